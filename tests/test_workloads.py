@@ -50,7 +50,7 @@ def test_smoothed_slab_orbitals():
 def test_fermi_dirac_occupations():
     w = wl.WORKLOADS[3]
     occ = wl.occupations(w)
-    assert occ.shape == (256,) and np.all(np.diff(occ) < 0) and occ[0] > 2 - 1e-12 and 0 < occ[-1] < 1e-12
+    assert occ.shape == (256,) and np.all(np.diff(occ) <= 0) and occ[0] > 2 - 1e-12 and 0 < occ[-1] < 1e-12
     i_mu = int(round(0.7 * 255))
     assert abs(occ[i_mu] - 1.0) < 0.2
     assert np.all(wl.occupations(wl.WORKLOADS[2]) == 2.0)
