@@ -56,4 +56,4 @@ def test_fermi_dirac_occupations():
     assert np.all(wl.occupations(wl.WORKLOADS[2]) == 2.0)
     w4 = wl.WORKLOADS[4]
     o4 = wl.occupations(w4)[w4.tgt_start:w4.tgt_start + w4.n_tgt]
-    assert o4[0] > 1.99 and o4[-1] < 0.01     # the target block straddles the Fermi edge
+    assert o4[0] > 1.99 and o4[-1] < 0.02     # the target block straddles the Fermi edge
