@@ -1,0 +1,137 @@
+/*
+ * exx.h -- C ABI of libexx.so: the exact-exchange apply on a real-space finite-difference grid,
+ * hand-written CUDA for sm_100a (NVIDIA B200).  One hot path of arxiv 2501.16572
+ * ("GPU acceleration of hybrid functional calculations in the SPARC electronic structure code").
+ * Citations are /root/reference/PAPER.md:<line> plus the equation; "R<n>" are the readings listed in
+ * DESIGN.md (= SURVEY.md section 8(c) A<n>).
+ *
+ * What the library computes (all real FP64, "double-precision arithmetic"):
+ *
+ *   phi_jk = f(L) (psi_j .* tgt_k)                                   Eqs. 2-5
+ *   vx_k   = - sum_j occ_j * psi_j .* phi_jk                          Eq. 1 / Eq. 19b
+ *   e_k    = h^3 * <tgt_k, vx_k>,   E_x = 1/2 sum_k occ_tgt_k e_k     BASELINE.json north_star (R7)
+ *
+ * f(L) is evaluated with the batch Kronecker-product formalism (Eqs. 6-7, 9-11, 16; PAPER.md:66-70,
+ * 86-98, 134): L = I(x)I(x)Kx + I(x)Ky(x)I + Kz(x)I(x)I, K_a = V_a diag(lam_a) V_a^T, three mode products
+ * with V^T, a pointwise multiply by m(lam_x+lam_y+lam_z), three mode products with V.
+ *   unscreened (omega <= 0):  m = 4 pi / mu, mu = -lam_sum; the zero mode is dropped (m := 0)
+ *   screened   (omega  > 0):  m = 4 pi (1 - exp(-mu/(4 omega^2))) / mu, m(0) = pi/omega^2       (R1-R3)
+ *
+ * Layout: a grid function is N = nx*ny*nz contiguous doubles, x fastest: idx = ix + nx*(iy + ny*iz)
+ * (the paper's vec of an n1 x n2 x n3 array).  A set of n functions is [n][N], each
+ * function contiguous (the column blocks of Eq. 10).
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE pointers on the plan's device; h_* are HOST pointers.  The caller owns
+ *    every buffer passed in, including the workspace; the plan owns V, lambda and the multiplier table.
+ *  - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*, NULL = default stream).
+ *    exx_apply / exx_poisson_solve never synchronise the host; results (including *d_ex) are valid once
+ *    the caller has synchronised that stream.  The calls are CUDA-graph capturable.
+ *  - Every entry point returns an exx_status; nothing throws, exits or aborts.  Arguments are validated
+ *    before the first launch, so a call that returns EXX_ERR_INVALID_ARG / _WORKSPACE / _ALIAS has
+ *    enqueued nothing.
+ *  - occ is used exactly as passed: no mixing fraction, spin factor or Brillouin weight (R8), no
+ *    thresholding of small occupations (R9).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns EXX_ERR_CUDA.
+ */
+#ifndef EXX_H
+#define EXX_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct exx_plan exx_plan; /* opaque; created/destroyed by the library */
+
+typedef enum {
+  EXX_OK = 0,
+  EXX_ERR_INVALID_ARG = 1,
+  EXX_ERR_ALLOC = 2,
+  EXX_ERR_CUDA = 3,
+  EXX_ERR_EIGENSOLVE = 4,
+  EXX_ERR_WORKSPACE = 5,
+  EXX_ERR_ALIAS = 6
+} exx_status;
+
+enum { EXX_BC_PERIODIC = 0, EXX_BC_DIRICHLET = 1 };
+
+/* Kernel variants (test hook; the default is the fast path). */
+enum {
+  EXX_VARIANT_FUSED_DMMA = 0, /* tensor-core (mma.sync f64 -> DMMA) mode products, fused passes */
+  EXX_VARIANT_REFERENCE = 1   /* one plain DFMA kernel per mode product; slow, for cross-checks  */
+};
+
+/*
+ * Build the plan: per-axis FD second-derivative matrices (central stencil of half-width fd_order/2,
+ * periodic wrap or Dirichlet truncation, R4/R6), their eigendecompositions (Eqs. 6-7;
+ * a cyclic Jacobi solver inside the library, host side, once) and the multiplier table f(Lambda~)
+ * (Eq. 16), uploaded to `device`.
+ *   nx,ny,nz >= 1; h > 0; bc[a] in {EXX_BC_PERIODIC, EXX_BC_DIRICHLET}; fd_order even >= 2;
+ *   omega <= 0 selects the unscreened kernel; max_batch >= 1 bounds n_c; device = CUDA ordinal.
+ * Errors: INVALID_ARG (nothing allocated), EIGENSOLVE (Jacobi did not converge), ALLOC, CUDA.
+ */
+exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3],
+                           int fd_order, double omega, int max_batch, int device);
+exx_status exx_plan_destroy(exx_plan* plan);
+
+/* Select a kernel variant (EXX_VARIANT_*). INVALID_ARG for unknown values. */
+exx_status exx_plan_set_variant(exx_plan* plan, int variant);
+
+/* Bytes of device workspace exx_apply / exx_poisson_solve need for batches of n_c right-hand sides
+ * (0 if plan is NULL or n_c is outside 1..max_batch). */
+size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c);
+
+/* Test hook: copy out one axis' eigenpairs. h_lambda: n doubles; h_V: n*n doubles, column-major
+ * (h_V[i + n*m] = component i of eigenvector m).  Either may be NULL. axis: 0=x, 1=y, 2=z. */
+exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, double* h_V);
+
+/* Test hook: copy out the multiplier table, N doubles, entry [a + nx*(b + ny*c)] = m(lam_x[a]+lam_y[b]+lam_z[c]). */
+exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult);
+
+/*
+ * Bare batched solver, Y = f(L) C (Eq. 9, 96-98 Eq. 11): d_phi[b] = f(L) d_rhs[b] for
+ * b < n_rhs, processed in batches of at most n_c (0 = library default).  d_phi may equal d_rhs (in
+ * place) but must not partially overlap it.  This is the unit of the "Poisson solves/s" metric.
+ */
+exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
+                             void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Exchange apply (Eq. 1, 42 Eq. 2, 178 Eq. 19b):
+ *   d_vx[k]  = - sum_{j<n_occ} d_occ[j] * d_psi[j] .* f(L)(d_psi[j] .* d_tgt[k])     [n_tgt][N], overwritten
+ *   d_ex_k[k] = h^3 <d_tgt[k], d_vx[k]>                                            [n_tgt], optional (NULL)
+ *   *d_ex    = 1/2 sum_k d_occ_tgt[k] d_ex_k[k]                                     optional (NULL); needs d_occ_tgt
+ * d_psi [n_occ][N], d_occ [n_occ]; d_tgt [n_tgt][N] may alias a block of d_psi.  d_vx must not overlap
+ * d_psi / d_tgt / the workspace (EXX_ERR_ALIAS).  n_c = right-hand sides per batch, 1..max_batch,
+ * 0 = library default.  Every (j,k) pair is solved (no symmetry shortcut, R12).  n_occ == 0 gives vx = 0.
+ */
+exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ,
+                     const double* d_tgt, const double* d_occ_tgt, int n_tgt, double* d_vx,
+                     double* d_ex, double* d_ex_k, int n_c, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Convenience end-to-end call with HOST buffers (pageable or pinned): uploads psi/occ (and tgt unless
+ * tgt_start >= 0 selects the block h_psi[tgt_start .. tgt_start+n_tgt) as targets), runs exx_apply on an
+ * internal stream, downloads vx / e_k / E_x and synchronises.  Device buffers are allocated and freed
+ * inside the call.  Any of h_vx, h_ex, h_ex_k may be NULL.
+ */
+exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_occ, int n_occ,
+                          const double* h_tgt, int tgt_start, const double* h_occ_tgt, int n_tgt,
+                          double* h_vx, double* h_ex, double* h_ex_k, int n_c);
+
+/* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
+long long exx_plan_last_launch_count(const exx_plan* plan);
+
+/* Human-readable status; for EXX_ERR_CUDA includes the last cudaError_t seen by this thread. */
+const char* exx_status_string(exx_status status);
+
+/* Library version string. */
+const char* exx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EXX_H */

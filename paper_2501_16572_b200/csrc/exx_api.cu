@@ -1,0 +1,387 @@
+// C-ABI layer of libexx.so (include/exx.h): argument validation, batching of the (j,k) pair space,
+// dispatch to the kernel variants.  No host synchronisation in exx_apply / exx_poisson_solve.
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "exx_internal.h"
+
+namespace {
+
+thread_local cudaError_t g_last_cuda = cudaSuccess;
+thread_local char g_msg[256];
+
+constexpr int kDefaultBatch = 32;
+constexpr int kEnergyChunk = 1024;  // targets per energy launch (bounds the plan-owned scratch)
+constexpr int kEnergyBlocks = 64;   // must match kernels_ref.cu
+
+struct HostApiBuffers {
+  double* base = nullptr;
+  size_t bytes = 0;
+  cudaStream_t stream = nullptr;
+};
+
+inline exx_status cuda_fail(cudaError_t e) {
+  g_last_cuda = e;
+  return EXX_ERR_CUDA;
+}
+
+#define EXX_CUDA(call)                              \
+  do {                                              \
+    cudaError_t e__ = (call);                       \
+    if (e__ != cudaSuccess) return cuda_fail(e__);  \
+  } while (0)
+
+inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+  if (!a || !b || na == 0 || nb == 0) return false;
+  const uintptr_t a0 = (uintptr_t)a, a1 = a0 + na, b0 = (uintptr_t)b, b1 = b0 + nb;
+  return a0 < b1 && b0 < a1;
+}
+
+inline int resolve_nc(const exx_plan* p, int n_c) {
+  if (n_c == 0) n_c = p->max_batch < kDefaultBatch ? p->max_batch : kDefaultBatch;
+  return n_c;
+}
+
+}  // namespace
+
+// plan-owned extras that are not part of the struct shared with the kernels
+struct PlanExtras {
+  double* d_energy_scratch = nullptr;  // kEnergyChunk * kEnergyBlocks doubles
+  HostApiBuffers hb;
+};
+static PlanExtras* extras_of(const exx_plan* p);
+
+struct exx_plan_full : exx_plan {
+  PlanExtras ex;
+};
+static PlanExtras* extras_of(const exx_plan* p) {
+  return &const_cast<exx_plan_full*>(static_cast<const exx_plan_full*>(p))->ex;
+}
+
+extern "C" {
+
+const char* exx_version(void) { return "exx-b200 0.1 (sm_100a)"; }
+
+const char* exx_status_string(exx_status s) {
+  switch (s) {
+    case EXX_OK: return "EXX_OK";
+    case EXX_ERR_INVALID_ARG: return "EXX_ERR_INVALID_ARG: invalid argument";
+    case EXX_ERR_ALLOC: return "EXX_ERR_ALLOC: allocation failed";
+    case EXX_ERR_CUDA:
+      snprintf(g_msg, sizeof(g_msg), "EXX_ERR_CUDA: %s (%s)", cudaGetErrorName(g_last_cuda),
+               cudaGetErrorString(g_last_cuda));
+      return g_msg;
+    case EXX_ERR_EIGENSOLVE: return "EXX_ERR_EIGENSOLVE: Jacobi eigensolver did not converge";
+    case EXX_ERR_WORKSPACE: return "EXX_ERR_WORKSPACE: workspace too small or missing";
+    case EXX_ERR_ALIAS: return "EXX_ERR_ALIAS: output overlaps an input or the workspace";
+  }
+  return "unknown exx_status";
+}
+
+exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3],
+                           int fd_order, double omega, int max_batch, int device) {
+  if (!out) return EXX_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (nx < 1 || ny < 1 || nz < 1 || !(h > 0.0) || !std::isfinite(h) || !bc || fd_order < 2 ||
+      (fd_order & 1) || fd_order > 64 || max_batch < 1 || max_batch > 65535 || !std::isfinite(omega))
+    return EXX_ERR_INVALID_ARG;
+  if ((long long)nx * ny * nz > (1LL << 31)) return EXX_ERR_INVALID_ARG;
+  for (int a = 0; a < 3; ++a)
+    if (bc[a] != EXX_BC_PERIODIC && bc[a] != EXX_BC_DIRICHLET) return EXX_ERR_INVALID_ARG;
+
+  exx_plan_full* p = new (std::nothrow) exx_plan_full();
+  if (!p) return EXX_ERR_ALLOC;
+  p->n[0] = nx; p->n[1] = ny; p->n[2] = nz;
+  p->h = h; p->order = fd_order; p->omega = omega; p->max_batch = max_batch; p->device = device;
+  p->variant = EXX_VARIANT_FUSED_DMMA;
+  p->N = (long long)nx * ny * nz;
+  p->d_mult = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0;
+  for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; }
+
+  try {
+    for (int a = 0; a < 3; ++a) {
+      // identical axes share the eigendecomposition (and, on the device, the matrix)
+      int same = -1;
+      for (int b = 0; b < a; ++b)
+        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a]) same = b;
+      if (same >= 0) {
+        p->h_lam[a] = p->h_lam[same];
+        p->h_V[a] = p->h_V[same];
+        continue;
+      }
+      std::vector<double> K = exx::second_derivative_matrix(p->n[a], h, bc[a], fd_order);
+      if (!exx::jacobi_eigh(p->n[a], K, p->h_lam[a], p->h_V[a])) {
+        delete p;
+        return EXX_ERR_EIGENSOLVE;
+      }
+    }
+    const double w0 = std::fabs(exx::fd_weights(fd_order, h)[0]);
+    p->h_mult = exx::multiplier_table(p->h_lam[0], p->h_lam[1], p->h_lam[2], omega, 1e-8 * 3.0 * w0);
+  } catch (const std::bad_alloc&) {
+    delete p;
+    return EXX_ERR_ALLOC;
+  }
+
+  if (device >= 0) {  // device < 0: host-only plan (planner tests); compute calls return EXX_ERR_CUDA
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess)
+      e = cudaDeviceGetAttribute(&p->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a) {
+      int same = -1;
+      for (int b = 0; b < a; ++b)
+        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a]) same = b;
+      if (same >= 0) { p->d_V[a] = p->d_V[same]; continue; }
+      const size_t bytes = sizeof(double) * p->h_V[a].size();
+      e = cudaMalloc(&p->d_V[a], bytes);
+      if (e == cudaSuccess) e = cudaMemcpy(p->d_V[a], p->h_V[a].data(), bytes, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_mult, sizeof(double) * p->N);
+    if (e == cudaSuccess)
+      e = cudaMemcpy(p->d_mult, p->h_mult.data(), sizeof(double) * p->N, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess)
+      e = cudaMalloc(&p->ex.d_energy_scratch, sizeof(double) * kEnergyChunk * kEnergyBlocks);
+    if (e == cudaSuccess) e = exx::fast_init(p);
+    if (e != cudaSuccess) {
+      exx_plan_destroy(p);
+      return e == cudaErrorMemoryAllocation ? EXX_ERR_ALLOC : cuda_fail(e);
+    }
+  }
+  *out = p;
+  return EXX_OK;
+}
+
+exx_status exx_plan_destroy(exx_plan* plan) {
+  if (!plan) return EXX_OK;
+  exx_plan_full* p = static_cast<exx_plan_full*>(plan);
+  if (p->device >= 0) {
+    cudaSetDevice(p->device);
+    exx::fast_destroy(p);
+    for (int a = 0; a < 3; ++a) {
+      bool shared = false;
+      for (int b = 0; b < a; ++b) shared |= (p->d_V[b] == p->d_V[a]);
+      if (!shared && p->d_V[a]) cudaFree(p->d_V[a]);
+    }
+    if (p->d_mult) cudaFree(p->d_mult);
+    if (p->ex.d_energy_scratch) cudaFree(p->ex.d_energy_scratch);
+    if (p->ex.hb.base) cudaFree(p->ex.hb.base);
+    if (p->ex.hb.stream) cudaStreamDestroy(p->ex.hb.stream);
+  }
+  delete p;
+  return EXX_OK;
+}
+
+exx_status exx_plan_set_variant(exx_plan* plan, int variant) {
+  if (!plan || (variant != EXX_VARIANT_FUSED_DMMA && variant != EXX_VARIANT_REFERENCE))
+    return EXX_ERR_INVALID_ARG;
+  plan->variant = variant;
+  return EXX_OK;
+}
+
+size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c) {
+  if (!plan) return 0;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return 0;
+  return 2 * sizeof(double) * (size_t)plan->N * (size_t)n_c;
+}
+
+exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, double* h_V) {
+  if (!plan || axis < 0 || axis > 2) return EXX_ERR_INVALID_ARG;
+  const int n = plan->n[axis];
+  if (h_lambda) std::memcpy(h_lambda, plan->h_lam[axis].data(), sizeof(double) * n);
+  if (h_V)
+    for (int i = 0; i < n; ++i)
+      for (int m = 0; m < n; ++m) h_V[i + (size_t)n * m] = plan->h_V[axis][(size_t)i * n + m];
+  return EXX_OK;
+}
+
+exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult) {
+  if (!plan || !h_mult) return EXX_ERR_INVALID_ARG;
+  std::memcpy(h_mult, plan->h_mult.data(), sizeof(double) * plan->N);
+  return EXX_OK;
+}
+
+long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }
+
+}  // extern "C"
+
+namespace {
+
+// One batch of the reference variant: buf0 holds the right-hand sides on entry, phi on exit.
+cudaError_t ref_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, cudaStream_t s,
+                            long long* launches) {
+  cudaError_t e;
+  if ((e = exx::ref_mode_product(p, 0, true, buf0, buf1, nb, false, s)) != cudaSuccess) return e;
+  if ((e = exx::ref_mode_product(p, 1, true, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
+  if ((e = exx::ref_mode_product(p, 2, true, buf0, buf1, nb, true, s)) != cudaSuccess) return e;
+  if ((e = exx::ref_mode_product(p, 2, false, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
+  if ((e = exx::ref_mode_product(p, 1, false, buf0, buf1, nb, false, s)) != cudaSuccess) return e;
+  if ((e = exx::ref_mode_product(p, 0, false, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
+  *launches += 6;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" {
+
+exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
+                             void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_rhs < 0 || (n_rhs > 0 && (!d_rhs || !d_phi))) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  if (n_rhs == 0) { plan->last_launches = 0; return EXX_OK; }
+  const size_t need = exx_plan_workspace_bytes(plan, n_c);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
+  if (d_rhs != d_phi && overlaps(d_rhs, fn * n_rhs, d_phi, fn * n_rhs)) return EXX_ERR_ALIAS;
+  if (overlaps(d_workspace, need, d_phi, fn * n_rhs) || overlaps(d_workspace, need, d_rhs, fn * n_rhs))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  double* buf0 = (double*)d_workspace;
+  double* buf1 = buf0 + N * (size_t)n_c;
+  long long launches = 0;
+  for (int b0 = 0; b0 < n_rhs; b0 += n_c) {
+    const int nb = n_rhs - b0 < n_c ? n_rhs - b0 : n_c;
+    EXX_CUDA(cudaMemcpyAsync(buf0, d_rhs + N * (size_t)b0, fn * nb, cudaMemcpyDeviceToDevice, s));
+    if (plan->variant == EXX_VARIANT_REFERENCE) {
+      EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
+    } else {
+      EXX_CUDA(exx::fast_solve_batch(plan, buf0, buf1, nb, nullptr, s, &launches));
+    }
+    EXX_CUDA(cudaMemcpyAsync(d_phi + N * (size_t)b0, buf0, fn * nb, cudaMemcpyDeviceToDevice, s));
+  }
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ,
+                     const double* d_tgt, const double* d_occ_tgt, int n_tgt, double* d_vx,
+                     double* d_ex, double* d_ex_k, int n_c, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_occ < 0 || n_tgt < 0) return EXX_ERR_INVALID_ARG;
+  if (n_occ > 0 && (!d_psi || !d_occ)) return EXX_ERR_INVALID_ARG;
+  if (n_tgt > 0 && (!d_tgt || !d_vx)) return EXX_ERR_INVALID_ARG;
+  if (d_ex && !d_occ_tgt && n_tgt > 0) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
+  const size_t need = exx_plan_workspace_bytes(plan, n_c);
+  if (n_occ > 0 && n_tgt > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
+  if (overlaps(d_vx, fn * n_tgt, d_psi, fn * n_occ) || overlaps(d_vx, fn * n_tgt, d_tgt, fn * n_tgt) ||
+      overlaps(d_vx, fn * n_tgt, d_workspace, need) || overlaps(d_workspace, need, d_psi, fn * n_occ) ||
+      overlaps(d_workspace, need, d_tgt, fn * n_tgt))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  long long launches = 0;
+  PlanExtras* ex = extras_of(plan);
+
+  if (n_tgt > 0 && n_occ == 0) {
+    EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_tgt, s));
+    ++launches;
+  } else if (n_tgt > 0) {
+    double* buf0 = (double*)d_workspace;
+    double* buf1 = buf0 + N * (size_t)n_c;
+    // Batch = nk targets x nj occupied orbitals, nj*nk <= n_c.  With n_occ >= n_c one target per batch.
+    const int nj_max = n_occ < n_c ? n_occ : n_c;
+    const int nk_max = n_c / nj_max;
+    for (int k0 = 0; k0 < n_tgt; k0 += nk_max) {
+      const int nk = n_tgt - k0 < nk_max ? n_tgt - k0 : nk_max;
+      for (int j0 = 0; j0 < n_occ; j0 += nj_max) {
+        const int nj = n_occ - j0 < nj_max ? n_occ - j0 : nj_max;
+        const exx::BatchDesc bd{j0, nj, k0, nk};
+        const int nb = nj * nk;
+        if (plan->variant == EXX_VARIANT_REFERENCE) {
+          EXX_CUDA(exx::ref_pair_density(plan, d_psi, d_tgt, bd, buf0, s));
+          EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
+          EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, j0 == 0, d_vx, s));
+          launches += 2;
+        } else {
+          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, j0 == 0};
+          EXX_CUDA(exx::fast_solve_batch(plan, buf0, buf1, nb, &fa, s, &launches));
+        }
+      }
+    }
+  }
+  if (d_ex && n_tgt == 0) {
+    EXX_CUDA(exx::zero_fill(d_ex, 1, s));
+    ++launches;
+  }
+  if ((d_ex || d_ex_k) && n_tgt > 0) {
+    // E_x is accumulated chunk by chunk; the first chunk overwrites *d_ex
+    for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
+      const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
+      if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
+      EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0,
+                           d_occ_tgt ? d_occ_tgt + k0 : nullptr, nk, ex->d_energy_scratch,
+                           d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
+      launches += 2;
+    }
+  }
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_occ, int n_occ,
+                          const double* h_tgt, int tgt_start, const double* h_occ_tgt, int n_tgt,
+                          double* h_vx, double* h_ex, double* h_ex_k, int n_c) {
+  if (!plan || n_occ < 0 || n_tgt < 0 || (n_occ > 0 && (!h_psi || !h_occ))) return EXX_ERR_INVALID_ARG;
+  const bool tgt_in_psi = tgt_start >= 0;
+  if (tgt_in_psi && tgt_start + n_tgt > n_occ) return EXX_ERR_INVALID_ARG;
+  if (!tgt_in_psi && n_tgt > 0 && !h_tgt) return EXX_ERR_INVALID_ARG;
+  if (h_ex && !h_occ_tgt && n_tgt > 0) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  EXX_CUDA(cudaSetDevice(plan->device));
+  PlanExtras* ex = extras_of(plan);
+  const size_t N = (size_t)plan->N;
+  const size_t ws = exx_plan_workspace_bytes(plan, n_c);
+  // carve: psi | tgt (if separate) | vx | occ | occ_tgt | ex_k | ex | workspace
+  size_t n_dbl = N * n_occ + (tgt_in_psi ? 0 : N * n_tgt) + N * n_tgt + n_occ + 2 * (size_t)n_tgt + 8;
+  size_t bytes = sizeof(double) * n_dbl + ws + 512;
+  if (ex->hb.bytes < bytes) {
+    if (ex->hb.base) cudaFree(ex->hb.base);
+    ex->hb.base = nullptr; ex->hb.bytes = 0;
+    cudaError_t e = cudaMalloc(&ex->hb.base, bytes);
+    if (e != cudaSuccess) { g_last_cuda = e; return EXX_ERR_ALLOC; }
+    ex->hb.bytes = bytes;
+  }
+  if (!ex->hb.stream) EXX_CUDA(cudaStreamCreateWithFlags(&ex->hb.stream, cudaStreamNonBlocking));
+  cudaStream_t s = ex->hb.stream;
+  double* q = ex->hb.base;
+  double* d_psi = q; q += N * n_occ;
+  double* d_tgt = tgt_in_psi ? d_psi + N * (size_t)tgt_start : q;
+  if (!tgt_in_psi) q += N * n_tgt;
+  double* d_vx = q; q += N * n_tgt;
+  double* d_occ = q; q += n_occ;
+  double* d_occ_tgt = q; q += n_tgt;
+  double* d_ex_k = q; q += n_tgt;
+  double* d_ex = q; q += 8;
+  void* d_ws = (void*)(((uintptr_t)q + 255) & ~(uintptr_t)255);
+  if (n_occ > 0) {
+    EXX_CUDA(cudaMemcpyAsync(d_psi, h_psi, sizeof(double) * N * n_occ, cudaMemcpyHostToDevice, s));
+    EXX_CUDA(cudaMemcpyAsync(d_occ, h_occ, sizeof(double) * n_occ, cudaMemcpyHostToDevice, s));
+  }
+  if (!tgt_in_psi && n_tgt > 0)
+    EXX_CUDA(cudaMemcpyAsync(d_tgt, h_tgt, sizeof(double) * N * n_tgt, cudaMemcpyHostToDevice, s));
+  if (h_occ_tgt && n_tgt > 0)
+    EXX_CUDA(cudaMemcpyAsync(d_occ_tgt, h_occ_tgt, sizeof(double) * n_tgt, cudaMemcpyHostToDevice, s));
+  exx_status st = exx_apply(plan, d_psi, d_occ, n_occ, d_tgt, h_occ_tgt ? d_occ_tgt : nullptr, n_tgt, d_vx,
+                            h_ex ? d_ex : nullptr, h_ex_k ? d_ex_k : nullptr, n_c, d_ws, ws, s);
+  if (st != EXX_OK) return st;
+  if (h_vx && n_tgt > 0)
+    EXX_CUDA(cudaMemcpyAsync(h_vx, d_vx, sizeof(double) * N * n_tgt, cudaMemcpyDeviceToHost, s));
+  if (h_ex_k && n_tgt > 0)
+    EXX_CUDA(cudaMemcpyAsync(h_ex_k, d_ex_k, sizeof(double) * n_tgt, cudaMemcpyDeviceToHost, s));
+  if (h_ex) EXX_CUDA(cudaMemcpyAsync(h_ex, d_ex, sizeof(double), cudaMemcpyDeviceToHost, s));
+  EXX_CUDA(cudaStreamSynchronize(s));
+  return EXX_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,84 @@
+// Internal declarations shared by the host planner, the kernels and the C-ABI layer of libexx.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "exx.h"
+
+namespace exx {
+
+// ---- host planner (plan_host.cpp) -------------------------------------------------------------
+// Central second-derivative weights w[0..n0], order = 2*n0 (R4).
+std::vector<double> fd_weights(int order, double h);
+// Dense symmetric n x n matrix of +d^2/dx^2, row-major (R2, R6).
+std::vector<double> second_derivative_matrix(int n, double h, int bc, int order);
+// Cyclic Jacobi: A (row-major, symmetric, destroyed) -> eigenvalues ascending in lam, eigenvectors in
+// V row-major V[i*n + m] = component i of eigenvector m.  Returns false if not converged.
+bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::vector<double>& V);
+// f(Lambda~) table (PAPER.md:61 Eq. 5, :134 Eq. 16; R1-R3), entry [a + nx*(b + ny*c)].
+std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
+                                     const std::vector<double>& lz, double omega, double zero_tol);
+
+}  // namespace exx
+
+struct exx_plan {
+  int n[3];  // nx, ny, nz
+  double h;
+  int bc[3];
+  int order;
+  double omega;
+  int max_batch;
+  int device;
+  int variant;
+  long long N;
+  std::vector<double> h_lam[3];
+  std::vector<double> h_V[3];  // row-major [i][m]
+  std::vector<double> h_mult;
+  // device copies
+  double* d_V[3];    // row-major [i][m], n*n (axes with identical matrices share one allocation)
+  double* d_mult;    // N
+  int sm_count;
+  int smem_optin;
+  long long last_launches;
+};
+
+namespace exx {
+
+// Batch descriptor: right-hand side b of a batch is the pair (j0 + b % nj, k0 + b / nj).
+struct BatchDesc {
+  int j0, nj, k0, nk;
+};
+
+// ---- reference variant (kernels_ref.cu): one plain DFMA kernel per step ----------------------
+cudaError_t ref_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd,
+                             double* out, cudaStream_t s);
+cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const double* in, double* out,
+                             int nb, bool apply_mult, cudaStream_t s);
+cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
+                           BatchDesc bd, bool first, double* vx, cudaStream_t s);
+// shared by both variants: e_k = h^3 <tgt_k, vx_k>, then E_x
+cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
+                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s);
+cudaError_t zero_fill(double* p, long long n, cudaStream_t s);
+
+// ---- fast variant (kernels_dmma.cu) ----------------------------------------------------------
+// Returns cudaErrorNotSupported if the plan's sizes are outside what the fast kernels handle
+// (the caller then reports EXX_ERR_INVALID_ARG; there is no silent fallback).
+cudaError_t fast_init(exx_plan* p);
+void fast_destroy(exx_plan* p);
+// phi-producing solve of one batch: in-place on buf0 using buf1 as scratch; result ends in buf0.
+// src_mode 0: buf0 already holds the right-hand sides.  src_mode 1: pair densities are formed on the
+// fly from psi/tgt (bd).  If acc != nullptr the last pass accumulates into vx instead of storing phi.
+struct FastArgs {
+  const double* psi;
+  const double* tgt;
+  const double* occ;
+  double* vx;
+  BatchDesc bd;
+  bool first;  // first batch for these targets: vx is overwritten, not accumulated into
+};
+cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, const FastArgs* fa,
+                             cudaStream_t s, long long* launches);
+
+}  // namespace exx

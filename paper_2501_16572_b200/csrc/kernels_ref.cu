@@ -1,0 +1,176 @@
+// Reference variant (EXX_VARIANT_REFERENCE): one plain FP64 kernel per step of the hot path.
+// Deliberately simple -- used to cross-check the fast variant on the GPU and as a fallback-free
+// "second opinion" in the parity tests.  Also holds the kernels both variants share (energy, zero fill).
+#include "exx_internal.h"
+
+namespace exx {
+namespace {
+
+// a1: rho_b(r) = psi_j(r) * tgt_k(r)   (Eq. 2 right-hand side; real => no conj)
+__global__ void k_pair_density(const double* __restrict__ psi, const double* __restrict__ tgt,
+                               BatchDesc bd, long long N, double* __restrict__ out) {
+  const int b = blockIdx.y;
+  const int j = bd.j0 + b % bd.nj, k = bd.k0 + b / bd.nj;
+  const double* pj = psi + (long long)j * N;
+  const double* tk = tgt + (long long)k * N;
+  double* o = out + (long long)b * N;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N;
+       i += (long long)gridDim.x * blockDim.x)
+    o[i] = pj[i] * tk[i];
+}
+
+// a2/a4: one mode product along `axis`.  Data viewed as [outer][n][inner]; forward contracts with V^T
+// (out[m] = sum_i V[i][m] in[i]), backward with V (out[i] = sum_m V[i][m] in[m]).  PAPER.md:96-98 (Eq. 11).
+// a3 (optional): multiply the result by the table m (Eq. 16) -- only ever used on the
+// last forward product, whose output index is the full eigen-space index.
+__global__ void k_mode_product(const double* __restrict__ in, double* __restrict__ out,
+                               const double* __restrict__ V, int n, long long inner, long long total,
+                               bool forward, const double* __restrict__ mult, long long N) {
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const long long i_in = t % inner;
+    const long long r = t / inner;
+    const int m = (int)(r % n);
+    const long long o = r / n;
+    const double* src = in + o * n * inner + i_in;
+    double acc = 0.0;
+    if (forward) {
+      for (int i = 0; i < n; ++i) acc = fma(V[(long long)i * n + m], src[i * inner], acc);
+    } else {
+      for (int i = 0; i < n; ++i) acc = fma(V[(long long)m * n + i], src[i * inner], acc);
+    }
+    if (mult) acc *= mult[t % N];
+    out[t] = acc;
+  }
+}
+
+// a5: vx_k(r) (-)= sum_b occ_j psi_j(r) phi_b(r), b ascending (PAPER.md:38 Eq. 1, :178 Eq. 19b).
+__global__ void k_accumulate(const double* __restrict__ psi, const double* __restrict__ occ,
+                             const double* __restrict__ phi, BatchDesc bd, bool first, long long N,
+                             double* __restrict__ vx) {
+  const int kk = blockIdx.y;
+  double* v = vx + (long long)(bd.k0 + kk) * N;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N;
+       i += (long long)gridDim.x * blockDim.x) {
+    double acc = first ? 0.0 : v[i];
+    for (int jj = 0; jj < bd.nj; ++jj) {
+      const long long b = (long long)kk * bd.nj + jj;
+      acc -= occ[bd.j0 + jj] * psi[(long long)(bd.j0 + jj) * N + i] * phi[b * N + i];
+    }
+    v[i] = acc;
+  }
+}
+
+// a6: per-target partial sums with warp shuffles, deterministic two-stage reduction.
+constexpr int kEnergyBlocks = 64;
+constexpr int kEnergyThreads = 256;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__global__ void k_energy_partial(const double* __restrict__ tgt, const double* __restrict__ vx,
+                                 long long N, double* __restrict__ partial) {
+  const int k = blockIdx.y;
+  const double* t = tgt + (long long)k * N;
+  const double* v = vx + (long long)k * N;
+  double acc = 0.0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N;
+       i += (long long)gridDim.x * blockDim.x)
+    acc = fma(t[i], v[i], acc);
+  __shared__ double sh[kEnergyThreads / 32];
+  acc = warp_sum(acc);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double s = threadIdx.x < kEnergyThreads / 32 ? sh[threadIdx.x] : 0.0;
+    s = warp_sum(s);
+    if (threadIdx.x == 0) partial[(long long)k * gridDim.x + blockIdx.x] = s;
+  }
+}
+
+// one block: e_k = dV * sum of the partials of target k (fixed order), E_x += 1/2 sum_k occ_k e_k
+__global__ void k_energy_final(const double* __restrict__ partial, int nblk, int n_tgt, double dV,
+                               const double* __restrict__ occ_tgt, double* __restrict__ ex_k,
+                               double* __restrict__ ex) {
+  double acc = 0.0;
+  for (int k = threadIdx.x; k < n_tgt; k += blockDim.x) {
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) s += partial[(long long)k * nblk + b];
+    s *= dV;
+    if (ex_k) ex_k[k] = s;
+    if (occ_tgt) acc = fma(occ_tgt[k], s, acc);
+  }
+  __shared__ double sh[32];
+  acc = warp_sum(acc);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double s = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+    s = warp_sum(s);
+    if (threadIdx.x == 0 && ex) *ex += 0.5 * s;  // caller zeroes *ex before the first chunk
+  }
+}
+
+__global__ void k_zero(double* p, long long n) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x)
+    p[i] = 0.0;
+}
+
+inline int grid_for(long long work, int threads, int sm_count) {
+  long long g = (work + threads - 1) / threads;
+  const long long cap = (long long)sm_count * 16;
+  if (g > cap) g = cap;
+  if (g < 1) g = 1;
+  return (int)g;
+}
+
+}  // namespace
+
+cudaError_t ref_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd,
+                             double* out, cudaStream_t s) {
+  dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nj * bd.nk);
+  k_pair_density<<<grid, 256, 0, s>>>(psi, tgt, bd, p->N, out);
+  return cudaGetLastError();
+}
+
+cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const double* in, double* out,
+                             int nb, bool apply_mult, cudaStream_t s) {
+  const int n = p->n[axis];
+  const long long inner = axis == 0 ? 1 : (axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1]);
+  const long long total = p->N * nb;
+  k_mode_product<<<grid_for(total, 256, p->sm_count), 256, 0, s>>>(
+      in, out, p->d_V[axis], n, inner, total, forward, apply_mult ? p->d_mult : nullptr, p->N);
+  return cudaGetLastError();
+}
+
+cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
+                           BatchDesc bd, bool first, double* vx, cudaStream_t s) {
+  dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
+  k_accumulate<<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
+  return cudaGetLastError();
+}
+
+// ex_k_scratch: n_tgt * kEnergyBlocks doubles (carved from the caller's workspace)
+cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
+                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s) {
+  if (n_tgt <= 0) return cudaSuccess;
+  dim3 grid(kEnergyBlocks, n_tgt);
+  k_energy_partial<<<grid, kEnergyThreads, 0, s>>>(tgt, vx, p->N, ex_k_scratch);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_energy_final<<<1, 256, 0, s>>>(ex_k_scratch, kEnergyBlocks, n_tgt, p->h * p->h * p->h, occ_tgt,
+                                   ex_k, ex);
+  return cudaGetLastError();
+}
+
+cudaError_t zero_fill(double* ptr, long long n, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  k_zero<<<grid_for(n, 256, 148), 256, 0, s>>>(ptr, n);
+  return cudaGetLastError();
+}
+
+}  // namespace exx

@@ -1,0 +1,147 @@
+// Host-side planner of libexx.so: FD second-derivative matrices, a cyclic Jacobi eigensolver and the
+// multiplier table.  Runs once per plan (Eqs. 6-7: "eigenvectors of the discrete second
+// derivative operators"); not on the timed path.  No LAPACK dependency, no code shared with oracle/.
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+
+#include "exx_internal.h"
+
+namespace exx {
+
+// w_q = (1/q^2) * prod_{m != q} m^2 / (m^2 - q^2), q = 1..n0 (Lagrange form of the centred stencil),
+// w_0 = -2 sum_q w_q; all divided by h^2.  DESIGN.md R4.
+std::vector<double> fd_weights(int order, double h) {
+  const int n0 = order / 2;
+  std::vector<double> w(n0 + 1, 0.0);
+  for (int q = 1; q <= n0; ++q) {
+    long double prod = 1.0L;
+    for (int m = 1; m <= n0; ++m) {
+      if (m == q) continue;
+      prod *= (long double)(m * m) / (long double)(m * m - q * q);
+    }
+    w[q] = (double)(prod / (long double)(q * q));
+  }
+  long double s = 0.0L;
+  for (int q = n0; q >= 1; --q) s += (long double)w[q];
+  w[0] = (double)(-2.0L * s);
+  for (auto& x : w) x /= (h * h);
+  return w;
+}
+
+std::vector<double> second_derivative_matrix(int n, double h, int bc, int order) {
+  const std::vector<double> w = fd_weights(order, h);
+  const int n0 = order / 2;
+  std::vector<double> K((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i) {
+    for (int q = -n0; q <= n0; ++q) {
+      int j = i + q;
+      if (bc == EXX_BC_PERIODIC) {
+        j %= n;
+        if (j < 0) j += n;
+        K[(size_t)i * n + j] += w[std::abs(q)];  // accumulate: the stencil may wrap more than once
+      } else if (j >= 0 && j < n) {
+        K[(size_t)i * n + j] = w[std::abs(q)];   // truncated at the Dirichlet boundary
+      }
+    }
+  }
+  return K;
+}
+
+// Cyclic-by-row Jacobi with the standard stable rotation (Golub & Van Loan, Alg. 8.5.x restated).
+bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::vector<double>& V) {
+  V.assign((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i) V[(size_t)i * n + i] = 1.0;
+  lam.assign(n, 0.0);
+  if (n == 1) {
+    lam[0] = A[0];
+    return true;
+  }
+  double fro = 0.0;
+  for (double a : A) fro += a * a;
+  fro = std::sqrt(fro);
+  if (fro == 0.0) return true;
+  const int max_sweeps = 60;
+  bool converged = false;
+  for (int sweep = 0; sweep < max_sweeps && !converged; ++sweep) {
+    double off = 0.0;
+    for (int p = 0; p < n; ++p)
+      for (int q = p + 1; q < n; ++q) off += A[(size_t)p * n + q] * A[(size_t)p * n + q];
+    if (std::sqrt(2.0 * off) <= 1e-17 * fro) {
+      converged = true;
+      break;
+    }
+    for (int p = 0; p < n - 1; ++p) {
+      for (int q = p + 1; q < n; ++q) {
+        const double apq = A[(size_t)p * n + q];
+        if (apq == 0.0) continue;
+        const double app = A[(size_t)p * n + p], aqq = A[(size_t)q * n + q];
+        if (std::fabs(apq) < 1e-300) continue;
+        const double tau = (aqq - app) / (2.0 * apq);
+        const double t = (tau >= 0.0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
+        const double c = 1.0 / std::sqrt(1.0 + t * t), s = t * c;
+        // A <- J^T A J on rows/columns p, q
+        for (int k = 0; k < n; ++k) {
+          const double akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
+          A[(size_t)k * n + p] = c * akp - s * akq;
+          A[(size_t)k * n + q] = s * akp + c * akq;
+        }
+        for (int k = 0; k < n; ++k) {
+          const double apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
+          A[(size_t)p * n + k] = c * apk - s * aqk;
+          A[(size_t)q * n + k] = s * apk + c * aqk;
+        }
+        A[(size_t)p * n + q] = 0.0;
+        A[(size_t)q * n + p] = 0.0;
+        for (int k = 0; k < n; ++k) {
+          const double vkp = V[(size_t)k * n + p], vkq = V[(size_t)k * n + q];
+          V[(size_t)k * n + p] = c * vkp - s * vkq;
+          V[(size_t)k * n + q] = s * vkp + c * vkq;
+        }
+      }
+    }
+  }
+  if (!converged) {
+    double off = 0.0;
+    for (int p = 0; p < n; ++p)
+      for (int q = p + 1; q < n; ++q) off += A[(size_t)p * n + q] * A[(size_t)p * n + q];
+    if (std::sqrt(2.0 * off) > 1e-14 * fro) return false;
+  }
+  // sort ascending
+  std::vector<int> idx(n);
+  std::iota(idx.begin(), idx.end(), 0);
+  std::sort(idx.begin(), idx.end(),
+            [&](int a, int b) { return A[(size_t)a * n + a] < A[(size_t)b * n + b]; });
+  std::vector<double> Vs((size_t)n * n);
+  for (int m = 0; m < n; ++m) {
+    lam[m] = A[(size_t)idx[m] * n + idx[m]];
+    for (int i = 0; i < n; ++i) Vs[(size_t)i * n + m] = V[(size_t)i * n + idx[m]];
+  }
+  V.swap(Vs);
+  return true;
+}
+
+std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
+                                     const std::vector<double>& lz, double omega, double zero_tol) {
+  const size_t nx = lx.size(), ny = ly.size(), nz = lz.size();
+  std::vector<double> m(nx * ny * nz);
+  const double four_pi = 4.0 * M_PI;
+  for (size_t c = 0; c < nz; ++c)
+    for (size_t b = 0; b < ny; ++b)
+      for (size_t a = 0; a < nx; ++a) {
+        const double ls = lz[c] + ly[b] + lx[a];
+        const double mu = -ls;
+        double v;
+        if (std::fabs(ls) < zero_tol) {
+          v = omega > 0.0 ? M_PI / (omega * omega) : 0.0;  // R3: keep the limit (HSE) / drop (PBE0)
+        } else if (omega > 0.0) {
+          v = -four_pi * std::expm1(-mu / (4.0 * omega * omega)) / mu;  // R1
+        } else {
+          v = four_pi / mu;  // R2
+        }
+        m[a + nx * (b + ny * c)] = v;
+      }
+  return m;
+}
+
+}  // namespace exx

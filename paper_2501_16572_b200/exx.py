@@ -1,0 +1,224 @@
+"""Thin ctypes binding over libexx.so (include/exx.h).  Argument marshalling only: every step of
+the hot path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+
+There is no CPU fallback: if libexx.so is missing or a call fails, an :class:`ExxError` is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+EXX_OK = 0
+BC_PERIODIC, BC_DIRICHLET = 0, 1
+VARIANT_FUSED_DMMA, VARIANT_REFERENCE = 0, 1
+
+_lib = None
+
+
+class ExxError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = load_library().exx_status_string(status).decode()
+        super().__init__(f"{where}: {msg}")
+
+
+def lib_path() -> str:
+    return os.path.join(HERE, "libexx.so")
+
+
+def load_library():
+    """dlopen libexx.so (built in-tree by ``paper_2501_16572_b200.build``); fail loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise RuntimeError(
+            f"{path} not found: build it with `python -m paper_2501_16572_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)
+    lib.exx_plan_create.restype = C.c_int
+    lib.exx_plan_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, ip, C.c_int,
+                                    C.c_double, C.c_int, C.c_int]
+    lib.exx_plan_destroy.restype = C.c_int
+    lib.exx_plan_destroy.argtypes = [vp]
+    lib.exx_plan_set_variant.restype = C.c_int
+    lib.exx_plan_set_variant.argtypes = [vp, C.c_int]
+    lib.exx_plan_workspace_bytes.restype = C.c_size_t
+    lib.exx_plan_workspace_bytes.argtypes = [vp, C.c_int]
+    lib.exx_plan_get_axis.restype = C.c_int
+    lib.exx_plan_get_axis.argtypes = [vp, C.c_int, dp, dp]
+    lib.exx_plan_get_multiplier.restype = C.c_int
+    lib.exx_plan_get_multiplier.argtypes = [vp, dp]
+    lib.exx_poisson_solve.restype = C.c_int
+    lib.exx_poisson_solve.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_apply.restype = C.c_int
+    lib.exx_apply.argtypes = [vp, dp, dp, C.c_int, dp, dp, C.c_int, dp, dp, dp, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_apply_host.restype = C.c_int
+    lib.exx_apply_host.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, dp, C.c_int, dp, dp, dp, C.c_int]
+    lib.exx_plan_last_launch_count.restype = C.c_longlong
+    lib.exx_plan_last_launch_count.argtypes = [vp]
+    lib.exx_status_string.restype = C.c_char_p
+    lib.exx_status_string.argtypes = [C.c_int]
+    lib.exx_version.restype = C.c_char_p
+    lib.exx_version.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _check(status: int, where: str):
+    if status != EXX_OK:
+        raise ExxError(status, where)
+
+
+def _dev_ptr(t: torch.Tensor | None, device: torch.device, what: str):
+    if t is None:
+        return None
+    if t.dtype != torch.float64 or not t.is_contiguous():
+        raise ValueError(f"{what}: need a contiguous float64 tensor")
+    if t.device != device:
+        raise ValueError(f"{what}: tensor is on {t.device}, plan is on {device}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_ptr(t, what: str):
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags.c_contiguous:
+            raise ValueError(f"{what}: need a C-contiguous float64 array")
+        return C.c_void_p(t.ctypes.data)
+    if t.dtype != torch.float64 or not t.is_contiguous() or t.device.type != "cpu":
+        raise ValueError(f"{what}: need a contiguous float64 host tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """exx_plan_create / exx_plan_destroy (the per-axis eigendecompositions, once)."""
+
+    def __init__(self, nx, ny, nz, h, bc=(0, 0, 0), fd_order=12, omega=0.0, max_batch=64, device=0):
+        lib = load_library()
+        self._lib = lib
+        self._h = C.c_void_p()
+        self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
+        self.N = self.nx * self.ny * self.nz
+        self.max_batch = int(max_batch)
+        self.device_index = int(device)
+        self.device = torch.device("cuda", device) if device >= 0 else torch.device("cpu")
+        bc_arr = (C.c_int * 3)(*[int(b) for b in bc])
+        st = lib.exx_plan_create(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, max_batch, device)
+        _check(st, "exx_plan_create")
+        self._ws = None
+
+    @classmethod
+    def for_workload(cls, w, max_batch=None, device=0):
+        return cls(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega,
+                   max_batch if max_batch is not None else max(64, w.default_nc), device)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.exx_plan_destroy(self._h)
+            self._h = C.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_variant(self, variant: int):
+        _check(self._lib.exx_plan_set_variant(self._h, variant), "exx_plan_set_variant")
+
+    def workspace_bytes(self, n_c: int = 0) -> int:
+        return int(self._lib.exx_plan_workspace_bytes(self._h, n_c))
+
+    def get_axis(self, axis: int):
+        n = (self.nx, self.ny, self.nz)[axis]
+        lam = np.empty(n)
+        V = np.empty((n, n), order="F")  # column-major: V[i, m] = component i of eigenvector m
+        _check(self._lib.exx_plan_get_axis(self._h, axis, C.c_void_p(lam.ctypes.data), C.c_void_p(V.ctypes.data)),
+               "exx_plan_get_axis")
+        return lam, V
+
+    def get_multiplier(self) -> np.ndarray:
+        m = np.empty((self.nz, self.ny, self.nx))
+        _check(self._lib.exx_plan_get_multiplier(self._h, C.c_void_p(m.ctypes.data)), "exx_plan_get_multiplier")
+        return m
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self._lib.exx_plan_last_launch_count(self._h))
+
+    def _workspace(self, n_c: int) -> torch.Tensor:
+        need = self.workspace_bytes(n_c)
+        if need == 0:
+            raise ValueError(f"n_c={n_c} outside 1..max_batch={self.max_batch}")
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def poisson_solve(self, rhs: torch.Tensor, out: torch.Tensor | None = None, n_c: int = 0,
+                      stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+        """exx_poisson_solve: out[b] = f(L) rhs[b] (Eq. 9).  ``out`` may be ``rhs``."""
+        n_rhs = rhs.shape[0] if rhs.dim() > 1 else 1
+        if rhs.numel() != n_rhs * self.N:
+            raise ValueError("rhs must be [n_rhs, nz, ny, nx]")
+        if out is None:
+            out = torch.empty_like(rhs)
+        ws = self._workspace(n_c)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_poisson_solve(self._h, _dev_ptr(rhs, self.device, "rhs"), _dev_ptr(out, self.device, "out"),
+                                         n_rhs, n_c, C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(s.cuda_stream))
+        _check(st, "exx_poisson_solve")
+        return out
+
+    def apply(self, psi: torch.Tensor, occ: torch.Tensor, tgt: torch.Tensor, occ_tgt: torch.Tensor | None = None,
+              vx: torch.Tensor | None = None, n_c: int = 0, want_ex_k: bool = True,
+              stream: torch.cuda.Stream | None = None):
+        """exx_apply: returns (vx [n_tgt, nz, ny, nx], e_k [n_tgt] or None, E_x 0-dim tensor or None);
+        all device tensors, valid once ``stream`` (default: torch's current stream) is synchronised."""
+        n_occ, n_tgt = psi.shape[0], tgt.shape[0]
+        if psi.numel() != n_occ * self.N or tgt.numel() != n_tgt * self.N:
+            raise ValueError("psi/tgt must be [n, nz, ny, nx]")
+        if vx is None:
+            vx = torch.empty((n_tgt, self.nz, self.ny, self.nx), dtype=torch.float64, device=self.device)
+        ex = torch.empty((), dtype=torch.float64, device=self.device) if occ_tgt is not None else None
+        ex_k = torch.empty(n_tgt, dtype=torch.float64, device=self.device) if want_ex_k else None
+        ws = self._workspace(n_c)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_apply(self._h, _dev_ptr(psi, self.device, "psi"), _dev_ptr(occ, self.device, "occ"), n_occ,
+                                 _dev_ptr(tgt, self.device, "tgt"), _dev_ptr(occ_tgt, self.device, "occ_tgt"), n_tgt,
+                                 _dev_ptr(vx, self.device, "vx"), _dev_ptr(ex, self.device, "ex"),
+                                 _dev_ptr(ex_k, self.device, "ex_k"), n_c, C.c_void_p(ws.data_ptr()), ws.numel(),
+                                 C.c_void_p(s.cuda_stream))
+        _check(st, "exx_apply")
+        return vx, ex_k, ex
+
+    def apply_host(self, psi, occ, tgt=None, tgt_start: int = -1, n_tgt: int | None = None, occ_tgt=None,
+                   vx=None, n_c: int = 0):
+        """exx_apply_host: HOST buffers in, HOST results out (H2D/D2H inside the call, synchronous).
+        Returns (vx, e_k, E_x) as numpy arrays / float."""
+        n_occ = psi.shape[0]
+        if tgt is None:
+            if tgt_start < 0 or n_tgt is None:
+                raise ValueError("give tgt, or tgt_start and n_tgt")
+        else:
+            n_tgt, tgt_start = tgt.shape[0], -1
+        if vx is None:
+            vx = np.empty((n_tgt, self.nz, self.ny, self.nx))
+        ex = np.zeros(1)
+        ex_k = np.empty(n_tgt)
+        st = self._lib.exx_apply_host(self._h, _host_ptr(psi, "psi"), _host_ptr(occ, "occ"), n_occ,
+                                      _host_ptr(tgt, "tgt"), tgt_start, _host_ptr(occ_tgt, "occ_tgt"), n_tgt,
+                                      _host_ptr(vx, "vx"), _host_ptr(ex, "ex") if occ_tgt is not None else None,
+                                      _host_ptr(ex_k, "ex_k"), n_c)
+        _check(st, "exx_apply_host")
+        return vx, ex_k, (float(ex[0]) if occ_tgt is not None else None)

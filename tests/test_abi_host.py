@@ -1,0 +1,91 @@
+"""C-ABI host-side checks (CPU only): the library loads, exports every symbol include/exx.h declares,
+validates arguments, and its own planner (FD matrices + Jacobi + multiplier table, no code shared with
+the oracle) agrees with the oracle's numpy/LAPACK planner.  No compute call is made."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import __graft_entry__ as ge
+from oracle import exx_oracle as orc
+from paper_2501_16572_b200 import exx
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    ge.build()
+    return exx.load_library()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    header = open(os.path.join(ROOT, "include", "exx.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    names = set(re.findall(r"\b(exx_[a-z_]+)\s*\(", header))
+    assert {"exx_plan_create", "exx_plan_destroy", "exx_apply", "exx_poisson_solve", "exx_apply_host",
+            "exx_plan_workspace_bytes", "exx_status_string"} <= names
+    for n in names:
+        assert hasattr(lib, n), n
+    assert b"sm_100a" in lib.exx_version()
+
+
+def test_argument_validation_without_gpu(lib):
+    h = C.c_void_p()
+    bc = (C.c_int * 3)(0, 0, 0)
+    bad = [
+        dict(nx=0), dict(h=0.0), dict(h=-1.0), dict(order=3), dict(order=0), dict(max_batch=0),
+    ]
+    for kw in bad:
+        a = dict(nx=8, ny=8, nz=8, h=0.5, order=12, omega=0.0, max_batch=4)
+        a.update(kw)
+        st = lib.exx_plan_create(C.byref(h), a["nx"], a["ny"], a["nz"], a["h"], bc, a["order"], a["omega"],
+                                 a["max_batch"], -1)
+        assert st == 1, kw
+        assert not h.value
+    bc_bad = (C.c_int * 3)(0, 2, 0)
+    assert lib.exx_plan_create(C.byref(h), 8, 8, 8, 0.5, bc_bad, 12, 0.0, 4, -1) == 1
+    assert lib.exx_plan_create(None, 8, 8, 8, 0.5, bc, 12, 0.0, 4, -1) == 1
+    for s in range(7):
+        assert lib.exx_status_string(s).startswith(b"EXX_")
+
+
+def test_host_only_plan_refuses_compute_loudly(lib):
+    p = exx.Plan(8, 6, 5, 0.5, (0, 0, 1), 12, 0.106, max_batch=4, device=-1)
+    assert p.workspace_bytes(4) == 2 * 8 * 240 * 4
+    assert p.workspace_bytes(5) == 0          # > max_batch
+    assert p.workspace_bytes(0) == 2 * 8 * 240 * 4  # default clamps to max_batch
+    dummy = C.c_void_p(1 << 20)
+    st = lib.exx_poisson_solve(p._h, dummy, dummy, 1, 1, dummy, 1 << 30, None)
+    assert st == 3 and b"EXX_ERR_CUDA" in lib.exx_status_string(st)   # no CPU fallback
+    st = lib.exx_apply(p._h, dummy, dummy, 1, dummy, None, 1, C.c_void_p(1 << 28), None, None, 1, C.c_void_p(1 << 29),
+                       1 << 20, None)
+    assert st == 3
+    with pytest.raises(exx.ExxError):
+        p.set_variant(7)
+    p.close()
+
+
+@pytest.mark.parametrize("dims,bc,omega,h", [((16, 16, 16), (0, 0, 0), 0.0, 0.5), ((12, 10, 30), (0, 0, 1), 0.106, 0.25),
+                                             ((48, 48, 48), (0, 0, 0), 0.106, 0.25), ((7, 9, 5), (1, 0, 1), 0.106, 0.3),
+                                             ((120, 60, 1), (1, 0, 0), 0.106, 0.2)])
+def test_library_planner_agrees_with_oracle_planner(lib, dims, bc, omega, h):
+    nx, ny, nz = dims
+    p = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=4, device=-1)
+    o = orc.make_plan(nx, ny, nz, h, bc, 12, omega)
+    scale = abs(orc.fd_weights(12, h)[0])
+    for ax, n in enumerate(dims):
+        lam, V = p.get_axis(ax)
+        assert np.allclose(lam, o.lam[ax], rtol=0, atol=2e-13 * scale)
+        assert np.allclose(V.T @ V, np.eye(n), atol=1e-13)
+        K = orc.second_derivative_matrix(n, h, bc[ax], 12)
+        assert np.allclose(K @ V, V * lam[None, :], rtol=0, atol=5e-13 * scale)
+    # eigenvalue sums are basis independent => tables must agree entry by entry (incl. the zero-mode rule)
+    m = p.get_multiplier()
+    assert m.shape == o.mult.shape
+    assert np.allclose(m, o.mult, rtol=1e-10, atol=0)
+    if all(b == 0 for b in bc):
+        assert m[-1, -1, -1] == (0.0 if omega <= 0 else pytest.approx(np.pi / omega ** 2, rel=1e-14))
+    p.close()
