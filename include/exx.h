@@ -125,6 +125,14 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);
 
+/*
+ * Diagnostic: sustained FP64 throughput of this GPU in TFLOP/s over about `seconds` (0 < seconds <= 30) of
+ * back-to-back launches of a register-resident issue loop.  kind 0 = DFMA (FP64 FMA pipe), kind 1 = DMMA
+ * (mma.sync m8n8k4 f64).  Synchronises the device.  Used by bench.py for the roofline denominator
+ * (MEASURED_PEAKS.json has no FP64 figure).
+ */
+exx_status exx_probe_fp64_peak(int kind, int device, double seconds, double* h_tflops);
+
 /* Human-readable status; for EXX_ERR_CUDA includes the last cudaError_t seen by this thread. */
 const char* exx_status_string(exx_status status);
 

@@ -66,6 +66,8 @@ def load_library():
     lib.exx_plan_last_launch_count.argtypes = [vp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
+    lib.exx_probe_fp64_peak.restype = C.c_int
+    lib.exx_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double)]
     lib.exx_version.restype = C.c_char_p
     lib.exx_version.argtypes = []
     _lib = lib
@@ -97,6 +99,13 @@ def _host_ptr(t, what: str):
     if t.dtype != torch.float64 or not t.is_contiguous() or t.device.type != "cpu":
         raise ValueError(f"{what}: need a contiguous float64 host tensor")
     return C.c_void_p(t.data_ptr())
+
+
+def probe_fp64_peak(kind: int, device: int = 0, seconds: float = 1.0) -> float:
+    """exx_probe_fp64_peak: sustained TFLOP/s of a DFMA (kind 0) or DMMA (kind 1) issue loop."""
+    out = C.c_double(0.0)
+    _check(load_library().exx_probe_fp64_peak(kind, device, seconds, C.byref(out)), "exx_probe_fp64_peak")
+    return out.value
 
 
 class Plan:

@@ -1,0 +1,204 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerance 1e-10 relative in the max norm on vx and on E_x
+(BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import exx_oracle as orc
+from paper_2501_16572_b200 import exx, workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+VARIANTS = [pytest.param(exx.VARIANT_FUSED_DMMA, id="fused_dmma"), pytest.param(exx.VARIANT_REFERENCE, id="reference")]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    import __graft_entry__ as ge
+    ge.build()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device; there is no CPU fallback"
+
+
+def _rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _oracle_plan(w):
+    return orc.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega)
+
+
+SOLVE_CASES = [
+    # (nx, ny, nz, h, bc, omega, n_rhs, n_c): ragged sizes (not multiples of 4/8), all BC mixes, tails
+    (16, 16, 16, 0.5, (0, 0, 0), 0.0, 5, 2),
+    (16, 16, 16, 0.5, (0, 0, 0), 0.106, 8, 8),
+    (20, 12, 9, 0.3, (0, 1, 0), 0.106, 7, 3),
+    (13, 17, 11, 0.4, (1, 1, 1), 0.0, 4, 4),
+    (48, 48, 48, 0.25, (0, 0, 0), 0.106, 6, 4),
+    (60, 60, 120, 0.25, (0, 0, 1), 0.106, 3, 2),
+    (33, 8, 70, 0.25, (0, 0, 1), 0.0, 3, 1),
+    (1, 1, 40, 0.25, (0, 0, 1), 0.106, 2, 2),
+    (96, 96, 96, 0.2, (0, 0, 0), 0.106, 2, 2),
+    (120, 120, 120, 0.2, (0, 0, 0), 0.106, 1, 1),
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("case", SOLVE_CASES, ids=lambda c: f"{c[0]}x{c[1]}x{c[2]}_nrhs{c[6]}_nc{c[7]}")
+def test_poisson_solve_matches_oracle(case, variant):
+    nx, ny, nz, h, bc, omega, n_rhs, n_c = case
+    plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=8, device=0)
+    plan.set_variant(variant)
+    rng = np.random.default_rng(99)
+    C = rng.standard_normal((n_rhs, nz, ny, nx))
+    ref = orc.poisson_solve(orc.make_plan(nx, ny, nz, h, bc, 12, omega), C)
+    d = torch.from_numpy(C).cuda()
+    keep = d.clone()
+    out = plan.poisson_solve(d, n_c=n_c)
+    torch.cuda.synchronize()
+    assert torch.equal(d, keep)                                  # input untouched
+    assert _rel(out.cpu().numpy(), ref) < TOL
+    out2 = plan.poisson_solve(d, out=d, n_c=n_c)                 # in place
+    torch.cuda.synchronize()
+    assert torch.equal(out2, out)
+    plan.close()
+
+
+APPLY_CASES = [
+    # (cfg, n_orb, n_tgt, tgt_start, n_c)
+    (1, 8, 8, 0, 0),        # BASELINE config 1, full: 64 pair solves
+    (1, 8, 8, 0, 3),        # ragged batches
+    (1, 8, 3, 5, 64),       # several targets per batch
+    (2, 12, 12, 0, 5),
+    (3, 10, 4, 3, 4),
+    (4, 6, 2, 4, 4),
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("case", APPLY_CASES, ids=lambda c: f"cfg{c[0]}_o{c[1]}_t{c[2]}_nc{c[4]}")
+def test_apply_matches_oracle(case, variant):
+    cfg, n_orb, n_tgt, t0, n_c = case
+    w = wl.scaled(wl.WORKLOADS[cfg], n_orb, n_tgt, t0)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    if w.fermi:   # exercise fractional, tiny and exactly-zero occupations on the small case
+        occ = occ.clone()
+        occ[:] = torch.tensor(np.linspace(2.0, 0.05, n_orb))
+        occ[-1] = 1e-13
+        occ[1] = 0.0
+        occ_t = occ[t0:t0 + n_tgt]
+    plan = exx.Plan.for_workload(w, max_batch=64, device=0)
+    plan.set_variant(variant)
+    dpsi = psi.cuda()
+    vx, e_k, ex = plan.apply(dpsi, occ.cuda(), dpsi[t0:t0 + n_tgt], occ_t.cuda(), n_c=n_c)
+    torch.cuda.synchronize()
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy())
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL
+    assert np.abs(e_k.cpu().numpy() - e_o).max() / np.abs(e_o).max() < TOL
+    assert abs(ex.item() - ex_o) / abs(ex_o) < TOL
+    assert plan.last_launch_count > 0
+    plan.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config2_full_size(variant):
+    # BASELINE config 2 as bench.py runs it (64 orbitals, 4,096 pair solves, default n_c)
+    w = wl.WORKLOADS[2]
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    plan = exx.Plan.for_workload(w, device=0)
+    plan.set_variant(variant)
+    dpsi = psi.cuda()
+    vx, e_k, ex = plan.apply(dpsi, occ.cuda(), dpsi, occ_t.cuda())
+    torch.cuda.synchronize()
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy())
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL
+    assert abs(ex.item() - ex_o) / abs(ex_o) < TOL
+    # properties that hold at any size: Hermiticity and negativity of M = Psi^T Vx Psi
+    M = (dpsi.view(64, -1) @ vx.view(64, -1).T).cpu().numpy()
+    assert np.abs(M - M.T).max() < 1e-10 * np.abs(M).max()
+    assert np.linalg.eigvalsh(0.5 * (M + M.T)).max() < 1e-9 * np.abs(M).max()
+    plan.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_batch_size_invariance_and_determinism(variant):
+    # same linear map for every n_c; only the j-summation grouping changes (rounding)
+    w = wl.scaled(wl.WORKLOADS[2], 9, 4, 2)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cuda")
+    plan = exx.Plan.for_workload(w, max_batch=64, device=0)
+    plan.set_variant(variant)
+    base, _, ex0 = plan.apply(psi, occ, tgt, occ_t, n_c=1)
+    base = base.clone()
+    for n_c in (2, 4, 9, 18, 64):
+        v, _, ex = plan.apply(psi, occ, tgt, occ_t, n_c=n_c)
+        assert float((v - base).abs().max() / base.abs().max()) < 1e-12
+        assert abs(ex.item() - ex0.item()) < 1e-12 * abs(ex0.item())
+    a, _, _ = plan.apply(psi, occ, tgt, occ_t, n_c=4)
+    a = a.clone()
+    b, _, _ = plan.apply(psi, occ, tgt, occ_t, n_c=4)
+    assert torch.equal(a, b)                                  # bitwise reproducible run to run
+    plan.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_edge_cases_and_errors(variant):
+    w = wl.scaled(wl.WORKLOADS[1], 4, 2, 0)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cuda")
+    plan = exx.Plan.for_workload(w, max_batch=8, device=0)
+    plan.set_variant(variant)
+    # no occupied orbitals: vx = 0, E_x = 0
+    vx, e_k, ex = plan.apply(psi[:0], occ[:0], tgt, occ_t)
+    torch.cuda.synchronize()
+    assert float(vx.abs().max()) == 0.0 and ex.item() == 0.0 and float(e_k.abs().max()) == 0.0
+    # no targets
+    vx, e_k, ex = plan.apply(psi, occ, tgt[:0], occ_t[:0])
+    torch.cuda.synchronize()
+    assert vx.shape[0] == 0 and ex.item() == 0.0
+    # all occupations zero
+    vx, _, ex = plan.apply(psi, torch.zeros_like(occ), tgt, occ_t)
+    torch.cuda.synchronize()
+    assert float(vx.abs().max()) == 0.0
+    # errors: n_c beyond max_batch, aliasing vx with psi, short workspace
+    with pytest.raises((exx.ExxError, ValueError)):
+        plan.apply(psi, occ, tgt, occ_t, n_c=9)
+    with pytest.raises(exx.ExxError) as ei:
+        plan.apply(psi, occ, tgt, occ_t, vx=psi[:2])
+    assert ei.value.status == 6
+    import ctypes as C
+    lib = exx.load_library()
+    vx = torch.empty_like(tgt)
+    st = lib.exx_apply(plan._h, psi.data_ptr(), occ.data_ptr(), 4, tgt.data_ptr(), None, 2, vx.data_ptr(), None, None,
+                       4, C.c_void_p(plan._workspace(8).data_ptr()), 16, None)
+    assert st == 5
+    plan.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_apply_host_end_to_end(variant):
+    w = wl.scaled(wl.WORKLOADS[2], 6, 3, 2)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    plan = exx.Plan.for_workload(w, max_batch=16, device=0)
+    plan.set_variant(variant)
+    vx_h, e_h, ex_h = plan.apply_host(psi.numpy(), occ.numpy(), tgt_start=2, n_tgt=3, occ_tgt=occ_t.numpy(), n_c=4)
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy())
+    assert _rel(vx_h, vx_o) < TOL and abs(ex_h - ex_o) < TOL * abs(ex_o)
+    # separate target block
+    vx_h2, _, _ = plan.apply_host(psi.numpy(), occ.numpy(), tgt=np.ascontiguousarray(tgt.numpy()), occ_tgt=occ_t.numpy())
+    assert _rel(vx_h2, vx_o) < TOL
+    plan.close()
+
+
+def test_fast_variant_agrees_with_reference_variant_bitwise_close():
+    w = wl.scaled(wl.WORKLOADS[3], 8, 3, 1)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cuda")
+    plan = exx.Plan.for_workload(w, max_batch=16, device=0)
+    out = {}
+    for v in (exx.VARIANT_REFERENCE, exx.VARIANT_FUSED_DMMA):
+        plan.set_variant(v)
+        vx, _, ex = plan.apply(psi, occ, tgt, occ_t, n_c=8)
+        out[v] = (vx.clone(), ex.item())
+    a, b = out[exx.VARIANT_REFERENCE], out[exx.VARIANT_FUSED_DMMA]
+    assert float((a[0] - b[0]).abs().max() / a[0].abs().max()) < 1e-12
+    assert abs(a[1] - b[1]) < 1e-12 * abs(a[1])
+    plan.close()
