@@ -152,13 +152,15 @@ def poisson_solve(plan: OraclePlan, C: np.ndarray) -> np.ndarray:
     if squeeze:
         C = C[None]
     Vx, Vy, Vz = plan.V
-    T = np.einsum("bzyx,xa->bzya", C, Vx)
-    T = np.einsum("bzya,yB->bzBa", T, Vy)
-    T = np.einsum("bzBa,zc->bcBa", T, Vz)
-    T = T * plan.mult[None]
-    Y = np.einsum("bcBa,zc->bzBa", T, Vz)
-    Y = np.einsum("bzBa,yB->bzya", Y, Vy)
-    Y = np.einsum("bzya,xa->bzyx", Y, Vx)
+    nb, nz, ny, nx = C.shape
+    # each mode product is one (broadcast) matmul -- a library primitive as a step, in Eq. 11's order
+    T = np.matmul(C, Vx)                                          # T[b,z,y,a] = sum_x C[b,z,y,x] Vx[x,a]
+    T = np.matmul(Vy.T, T)                                        # T[b,z,B,a] = sum_y Vy[y,B] T[b,z,y,a]
+    T = np.matmul(Vz.T, T.reshape(nb, nz, ny * nx))               # T[b,c,(B,a)] = sum_z Vz[z,c] T[b,z,(B,a)]
+    T = T * plan.mult.reshape(1, nz, ny * nx)                     # Hadamard with f(Lambda~), Eq. 16
+    Y = np.matmul(Vz, T).reshape(nb, nz, ny, nx)                  # expand back: z, then y, then x
+    Y = np.matmul(Vy, Y)
+    Y = np.matmul(Y, Vx.T)
     return Y[0] if squeeze else Y
 
 
