@@ -126,6 +126,17 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
 long long exx_plan_last_launch_count(const exx_plan* plan);
 
 /*
+ * Per-kernel-class timing (bench instrumentation).  With profiling on, every kernel the library launches
+ * is bracketed by a CUDA-event pair on the caller's stream (this perturbs the stream slightly: do not
+ * report whole-call times taken with it on).  exx_plan_get_profile synchronises the recorded events, adds
+ * the durations per class into h_ms[4] / h_count[4] and clears the records.  Classes: 0 = mode products
+ * (a2-a4, with fused a1/a3/a5 where the variant fuses them), 1 = pair density (a1), 2 = accumulate (a5),
+ * 3 = energy and housekeeping (a6).
+ */
+exx_status exx_plan_set_profiling(exx_plan* plan, int on);
+exx_status exx_plan_get_profile(exx_plan* plan, double* h_ms, long long* h_count);
+
+/*
  * Diagnostic: sustained FP64 throughput of this GPU in TFLOP/s over about `seconds` (0 < seconds <= 30) of
  * back-to-back launches of a register-resident issue loop.  kind 0 = DFMA (FP64 FMA pipe), kind 1 = DMMA
  * (mma.sync m8n8k4 f64).  Synchronises the device.  Used by bench.py for the roofline denominator

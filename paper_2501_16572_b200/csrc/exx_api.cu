@@ -99,6 +99,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->variant = EXX_VARIANT_FUSED_DMMA;
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0;
+  p->prof_on = false;
   for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; }
 
   try {
@@ -206,6 +207,29 @@ exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult) {
 
 long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }
 
+exx_status exx_plan_set_profiling(exx_plan* plan, int on) {
+  if (!plan) return EXX_ERR_INVALID_ARG;
+  plan->prof_on = on != 0;
+  return EXX_OK;
+}
+
+exx_status exx_plan_get_profile(exx_plan* plan, double* h_ms, long long* h_count) {
+  if (!plan || !h_ms || !h_count) return EXX_ERR_INVALID_ARG;
+  for (int c = 0; c < exx::KC_COUNT; ++c) { h_ms[c] = 0.0; h_count[c] = 0; }
+  cudaError_t err = cudaSuccess;
+  for (auto& r : plan->prof) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(r.e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.e0, r.e1);
+    if (e != cudaSuccess) err = e;
+    else { h_ms[r.cls] += ms; h_count[r.cls] += 1; }
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
+  }
+  plan->prof.clear();
+  return err == cudaSuccess ? EXX_OK : cuda_fail(err);
+}
+
 }  // extern "C"
 
 namespace {
@@ -214,12 +238,16 @@ namespace {
 cudaError_t ref_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, cudaStream_t s,
                             long long* launches) {
   cudaError_t e;
-  if ((e = exx::ref_mode_product(p, 0, true, buf0, buf1, nb, false, s)) != cudaSuccess) return e;
-  if ((e = exx::ref_mode_product(p, 1, true, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
-  if ((e = exx::ref_mode_product(p, 2, true, buf0, buf1, nb, true, s)) != cudaSuccess) return e;
-  if ((e = exx::ref_mode_product(p, 2, false, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
-  if ((e = exx::ref_mode_product(p, 1, false, buf0, buf1, nb, false, s)) != cudaSuccess) return e;
-  if ((e = exx::ref_mode_product(p, 0, false, buf1, buf0, nb, false, s)) != cudaSuccess) return e;
+  const int axis[6] = {0, 1, 2, 2, 1, 0};
+  double *src = buf0, *dst = buf1;
+  for (int i = 0; i < 6; ++i) {
+    {
+      exx::ProfScope ps(p, exx::KC_MODE_PRODUCT, s);
+      e = exx::ref_mode_product(p, axis[i], i < 3, src, dst, nb, i == 2, s);
+    }
+    if (e != cudaSuccess) return e;
+    double* t = src; src = dst; dst = t;
+  }
   *launches += 6;
   return cudaSuccess;
 }
@@ -297,9 +325,15 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
         const exx::BatchDesc bd{j0, nj, k0, nk};
         const int nb = nj * nk;
         if (plan->variant == EXX_VARIANT_REFERENCE) {
-          EXX_CUDA(exx::ref_pair_density(plan, d_psi, d_tgt, bd, buf0, s));
+          {
+            exx::ProfScope ps(plan, exx::KC_PAIR_DENSITY, s);
+            EXX_CUDA(exx::ref_pair_density(plan, d_psi, d_tgt, bd, buf0, s));
+          }
           EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
-          EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, j0 == 0, d_vx, s));
+          {
+            exx::ProfScope ps(plan, exx::KC_ACCUMULATE, s);
+            EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, j0 == 0, d_vx, s));
+          }
           launches += 2;
         } else {
           const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, j0 == 0};
@@ -317,9 +351,12 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
       const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
       if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
-      EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0,
-                           d_occ_tgt ? d_occ_tgt + k0 : nullptr, nk, ex->d_energy_scratch,
-                           d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
+      {
+        exx::ProfScope ps(plan, exx::KC_OTHER, s);
+        EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0,
+                             d_occ_tgt ? d_occ_tgt + k0 : nullptr, nk, ex->d_energy_scratch,
+                             d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
+      }
       launches += 2;
     }
   }

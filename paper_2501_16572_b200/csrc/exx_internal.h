@@ -22,6 +22,14 @@ std::vector<double> multiplier_table(const std::vector<double>& lx, const std::v
 
 }  // namespace exx
 
+namespace exx {
+enum KernelClass { KC_MODE_PRODUCT = 0, KC_PAIR_DENSITY = 1, KC_ACCUMULATE = 2, KC_OTHER = 3, KC_COUNT = 4 };
+struct ProfRec {
+  cudaEvent_t e0, e1;
+  int cls;
+};
+}  // namespace exx
+
 struct exx_plan {
   int n[3];  // nx, ny, nz
   double h;
@@ -41,6 +49,9 @@ struct exx_plan {
   int sm_count;
   int smem_optin;
   long long last_launches;
+  // optional per-kernel-class CUDA-event timing (exx_plan_set_profiling)
+  bool prof_on;
+  std::vector<exx::ProfRec> prof;
 };
 
 namespace exx {
@@ -61,6 +72,24 @@ cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* o
 cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
                    int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s);
 cudaError_t zero_fill(double* p, long long n, cudaStream_t s);
+
+// RAII event pair around one launch when profiling is on (no-op otherwise).
+struct ProfScope {
+  exx_plan* p;
+  cudaStream_t s;
+  cudaEvent_t e1;
+  ProfScope(exx_plan* plan, int cls, cudaStream_t stream) : p(plan), s(stream), e1(nullptr) {
+    if (!p->prof_on) return;
+    cudaEvent_t e0;
+    if (cudaEventCreate(&e0) != cudaSuccess) return;
+    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); e1 = nullptr; return; }
+    cudaEventRecord(e0, s);
+    p->prof.push_back(ProfRec{e0, e1, cls});
+  }
+  ~ProfScope() {
+    if (e1) cudaEventRecord(e1, s);
+  }
+};
 
 // ---- fast variant (kernels_dmma.cu) ----------------------------------------------------------
 // Returns cudaErrorNotSupported if the plan's sizes are outside what the fast kernels handle

@@ -335,6 +335,7 @@ void fast_destroy(exx_plan*) {}
 // (still CUDA, still in the library; stated in DESIGN.md).  buf1 is only needed in that case.
 static cudaError_t one_product(exx_plan* p, int axis, bool fwd, double*& cur, double*& other, int nb,
                                bool mult, cudaStream_t s) {
+  ProfScope ps(p, KC_MODE_PRODUCT, s);
   cudaError_t e = fast_mode_product(p, axis, fwd, cur, cur, nb, mult, s);
   if (e == cudaErrorNotSupported) {
     e = ref_mode_product(p, axis, fwd, cur, other, nb, mult, s);
@@ -350,7 +351,11 @@ cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, co
   cudaError_t e;
   double *cur = buf0, *other = buf1;
   if (fa) {
-    if ((e = ref_pair_density(p, fa->psi, fa->tgt, fa->bd, cur, s)) != cudaSuccess) return e;
+    {
+      ProfScope ps(p, KC_PAIR_DENSITY, s);
+      e = ref_pair_density(p, fa->psi, fa->tgt, fa->bd, cur, s);
+    }
+    if (e != cudaSuccess) return e;
     ++*launches;
   }
   if ((e = one_product(p, 0, true, cur, other, nb, false, s)) != cudaSuccess) return e;
@@ -361,7 +366,11 @@ cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, co
   if ((e = one_product(p, 0, false, cur, other, nb, false, s)) != cudaSuccess) return e;
   *launches += 6;
   if (fa) {
-    if ((e = ref_accumulate(p, fa->psi, fa->occ, cur, fa->bd, fa->first, fa->vx, s)) != cudaSuccess) return e;
+    {
+      ProfScope ps(p, KC_ACCUMULATE, s);
+      e = ref_accumulate(p, fa->psi, fa->occ, cur, fa->bd, fa->first, fa->vx, s);
+    }
+    if (e != cudaSuccess) return e;
     ++*launches;
   } else if (cur != buf0) {
     e = cudaMemcpyAsync(buf0, cur, sizeof(double) * (size_t)p->N * nb, cudaMemcpyDeviceToDevice, s);

@@ -66,6 +66,10 @@ def load_library():
     lib.exx_plan_last_launch_count.argtypes = [vp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
+    lib.exx_plan_set_profiling.restype = C.c_int
+    lib.exx_plan_set_profiling.argtypes = [vp, C.c_int]
+    lib.exx_plan_get_profile.restype = C.c_int
+    lib.exx_plan_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     lib.exx_probe_fp64_peak.restype = C.c_int
     lib.exx_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double)]
     lib.exx_version.restype = C.c_char_p
@@ -160,6 +164,18 @@ class Plan:
         m = np.empty((self.nz, self.ny, self.nx))
         _check(self._lib.exx_plan_get_multiplier(self._h, C.c_void_p(m.ctypes.data)), "exx_plan_get_multiplier")
         return m
+
+    def set_profiling(self, on: bool):
+        _check(self._lib.exx_plan_set_profiling(self._h, 1 if on else 0), "exx_plan_set_profiling")
+
+    def get_profile(self):
+        """exx_plan_get_profile: {class: (ms, launches)} for classes mode_product / pair_density /
+        accumulate / other, accumulated since the last call (synchronises)."""
+        ms = (C.c_double * 4)()
+        cnt = (C.c_longlong * 4)()
+        _check(self._lib.exx_plan_get_profile(self._h, ms, cnt), "exx_plan_get_profile")
+        names = ("mode_product", "pair_density", "accumulate", "other")
+        return {n: (ms[i], int(cnt[i])) for i, n in enumerate(names)}
 
     @property
     def last_launch_count(self) -> int:
