@@ -1,21 +1,31 @@
 // Fast variant (EXX_VARIANT_FUSED_DMMA): mode products on the FP64 tensor pipe.
 //
-// Every mode product of Eq. 11 is a "small stationary matrix times a very wide
-// matrix": out[:, c] = M in[:, c] with M = V^T (forward) or V (backward), n x n, n <= 128, and c running
-// over N*n_c/n columns.  One persistent CTA per SM keeps V resident in shared memory for the whole
-// launch and streams column tiles through a 2-stage cp.async pipeline; warps issue
-// mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4, measured 37.1 TFLOP/s on B200 = 128 flop/clk/SM) with
-// MT x NT register blocking so that shared-memory operand traffic stays below 40 % of the LSU pipe.
+// Every mode product of Eq. 11 is "a small stationary matrix times a very wide one":
+// out[:, c] = M in[:, c], M = V^T (forward) or V (backward), n x n with n <= 128, c running over
+// N*n_c/n columns.  Design (measured facts in profiles/r1_dmma_issue_vs_occupancy.txt):
+//   * mma.sync.m8n8k4.f64 lowers to DMMA.8x8x4; one warp per SM sub-partition with >= 2 independent
+//     accumulators already saturates the pipe (37.1 TFLOP/s = 128 flop/clk/SM), every DMMA blocks its
+//     warp for 16 issue cycles.  So the kernel is built from fully independent warps, 2 per
+//     sub-partition, and everything that is not a DMMA must fit in the shadow of the other warp's DMMAs.
+//   * V (<= 132 KB padded) is staged once per CTA in shared memory with a row stride == 4 (mod 8)
+//     doubles, which makes both the V and the V^T fragment reads bank-conflict free.
+//   * The data operand is never shared between warps: each element is used by exactly one warp (a warp
+//     owns 8*NT columns for ALL n output rows), so every lane fetches exactly its own B-fragment elements
+//     with 8-byte cp.async copies into a private D-deep ring of shared-memory slots (full 32 B sectors:
+//     8 consecutive columns x 4 rows in L-mode, 4 consecutive x x 8 rows in X-mode).  cp.async groups,
+//     not the register scoreboard, track completion; no block or warp barrier exists in the steady state.
+//   * Accumulators (ceil(n/8) x NT tiles) live in registers; results are stored straight from the
+//     fragments, so every pass runs in place.
+// Fused into the passes: the pair density psi_j*tgt_k in the load path of the first product (a1), the
+// multiplier f(Lambda~) in the store path of the last forward product (a3).
 //
-// Two global<->tile mappings share the MMA core:
-//   L-mode (axis y or z, contracted index strided by `inner`): tile = [k][w columns], columns are the
-//           flattened (outer, inner) index, so there is no ragged waste except at the very end;
-//   X-mode (axis x, contracted index contiguous): tile = [w rows][k], the transposed product
-//           out^T = M in^T is computed, so the data rows are the MMA's N dimension.
-// Results are stored straight from the accumulator fragments; all passes are in place.
+// Two global<->fragment mappings share the MMA core:
+//   L-mode (axis y or z; contracted index strided by `inner`): columns = flattened (outer, inner) index;
+//   X-mode (axis x; contracted index contiguous): the transposed product out^T = M in^T, columns = rows
+//           of nx contiguous points, tiled per right-hand side.
 //
 // The paper's four data reorganisations (Eqs. 12-15) do not exist here: they are
-// artefacts of calling a 2-D GEMM library and are replaced by the strided tile addressing above.
+// artefacts of calling a 2-D GEMM library and are replaced by the strided fragment addressing above.
 #include <cstdint>
 
 #include "exx_internal.h"
@@ -23,194 +33,226 @@
 namespace exx {
 namespace {
 
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-               : "+d"(c[0]), "+d"(c[1])
-               : "d"(a), "d"(b));
-}
+constexpr int kWarps = 8;
+constexpr int kThreads = 32 * kWarps;
+constexpr int kRing = 8;  // depth of the per-lane B-fragment ring (cp.async stages), in k-steps
 
-template <int BYTES>
-__device__ __forceinline__ void cp_async(void* smem, const void* gmem) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;\n" ::"r"(s), "l"(gmem), "n"(BYTES));
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+      : "+d"(c[0]), "+d"(c[1])
+      : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+__device__ __forceinline__ double lds64(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
+  return v;
+}
+// 8-byte asynchronous global->shared copy; src_bytes = 0 writes zeros (used for k >= n and ragged tails).
+// Completion is tracked by cp.async groups, not by the register scoreboard, so a D-deep ring really is
+// D steps of latency tolerance (plain LDG prefetches shared scoreboard slots with the DMMAs and stalled).
+__device__ __forceinline__ void cp_async8(unsigned smem_addr, const double* gmem, bool valid) {
+  const int src_bytes = valid ? 8 : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_addr), "l"(gmem), "r"(src_bytes)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
-struct ModeArgs {
+struct WArgs {
   const double* in;
   double* out;
-  const double* V;      // row-major [i][m], n x n
-  const double* mult;   // optional (L-mode only): multiplier table indexed [m*inner + i]
-  int n;                // contracted extent
-  int KT;               // ceil(n/4)
-  int ldv;              // smem row stride of V (== 4 mod 8)
-  int ldt;              // smem row stride of a data tile (== 4 mod 8)
-  int fwd;              // 1: M = V^T, 0: M = V
-  int inner;            // L-mode: length of the contiguous run below the contracted axis
-  long long total;      // L-mode: number of columns (outer*inner); X-mode: number of rows
-  int n_tiles;
+  const double* V;     // row-major [i][m], n x n
+  const double* mult;  // optional (L-mode): table indexed [m*inner + i]
+  const double* psi;   // PD only
+  const double* tgt;   // PD only
+  int n;
+  int KT;                // ceil(n/4)
+  int inner;             // L-mode: contiguous run below the contracted axis
+  long long total;       // L-mode: number of columns (outer*inner)
+  int rows_per_rhs;      // X-mode: N / nx
+  int tiles_per_rhs;     // X-mode: ceil(rows_per_rhs / (8*NT))
+  long long n_tiles;     // warp tiles in this launch
+  long long N;           // points per right-hand side
+  BatchDesc bd;          // PD only
+  int vec2;              // L-mode: 16-byte stores are aligned
 };
 
-// smem layout (doubles): [ V: R8 x ldv ][ stage0 ][ stage1 ],  R8 = roundup(n, 8)
-template <int MT, int WR, int NT, int WC, bool XMODE, int VEC>
-__global__ void __launch_bounds__(32 * WR * WC, 1) k_mode_dmma(const ModeArgs a) {
-  constexpr int kThreads = 32 * WR * WC;
-  constexpr int kW = 8 * NT * WC;
-  extern __shared__ __align__(16) double smem[];
+// MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
+template <int MTOT, int NT, bool XMODE, bool FWD, bool PD>
+__global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
+  static_assert(!PD || (XMODE && FWD), "pair density is fused into the first (x, forward) product only");
+  constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): conflict-free for both fragment orientations
+  extern __shared__ __align__(16) double Vs[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g = lane >> 2, q = lane & 3;
-  const int wr = warp % WR, wc = warp / WR;
-  const int n = a.n, KT = a.KT, ldv = a.ldv, ldt = a.ldt;
-  const int R8 = (n + 7) & ~7;
-  double* Vs = smem;
-  const int stage_elems = XMODE ? kW * ldt : 4 * KT * ldt;
-  double* stage0 = Vs + R8 * ldv;
+  const int n = a.n, KT = a.KT;
 
-  // ---- one-time: zero everything (k-padding must be exact zeros), then stage V --------------------
-  {
-    const int tot = R8 * ldv + 2 * stage_elems;
-    for (int i = tid; i < tot; i += kThreads) smem[i] = 0.0;
-    __syncthreads();
-    for (int i = tid; i < n * n; i += kThreads) {
-      const int r = i / n, c = i - r * n;
-      Vs[r * ldv + c] = a.V[i];
-    }
+  // ---- stage V once per CTA: zero padding (k >= n must contribute exact zeros), then the n x n block ----
+  for (int i = tid; i < 8 * MTOT * LDV; i += kThreads) Vs[i] = 0.0;
+  __syncthreads();
+  for (int i = tid; i < n * n; i += kThreads) {
+    const int r = i / n, c = i - r * n;
+    Vs[r * LDV + c] = a.V[i];
   }
+  __syncthreads();
 
-  // A operand (M): element (m,k) at Vs[m*a_sm + k*a_sk]
-  const int a_sm = a.fwd ? 1 : ldv, a_sk = a.fwd ? ldv : 1;
-  // B operand (data): element (k, col) at tile[k*b_sk + col*b_sn]
-  const int b_sk = XMODE ? 1 : ldt, b_sn = XMODE ? ldt : 1;
-  const int m_base = 8 * MT * wr, n_base = 8 * NT * wc;
-  int mt_valid = 0;
-#pragma unroll
-  for (int mt = 0; mt < MT; ++mt) mt_valid += (m_base + 8 * mt < n) ? 1 : 0;
-  const double* ap = Vs + (m_base + g) * a_sm + q * a_sk;
+  // A fragment (M[m][k]) shared address for (mt, kt): base + mt*A_MT + kt*A_KT   (bytes)
+  //   FWD: M[m][k] = V[k][m] -> Vs[(4kt+q)*LDV + 8mt+g];   BWD: M[m][k] = V[m][k] -> Vs[(8mt+g)*LDV + 4kt+q]
+  constexpr unsigned A_MT = FWD ? 64u : 64u * LDV;
+  constexpr unsigned A_KT = FWD ? 32u * LDV : 32u;
+  const unsigned a_base = (unsigned)__cvta_generic_to_shared(Vs) + 8u * (FWD ? (q * LDV + g) : (g * LDV + q));
 
-  auto load_tile = [&](int t, double* st) {
+  // per-lane B-fragment ring: slot (d, nt, s) of this lane at ring_base + ((d*NT + nt)*NS + s)*256
+  constexpr int NS = PD ? 2 : 1;  // PD stages psi and tgt separately and multiplies on consumption
+  constexpr unsigned kRingWarpBytes = kRing * NT * NS * 256u;
+  const unsigned ring_base = (unsigned)__cvta_generic_to_shared(Vs) + 8u * (8 * MTOT * LDV) +
+                             warp * kRingWarpBytes + lane * 8u;
+
+  const long long gw = (long long)blockIdx.x * kWarps + warp;
+  const long long gstride = (long long)gridDim.x * kWarps;
+
+  for (long long wt = gw; wt < a.n_tiles; wt += gstride) {
+    // ---- per-lane source pointers of the B fragments: element (k = 4kt+q, column 8nt+g) ------------------
+    const double* bp[NT];
+    const double* tp[NT];   // PD: the target function's pointer
+    bool cv[NT];
+    long long kstep;        // elements between consecutive k-steps
+    int rhs = 0, rb = 0;
     if (XMODE) {
-      // rows [t*kW, ...) of n contiguous doubles each; 16 threads per row
-      const long long r0 = (long long)t * kW;
-      const int rows = (int)((a.total - r0) < kW ? (a.total - r0) : kW);
-      const double* src = a.in + r0 * n;
-      const int trow = tid >> 4, tcol = (tid & 15) * VEC;
-      for (int r = trow; r < rows; r += kThreads / 16)
-        for (int c = tcol; c < n; c += 16 * VEC) cp_async<8 * VEC>(st + r * ldt + c, src + (long long)r * n + c);
+      rhs = (int)(wt / a.tiles_per_rhs);
+      rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
+      kstep = 4;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+        const int rr = rb * 8 * NT + 8 * nt + g;
+        cv[nt] = rr < a.rows_per_rhs;
+        const long long off = (long long)(cv[nt] ? rr : 0) * n + q;
+        if (PD) {
+          const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
+          bp[nt] = a.psi + (long long)j * a.N + off;
+          tp[nt] = a.tgt + (long long)k * a.N + off;
+        } else {
+          bp[nt] = a.in + (long long)rhs * a.N + off;
+          tp[nt] = nullptr;
+        }
+      }
     } else {
-      // columns [t*kW, ...) of the flattened (outer, inner) index; each thread owns one column group
-      constexpr int kCG = kW / VEC;             // column groups per row
-      constexpr int kRowsPerPass = kThreads / kCG;
-      static_assert(kThreads % kCG == 0, "thread/column mapping");
-      const int cg = tid % kCG, k0 = tid / kCG;
-      const long long cidx = (long long)t * kW + cg * VEC;
-      if (cidx < a.total) {
-        const long long o = cidx / a.inner;
-        const int i = (int)(cidx - o * a.inner);
-        const double* src = a.in + (o * n) * a.inner + i;
-        double* dst = st + cg * VEC;
-        for (int k = k0; k < n; k += kRowsPerPass) cp_async<8 * VEC>(dst + k * ldt, src + (long long)k * a.inner);
+      kstep = 4LL * a.inner;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+        const long long c = wt * (8 * NT) + 8 * nt + g;
+        cv[nt] = c < a.total;
+        const long long cc = cv[nt] ? c : 0;
+        const long long o = cc / a.inner;
+        const int i = (int)(cc - o * a.inner);
+        bp[nt] = a.in + (o * n + q) * a.inner + i;
+        tp[nt] = nullptr;
       }
     }
-  };
-
-  int t = blockIdx.x;
-  int buf = 0;
-  if (t < a.n_tiles) load_tile(t, stage0);
-  cp_async_commit();
-  __syncthreads();  // V staged (plain stores) before anyone reads it
-
-  for (; t < a.n_tiles; t += gridDim.x) {
-    double* cur = stage0 + buf * stage_elems;
-    const int tn = t + gridDim.x;
-    if (tn < a.n_tiles) load_tile(tn, stage0 + (buf ^ 1) * stage_elems);
-    cp_async_commit();
-    cp_async_wait<1>();
-    __syncthreads();
-
-    double acc[MT][NT][2];
+    // issue the copies of k-step kt into ring stage d (always one commit group per call)
+    auto issue = [&](int kt, int d) {
 #pragma unroll
-    for (int mt = 0; mt < MT; ++mt)
+      for (int nt = 0; nt < NT; ++nt) {
+        const bool ok = cv[nt] && (4 * kt + q < n);
+        const long long off = ok ? kt * kstep : 0;
+        cp_async8(ring_base + ((d * NT + nt) * NS) * 256u, bp[nt] + off, ok);
+        if (PD) cp_async8(ring_base + ((d * NT + nt) * NS + 1) * 256u, tp[nt] + off, ok);
+      }
+      cp_async_commit();
+    };
+
+    double acc[MTOT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MTOT; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-    const double* bp = cur + (n_base + g) * b_sn + q * b_sk;
-#pragma unroll 2
-    for (int kt = 0; kt < KT; ++kt) {
-      double af[MT], bf[NT];
 #pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-        if (mt < mt_valid) af[mt] = ap[mt * 8 * a_sm + kt * 4 * a_sk];
-#pragma unroll
-      for (int nt = 0; nt < NT; ++nt) bf[nt] = bp[nt * 8 * b_sn + kt * 4 * b_sk];
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-        if (mt < mt_valid) {
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
-        }
-    }
+    for (int d = 0; d < kRing; ++d) issue(d, d);
 
-    // ---- epilogue: store accumulator fragments ------------------------------------------------------
+    for (int kt0 = 0; kt0 < KT; kt0 += kRing) {
+#pragma unroll
+      for (int d = 0; d < kRing; ++d) {
+        const int kt = kt0 + d;
+        if (kt < KT) {
+          cp_async_wait<kRing - 1>();  // the group of step kt has landed (each lane reads only its own slots)
+          double bf[NT];
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            bf[nt] = lds64(ring_base + ((d * NT + nt) * NS) * 256u);
+            if (PD) bf[nt] *= lds64(ring_base + ((d * NT + nt) * NS + 1) * 256u);
+          }
+          double af[MTOT];
+          const unsigned aaddr = a_base + kt * A_KT;
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aaddr + mt * A_MT);
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+          // refill this stage; the DMMAs above consumed bf, so the LDS of the stage have completed
+          issue(kt + kRing, d);
+        }
+      }
+    }
+    cp_async_wait<0>();
+
+    // ---- epilogue: C[m = 8mt+g][column 8nt + 2q + e] straight from the fragments --------------------------
     if (XMODE) {
-      // C[m = a-index][col = row r]: out[(r0 + r) * n + m]
-      const long long r0 = (long long)t * kW;
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          const long long r = r0 + n_base + 8 * nt + 2 * q + e;
-          if (r < a.total) {
-            double* dst = a.out + r * n;
+          const int rr = rb * 8 * NT + 8 * nt + 2 * q + e;
+          if (rr < a.rows_per_rhs) {
+            double* dst = a.out + (long long)rhs * a.N + (long long)rr * n + g;
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-              const int m = m_base + 8 * mt + g;
-              if (mt < mt_valid && m < n) dst[m] = acc[mt][nt][e];
-            }
+            for (int mt = 0; mt < MTOT; ++mt)
+              if (8 * mt + g < n) dst[8 * mt] = acc[mt][nt][e];
           }
         }
       }
     } else {
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const long long cidx = (long long)t * kW + n_base + 8 * nt + 2 * q;
-        if (VEC == 2) {
-          if (cidx < a.total) {
-            const long long o = cidx / a.inner;
-            const int i = (int)(cidx - o * a.inner);
-            double* dst = a.out + (o * n) * a.inner + i;
+        const long long c = wt * (8 * NT) + 8 * nt + 2 * q;
+        if (a.vec2) {
+          if (c < a.total) {
+            const long long o = c / a.inner;
+            const int i = (int)(c - o * a.inner);
+            double* dst = a.out + (o * n + g) * a.inner + i;
+            const double* mp = a.mult ? a.mult + (long long)g * a.inner + i : nullptr;
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-              const int m = m_base + 8 * mt + g;
-              if (mt < mt_valid && m < n) {
+            for (int mt = 0; mt < MTOT; ++mt) {
+              if (8 * mt + g < n) {
                 double2 v = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-                if (a.mult) {
-                  const double2 mm = __ldg(reinterpret_cast<const double2*>(a.mult + (long long)m * a.inner + i));
+                if (mp) {
+                  const double2 mm = __ldg(reinterpret_cast<const double2*>(mp + (long long)(8 * mt) * a.inner));
                   v.x *= mm.x;
                   v.y *= mm.y;
                 }
-                *reinterpret_cast<double2*>(dst + (long long)m * a.inner) = v;
+                *reinterpret_cast<double2*>(dst + (long long)(8 * mt) * a.inner) = v;
               }
             }
           }
         } else {
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
-            const long long ce = cidx + e;
+            const long long ce = c + e;
             if (ce < a.total) {
               const long long o = ce / a.inner;
               const int i = (int)(ce - o * a.inner);
-              double* dst = a.out + (o * n) * a.inner + i;
+              double* dst = a.out + (o * n + g) * a.inner + i;
+              const double* mp = a.mult ? a.mult + (long long)g * a.inner + i : nullptr;
 #pragma unroll
-              for (int mt = 0; mt < MT; ++mt) {
-                const int m = m_base + 8 * mt + g;
-                if (mt < mt_valid && m < n) {
+              for (int mt = 0; mt < MTOT; ++mt) {
+                if (8 * mt + g < n) {
                   double v = acc[mt][nt][e];
-                  if (a.mult) v *= __ldg(a.mult + (long long)m * a.inner + i);
-                  dst[(long long)m * a.inner] = v;
+                  if (mp) v *= __ldg(mp + (long long)(8 * mt) * a.inner);
+                  dst[(long long)(8 * mt) * a.inner] = v;
                 }
               }
             }
@@ -218,112 +260,99 @@ __global__ void __launch_bounds__(32 * WR * WC, 1) k_mode_dmma(const ModeArgs a)
         }
       }
     }
-    __syncthreads();  // everyone is done with `cur` before the next iteration's prefetch overwrites it
-    buf ^= 1;
   }
-  cp_async_wait<0>();
 }
 
 // ---- host side ------------------------------------------------------------------------------------
 
-struct Shape {
-  int MT, WR, NT, WC;
-};
-
-inline bool pick_shape(int n, Shape* s) {
-  if (n <= 16) *s = {2, 1, 2, 8};
-  else if (n <= 32) *s = {2, 2, 2, 4};
-  else if (n <= 48) *s = {3, 2, 2, 4};
-  else if (n <= 64) *s = {4, 2, 2, 4};
-  else if (n <= 96) *s = {3, 4, 2, 2};
-  else if (n <= 128) *s = {4, 4, 2, 2};
+// supported classes of ceil(n/8) and the columns-per-warp choice for each
+inline bool pick_class(int n, int* mtot, int* nt) {
+  const int need = (n + 7) / 8;
+  if (need <= 2) { *mtot = 2; *nt = 4; }
+  else if (need <= 4) { *mtot = 4; *nt = 4; }
+  else if (need <= 6) { *mtot = 6; *nt = 4; }
+  else if (need <= 8) { *mtot = 8; *nt = 2; }
+  else if (need <= 12) { *mtot = 12; *nt = 2; }
+  else if (need <= 15) { *mtot = 15; *nt = 2; }
+  else if (need <= 16) { *mtot = 16; *nt = 2; }
   else return false;
   return true;
 }
 
-struct Layout {
-  int KT, ldv, ldt, R8, kW;
-  size_t smem_bytes;
-};
-
-inline Layout make_layout(int n, const Shape& s, bool xmode) {
-  Layout L;
-  L.KT = (n + 3) / 4;
-  L.R8 = (n + 7) & ~7;
-  L.ldv = L.R8 + 4;
-  L.kW = 8 * s.NT * s.WC;
-  if (xmode) {
-    const int k4 = 4 * L.KT;
-    L.ldt = (k4 % 8 == 4) ? k4 : k4 + 4;
-    L.smem_bytes = sizeof(double) * ((size_t)L.R8 * L.ldv + 2 * (size_t)L.kW * L.ldt);
-  } else {
-    L.ldt = L.kW + 4;
-    L.smem_bytes = sizeof(double) * ((size_t)L.R8 * L.ldv + 2 * (size_t)4 * L.KT * L.ldt);
-  }
-  return L;
-}
-
-template <int MT, int WR, int NT, int WC>
-cudaError_t launch_shape(bool xmode, int vec, const ModeArgs& a, int grid, size_t smem, cudaStream_t s) {
-  constexpr int kThreads = 32 * WR * WC;
-#define EXX_LAUNCH(XM, VC)                                                                              \
+template <int MTOT, int NT>
+cudaError_t launch_class(bool xmode, bool fwd, bool pd, const WArgs& a, int grid, cudaStream_t s) {
+  constexpr size_t smem_v = sizeof(double) * 8 * MTOT * (8 * MTOT + 4);
+#define EXX_LAUNCH(XM, FW, PDD)                                                                         \
   do {                                                                                                  \
-    auto kern = k_mode_dmma<MT, WR, NT, WC, XM, VC>;                                                    \
+    const size_t smem = smem_v + (size_t)kWarps * kRing * NT * ((PDD) ? 2 : 1) * 256;                   \
+    auto kern = k_mode_w<MTOT, NT, XM, FW, PDD>;                                                        \
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
     if (e != cudaSuccess) return e;                                                                     \
     kern<<<grid, kThreads, smem, s>>>(a);                                                               \
     return cudaGetLastError();                                                                          \
   } while (0)
   if (xmode) {
-    if (vec == 2) EXX_LAUNCH(true, 2);
-    EXX_LAUNCH(true, 1);
+    if (fwd && pd) EXX_LAUNCH(true, true, true);
+    if (fwd) EXX_LAUNCH(true, true, false);
+    EXX_LAUNCH(true, false, false);
   } else {
-    if (vec == 2) EXX_LAUNCH(false, 2);
-    EXX_LAUNCH(false, 1);
+    if (fwd) EXX_LAUNCH(false, true, false);
+    EXX_LAUNCH(false, false, false);
   }
 #undef EXX_LAUNCH
   return cudaErrorUnknown;
 }
 
-// One mode product along `axis`, in place or out of place, nb right-hand sides.
+// One mode product along `axis` for nb right-hand sides; in == out is allowed (and is the normal case).
+// pd != nullptr (axis 0, forward only): the input is psi_j .* tgt_k formed on the fly.
 cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const double* in, double* out,
-                              int nb, bool apply_mult, cudaStream_t s) {
+                              int nb, bool apply_mult, const FastArgs* pd, cudaStream_t s) {
   const int n = p->n[axis];
-  Shape sh;
-  if (!pick_shape(n, &sh)) return cudaErrorNotSupported;
+  int mtot, nt;
+  if (!pick_class(n, &mtot, &nt)) return cudaErrorNotSupported;
   const bool xmode = axis == 0;
-  const Layout L = make_layout(n, sh, xmode);
-  if (L.smem_bytes > (size_t)p->smem_optin) return cudaErrorNotSupported;
-  ModeArgs a;
+  if (pd && !(xmode && forward)) return cudaErrorInvalidValue;
+  WArgs a{};
   a.in = in;
   a.out = out;
   a.V = p->d_V[axis];
   a.mult = apply_mult ? p->d_mult : nullptr;
+  a.psi = pd ? pd->psi : nullptr;
+  a.tgt = pd ? pd->tgt : nullptr;
+  if (pd) a.bd = pd->bd;
   a.n = n;
-  a.KT = L.KT;
-  a.ldv = L.ldv;
-  a.ldt = L.ldt;
-  a.fwd = forward ? 1 : 0;
-  const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
-  a.inner = xmode ? 1 : (int)inner;
-  a.total = p->N / n * nb;  // columns (L-mode) or rows (X-mode)
-  const long long tiles = (a.total + L.kW - 1) / L.kW;
-  if (tiles > 0x7fffffffLL) return cudaErrorNotSupported;
-  a.n_tiles = (int)tiles;
-  const bool aligned = (((uintptr_t)in | (uintptr_t)out) & 15) == 0 &&
-                       (!apply_mult || ((uintptr_t)p->d_mult & 15) == 0);
-  int vec = 1;
-  if (aligned) {
-    if (xmode) vec = (n % 2 == 0) ? 2 : 1;
-    else vec = (inner % 2 == 0) ? 2 : 1;
+  a.KT = (n + 3) / 4;
+  a.N = p->N;
+  const int cols_per_tile = 8 * nt;
+  if (xmode) {
+    a.inner = 1;
+    a.rows_per_rhs = (int)(p->N / n);
+    a.tiles_per_rhs = (a.rows_per_rhs + cols_per_tile - 1) / cols_per_tile;
+    a.total = (long long)a.rows_per_rhs * nb;
+    a.n_tiles = (long long)a.tiles_per_rhs * nb;
+    a.vec2 = 0;
+  } else {
+    const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
+    a.inner = (int)inner;
+    a.total = p->N / n * nb;
+    a.n_tiles = (a.total + cols_per_tile - 1) / cols_per_tile;
+    a.rows_per_rhs = 0;
+    a.tiles_per_rhs = 1;
+    const bool aligned = (((uintptr_t)out) & 15) == 0 && (!apply_mult || ((uintptr_t)p->d_mult & 15) == 0);
+    a.vec2 = (aligned && inner % 2 == 0) ? 1 : 0;
   }
-  const int grid = (int)(tiles < p->sm_count ? tiles : p->sm_count);
-  if (sh.MT == 2 && sh.WR == 1) return launch_shape<2, 1, 2, 8>(xmode, vec, a, grid, L.smem_bytes, s);
-  if (sh.MT == 2 && sh.WR == 2) return launch_shape<2, 2, 2, 4>(xmode, vec, a, grid, L.smem_bytes, s);
-  if (sh.MT == 3 && sh.WR == 2) return launch_shape<3, 2, 2, 4>(xmode, vec, a, grid, L.smem_bytes, s);
-  if (sh.MT == 4 && sh.WR == 2) return launch_shape<4, 2, 2, 4>(xmode, vec, a, grid, L.smem_bytes, s);
-  if (sh.MT == 3 && sh.WR == 4) return launch_shape<3, 4, 2, 2>(xmode, vec, a, grid, L.smem_bytes, s);
-  return launch_shape<4, 4, 2, 2>(xmode, vec, a, grid, L.smem_bytes, s);
+  if (a.n_tiles <= 0) return cudaSuccess;
+  const long long ctas = (a.n_tiles + kWarps - 1) / kWarps;
+  const int grid = (int)(ctas < p->sm_count ? ctas : p->sm_count);
+  switch (mtot) {
+    case 2: return launch_class<2, 4>(xmode, forward, pd != nullptr, a, grid, s);
+    case 4: return launch_class<4, 4>(xmode, forward, pd != nullptr, a, grid, s);
+    case 6: return launch_class<6, 4>(xmode, forward, pd != nullptr, a, grid, s);
+    case 8: return launch_class<8, 2>(xmode, forward, pd != nullptr, a, grid, s);
+    case 12: return launch_class<12, 2>(xmode, forward, pd != nullptr, a, grid, s);
+    case 15: return launch_class<15, 2>(xmode, forward, pd != nullptr, a, grid, s);
+    default: return launch_class<16, 2>(xmode, forward, pd != nullptr, a, grid, s);
+  }
 }
 
 }  // namespace
@@ -336,7 +365,7 @@ void fast_destroy(exx_plan*) {}
 static cudaError_t one_product(exx_plan* p, int axis, bool fwd, double*& cur, double*& other, int nb,
                                bool mult, cudaStream_t s) {
   ProfScope ps(p, KC_MODE_PRODUCT, s);
-  cudaError_t e = fast_mode_product(p, axis, fwd, cur, cur, nb, mult, s);
+  cudaError_t e = fast_mode_product(p, axis, fwd, cur, cur, nb, mult, nullptr, s);
   if (e == cudaErrorNotSupported) {
     e = ref_mode_product(p, axis, fwd, cur, other, nb, mult, s);
     double* t = cur;
@@ -350,15 +379,23 @@ cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, co
                              cudaStream_t s, long long* launches) {
   cudaError_t e;
   double *cur = buf0, *other = buf1;
+  bool first_done = false;
   if (fa) {
+    // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
+      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      e = fast_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
+    }
+    if (e == cudaSuccess) {
+      first_done = true;
+    } else if (e == cudaErrorNotSupported) {
       ProfScope ps(p, KC_PAIR_DENSITY, s);
       e = ref_pair_density(p, fa->psi, fa->tgt, fa->bd, cur, s);
+      ++*launches;
     }
     if (e != cudaSuccess) return e;
-    ++*launches;
   }
-  if ((e = one_product(p, 0, true, cur, other, nb, false, s)) != cudaSuccess) return e;
+  if (!first_done && (e = one_product(p, 0, true, cur, other, nb, false, s)) != cudaSuccess) return e;
   if ((e = one_product(p, 1, true, cur, other, nb, false, s)) != cudaSuccess) return e;
   if ((e = one_product(p, 2, true, cur, other, nb, true, s)) != cudaSuccess) return e;
   if ((e = one_product(p, 2, false, cur, other, nb, false, s)) != cudaSuccess) return e;
