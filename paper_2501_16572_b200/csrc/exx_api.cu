@@ -275,13 +275,16 @@ exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi,
   long long launches = 0;
   for (int b0 = 0; b0 < n_rhs; b0 += n_c) {
     const int nb = n_rhs - b0 < n_c ? n_rhs - b0 : n_c;
-    EXX_CUDA(cudaMemcpyAsync(buf0, d_rhs + N * (size_t)b0, fn * nb, cudaMemcpyDeviceToDevice, s));
     if (plan->variant == EXX_VARIANT_REFERENCE) {
+      EXX_CUDA(cudaMemcpyAsync(buf0, d_rhs + N * (size_t)b0, fn * nb, cudaMemcpyDeviceToDevice, s));
       EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
+      EXX_CUDA(cudaMemcpyAsync(d_phi + N * (size_t)b0, buf0, fn * nb, cudaMemcpyDeviceToDevice, s));
     } else {
-      EXX_CUDA(exx::fast_solve_batch(plan, buf0, buf1, nb, nullptr, s, &launches));
+      // first product reads the right-hand sides where they are and writes phi's storage; the other five
+      // run in place there (no staging copies)
+      EXX_CUDA(exx::fast_solve_batch(plan, d_rhs + N * (size_t)b0, d_phi + N * (size_t)b0, buf0, nb, nullptr, s,
+                                     &launches));
     }
-    EXX_CUDA(cudaMemcpyAsync(d_phi + N * (size_t)b0, buf0, fn * nb, cudaMemcpyDeviceToDevice, s));
   }
   plan->last_launches = launches;
   return EXX_OK;
@@ -337,7 +340,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
           launches += 2;
         } else {
           const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, j0 == 0};
-          EXX_CUDA(exx::fast_solve_batch(plan, buf0, buf1, nb, &fa, s, &launches));
+          EXX_CUDA(exx::fast_solve_batch(plan, nullptr, buf0, buf1, nb, &fa, s, &launches));
         }
       }
     }

@@ -96,9 +96,7 @@ struct ProfScope {
 // (the caller then reports EXX_ERR_INVALID_ARG; there is no silent fallback).
 cudaError_t fast_init(exx_plan* p);
 void fast_destroy(exx_plan* p);
-// phi-producing solve of one batch: in-place on buf0 using buf1 as scratch; result ends in buf0.
-// src_mode 0: buf0 already holds the right-hand sides.  src_mode 1: pair densities are formed on the
-// fly from psi/tgt (bd).  If acc != nullptr the last pass accumulates into vx instead of storing phi.
+// One batch of solves; see kernels_dmma.cu.
 struct FastArgs {
   const double* psi;
   const double* tgt;
@@ -107,7 +105,7 @@ struct FastArgs {
   BatchDesc bd;
   bool first;  // first batch for these targets: vx is overwritten, not accumulated into
 };
-cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, const FastArgs* fa,
-                             cudaStream_t s, long long* launches);
+cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,
+                             const FastArgs* fa, cudaStream_t s, long long* launches);
 
 }  // namespace exx

@@ -81,9 +81,10 @@ struct WArgs {
 };
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
-template <int MTOT, int NT, bool XMODE, bool FWD, bool PD>
+template <int MTOT, int NT, bool XMODE, bool FWD, bool TWO>
 __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
-  static_assert(!PD || (XMODE && FWD), "pair density is fused into the first (x, forward) product only");
+  static_assert(!TWO || (XMODE && FWD) || (!XMODE && !FWD), "second stream: pair density (x fwd) or multiplier (z bwd)");
+  static_assert((kRing & (kRing - 1)) == 0, "ring depth must be a power of two");
   constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): conflict-free for both fragment orientations
   extern __shared__ __align__(16) double Vs[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -106,31 +107,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   const unsigned a_base = (unsigned)__cvta_generic_to_shared(Vs) + 8u * (FWD ? (q * LDV + g) : (g * LDV + q));
 
   // per-lane B-fragment ring: slot (d, nt, s) of this lane at ring_base + ((d*NT + nt)*NS + s)*256
-  constexpr int NS = PD ? 2 : 1;  // PD stages psi and tgt separately and multiplies on consumption
+  constexpr int NS = TWO ? 2 : 1;  // two streams are staged separately and multiplied on consumption
   constexpr unsigned kRingWarpBytes = kRing * NT * NS * 256u;
   const unsigned ring_base = (unsigned)__cvta_generic_to_shared(Vs) + 8u * (8 * MTOT * LDV) +
                              warp * kRingWarpBytes + lane * 8u;
 
   const long long gw = (long long)blockIdx.x * kWarps + warp;
   const long long gstride = (long long)gridDim.x * kWarps;
+  const long long kstep = XMODE ? 4 : 4LL * a.inner;  // elements between consecutive k-steps
 
-  for (long long wt = gw; wt < a.n_tiles; wt += gstride) {
-    // ---- per-lane source pointers of the B fragments: element (k = 4kt+q, column 8nt+g) ------------------
-    const double* bp[NT];
-    const double* tp[NT];   // PD: the target function's pointer
-    bool cv[NT];
-    long long kstep;        // elements between consecutive k-steps
-    int rhs = 0, rb = 0;
+  // Per-lane source pointers of the B fragments of warp tile wt: element (k = 4kt+q, column 8nt+g).
+  // TWO: a second stream with the same stride is multiplied in on consumption -- the target function in
+  // X-mode (pair density, a1), the multiplier table in L-mode (a3, applied while loading the z-backward pass).
+  auto setup = [&](long long wt, const double* (&bp)[NT], const double* (&tp)[NT], bool (&cv)[NT]) {
     if (XMODE) {
-      rhs = (int)(wt / a.tiles_per_rhs);
-      rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
-      kstep = 4;
+      const int rhs = (int)(wt / a.tiles_per_rhs);
+      const int rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
         const int rr = rb * 8 * NT + 8 * nt + g;
         cv[nt] = rr < a.rows_per_rhs;
         const long long off = (long long)(cv[nt] ? rr : 0) * n + q;
-        if (PD) {
+        if (TWO) {
           const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
           bp[nt] = a.psi + (long long)j * a.N + off;
           tp[nt] = a.tgt + (long long)k * a.N + off;
@@ -140,7 +138,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
         }
       }
     } else {
-      kstep = 4LL * a.inner;
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
         const long long c = wt * (8 * NT) + 8 * nt + g;
@@ -149,56 +146,75 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
         const long long o = cc / a.inner;
         const int i = (int)(cc - o * a.inner);
         bp[nt] = a.in + (o * n + q) * a.inner + i;
-        tp[nt] = nullptr;
+        tp[nt] = TWO ? a.mult + (long long)q * a.inner + i : nullptr;
       }
     }
-    // issue the copies of k-step kt into ring stage d (always one commit group per call)
-    auto issue = [&](int kt, int d) {
+  };
+
+  // ---- producer state: runs kRing k-steps ahead of the consumer, straight across tile boundaries ----------
+  long long wt_i = gw;
+  int kt_i = 0;
+  const double* bp_i[NT];
+  const double* tp_i[NT];
+  bool cv_i[NT];
+  if (wt_i < a.n_tiles) setup(wt_i, bp_i, tp_i, cv_i);
+  // issue the copies of the producer's current k-step into ring stage `st` (always exactly one commit group)
+  auto issue_next = [&](int st) {
+    if (wt_i < a.n_tiles) {
+      const unsigned slot = ring_base + st * (NT * NS * 256u);
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const bool ok = cv[nt] && (4 * kt + q < n);
-        const long long off = ok ? kt * kstep : 0;
-        cp_async8(ring_base + ((d * NT + nt) * NS) * 256u, bp[nt] + off, ok);
-        if (PD) cp_async8(ring_base + ((d * NT + nt) * NS + 1) * 256u, tp[nt] + off, ok);
+        const bool ok = cv_i[nt] && (4 * kt_i + q < n);
+        const long long off = ok ? kt_i * kstep : 0;
+        cp_async8(slot + (nt * NS) * 256u, bp_i[nt] + off, ok);
+        if (TWO) cp_async8(slot + (nt * NS + 1) * 256u, tp_i[nt] + off, ok);
       }
-      cp_async_commit();
-    };
+      if (++kt_i == KT) {
+        kt_i = 0;
+        wt_i += gstride;
+        if (wt_i < a.n_tiles) setup(wt_i, bp_i, tp_i, cv_i);
+      }
+    }
+    cp_async_commit();
+  };
+#pragma unroll
+  for (int d = 0; d < kRing; ++d) issue_next(d);
+  int stage = 0;
 
+  for (long long wt = gw; wt < a.n_tiles; wt += gstride) {
+    int rhs = 0, rb = 0;
+    if (XMODE) {
+      rhs = (int)(wt / a.tiles_per_rhs);
+      rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
+    }
     double acc[MTOT][NT][2];
 #pragma unroll
     for (int mt = 0; mt < MTOT; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
+#pragma unroll 2
+    for (int kt = 0; kt < KT; ++kt) {
+      cp_async_wait<kRing - 1>();  // this step's group has landed (each lane reads only its own slots)
+      const unsigned slot = ring_base + stage * (NT * NS * 256u);
+      double bf[NT];
 #pragma unroll
-    for (int d = 0; d < kRing; ++d) issue(d, d);
-
-    for (int kt0 = 0; kt0 < KT; kt0 += kRing) {
-#pragma unroll
-      for (int d = 0; d < kRing; ++d) {
-        const int kt = kt0 + d;
-        if (kt < KT) {
-          cp_async_wait<kRing - 1>();  // the group of step kt has landed (each lane reads only its own slots)
-          double bf[NT];
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) {
-            bf[nt] = lds64(ring_base + ((d * NT + nt) * NS) * 256u);
-            if (PD) bf[nt] *= lds64(ring_base + ((d * NT + nt) * NS + 1) * 256u);
-          }
-          double af[MTOT];
-          const unsigned aaddr = a_base + kt * A_KT;
-#pragma unroll
-          for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aaddr + mt * A_MT);
-#pragma unroll
-          for (int mt = 0; mt < MTOT; ++mt)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
-          // refill this stage; the DMMAs above consumed bf, so the LDS of the stage have completed
-          issue(kt + kRing, d);
-        }
+      for (int nt = 0; nt < NT; ++nt) {
+        bf[nt] = lds64(slot + (nt * NS) * 256u);
+        if (TWO) bf[nt] *= lds64(slot + (nt * NS + 1) * 256u);
       }
+      double af[MTOT];
+      const unsigned aaddr = a_base + kt * A_KT;
+#pragma unroll
+      for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aaddr + mt * A_MT);
+#pragma unroll
+      for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+      // refill this stage: the DMMAs above consumed bf, so the LDS of the stage have completed
+      issue_next(stage);
+      stage = (stage + 1) & (kRing - 1);
     }
-    cp_async_wait<0>();
 
     // ---- epilogue: C[m = 8mt+g][column 8nt + 2q + e] straight from the fragments --------------------------
     if (XMODE) {
@@ -224,18 +240,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
             const long long o = c / a.inner;
             const int i = (int)(c - o * a.inner);
             double* dst = a.out + (o * n + g) * a.inner + i;
-            const double* mp = a.mult ? a.mult + (long long)g * a.inner + i : nullptr;
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
-              if (8 * mt + g < n) {
-                double2 v = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-                if (mp) {
-                  const double2 mm = __ldg(reinterpret_cast<const double2*>(mp + (long long)(8 * mt) * a.inner));
-                  v.x *= mm.x;
-                  v.y *= mm.y;
-                }
-                *reinterpret_cast<double2*>(dst + (long long)(8 * mt) * a.inner) = v;
-              }
+              if (8 * mt + g < n)
+                *reinterpret_cast<double2*>(dst + (long long)(8 * mt) * a.inner) =
+                    make_double2(acc[mt][nt][0], acc[mt][nt][1]);
             }
           }
         } else {
@@ -246,14 +255,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
               const long long o = ce / a.inner;
               const int i = (int)(ce - o * a.inner);
               double* dst = a.out + (o * n + g) * a.inner + i;
-              const double* mp = a.mult ? a.mult + (long long)g * a.inner + i : nullptr;
 #pragma unroll
               for (int mt = 0; mt < MTOT; ++mt) {
-                if (8 * mt + g < n) {
-                  double v = acc[mt][nt][e];
-                  if (mp) v *= __ldg(mp + (long long)(8 * mt) * a.inner);
-                  dst[(long long)(8 * mt) * a.inner] = v;
-                }
+                if (8 * mt + g < n) dst[(long long)(8 * mt) * a.inner] = acc[mt][nt][e];
               }
             }
           }
@@ -280,7 +284,7 @@ inline bool pick_class(int n, int* mtot, int* nt) {
 }
 
 template <int MTOT, int NT>
-cudaError_t launch_class(bool xmode, bool fwd, bool pd, const WArgs& a, int grid, cudaStream_t s) {
+cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int grid, cudaStream_t s) {
   constexpr size_t smem_v = sizeof(double) * 8 * MTOT * (8 * MTOT + 4);
 #define EXX_LAUNCH(XM, FW, PDD)                                                                         \
   do {                                                                                                  \
@@ -292,11 +296,12 @@ cudaError_t launch_class(bool xmode, bool fwd, bool pd, const WArgs& a, int grid
     return cudaGetLastError();                                                                          \
   } while (0)
   if (xmode) {
-    if (fwd && pd) EXX_LAUNCH(true, true, true);
+    if (fwd && two) EXX_LAUNCH(true, true, true);
     if (fwd) EXX_LAUNCH(true, true, false);
     EXX_LAUNCH(true, false, false);
   } else {
     if (fwd) EXX_LAUNCH(false, true, false);
+    if (two) EXX_LAUNCH(false, false, true);
     EXX_LAUNCH(false, false, false);
   }
 #undef EXX_LAUNCH
@@ -305,6 +310,7 @@ cudaError_t launch_class(bool xmode, bool fwd, bool pd, const WArgs& a, int grid
 
 // One mode product along `axis` for nb right-hand sides; in == out is allowed (and is the normal case).
 // pd != nullptr (axis 0, forward only): the input is psi_j .* tgt_k formed on the fly.
+// apply_mult (axis 2, backward only): the input is multiplied by f(Lambda~) while it is loaded.
 cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const double* in, double* out,
                               int nb, bool apply_mult, const FastArgs* pd, cudaStream_t s) {
   const int n = p->n[axis];
@@ -312,6 +318,8 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
   if (!pick_class(n, &mtot, &nt)) return cudaErrorNotSupported;
   const bool xmode = axis == 0;
   if (pd && !(xmode && forward)) return cudaErrorInvalidValue;
+  if (apply_mult && !(axis == 2 && !forward)) return cudaErrorInvalidValue;
+  const bool two = pd != nullptr || apply_mult;
   WArgs a{};
   a.in = in;
   a.out = out;
@@ -338,20 +346,20 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
     a.n_tiles = (a.total + cols_per_tile - 1) / cols_per_tile;
     a.rows_per_rhs = 0;
     a.tiles_per_rhs = 1;
-    const bool aligned = (((uintptr_t)out) & 15) == 0 && (!apply_mult || ((uintptr_t)p->d_mult & 15) == 0);
+    const bool aligned = (((uintptr_t)out) & 15) == 0;
     a.vec2 = (aligned && inner % 2 == 0) ? 1 : 0;
   }
   if (a.n_tiles <= 0) return cudaSuccess;
   const long long ctas = (a.n_tiles + kWarps - 1) / kWarps;
   const int grid = (int)(ctas < p->sm_count ? ctas : p->sm_count);
   switch (mtot) {
-    case 2: return launch_class<2, 4>(xmode, forward, pd != nullptr, a, grid, s);
-    case 4: return launch_class<4, 4>(xmode, forward, pd != nullptr, a, grid, s);
-    case 6: return launch_class<6, 4>(xmode, forward, pd != nullptr, a, grid, s);
-    case 8: return launch_class<8, 2>(xmode, forward, pd != nullptr, a, grid, s);
-    case 12: return launch_class<12, 2>(xmode, forward, pd != nullptr, a, grid, s);
-    case 15: return launch_class<15, 2>(xmode, forward, pd != nullptr, a, grid, s);
-    default: return launch_class<16, 2>(xmode, forward, pd != nullptr, a, grid, s);
+    case 2: return launch_class<2, 4>(xmode, forward, two, a, grid, s);
+    case 4: return launch_class<4, 4>(xmode, forward, two, a, grid, s);
+    case 6: return launch_class<6, 4>(xmode, forward, two, a, grid, s);
+    case 8: return launch_class<8, 2>(xmode, forward, two, a, grid, s);
+    case 12: return launch_class<12, 2>(xmode, forward, two, a, grid, s);
+    case 15: return launch_class<15, 2>(xmode, forward, two, a, grid, s);
+    default: return launch_class<16, 2>(xmode, forward, two, a, grid, s);
   }
 }
 
@@ -361,25 +369,40 @@ cudaError_t fast_init(exx_plan*) { return cudaSuccess; }
 void fast_destroy(exx_plan*) {}
 
 // Axes longer than 128 points do not fit the resident-V kernels; they run on the plain DFMA kernel
-// (still CUDA, still in the library; stated in DESIGN.md).  buf1 is only needed in that case.
-static cudaError_t one_product(exx_plan* p, int axis, bool fwd, double*& cur, double*& other, int nb,
-                               bool mult, cudaStream_t s) {
+// (still CUDA, still in the library; stated in DESIGN.md).  `scratch` is only needed in that case.
+// The multiplier (a3) is applied by the z-forward store in the plain kernel and by the z-backward load
+// in the DMMA kernel; `mult_pending` carries it from one to the other.
+static cudaError_t one_product(exx_plan* p, int axis, bool fwd, const double* src, double*& cur, double*& other,
+                               int nb, bool& mult_pending, cudaStream_t s) {
   ProfScope ps(p, KC_MODE_PRODUCT, s);
-  cudaError_t e = fast_mode_product(p, axis, fwd, cur, cur, nb, mult, nullptr, s);
-  if (e == cudaErrorNotSupported) {
-    e = ref_mode_product(p, axis, fwd, cur, other, nb, mult, s);
+  const bool z_bwd = axis == 2 && !fwd;
+  cudaError_t e = fast_mode_product(p, axis, fwd, src, cur, nb, z_bwd && mult_pending, nullptr, s);
+  if (e == cudaSuccess) {
+    if (z_bwd) mult_pending = false;
+    return e;
+  }
+  if (e != cudaErrorNotSupported) return e;
+  const bool z_fwd = axis == 2 && fwd;
+  if (src == cur) {
+    e = ref_mode_product(p, axis, fwd, cur, other, nb, z_fwd, s);
     double* t = cur;
     cur = other;
     other = t;
+  } else {
+    e = ref_mode_product(p, axis, fwd, src, cur, nb, z_fwd, s);
   }
+  if (z_fwd) mult_pending = false;
   return e;
 }
 
-cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, const FastArgs* fa,
-                             cudaStream_t s, long long* launches) {
+// One batch: `src` holds nb right-hand sides (ignored when fa != nullptr: the pair densities are formed on
+// the fly), `work` receives phi (src == work allowed), `scratch` is a second nb*N buffer used only by the
+// plain-kernel fallback.  With fa, phi is then accumulated into vx (a5).
+cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,
+                             const FastArgs* fa, cudaStream_t s, long long* launches) {
   cudaError_t e;
-  double *cur = buf0, *other = buf1;
-  bool first_done = false;
+  double *cur = work, *other = scratch;
+  bool first_done = false, mult_pending = true;
   if (fa) {
     // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
@@ -392,15 +415,17 @@ cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, co
       ProfScope ps(p, KC_PAIR_DENSITY, s);
       e = ref_pair_density(p, fa->psi, fa->tgt, fa->bd, cur, s);
       ++*launches;
+      src = cur;
     }
     if (e != cudaSuccess) return e;
   }
-  if (!first_done && (e = one_product(p, 0, true, cur, other, nb, false, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 1, true, cur, other, nb, false, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 2, true, cur, other, nb, true, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 2, false, cur, other, nb, false, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 1, false, cur, other, nb, false, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 0, false, cur, other, nb, false, s)) != cudaSuccess) return e;
+  if (!first_done && (e = one_product(p, 0, true, src, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if ((e = one_product(p, 1, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if ((e = one_product(p, 2, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if ((e = one_product(p, 2, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if (mult_pending) return cudaErrorUnknown;  // cannot happen: same axis, same support decision
+  if ((e = one_product(p, 1, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if ((e = one_product(p, 0, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
   *launches += 6;
   if (fa) {
     {
@@ -409,8 +434,8 @@ cudaError_t fast_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, co
     }
     if (e != cudaSuccess) return e;
     ++*launches;
-  } else if (cur != buf0) {
-    e = cudaMemcpyAsync(buf0, cur, sizeof(double) * (size_t)p->N * nb, cudaMemcpyDeviceToDevice, s);
+  } else if (cur != work) {
+    e = cudaMemcpyAsync(work, cur, sizeof(double) * (size_t)p->N * nb, cudaMemcpyDeviceToDevice, s);
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
