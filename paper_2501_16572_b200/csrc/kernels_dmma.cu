@@ -27,6 +27,7 @@
 // The paper's four data reorganisations (Eqs. 12-15) do not exist here: they are
 // artefacts of calling a 2-D GEMM library and are replaced by the strided fragment addressing above.
 #include <cstdint>
+#include <cstdlib>
 
 #include "exx_internal.h"
 
@@ -35,6 +36,7 @@ namespace {
 
 constexpr int kWarps = 8;
 constexpr int kThreads = 32 * kWarps;
+constexpr size_t kMinSmem = 117 * 1024;  // > half of the 227 KB per-SM limit
 constexpr int kRing = 8;  // depth of the per-lane B-fragment ring (cp.async stages), in k-steps
 
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
@@ -99,6 +101,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
     Vs[r * LDV + c] = a.V[i];
   }
   __syncthreads();
+  // Programmatic dependent launch: everything above touched only the plan's constant V, so it overlaps
+  // the tail of the previous pass; from here on we read that pass's output.
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
 
   // A fragment (M[m][k]) shared address for (mt, kt): base + mt*A_MT + kt*A_KT   (bytes)
   //   FWD: M[m][k] = V[k][m] -> Vs[(4kt+q)*LDV + 8mt+g];   BWD: M[m][k] = V[m][k] -> Vs[(8mt+g)*LDV + 4kt+q]
@@ -121,8 +127,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   // X-mode (pair density, a1), the multiplier table in L-mode (a3, applied while loading the z-backward pass).
   auto setup = [&](long long wt, const double* (&bp)[NT], const double* (&tp)[NT], bool (&cv)[NT]) {
     if (XMODE) {
-      const int rhs = (int)(wt / a.tiles_per_rhs);
-      const int rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
+      const int rhs = (int)((unsigned)wt / (unsigned)a.tiles_per_rhs);
+      const int rb = (int)wt - rhs * a.tiles_per_rhs;
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
         const int rr = rb * 8 * NT + 8 * nt + g;
@@ -140,12 +146,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
     } else {
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const long long c = wt * (8 * NT) + 8 * nt + g;
-        cv[nt] = c < a.total;
-        const long long cc = cv[nt] ? c : 0;
-        const long long o = cc / a.inner;
-        const int i = (int)(cc - o * a.inner);
-        bp[nt] = a.in + (o * n + q) * a.inner + i;
+        const unsigned c = (unsigned)wt * (8 * NT) + 8 * nt + g;   // host guarantees total < 2^31
+        cv[nt] = c < (unsigned)a.total;
+        const unsigned cc = cv[nt] ? c : 0u;
+        const unsigned o = cc / (unsigned)a.inner;
+        const int i = (int)(cc - o * (unsigned)a.inner);
+        bp[nt] = a.in + ((long long)o * n + q) * a.inner + i;
         tp[nt] = TWO ? a.mult + (long long)q * a.inner + i : nullptr;
       }
     }
@@ -184,8 +190,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   for (long long wt = gw; wt < a.n_tiles; wt += gstride) {
     int rhs = 0, rb = 0;
     if (XMODE) {
-      rhs = (int)(wt / a.tiles_per_rhs);
-      rb = (int)(wt - (long long)rhs * a.tiles_per_rhs);
+      rhs = (int)((unsigned)wt / (unsigned)a.tiles_per_rhs);
+      rb = (int)wt - rhs * a.tiles_per_rhs;
     }
     double acc[MTOT][NT][2];
 #pragma unroll
@@ -234,12 +240,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
     } else {
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const long long c = wt * (8 * NT) + 8 * nt + 2 * q;
+        const unsigned c = (unsigned)wt * (8 * NT) + 8 * nt + 2 * q;
         if (a.vec2) {
-          if (c < a.total) {
-            const long long o = c / a.inner;
-            const int i = (int)(c - o * a.inner);
-            double* dst = a.out + (o * n + g) * a.inner + i;
+          if (c < (unsigned)a.total) {
+            const unsigned o = c / (unsigned)a.inner;
+            const int i = (int)(c - o * (unsigned)a.inner);
+            double* dst = a.out + ((long long)o * n + g) * a.inner + i;
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
               if (8 * mt + g < n)
@@ -250,11 +256,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
         } else {
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
-            const long long ce = c + e;
-            if (ce < a.total) {
-              const long long o = ce / a.inner;
-              const int i = (int)(ce - o * a.inner);
-              double* dst = a.out + (o * n + g) * a.inner + i;
+            const unsigned ce = c + e;
+            if (ce < (unsigned)a.total) {
+              const unsigned o = ce / (unsigned)a.inner;
+              const int i = (int)(ce - o * (unsigned)a.inner);
+              double* dst = a.out + ((long long)o * n + g) * a.inner + i;
 #pragma unroll
               for (int mt = 0; mt < MTOT; ++mt) {
                 if (8 * mt + g < n) dst[(long long)(8 * mt) * a.inner] = acc[mt][nt][e];
@@ -283,17 +289,43 @@ inline bool pick_class(int n, int* mtot, int* nt) {
   return true;
 }
 
+// EXX_NO_PDL=1 disables programmatic dependent launch (debug / A-B measurements)
+inline bool use_pdl() {
+  static const bool on = [] {
+    const char* e = getenv("EXX_NO_PDL");
+    return !(e && e[0] == '1');
+  }();
+  return on;
+}
+
 template <int MTOT, int NT>
 cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int grid, cudaStream_t s) {
   constexpr size_t smem_v = sizeof(double) * 8 * MTOT * (8 * MTOT + 4);
 #define EXX_LAUNCH(XM, FW, PDD)                                                                         \
   do {                                                                                                  \
-    const size_t smem = smem_v + (size_t)kWarps * kRing * NT * ((PDD) ? 2 : 1) * 256;                   \
+    /* at least half of the SM's shared memory, so that exactly one CTA fits per SM: the work split      \
+       assumes one persistent CTA per SM, and with programmatic dependent launch the block scheduler     \
+       would otherwise double up early-launched CTAs on whichever SMs free up first */                  \
+    const size_t smem_need = smem_v + (size_t)kWarps * kRing * NT * ((PDD) ? 2 : 1) * 256;              \
+    const size_t smem = smem_need > kMinSmem ? smem_need : kMinSmem;                                    \
     auto kern = k_mode_w<MTOT, NT, XM, FW, PDD>;                                                        \
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-    if (e != cudaSuccess) return e;                                                                     \
-    kern<<<grid, kThreads, smem, s>>>(a);                                                               \
-    return cudaGetLastError();                                                                          \
+    static bool attr_set = false; /* per instantiation; plans on one device share it */                \
+    if (!attr_set) {                                                                                    \
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+      if (e != cudaSuccess) return e;                                                                   \
+      attr_set = true;                                                                                  \
+    }                                                                                                   \
+    cudaLaunchConfig_t cfg = {};                                                                        \
+    cfg.gridDim = dim3(grid);                                                                           \
+    cfg.blockDim = dim3(kThreads);                                                                      \
+    cfg.dynamicSmemBytes = smem;                                                                        \
+    cfg.stream = s;                                                                                     \
+    cudaLaunchAttribute at[1];                                                                          \
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                      \
+    at[0].val.programmaticStreamSerializationAllowed = 1;                                               \
+    cfg.attrs = at;                                                                                     \
+    cfg.numAttrs = use_pdl() ? 1 : 0;                                                                   \
+    return cudaLaunchKernelEx(&cfg, kern, a);                                                           \
   } while (0)
   if (xmode) {
     if (fwd && two) EXX_LAUNCH(true, true, true);
@@ -350,6 +382,7 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
     a.vec2 = (aligned && inner % 2 == 0) ? 1 : 0;
   }
   if (a.n_tiles <= 0) return cudaSuccess;
+  if (a.total >= (1LL << 31) - 64 || a.n_tiles >= (1LL << 31) - 64) return cudaErrorNotSupported;  // 32-bit tile math
   const long long ctas = (a.n_tiles + kWarps - 1) / kWarps;
   const int grid = (int)(ctas < p->sm_count ? ctas : p->sm_count);
   switch (mtot) {
