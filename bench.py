@@ -202,7 +202,8 @@ def run_b200(args):
     psi, occ, tgt, occ_t = wl.make_inputs(w, gen_dev)
     d_psi, d_occ = psi.to(dev), occ.to(dev)
     # weak scaling: rank r applies Vx to n_tgt targets starting at tgt_start + r*n_tgt (wrapping)
-    idx = (w.tgt_start + rank * w.n_tgt + torch.arange(w.n_tgt)) % w.n_orb
+    from paper_2501_16572_b200 import sharding
+    idx = sharding.weak_scaling_targets(w.tgt_start, w.n_tgt, w.n_orb, rank)
     if world == 1:
         d_tgt = d_psi[w.tgt_start:w.tgt_start + w.n_tgt]
         d_occ_t = d_occ[w.tgt_start:w.tgt_start + w.n_tgt]
@@ -210,7 +211,7 @@ def run_b200(args):
         d_tgt = d_psi[idx.to(dev)].contiguous()
         d_occ_t = d_occ[idx.to(dev)].contiguous()
 
-    plan = exx.Plan.for_workload(w, max_batch=max(64, n_c), device=local)
+    plan = exx.Plan.for_workload(w, max_batch=max(128, n_c), device=local)
     plan.set_variant(args.variant)
     vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)

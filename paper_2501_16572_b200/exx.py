@@ -132,7 +132,7 @@ class Plan:
     @classmethod
     def for_workload(cls, w, max_batch=None, device=0):
         return cls(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega,
-                   max_batch if max_batch is not None else max(64, w.default_nc), device)
+                   max_batch if max_batch is not None else max(128, w.default_nc), device)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
