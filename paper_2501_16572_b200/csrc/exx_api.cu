@@ -100,7 +100,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0;
   p->prof_on = false;
-  for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; }
+  for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; }
 
   try {
     for (int a = 0; a < 3; ++a) {

@@ -45,6 +45,7 @@ struct exx_plan {
   std::vector<double> h_mult;
   // device copies
   double* d_V[3];    // row-major [i][m], n*n (axes with identical matrices share one allocation)
+  double* d_Vpad[3]; // zero-padded shared-memory images of V for the DMMA kernels (kernels_dmma.cu)
   double* d_mult;    // N
   int sm_count;
   int smem_optin;

@@ -63,10 +63,32 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
+// Exact n / d for n < 2^31 with a host-computed multiplier (d = 2^shift when mul == 0).
+struct FastDiv {
+  unsigned mul;
+  int shift;
+  unsigned d;
+};
+inline FastDiv make_fastdiv(unsigned d) {
+  FastDiv f{0u, 0, d};
+  if ((d & (d - 1)) == 0) {  // power of two (d >= 1)
+    while ((1u << f.shift) < d) ++f.shift;
+    return f;
+  }
+  int L = 0;
+  while ((1ull << L) < d) ++L;  // ceil(log2 d)
+  f.mul = (unsigned)(((1ull << (31 + L)) / d) + 1ull);
+  f.shift = L - 1;
+  return f;
+}
+__device__ __forceinline__ unsigned fast_div(unsigned n, const FastDiv& f) {
+  return f.mul ? (__umulhi(n, f.mul) >> f.shift) : (n >> f.shift);
+}
+
 struct WArgs {
   const double* in;
   double* out;
-  const double* V;     // row-major [i][m], n x n
+  const double* V;     // zero-padded image [8*MTOT][8*MTOT+4] of the row-major eigenvector matrix
   const double* mult;  // optional (L-mode): table indexed [m*inner + i]
   const double* psi;   // PD only
   const double* tgt;   // PD only
@@ -80,6 +102,8 @@ struct WArgs {
   long long N;           // points per right-hand side
   BatchDesc bd;          // PD only
   int vec2;              // L-mode: 16-byte stores are aligned
+  FastDiv div_inner;     // L-mode: / inner
+  FastDiv div_tiles;     // X-mode: / tiles_per_rhs
 };
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
@@ -93,12 +117,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   const int g = lane >> 2, q = lane & 3;
   const int n = a.n, KT = a.KT;
 
-  // ---- stage V once per CTA: zero padding (k >= n must contribute exact zeros), then the n x n block ----
-  for (int i = tid; i < 8 * MTOT * LDV; i += kThreads) Vs[i] = 0.0;
-  __syncthreads();
-  for (int i = tid; i < n * n; i += kThreads) {
-    const int r = i / n, c = i - r * n;
-    Vs[r * LDV + c] = a.V[i];
+  // ---- stage V once per CTA: the plan holds a zero-padded image in exactly this layout (k >= n must
+  // contribute exact zeros), so staging is one burst of 16-byte asynchronous copies ----------------------
+  {
+    const unsigned vs0 = (unsigned)__cvta_generic_to_shared(Vs);
+    for (int i = 2 * tid; i < 8 * MTOT * LDV; i += 2 * kThreads)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(vs0 + 8u * i), "l"(a.V + i) : "memory");
+    cp_async_commit();
+    cp_async_wait<0>();
   }
   __syncthreads();
   // Programmatic dependent launch: everything above touched only the plan's constant V, so it overlaps
@@ -127,32 +153,42 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   // X-mode (pair density, a1), the multiplier table in L-mode (a3, applied while loading the z-backward pass).
   auto setup = [&](long long wt, const double* (&bp)[NT], const double* (&tp)[NT], bool (&cv)[NT]) {
     if (XMODE) {
-      const int rhs = (int)((unsigned)wt / (unsigned)a.tiles_per_rhs);
+      const int rhs = (int)fast_div((unsigned)wt, a.div_tiles);
       const int rb = (int)wt - rhs * a.tiles_per_rhs;
+      const double* base0 = nullptr;
+      const double* base1 = nullptr;
+      if (TWO) {
+        const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
+        base0 = a.psi + (long long)j * a.N;
+        base1 = a.tgt + (long long)k * a.N;
+      } else {
+        base0 = a.in + (long long)rhs * a.N;
+      }
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
         const int rr = rb * 8 * NT + 8 * nt + g;
         cv[nt] = rr < a.rows_per_rhs;
-        const long long off = (long long)(cv[nt] ? rr : 0) * n + q;
-        if (TWO) {
-          const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
-          bp[nt] = a.psi + (long long)j * a.N + off;
-          tp[nt] = a.tgt + (long long)k * a.N + off;
-        } else {
-          bp[nt] = a.in + (long long)rhs * a.N + off;
-          tp[nt] = nullptr;
-        }
+        const int off = (cv[nt] ? rr : 0) * n + q;
+        bp[nt] = base0 + off;
+        tp[nt] = TWO ? base1 + off : nullptr;
       }
     } else {
+      // columns wt*8NT + 8nt + g: one division for the first, the rest by stepping 8 with carry
+      unsigned c = (unsigned)wt * (8 * NT) + g;               // host guarantees total < 2^31
+      const unsigned cfirst = c < (unsigned)a.total ? c : 0u;
+      unsigned o = fast_div(cfirst, a.div_inner);
+      int i = (int)(cfirst - o * (unsigned)a.inner);
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const unsigned c = (unsigned)wt * (8 * NT) + 8 * nt + g;   // host guarantees total < 2^31
         cv[nt] = c < (unsigned)a.total;
-        const unsigned cc = cv[nt] ? c : 0u;
-        const unsigned o = cc / (unsigned)a.inner;
-        const int i = (int)(cc - o * (unsigned)a.inner);
         bp[nt] = a.in + ((long long)o * n + q) * a.inner + i;
         tp[nt] = TWO ? a.mult + (long long)q * a.inner + i : nullptr;
+        c += 8;
+        i += 8;
+        while (i >= a.inner) {
+          i -= a.inner;
+          ++o;
+        }
       }
     }
   };
@@ -190,7 +226,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
   for (long long wt = gw; wt < a.n_tiles; wt += gstride) {
     int rhs = 0, rb = 0;
     if (XMODE) {
-      rhs = (int)((unsigned)wt / (unsigned)a.tiles_per_rhs);
+      rhs = (int)fast_div((unsigned)wt, a.div_tiles);
       rb = (int)wt - rhs * a.tiles_per_rhs;
     }
     double acc[MTOT][NT][2];
@@ -237,34 +273,43 @@ __global__ void __launch_bounds__(kThreads, 1) k_mode_w(const WArgs a) {
           }
         }
       }
+    } else if (a.vec2) {
+      // inner is even and c is even, so the pair (c, c+1) never straddles a row of the flattened index
+      unsigned c = (unsigned)wt * (8 * NT) + 2 * q;
+      const unsigned cfirst = c < (unsigned)a.total ? c : 0u;
+      unsigned o = fast_div(cfirst, a.div_inner);
+      int i = (int)(cfirst - o * (unsigned)a.inner);
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+        if (c < (unsigned)a.total) {
+          double* dst = a.out + ((long long)o * n + g) * a.inner + i;
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) {
+            if (8 * mt + g < n)
+              *reinterpret_cast<double2*>(dst + (long long)(8 * mt) * a.inner) =
+                  make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+          }
+        }
+        c += 8;
+        i += 8;
+        while (i >= a.inner) {
+          i -= a.inner;
+          ++o;
+        }
+      }
     } else {
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) {
-        const unsigned c = (unsigned)wt * (8 * NT) + 8 * nt + 2 * q;
-        if (a.vec2) {
-          if (c < (unsigned)a.total) {
-            const unsigned o = c / (unsigned)a.inner;
-            const int i = (int)(c - o * (unsigned)a.inner);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const unsigned ce = (unsigned)wt * (8 * NT) + 8 * nt + 2 * q + e;
+          if (ce < (unsigned)a.total) {
+            const unsigned o = fast_div(ce, a.div_inner);
+            const int i = (int)(ce - o * (unsigned)a.inner);
             double* dst = a.out + ((long long)o * n + g) * a.inner + i;
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
-              if (8 * mt + g < n)
-                *reinterpret_cast<double2*>(dst + (long long)(8 * mt) * a.inner) =
-                    make_double2(acc[mt][nt][0], acc[mt][nt][1]);
-            }
-          }
-        } else {
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const unsigned ce = c + e;
-            if (ce < (unsigned)a.total) {
-              const unsigned o = ce / (unsigned)a.inner;
-              const int i = (int)(ce - o * (unsigned)a.inner);
-              double* dst = a.out + ((long long)o * n + g) * a.inner + i;
-#pragma unroll
-              for (int mt = 0; mt < MTOT; ++mt) {
-                if (8 * mt + g < n) dst[(long long)(8 * mt) * a.inner] = acc[mt][nt][e];
-              }
+              if (8 * mt + g < n) dst[(long long)(8 * mt) * a.inner] = acc[mt][nt][e];
             }
           }
         }
@@ -355,7 +400,7 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
   WArgs a{};
   a.in = in;
   a.out = out;
-  a.V = p->d_V[axis];
+  a.V = p->d_Vpad[axis];
   a.mult = apply_mult ? p->d_mult : nullptr;
   a.psi = pd ? pd->psi : nullptr;
   a.tgt = pd ? pd->tgt : nullptr;
@@ -381,6 +426,8 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
     const bool aligned = (((uintptr_t)out) & 15) == 0;
     a.vec2 = (aligned && inner % 2 == 0) ? 1 : 0;
   }
+  a.div_inner = make_fastdiv((unsigned)a.inner);
+  a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
   if (a.n_tiles <= 0) return cudaSuccess;
   if (a.total >= (1LL << 31) - 64 || a.n_tiles >= (1LL << 31) - 64) return cudaErrorNotSupported;  // 32-bit tile math
   const long long ctas = (a.n_tiles + kWarps - 1) / kWarps;
@@ -398,8 +445,39 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
 
 }  // namespace
 
-cudaError_t fast_init(exx_plan*) { return cudaSuccess; }
-void fast_destroy(exx_plan*) {}
+// Upload, per axis, the zero-padded shared-memory image of V that k_mode_w stages verbatim.
+cudaError_t fast_init(exx_plan* p) {
+  for (int ax = 0; ax < 3; ++ax) {
+    p->d_Vpad[ax] = nullptr;
+    int mtot, nt;
+    if (!pick_class(p->n[ax], &mtot, &nt)) continue;  // this axis runs on the plain kernel
+    int same = -1;
+    for (int b = 0; b < ax; ++b)
+      if (p->d_V[b] == p->d_V[ax] && p->d_Vpad[b]) same = b;
+    if (same >= 0) {
+      p->d_Vpad[ax] = p->d_Vpad[same];
+      continue;
+    }
+    const int n = p->n[ax], rows = 8 * mtot, ldv = 8 * mtot + 4;
+    std::vector<double> img((size_t)rows * ldv, 0.0);
+    for (int r = 0; r < n; ++r)
+      for (int c = 0; c < n; ++c) img[(size_t)r * ldv + c] = p->h_V[ax][(size_t)r * n + c];
+    cudaError_t e = cudaMalloc(&p->d_Vpad[ax], sizeof(double) * img.size());
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpy(p->d_Vpad[ax], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+void fast_destroy(exx_plan* p) {
+  for (int ax = 0; ax < 3; ++ax) {
+    bool shared = false;
+    for (int b = 0; b < ax; ++b) shared |= (p->d_Vpad[b] == p->d_Vpad[ax]);
+    if (!shared && p->d_Vpad[ax]) cudaFree(p->d_Vpad[ax]);
+  }
+  for (int ax = 0; ax < 3; ++ax) p->d_Vpad[ax] = nullptr;
+}
 
 // Axes longer than 128 points do not fit the resident-V kernels; they run on the plain DFMA kernel
 // (still CUDA, still in the library; stated in DESIGN.md).  `scratch` is only needed in that case.
