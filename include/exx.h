@@ -59,8 +59,10 @@ enum { EXX_BC_PERIODIC = 0, EXX_BC_DIRICHLET = 1 };
 
 /* Kernel variants (test hook; the default is the fast path). */
 enum {
-  EXX_VARIANT_FUSED_DMMA = 0, /* tensor-core (mma.sync f64 -> DMMA) mode products, fused passes */
-  EXX_VARIANT_REFERENCE = 1   /* one plain DFMA kernel per mode product; slow, for cross-checks  */
+  EXX_VARIANT_FUSED_DMMA = 0, /* tensor-core (mma.sync f64 -> DMMA) mode products, operands staged by TMA */
+  EXX_VARIANT_REFERENCE = 1,  /* one plain DFMA kernel per mode product; slow, for cross-checks        */
+  EXX_VARIANT_CPASYNC = 2     /* DMMA mode products with per-lane cp.async staging (first generation;  */
+                              /* also what variant 0 uses for sizes TMA cannot address, e.g. odd nx)   */
 };
 
 /*
@@ -124,6 +126,11 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
 
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);
+
+/* Test hook: how many mode-product launches of this plan, since it was created, went through the TMA-staged
+ * kernels (the default path; sizes TMA cannot address -- odd nx, an axis longer than 128 points, buffers not
+ * 16-byte aligned -- use the cp.async or plain kernels instead, still on the GPU). */
+long long exx_plan_tma_launch_count(const exx_plan* plan);
 
 /*
  * Per-kernel-class timing (bench instrumentation).  With profiling on, every kernel the library launches

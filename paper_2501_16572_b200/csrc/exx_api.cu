@@ -98,7 +98,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->h = h; p->order = fd_order; p->omega = omega; p->max_batch = max_batch; p->device = device;
   p->variant = EXX_VARIANT_FUSED_DMMA;
   p->N = (long long)nx * ny * nz;
-  p->d_mult = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0;
+  p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->tma_launches = 0;
   p->prof_on = false;
   for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; }
 
@@ -146,6 +146,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
     if (e == cudaSuccess)
       e = cudaMalloc(&p->ex.d_energy_scratch, sizeof(double) * kEnergyChunk * kEnergyBlocks);
     if (e == cudaSuccess) e = exx::fast_init(p);
+    if (e == cudaSuccess) e = exx::tma_init(p);
     if (e != cudaSuccess) {
       exx_plan_destroy(p);
       return e == cudaErrorMemoryAllocation ? EXX_ERR_ALLOC : cuda_fail(e);
@@ -161,6 +162,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
   if (p->device >= 0) {
     cudaSetDevice(p->device);
     exx::fast_destroy(p);
+    exx::tma_destroy(p);
     for (int a = 0; a < 3; ++a) {
       bool shared = false;
       for (int b = 0; b < a; ++b) shared |= (p->d_V[b] == p->d_V[a]);
@@ -176,7 +178,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
 }
 
 exx_status exx_plan_set_variant(exx_plan* plan, int variant) {
-  if (!plan || (variant != EXX_VARIANT_FUSED_DMMA && variant != EXX_VARIANT_REFERENCE))
+  if (!plan || (variant != EXX_VARIANT_FUSED_DMMA && variant != EXX_VARIANT_REFERENCE && variant != EXX_VARIANT_CPASYNC))
     return EXX_ERR_INVALID_ARG;
   plan->variant = variant;
   return EXX_OK;
@@ -206,6 +208,8 @@ exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult) {
 }
 
 long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }
+
+long long exx_plan_tma_launch_count(const exx_plan* plan) { return plan ? plan->tma_launches : 0; }
 
 exx_status exx_plan_set_profiling(exx_plan* plan, int on) {
   if (!plan) return EXX_ERR_INVALID_ARG;
@@ -339,7 +343,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
           }
           launches += 2;
         } else {
-          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, j0 == 0};
+          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0};
           EXX_CUDA(exx::fast_solve_batch(plan, nullptr, buf0, buf1, nb, &fa, s, &launches));
         }
       }

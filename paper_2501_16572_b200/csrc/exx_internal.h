@@ -47,9 +47,11 @@ struct exx_plan {
   double* d_V[3];    // row-major [i][m], n*n (axes with identical matrices share one allocation)
   double* d_Vpad[3]; // zero-padded shared-memory images of V for the DMMA kernels (kernels_dmma.cu)
   double* d_mult;    // N
+  void* tma_state;   // TMA-staged kernels: permuted V images and the tensor-map cache (kernels_tma.cu)
   int sm_count;
   int smem_optin;
   long long last_launches;
+  long long tma_launches;  // cumulative count of TMA-staged mode-product launches (test hook)
   // optional per-kernel-class CUDA-event timing (exx_plan_set_profiling)
   bool prof_on;
   std::vector<exx::ProfRec> prof;
@@ -104,8 +106,14 @@ struct FastArgs {
   const double* occ;
   double* vx;
   BatchDesc bd;
+  int n_occ, n_tgt;  // extents of psi / tgt (tensor maps cover the whole arrays)
   bool first;  // first batch for these targets: vx is overwritten, not accumulated into
 };
+// ---- TMA-staged mode products (kernels_tma.cu), the default; cudaErrorNotSupported -> cp.async kernels ----
+cudaError_t tma_init(exx_plan* p);
+void tma_destroy(exx_plan* p);
+cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s);
 cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,
                              const FastArgs* fa, cudaStream_t s, long long* launches);
 

@@ -487,7 +487,11 @@ static cudaError_t one_product(exx_plan* p, int axis, bool fwd, const double* sr
                                int nb, bool& mult_pending, cudaStream_t s) {
   ProfScope ps(p, KC_MODE_PRODUCT, s);
   const bool z_bwd = axis == 2 && !fwd;
-  cudaError_t e = fast_mode_product(p, axis, fwd, src, cur, nb, z_bwd && mult_pending, nullptr, s);
+  cudaError_t e = cudaErrorNotSupported;
+  if (p->variant == EXX_VARIANT_FUSED_DMMA)
+    e = tma_mode_product(p, axis, fwd, src, cur, nb, z_bwd && mult_pending, nullptr, s);
+  if (e == cudaErrorNotSupported)
+    e = fast_mode_product(p, axis, fwd, src, cur, nb, z_bwd && mult_pending, nullptr, s);
   if (e == cudaSuccess) {
     if (z_bwd) mult_pending = false;
     return e;
@@ -518,7 +522,9 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
     // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
       ProfScope ps(p, KC_MODE_PRODUCT, s);
-      e = fast_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
+      e = cudaErrorNotSupported;
+      if (p->variant == EXX_VARIANT_FUSED_DMMA) e = tma_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
+      if (e == cudaErrorNotSupported) e = fast_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
     }
     if (e == cudaSuccess) {
       first_done = true;

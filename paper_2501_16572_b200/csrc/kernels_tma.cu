@@ -1,0 +1,617 @@
+// Default variant (EXX_VARIANT_FUSED_DMMA): mode products on the FP64 tensor pipe, operands staged by TMA.
+//
+// Every mode product of Eq. 11 is "a small stationary matrix times a very wide one":
+// out[:, c] = M in[:, c], M = V^T (forward) or V (backward), n x n with n <= 128, c running over N*n_c/n
+// columns.  What the measurements of the first-generation kernel (kernels_dmma.cu, profiles/
+// r1_cfg2_cpasync_ncu.md) say bounds it: not the DMMA pipe but everything around it -- per-lane 8-byte
+// LDGSTS copies (8 L1 wavefronts per 256 B), their 64-bit address arithmetic (5 other instructions per
+// DMMA), and only two warps per scheduler to hide it.  This kernel removes that work from the SM's issue
+// slots instead of tuning it:
+//   * The streamed operand arrives by TMA (cp.async.bulk.tensor, SASS UTMALDG): one elected lane per warp
+//     issues one or two box copies per 16 contraction indices; hardware computes the addresses, clips
+//     ragged edges (out-of-bounds elements arrive as zeros) and signals an mbarrier.  No LSU wavefronts,
+//     no per-lane pointers, no predicates.
+//   * Boxes are 16 doubles (128 B) wide and land with the hardware 128-byte swizzle, so the B-fragment
+//     reads are bank-conflict free without padding.  The order of the contraction index inside a block of
+//     16 is free (it is a sum), so the k <-> lane assignment is chosen to fit the swizzle and the rows of the
+//     plan's shared-memory image of V are permuted to match (tma_init).  Forward/backward and the axis only
+//     change that image: the kernel has no FWD/BWD variants.
+//   * Warps stay fully independent (a warp owns 8*NT columns for all n output rows; its accumulators never
+//     leave registers): each warp runs its own two-stage mbarrier pipeline, there is no block barrier in
+//     the steady state.  With the address work gone the kernel fits 12-16 warps per SM (3-4 per scheduler)
+//     instead of 8, which is what keeps the DMMA pipe fed while a warp waits, stores or sets up a tile.
+//   * Fused into the passes as before: the pair density psi_j*tgt_k (a1) as a second TMA stream of the first
+//     product, the multiplier f(Lambda~) (a3) as a second stream of the z-backward product.
+//
+// L-mode (axis y or z; contracted index strided by `inner`): the operand is the 3-D tensor
+// [outer][n][inner]; a warp tile is NT/2 chunks of 16 consecutive inner-columns, a stage is a
+// {16 cols, 16 rows} box per chunk.  X-mode (axis x; contracted index contiguous): the transposed product
+// out^T = M in^T, the operand is the 2-D tensor [rows][n]; a warp tile is 8*NT rows, a stage is a
+// {16 x, 8*NT rows} box.
+//
+// The paper's four data reorganisations (Eqs. 12-15) do not exist here: they are
+// artefacts of calling a 2-D GEMM library and are replaced by tensor-map strides.
+#include <cuda.h>  // CUtensorMap and its enums only; cuTensorMapEncodeTiled is resolved at run time
+
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+
+#include "exx_internal.h"
+
+namespace exx {
+namespace {
+
+constexpr int kDepth = 2;  // ring depth in stages of 16 contraction indices (4 k-steps, >= 96 DMMAs each)
+
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+      : "+d"(c[0]), "+d"(c[1])
+      : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double lds64(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+// Blocks until the phase with the given parity has completed.  A bounded spin turns a lost transaction (a
+// bug) into a trap instead of a hung GPU.
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  unsigned done = 0;
+  for (unsigned spin = 0; !done; ++spin) {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (spin > (1u << 24)) __trap();
+  }
+}
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+      "l"(tm), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int c0, int c1, int c2,
+                                            unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(
+          dst),
+      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+      : "memory");
+}
+
+// Exact n / d for n < 2^31 with a host-computed multiplier (d = 2^shift when mul == 0).
+struct FastDiv {
+  unsigned mul;
+  int shift;
+};
+inline FastDiv make_fastdiv(unsigned d) {
+  FastDiv f{0u, 0};
+  if ((d & (d - 1)) == 0) {
+    while ((1u << f.shift) < d) ++f.shift;
+    return f;
+  }
+  int L = 0;
+  while ((1ull << L) < d) ++L;
+  f.mul = (unsigned)(((1ull << (31 + L)) / d) + 1ull);
+  f.shift = L - 1;
+  return f;
+}
+__device__ __forceinline__ unsigned fast_div(unsigned n, const FastDiv& f) {
+  return f.mul ? (__umulhi(n, f.mul) >> f.shift) : (n >> f.shift);
+}
+
+struct TArgs {
+  double* out;
+  const double* V;  // permuted, zero-padded image [16*S][8*MTOT+4] (tma_init)
+  int n;
+  int S;        // stages per tile = ceil(n/16)
+  int kk_last;  // k-steps of the last stage that touch indices < n
+  unsigned n_tiles;
+  // L-mode
+  int inner;              // contiguous run below the contracted axis
+  int cpo;                // chunks of 16 columns per outer index = ceil(inner/16)
+  unsigned total_chunks;  // cpo * outer
+  int outer;
+  FastDiv div_cpo;
+  // X-mode
+  int rows_per_rhs;   // N / nx
+  int tiles_per_rhs;  // pair density only: ceil(rows_per_rhs / (8*NT))
+  int rows_total;     // rows of the output tensor
+  FastDiv div_tiles;
+  BatchDesc bd;  // pair density only
+};
+
+// MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_t(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const TArgs a) {
+  static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
+  constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): the A-fragment reads are bank-conflict free
+  constexpr int NS = TWO ? 2 : 1;    // two streams are staged separately and multiplied on consumption
+  constexpr unsigned kStage = 1024u * NT;  // bytes per stage and stream: 16 x (8*NT) doubles
+  constexpr int CH = NT / 2;               // L-mode: 16-column chunks per tile
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, S = a.S;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * S) * LDV;
+
+  // ---- stage the V image once per CTA (one burst of 16-byte asynchronous copies) -------------------------
+  for (unsigned i = 2 * tid; i < 16u * S * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;  // swizzled boxes need 1024-byte alignment
+  const unsigned my_ring = ring0 + warp * (kDepth * NS * kStage);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * NS * kStage) + warp * (kDepth * 8u);
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+  // Programmatic dependent launch: everything above touched only plan constants, so it overlaps the tail
+  // of the previous pass; from here on we read that pass's output.
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  // Tile t of this launch belongs to warp (b, w) = (t % grid, (t / grid) % WARPS): a ragged last round is
+  // spread over all SMs and, inside an SM, over all four schedulers.
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  const unsigned tstride = gridDim.x * WARPS;
+
+  // ---- producer (lane 0 of each warp): runs kDepth stages ahead, straight across tile boundaries ---------
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pc0[CH], pc2[CH];  // L-mode: column and outer coordinate of each chunk
+  int pr0 = 0, pr1 = 0;  // X-mode: first row in tm0 / tm1
+  auto tile_coords = [&](unsigned t) {
+    if (XMODE) {
+      if (TWO) {
+        const int rhs = (int)fast_div(t, a.div_tiles);
+        const int rb = (int)t - rhs * a.tiles_per_rhs;
+        const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
+        pr0 = j * a.rows_per_rhs + rb * (8 * NT);
+        pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+      } else {
+        pr0 = (int)t * (8 * NT);
+      }
+    } else {
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) {
+        const unsigned cc = t * CH + ch;
+        if (cc < a.total_chunks) {
+          const unsigned o = fast_div(cc, a.div_cpo);
+          pc2[ch] = (int)o;
+          pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
+        } else {  // past the end: an all-out-of-bounds box (zeros), never stored
+          pc2[ch] = a.outer;
+          pc0[ch] = 0;
+        }
+      }
+    }
+  };
+  auto produce = [&](int slot) {  // lane 0 only
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * (NS * kStage);
+    mbar_expect_tx(bar, NS * kStage);
+    if (XMODE) {
+      tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
+      if (TWO) tma_load_2d(dst + kStage, &tm1, 16 * s_p, pr1, bar);
+    } else {
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) {
+        tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
+        if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * s_p, 0, bar);
+      }
+    }
+    if (++s_p == S) {
+      s_p = 0;
+      t_p += tstride;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (lane == 0) {
+    if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) produce(d);
+  }
+
+  // ---- per-lane fragment addresses --------------------------------------------------------------------
+  // A fragment (M[m][k]) of (stage s, k-step kk, row tile mt): image row 16s + 4kk + q, column 8mt + g.
+  const unsigned a_base = smem0 + 8u * (q * LDV + g);
+  // B fragment of (k-step kk, column tile nt) inside a stage, 128-byte swizzle (16-byte chunk index XOR row%8):
+  //   X-mode: box row 8nt+g (a data row), x = (q&1) + 8(q>>1) + 2kk      -> xo[kk] + 1024 nt
+  //   L-mode: box row 2q + (kk&1) + 8(kk>>1) (a contraction index), column 8(nt&1)+g of chunk nt>>1
+  //                                                                       -> xo[2(nt&1) + (kk&1)] + 2048 (nt>>1) + 1024 (kk>>1)
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (XMODE) {
+      xo[i] = 128u * g + 16u * ((4u * (q >> 1) + i) ^ (unsigned)g) + 8u * (q & 1);
+    } else {
+      const unsigned row = 2u * q + (i & 1);
+      xo[i] = 128u * row + 16u * ((4u * (i >> 1) + (g >> 1)) ^ row) + 8u * (g & 1);
+    }
+  }
+
+  int slot = 0;
+  unsigned parity = 0;
+  for (unsigned t = tfirst; t < a.n_tiles; t += tstride) {
+    double acc[MTOT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+    for (int s = 0; s < S; ++s) {
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * (NS * kStage);
+      const unsigned aa = a_base + (unsigned)s * (16u * LDV * 8u);
+      const int nk = (s == S - 1) ? a.kk_last : 4;
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (kk < nk) {
+          double bf[NT];
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            const unsigned off = XMODE ? (sb + xo[kk] + 1024u * nt)
+                                       : (sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1));
+            bf[nt] = lds64(off);
+            if (TWO) bf[nt] *= lds64(off + kStage);
+          }
+          double af[MTOT];
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+        }
+      }
+      // every lane's reads of this stage have completed (their values fed the DMMAs above): refill it
+      __syncwarp();
+      if (lane == 0) produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+
+    // ---- epilogue: C[m = 8mt+g][column 8nt + 2q + e] straight from the fragments (every pass is in place) --
+    if (XMODE) {
+      int row0, limit;
+      if (TWO) {
+        const int rhs = (int)fast_div(t, a.div_tiles);
+        const int rb = (int)t - rhs * a.tiles_per_rhs;
+        row0 = rhs * a.rows_per_rhs + rb * (8 * NT);
+        limit = (rhs + 1) * a.rows_per_rhs;
+      } else {
+        row0 = (int)t * (8 * NT);
+        limit = a.rows_total;
+      }
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int r = row0 + 8 * nt + 2 * q + e;
+          if (r < limit) {
+            double* dst = a.out + (long long)r * n + g;
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt)
+              if (8 * mt + g < n) dst[8 * mt] = acc[mt][nt][e];
+          }
+        }
+      }
+    } else {
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) {
+        const unsigned cc = t * CH + ch;
+        if (cc < a.total_chunks) {
+          const unsigned o = fast_div(cc, a.div_cpo);
+          const int col0 = 16 * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
+          double* base = a.out + ((long long)o * n + g) * a.inner + col0;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const int nt = 2 * ch + h;
+            if (col0 + 8 * h < a.inner) {  // inner is even, so the pair (c, c+1) is inside or outside together
+#pragma unroll
+              for (int mt = 0; mt < MTOT; ++mt)
+                if (8 * mt + g < n)
+                  *reinterpret_cast<double2*>(base + (long long)(8 * mt) * a.inner + 8 * h) =
+                      make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+// ---- host side ----------------------------------------------------------------------------------------
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess ||
+        qr != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+
+struct MapKey {
+  const void* base;
+  unsigned long long d0, d1, d2;
+  unsigned b1;  // box rows (box is always 16 wide; third box dimension 1)
+  bool operator==(const MapKey& o) const {
+    return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b1 == o.b1;
+  }
+};
+struct MapEntry {
+  MapKey key;
+  CUtensorMap map;
+};
+
+struct TmaState {
+  double* d_img[3][2];  // [axis][0 = forward (V^T), 1 = backward (V)]
+  bool img_owned[3][2];
+  std::vector<MapEntry> cache;
+};
+
+// supported classes of ceil(n/8), the columns-per-warp choice and the warps per CTA for each
+struct ClassCfg {
+  int mtot, nt, warps, warps_two;
+};
+inline bool pick_class(int n, ClassCfg* c) {
+  const int need = (n + 7) / 8;
+  if (need <= 2) *c = {2, 4, 16, 12};
+  else if (need <= 4) *c = {4, 4, 16, 12};
+  else if (need <= 6) *c = {6, 4, 16, 12};
+  else if (need <= 8) *c = {8, 4, 12, 8};
+  else if (need <= 12) *c = {12, 2, 12, 12};
+  else if (need <= 15) *c = {15, 2, 12, 12};
+  else if (need <= 16) *c = {16, 2, 12, 8};
+  else return false;
+  return true;
+}
+
+// 2-D ([d1][d0]) or 3-D ([d2][d1][d0]) FP64 tensor, box {16, box_rows(, 1)}, 128-byte swizzle, zero fill.
+cudaError_t get_map(TmaState* st, const void* base, unsigned long long d0, unsigned long long d1,
+                    unsigned long long d2, unsigned box_rows, CUtensorMap* out) {
+  const MapKey key{base, d0, d1, d2, box_rows};
+  for (const auto& e : st->cache)
+    if (e.key == key) {
+      *out = e.map;
+      return cudaSuccess;
+    }
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return cudaErrorNotSupported;
+  const cuuint32_t rank = d2 ? 3 : 2;
+  cuuint64_t gdim[3] = {d0, d1, d2 ? d2 : 1};
+  cuuint64_t gstr[2] = {d0 * 8ull, d0 * d1 * 8ull};
+  cuuint32_t box[3] = {16u, box_rows, 1u};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  alignas(64) CUtensorMap m;
+  const CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, const_cast<void*>(base), gdim, gstr, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  if (st->cache.size() >= 64) st->cache.clear();
+  st->cache.push_back(MapEntry{key, m});
+  *out = m;
+  return cudaSuccess;
+}
+
+inline bool use_pdl() {
+  static const bool on = [] {
+    const char* e = getenv("EXX_NO_PDL");
+    return !(e && e[0] == '1');
+  }();
+  return on;
+}
+
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS>
+cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, cudaStream_t s) {
+  constexpr int LDV = 8 * MTOT + 4;
+  const size_t img = sizeof(double) * 16 * (size_t)a.S * LDV;
+  // image | (alignment slack) | rings | mbarriers.  The request always exceeds half of the SM's shared memory
+  // so that exactly one CTA is resident: the tile split assumes one persistent CTA per SM.
+  size_t smem = img + 1024 + (size_t)WARPS * kDepth * (TWO ? 2 : 1) * 1024 * NT + (size_t)WARPS * kDepth * 8;
+  if (smem < 117 * 1024) smem = 117 * 1024;
+  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS>;
+  static size_t attr_smem = 0;  // per instantiation
+  if (smem > attr_smem) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_smem = smem;
+  }
+  cudaLaunchConfig_t cfg = {};
+  const unsigned grid = a.n_tiles < (unsigned)sm_count ? a.n_tiles : (unsigned)sm_count;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * WARPS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = use_pdl() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
+}
+
+template <int MTOT, int NT, int WARPS, int WARPS_TWO>
+cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a,
+                         int sm_count, cudaStream_t s) {
+  if (xmode) {
+    if (two) return launch_one<MTOT, NT, true, true, WARPS_TWO>(m0, m1, a, sm_count, s);
+    return launch_one<MTOT, NT, true, false, WARPS>(m0, m1, a, sm_count, s);
+  }
+  if (two) return launch_one<MTOT, NT, false, true, WARPS_TWO>(m0, m1, a, sm_count, s);
+  return launch_one<MTOT, NT, false, false, WARPS>(m0, m1, a, sm_count, s);
+}
+
+inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+
+}  // namespace
+
+// One mode product along `axis` for nb right-hand sides; in == out is allowed (and is the normal case).
+// pd != nullptr (axis 0, forward only): the input is psi_j .* tgt_k formed on the fly (a1).
+// apply_mult (axis 2, backward only): the input is multiplied by f(Lambda~) while it is consumed (a3).
+// cudaErrorNotSupported: sizes or alignment outside what TMA can address (odd nx, n > 128, unaligned
+// buffers, no driver entry point); the caller then uses the cp.async kernels of kernels_dmma.cu.
+cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return cudaErrorNotSupported;
+  const int n = p->n[axis];
+  ClassCfg cc;
+  if (!pick_class(n, &cc)) return cudaErrorNotSupported;
+  const double* img = st->d_img[axis][forward ? 0 : 1];
+  if (!img) return cudaErrorNotSupported;
+  if ((p->n[0] & 1) || !aligned16(out) || (in && !aligned16(in))) return cudaErrorNotSupported;
+  const bool xmode = axis == 0;
+  if (pd && !(xmode && forward)) return cudaErrorInvalidValue;
+  if (apply_mult && !(axis == 2 && !forward)) return cudaErrorInvalidValue;
+  if (pd && (!aligned16(pd->psi) || !aligned16(pd->tgt))) return cudaErrorNotSupported;
+  const bool two = pd != nullptr || apply_mult;
+  const int NT = cc.nt;
+
+  TArgs a{};
+  a.out = out;
+  a.V = img;
+  a.n = n;
+  a.S = (n + 15) / 16;
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if (xmode) {
+    const int rem = n - 16 * (a.S - 1);
+    a.kk_last = rem > 0 ? 4 : 0;  // every k-step of an X-mode stage touches both halves of the 16-block
+    a.rows_per_rhs = (int)(p->N / n);
+    const long long rows_total = (long long)a.rows_per_rhs * nb;
+    if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    a.rows_total = (int)rows_total;
+    a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+    a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+    if (pd) {
+      a.bd = pd->bd;
+      a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
+      const long long rp = (long long)a.rows_per_rhs * pd->n_occ, rt = (long long)a.rows_per_rhs * pd->n_tgt;
+      if (rp >= (1LL << 31) - 64 || rt >= (1LL << 31) - 64) return cudaErrorNotSupported;
+      if ((e = get_map(st, pd->psi, n, rp, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+      if ((e = get_map(st, pd->tgt, n, rt, 0, 8 * NT, &m1)) != cudaSuccess) return e;
+    } else {
+      a.n_tiles = (unsigned)((rows_total + 8 * NT - 1) / (8 * NT));
+      if ((e = get_map(st, in, n, rows_total, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+      m1 = m0;
+    }
+  } else {
+    const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
+    const long long outer = p->N / (n * inner) * nb;
+    const int rem = n - 16 * (a.S - 1);
+    a.kk_last = rem > 8 ? 4 : 2;  // k-steps 0,1 cover rows 0..7 of a stage, k-steps 2,3 rows 8..15
+    a.inner = (int)inner;
+    a.cpo = (int)((inner + 15) / 16);
+    const long long chunks = (long long)a.cpo * outer;
+    if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    a.total_chunks = (unsigned)chunks;
+    a.outer = (int)outer;
+    a.div_cpo = make_fastdiv((unsigned)a.cpo);
+    const int CH = NT / 2;
+    a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+    if ((e = get_map(st, in, inner, n, outer, 16, &m0)) != cudaSuccess) return e;
+    if (apply_mult) {
+      if ((e = get_map(st, p->d_mult, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+    } else {
+      m1 = m0;
+    }
+  }
+  if (a.n_tiles == 0) return cudaSuccess;
+  ++p->tma_launches;
+  switch (cc.mtot) {
+    case 2: return launch_class<2, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 4: return launch_class<4, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 6: return launch_class<6, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 8: return launch_class<8, 4, 12, 8>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 12: return launch_class<12, 2, 12, 12>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 15: return launch_class<15, 2, 12, 12>(xmode, two, m0, m1, a, p->sm_count, s);
+    default: return launch_class<16, 2, 12, 8>(xmode, two, m0, m1, a, p->sm_count, s);
+  }
+}
+
+// Upload, per axis and direction, the shared-memory image of M (M[m][k] = V[k][m] forward, V[m][k] backward)
+// that k_mode_t stages verbatim: row 16s + 4kk + q holds the contraction index the lane with that q reads in
+// k-step kk of stage s (see the fragment-address comment in the kernel), zero beyond n.
+cudaError_t tma_init(exx_plan* p) {
+  p->tma_state = nullptr;
+  if (!encode_fn()) return cudaSuccess;  // no driver entry point: the cp.async kernels serve every pass
+  TmaState* st = new (std::nothrow) TmaState();
+  if (!st) return cudaErrorMemoryAllocation;
+  for (int ax = 0; ax < 3; ++ax)
+    for (int d = 0; d < 2; ++d) {
+      st->d_img[ax][d] = nullptr;
+      st->img_owned[ax][d] = false;
+    }
+  p->tma_state = st;
+  for (int ax = 0; ax < 3; ++ax) {
+    ClassCfg cc;
+    if (!pick_class(p->n[ax], &cc)) continue;  // this axis runs on the plain kernel
+    const bool xmode = ax == 0;
+    // axes 1 and 2 are both L-mode: identical matrices share the images
+    if (ax == 2 && p->d_V[2] == p->d_V[1] && st->d_img[1][0]) {
+      st->d_img[2][0] = st->d_img[1][0];
+      st->d_img[2][1] = st->d_img[1][1];
+      continue;
+    }
+    const int n = p->n[ax], S = (n + 15) / 16, ldv = 8 * cc.mtot + 4;
+    for (int d = 0; d < 2; ++d) {
+      std::vector<double> img((size_t)16 * S * ldv, 0.0);
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int within = xmode ? ((q & 1) + 8 * (q >> 1) + 2 * kk) : (2 * q + (kk & 1) + 8 * (kk >> 1));
+            const int k = 16 * s + within;
+            if (k >= n) continue;
+            double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];
+            for (int m = 0; m < n; ++m)
+              row[m] = d == 0 ? p->h_V[ax][(size_t)k * n + m] : p->h_V[ax][(size_t)m * n + k];
+          }
+      cudaError_t e = cudaMalloc(&st->d_img[ax][d], sizeof(double) * img.size());
+      if (e != cudaSuccess) return e;
+      st->img_owned[ax][d] = true;
+      e = cudaMemcpy(st->d_img[ax][d], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+    }
+  }
+  return cudaSuccess;
+}
+
+void tma_destroy(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return;
+  for (int ax = 0; ax < 3; ++ax)
+    for (int d = 0; d < 2; ++d)
+      if (st->img_owned[ax][d] && st->d_img[ax][d]) cudaFree(st->d_img[ax][d]);
+  delete st;
+  p->tma_state = nullptr;
+}
+
+}  // namespace exx

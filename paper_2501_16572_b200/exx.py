@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 
 EXX_OK = 0
 BC_PERIODIC, BC_DIRICHLET = 0, 1
-VARIANT_FUSED_DMMA, VARIANT_REFERENCE = 0, 1
+VARIANT_FUSED_DMMA, VARIANT_REFERENCE, VARIANT_CPASYNC = 0, 1, 2
 
 _lib = None
 
@@ -64,6 +64,8 @@ def load_library():
     lib.exx_apply_host.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, dp, C.c_int, dp, dp, dp, C.c_int]
     lib.exx_plan_last_launch_count.restype = C.c_longlong
     lib.exx_plan_last_launch_count.argtypes = [vp]
+    lib.exx_plan_tma_launch_count.restype = C.c_longlong
+    lib.exx_plan_tma_launch_count.argtypes = [vp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
     lib.exx_plan_set_profiling.restype = C.c_int
@@ -180,6 +182,10 @@ class Plan:
     @property
     def last_launch_count(self) -> int:
         return int(self._lib.exx_plan_last_launch_count(self._h))
+
+    @property
+    def tma_launch_count(self) -> int:
+        return int(self._lib.exx_plan_tma_launch_count(self._h))
 
     def _workspace(self, n_c: int) -> torch.Tensor:
         need = self.workspace_bytes(n_c)

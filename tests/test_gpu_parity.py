@@ -11,7 +11,8 @@ from paper_2501_16572_b200 import exx, workloads as wl
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-10
-VARIANTS = [pytest.param(exx.VARIANT_FUSED_DMMA, id="fused_dmma"), pytest.param(exx.VARIANT_REFERENCE, id="reference")]
+VARIANTS = [pytest.param(exx.VARIANT_FUSED_DMMA, id="fused_dmma"), pytest.param(exx.VARIANT_REFERENCE, id="reference"),
+            pytest.param(exx.VARIANT_CPASYNC, id="cpasync")]
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -62,6 +63,10 @@ def test_poisson_solve_matches_oracle(case, variant):
     out2 = plan.poisson_solve(d, out=d, n_c=n_c)                 # in place
     torch.cuda.synchronize()
     assert torch.equal(out2, out)
+    if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0 and max(nx, ny, nz) <= 128:
+        assert plan.tma_launch_count == 12 * ((n_rhs + n_c - 1) // n_c)   # every pass went through the TMA kernels
+    else:
+        assert plan.tma_launch_count == 0
     plan.close()
 
 
