@@ -127,8 +127,19 @@ struct TArgs {
   int tiles_per_rhs;  // pair density only: ceil(rows_per_rhs / (8*NT))
   int rows_total;     // rows of the output tensor
   FastDiv div_tiles;
-  BatchDesc bd;  // pair density only
+  FastDiv div_nj;  // pair density only
+  int exact;       // no ragged edge in this launch: the epilogue stores without predicates
+  BatchDesc bd;    // pair density only
 };
+
+__device__ __forceinline__ bool elect_one() {
+  unsigned pred;
+  asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ void stg_v2(double* p, double x, double y) {
+  asm volatile("st.global.v2.f64 [%0], {%1, %2};\n" ::"l"(p), "d"(x), "d"(y) : "memory");
+}
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
 template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS>
@@ -140,7 +151,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   constexpr unsigned kStage = 1024u * NT;  // bytes per stage and stream: 16 x (8*NT) doubles
   constexpr int CH = NT / 2;               // L-mode: 16-column chunks per tile
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
+  // warp index through a shuffle: the compiler then knows it is warp-uniform and keeps everything derived
+  // from it (ring and barrier addresses, tile counters) in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int g = lane >> 2, q = lane & 3;
   const int n = a.n, S = a.S;
   const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
@@ -171,7 +185,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   const unsigned tfirst = blockIdx.x + gridDim.x * warp;
   const unsigned tstride = gridDim.x * WARPS;
 
-  // ---- producer (lane 0 of each warp): runs kDepth stages ahead, straight across tile boundaries ---------
+  // ---- producer: warp-uniform bookkeeping, one elected lane issues the copies; runs kDepth stages ahead,
+  //      straight across tile boundaries ----------------------------------------------------------------
   unsigned t_p = tfirst;
   int s_p = 0;
   int pc0[CH], pc2[CH];  // L-mode: column and outer coordinate of each chunk
@@ -181,7 +196,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       if (TWO) {
         const int rhs = (int)fast_div(t, a.div_tiles);
         const int rb = (int)t - rhs * a.tiles_per_rhs;
-        const int j = a.bd.j0 + rhs % a.bd.nj, k = a.bd.k0 + rhs / a.bd.nj;
+        const int kq = (int)fast_div((unsigned)rhs, a.div_nj);
+        const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
         pr0 = j * a.rows_per_rhs + rb * (8 * NT);
         pr1 = k * a.rows_per_rhs + rb * (8 * NT);
       } else {
@@ -202,19 +218,21 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       }
     }
   };
-  auto produce = [&](int slot) {  // lane 0 only
+  auto produce = [&](int slot) {  // called by the whole (converged) warp
     if (t_p >= a.n_tiles) return;
     const unsigned bar = my_bar + 8u * slot;
     const unsigned dst = my_ring + slot * (NS * kStage);
-    mbar_expect_tx(bar, NS * kStage);
-    if (XMODE) {
-      tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
-      if (TWO) tma_load_2d(dst + kStage, &tm1, 16 * s_p, pr1, bar);
-    } else {
+    if (elect_one()) {
+      mbar_expect_tx(bar, NS * kStage);
+      if (XMODE) {
+        tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
+        if (TWO) tma_load_2d(dst + kStage, &tm1, 16 * s_p, pr1, bar);
+      } else {
 #pragma unroll
-      for (int ch = 0; ch < CH; ++ch) {
-        tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
-        if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * s_p, 0, bar);
+        for (int ch = 0; ch < CH; ++ch) {
+          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
+          if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * s_p, 0, bar);
+        }
       }
     }
     if (++s_p == S) {
@@ -223,15 +241,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       if (t_p < a.n_tiles) tile_coords(t_p);
     }
   };
-  if (lane == 0) {
-    if (t_p < a.n_tiles) tile_coords(t_p);
+  if (t_p < a.n_tiles) tile_coords(t_p);
 #pragma unroll
-    for (int d = 0; d < kDepth; ++d) produce(d);
-  }
+  for (int d = 0; d < kDepth; ++d) produce(d);
 
   // ---- per-lane fragment addresses --------------------------------------------------------------------
   // A fragment (M[m][k]) of (stage s, k-step kk, row tile mt): image row 16s + 4kk + q, column 8mt + g.
-  const unsigned a_base = smem0 + 8u * (q * LDV + g);
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
   // B fragment of (k-step kk, column tile nt) inside a stage, 128-byte swizzle (16-byte chunk index XOR row%8):
   //   X-mode: box row 8nt+g (a data row), x = (q&1) + 8(q>>1) + 2kk      -> xo[kk] + 1024 nt
   //   L-mode: box row 2q + (kk&1) + 8(kk>>1) (a contraction index), column 8(nt&1)+g of chunk nt>>1
@@ -257,9 +273,12 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
     for (int s = 0; s < S; ++s) {
+      // opaque uses: keep the per-lane fragment offsets in registers (at the register cap the compiler
+      // otherwise rebuilds them from %tid in every k-step, ~20 instructions ahead of the first LDS)
+      asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * (NS * kStage);
-      const unsigned aa = a_base + (unsigned)s * (16u * LDV * 8u);
+      const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
       const int nk = (s == S - 1) ? a.kk_last : 4;
 #pragma unroll
       for (int kk = 0; kk < 4; ++kk) {
@@ -283,14 +302,15 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       }
       // every lane's reads of this stage have completed (their values fed the DMMAs above): refill it
       __syncwarp();
-      if (lane == 0) produce(slot);
+      produce(slot);
       if (++slot == kDepth) {
         slot = 0;
         parity ^= 1u;
       }
     }
 
-    // ---- epilogue: C[m = 8mt+g][column 8nt + 2q + e] straight from the fragments (every pass is in place) --
+    // ---- epilogue: C[m = 8mt+g][column 8nt + 2q + e] straight from the fragments (every pass is in place).
+    //      a.exact: no ragged edge anywhere in this launch -> no per-store predicates ------------------------
     if (XMODE) {
       int row0, limit;
       if (TWO) {
@@ -302,36 +322,55 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
         row0 = (int)t * (8 * NT);
         limit = a.rows_total;
       }
+      double* base = a.out + ((long long)(row0 + 2 * q) * n + g);
+      if (a.exact) {
 #pragma unroll
-      for (int nt = 0; nt < NT; ++nt) {
+        for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const int r = row0 + 8 * nt + 2 * q + e;
-          if (r < limit) {
-            double* dst = a.out + (long long)r * n + g;
+          for (int e = 0; e < 2; ++e) {
+            double* dst = base + (long long)(8 * nt + e) * n;
 #pragma unroll
-            for (int mt = 0; mt < MTOT; ++mt)
-              if (8 * mt + g < n) dst[8 * mt] = acc[mt][nt][e];
+            for (int mt = 0; mt < MTOT; ++mt) dst[8 * mt] = acc[mt][nt][e];
           }
-        }
+      } else {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            if (row0 + 8 * nt + 2 * q + e < limit) {
+              double* dst = base + (long long)(8 * nt + e) * n;
+#pragma unroll
+              for (int mt = 0; mt < MTOT; ++mt)
+                if (8 * mt + g < n) dst[8 * mt] = acc[mt][nt][e];
+            }
+          }
       }
     } else {
+      const long long mstep = 8LL * a.inner;  // doubles between consecutive row tiles
 #pragma unroll
       for (int ch = 0; ch < CH; ++ch) {
         const unsigned cc = t * CH + ch;
         if (cc < a.total_chunks) {
           const unsigned o = fast_div(cc, a.div_cpo);
           const int col0 = 16 * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
-          double* base = a.out + ((long long)o * n + g) * a.inner + col0;
+          double* ptr = a.out + ((long long)o * n + g) * a.inner + col0;
+          if (a.exact) {
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int nt = 2 * ch + h;
-            if (col0 + 8 * h < a.inner) {  // inner is even, so the pair (c, c+1) is inside or outside together
+            for (int mt = 0; mt < MTOT; ++mt) {
+              stg_v2(ptr, acc[mt][2 * ch][0], acc[mt][2 * ch][1]);
+              stg_v2(ptr + 8, acc[mt][2 * ch + 1][0], acc[mt][2 * ch + 1][1]);
+              ptr += mstep;
+            }
+          } else {
+            // inner is even, so the pair (c, c+1) is inside or outside together
+            const bool in0 = col0 < a.inner, in1 = col0 + 8 < a.inner;
 #pragma unroll
-              for (int mt = 0; mt < MTOT; ++mt)
-                if (8 * mt + g < n)
-                  *reinterpret_cast<double2*>(base + (long long)(8 * mt) * a.inner + 8 * h) =
-                      make_double2(acc[mt][nt][0], acc[mt][nt][1]);
+            for (int mt = 0; mt < MTOT; ++mt) {
+              if (8 * mt + g < n) {
+                if (in0) stg_v2(ptr, acc[mt][2 * ch][0], acc[mt][2 * ch][1]);
+                if (in1) stg_v2(ptr + 8, acc[mt][2 * ch + 1][0], acc[mt][2 * ch + 1][1]);
+              }
+              ptr += mstep;
             }
           }
         }
@@ -511,8 +550,10 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
     a.rows_total = (int)rows_total;
     a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
     a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+    a.exact = (n == 8 * cc.mtot) && ((pd ? a.rows_per_rhs : rows_total) % (8 * NT) == 0);
     if (pd) {
       a.bd = pd->bd;
+      a.div_nj = make_fastdiv((unsigned)pd->bd.nj);
       a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
       const long long rp = (long long)a.rows_per_rhs * pd->n_occ, rt = (long long)a.rows_per_rhs * pd->n_tgt;
       if (rp >= (1LL << 31) - 64 || rt >= (1LL << 31) - 64) return cudaErrorNotSupported;
@@ -535,6 +576,7 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
     a.total_chunks = (unsigned)chunks;
     a.outer = (int)outer;
     a.div_cpo = make_fastdiv((unsigned)a.cpo);
+    a.exact = (n == 8 * cc.mtot) && (inner % 16 == 0);
     const int CH = NT / 2;
     a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
     if ((e = get_map(st, in, inner, n, outer, 16, &m0)) != cudaSuccess) return e;
