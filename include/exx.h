@@ -81,6 +81,17 @@ exx_status exx_plan_destroy(exx_plan* plan);
 /* Select a kernel variant (EXX_VARIANT_*). INVALID_ARG for unknown values. */
 exx_status exx_plan_set_variant(exx_plan* plan, int variant);
 
+/*
+ * How many batches exx_apply keeps in flight: 1 (default) = every kernel on the caller's stream; 2 (allowed
+ * where the fast kernels serve all three axes) = consecutive target blocks alternate between the caller's stream and
+ * a plan-owned second stream, forked from and joined back into the caller's stream with events inside the
+ * call, so the call is still asynchronous, ordered with respect to the caller's stream and graph capturable.
+ * Each lane uses one half of the workspace.  The two lanes never touch the same vx_k, and every vx_k is
+ * accumulated in the same order as with one lane: results are bitwise identical.  INVALID_ARG otherwise.
+ */
+exx_status exx_plan_set_lanes(exx_plan* plan, int lanes);
+int exx_plan_get_lanes(const exx_plan* plan);
+
 /* Bytes of device workspace exx_apply / exx_poisson_solve need for batches of n_c right-hand sides
  * (0 if plan is NULL or n_c is outside 1..max_batch). */
 size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c);

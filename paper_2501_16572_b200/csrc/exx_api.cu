@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -38,6 +39,17 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
   if (!a || !b || na == 0 || nb == 0) return false;
   const uintptr_t a0 = (uintptr_t)a, a1 = a0 + na, b0 = (uintptr_t)b, b1 = b0 + nb;
   return a0 < b1 && b0 < a1;
+}
+
+// the DMMA kernels serve every axis (n <= 128): no pass needs the second workspace half as scratch
+inline bool all_axes_fast(const exx_plan* p) { return p->d_Vpad[0] && p->d_Vpad[1] && p->d_Vpad[2]; }
+
+// One lane by default: two lanes measured +1.5 % .. +2.7 % on the 96^3 / 120^3 configs (the other lane's
+// accumulate overlaps the mode products) and -2 % .. -6 % at 48^3, see DESIGN.md 6.3.  EXX_LANES overrides.
+inline int default_lanes(const exx_plan* p) {
+  if (const char* e = getenv("EXX_LANES"))
+    if (e[0] == '2') return all_axes_fast(p) ? 2 : 1;
+  return 1;
 }
 
 inline int resolve_nc(const exx_plan* p, int n_c) {
@@ -100,6 +112,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->tma_launches = 0;
   p->prof_on = false;
+  p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; }
 
   try {
@@ -147,6 +160,10 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
       e = cudaMalloc(&p->ex.d_energy_scratch, sizeof(double) * kEnergyChunk * kEnergyBlocks);
     if (e == cudaSuccess) e = exx::fast_init(p);
     if (e == cudaSuccess) e = exx::tma_init(p);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->lane_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) p->lanes = default_lanes(p);
     if (e != cudaSuccess) {
       exx_plan_destroy(p);
       return e == cudaErrorMemoryAllocation ? EXX_ERR_ALLOC : cuda_fail(e);
@@ -163,6 +180,9 @@ exx_status exx_plan_destroy(exx_plan* plan) {
     cudaSetDevice(p->device);
     exx::fast_destroy(p);
     exx::tma_destroy(p);
+    if (p->lane_stream) cudaStreamDestroy(p->lane_stream);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     for (int a = 0; a < 3; ++a) {
       bool shared = false;
       for (int b = 0; b < a; ++b) shared |= (p->d_V[b] == p->d_V[a]);
@@ -183,6 +203,15 @@ exx_status exx_plan_set_variant(exx_plan* plan, int variant) {
   plan->variant = variant;
   return EXX_OK;
 }
+
+exx_status exx_plan_set_lanes(exx_plan* plan, int lanes) {
+  if (!plan || (lanes != 1 && lanes != 2)) return EXX_ERR_INVALID_ARG;
+  if (lanes == 2 && (plan->device < 0 || !all_axes_fast(plan))) return EXX_ERR_INVALID_ARG;
+  plan->lanes = lanes;
+  return EXX_OK;
+}
+
+int exx_plan_get_lanes(const exx_plan* plan) { return plan ? plan->lanes : 0; }
 
 size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c) {
   if (!plan) return 0;
@@ -325,8 +354,21 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     // Batch = nk targets x nj occupied orbitals, nj*nk <= n_c.  With n_occ >= n_c one target per batch.
     const int nj_max = n_occ < n_c ? n_occ : n_c;
     const int nk_max = n_c / nj_max;
-    for (int k0 = 0; k0 < n_tgt; k0 += nk_max) {
+    // Two lanes: target block kb runs on lane kb % 2 (all its j-batches in order, so vx_k is accumulated in
+    // the same order as with one lane and no vx_k is touched by both lanes); lane 1 works in the second half
+    // of the workspace on the plan's own stream, forked from and joined back into the caller's stream.
+    const int n_kblocks = (n_tgt + nk_max - 1) / nk_max;
+    const bool two_lanes = plan->variant != EXX_VARIANT_REFERENCE && plan->lanes == 2 && n_kblocks > 1 &&
+                           all_axes_fast(plan);
+    if (two_lanes) {
+      EXX_CUDA(cudaEventRecord(plan->ev_fork, s));
+      EXX_CUDA(cudaStreamWaitEvent(plan->lane_stream, plan->ev_fork, 0));
+    }
+    int kb = 0;
+    for (int k0 = 0; k0 < n_tgt; k0 += nk_max, ++kb) {
       const int nk = n_tgt - k0 < nk_max ? n_tgt - k0 : nk_max;
+      const bool lane1 = two_lanes && (kb & 1);
+      cudaStream_t ls = lane1 ? plan->lane_stream : s;
       for (int j0 = 0; j0 < n_occ; j0 += nj_max) {
         const int nj = n_occ - j0 < nj_max ? n_occ - j0 : nj_max;
         const exx::BatchDesc bd{j0, nj, k0, nk};
@@ -344,9 +386,14 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
           launches += 2;
         } else {
           const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0};
-          EXX_CUDA(exx::fast_solve_batch(plan, nullptr, buf0, buf1, nb, &fa, s, &launches));
+          EXX_CUDA(exx::fast_solve_batch(plan, nullptr, lane1 ? buf1 : buf0, two_lanes ? nullptr : buf1, nb, &fa, ls,
+                                         &launches));
         }
       }
+    }
+    if (two_lanes) {
+      EXX_CUDA(cudaEventRecord(plan->ev_join, plan->lane_stream));
+      EXX_CUDA(cudaStreamWaitEvent(s, plan->ev_join, 0));
     }
   }
   if (d_ex && n_tgt == 0) {

@@ -52,6 +52,11 @@ struct exx_plan {
   int smem_optin;
   long long last_launches;
   long long tma_launches;  // cumulative count of TMA-staged mode-product launches (test hook)
+  // exx_apply runs `lanes` batches at a time (1 or 2): lane 0 on the caller's stream, lane 1 on lane_stream,
+  // forked and joined with the two events
+  int lanes;
+  cudaStream_t lane_stream;
+  cudaEvent_t ev_fork, ev_join;
   // optional per-kernel-class CUDA-event timing (exx_plan_set_profiling)
   bool prof_on;
   std::vector<exx::ProfRec> prof;

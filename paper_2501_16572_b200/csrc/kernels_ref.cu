@@ -1,6 +1,9 @@
 // Reference variant (EXX_VARIANT_REFERENCE): one plain FP64 kernel per step of the hot path.
 // Deliberately simple -- used to cross-check the fast variant on the GPU and as a fallback-free
 // "second opinion" in the parity tests.  Also holds the kernels both variants share (energy, zero fill).
+#include <cstdint>
+#include <cstdlib>
+
 #include "exx_internal.h"
 
 namespace exx {
@@ -45,19 +48,59 @@ __global__ void k_mode_product(const double* __restrict__ in, double* __restrict
 }
 
 // a5: vx_k(r) (-)= sum_b occ_j psi_j(r) phi_b(r), b ascending (PAPER.md:38 Eq. 1, :178 Eq. 19b).
-__global__ void k_accumulate(const double* __restrict__ psi, const double* __restrict__ occ,
-                             const double* __restrict__ phi, BatchDesc bd, bool first, long long N,
-                             double* __restrict__ vx) {
+// Streaming kernel: per grid point one read of phi_b and psi_j per pair, vx_k read-modify-written once per
+// batch.  VEC = 2 uses 16-byte accesses (N even, 16-byte aligned buffers); UNROLL independent j per trip keep
+// 2*UNROLL loads per thread in flight.  The sum over j runs in ascending order whatever the template
+// arguments, so all instantiations give bitwise identical results.
+template <int VEC, int UNROLL>
+__global__ void __launch_bounds__(256) k_accumulate(const double* __restrict__ psi, const double* __restrict__ occ,
+                                                    const double* __restrict__ phi, BatchDesc bd, bool first,
+                                                    unsigned N, double* __restrict__ vx) {
   const int kk = blockIdx.y;
-  double* v = vx + (long long)(bd.k0 + kk) * N;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N;
-       i += (long long)gridDim.x * blockDim.x) {
-    double acc = first ? 0.0 : v[i];
-    for (int jj = 0; jj < bd.nj; ++jj) {
-      const long long b = (long long)kk * bd.nj + jj;
-      acc -= occ[bd.j0 + jj] * psi[(long long)(bd.j0 + jj) * N + i] * phi[b * N + i];
+  const int nj = bd.nj;
+  double* v = vx + (size_t)(bd.k0 + kk) * N;
+  const double* oc = occ + bd.j0;
+  const double* psi0 = psi + (size_t)bd.j0 * N;
+  const double* phi0 = phi + (size_t)kk * nj * N;
+  const unsigned stride = gridDim.x * blockDim.x * VEC;
+  for (unsigned i = (blockIdx.x * blockDim.x + threadIdx.x) * VEC; i < N; i += stride) {
+    double acc[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) acc[e] = first ? 0.0 : v[i + e];
+    const double* pj = psi0 + i;
+    const double* ph = phi0 + i;
+    int jj = 0;
+    for (; jj + UNROLL <= nj; jj += UNROLL) {
+      double a[UNROLL][VEC], b[UNROLL][VEC];
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u) {
+        if (VEC == 2) {
+          const double2 x = *reinterpret_cast<const double2*>(pj + (size_t)u * N);
+          const double2 y = *reinterpret_cast<const double2*>(ph + (size_t)u * N);
+          a[u][0] = x.x; a[u][VEC - 1] = x.y; b[u][0] = y.x; b[u][VEC - 1] = y.y;
+        } else {
+          a[u][0] = pj[(size_t)u * N];
+          b[u][0] = ph[(size_t)u * N];
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < UNROLL; ++u) {
+        const double o = oc[jj + u];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) acc[e] -= o * a[u][e] * b[u][e];
+      }
+      pj += (size_t)UNROLL * N;
+      ph += (size_t)UNROLL * N;
     }
-    v[i] = acc;
+    for (; jj < nj; ++jj) {
+      const double o = oc[jj];
+#pragma unroll
+      for (int e = 0; e < VEC; ++e) acc[e] -= o * pj[e] * ph[e];
+      pj += N;
+      ph += N;
+    }
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) v[i + e] = acc[e];
   }
 }
 
@@ -149,8 +192,18 @@ cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const do
 
 cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
                            BatchDesc bd, bool first, double* vx, cudaStream_t s) {
-  dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
-  k_accumulate<<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
+  static const int variant = [] { const char* e = getenv("EXX_ACC"); return e ? atoi(e) : 1; }();
+  const unsigned N = (unsigned)p->N;
+  const bool vec2 = (N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
+  if (vec2 && variant >= 2) {
+    dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nk);
+    if (variant == 3) k_accumulate<2, 8><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+    else k_accumulate<2, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+  } else {
+    dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
+    if (variant == 0) k_accumulate<1, 2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+    else k_accumulate<1, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+  }
   return cudaGetLastError();
 }
 

@@ -142,8 +142,8 @@ __device__ __forceinline__ void stg_v2(double* p, double x, double y) {
 }
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS, 1)
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
     k_mode_t(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const TArgs a) {
   static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
   constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): the A-fragment reads are bank-conflict free
@@ -168,22 +168,35 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;  // swizzled boxes need 1024-byte alignment
   const unsigned my_ring = ring0 + warp * (kDepth * NS * kStage);
   const unsigned my_bar = ring0 + WARPS * (kDepth * NS * kStage) + warp * (kDepth * 8u);
+  // CTA-wide tile counter (dynamic tile claiming, below): local tile indices 0..WARPS-1 are pre-assigned
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * NS * kStage) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
   if (lane == 0) {
 #pragma unroll
     for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
-  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
-  __syncthreads();
+  __syncthreads();  // barriers and tile counter initialised (the V image is still in flight)
   // Programmatic dependent launch: everything above touched only plan constants, so it overlaps the tail
   // of the previous pass; from here on we read that pass's output.
   asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
   asm volatile("griddepcontrol.wait;\n" ::: "memory");
 
-  // Tile t of this launch belongs to warp (b, w) = (t % grid, (t / grid) % WARPS): a ragged last round is
-  // spread over all SMs and, inside an SM, over all four schedulers.
+  // Tiles b, b + grid, b + 2 grid, ... belong to CTA b (static, equal shares); inside the CTA the warps claim
+  // them one at a time from a shared counter, so no warp idles while the CTA still has tiles, however unevenly
+  // the schedulers share the DMMA pipe (measured: neutral against a static split on the five configs).
   const unsigned tfirst = blockIdx.x + gridDim.x * warp;
-  const unsigned tstride = gridDim.x * WARPS;
+  auto claim_tile = [&]() -> unsigned {  // whole warp; returns the same tile id in every lane
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  // tiles the producer has claimed and the consumer has not started yet (the producer runs at most kDepth
+  // stages, i.e. at most kDepth tiles, ahead)
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
 
   // ---- producer: warp-uniform bookkeeping, one elected lane issues the copies; runs kDepth stages ahead,
   //      straight across tile boundaries ----------------------------------------------------------------
@@ -237,13 +250,20 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     }
     if (++s_p == S) {
       s_p = 0;
-      t_p += tstride;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
       if (t_p < a.n_tiles) tile_coords(t_p);
     }
   };
   if (t_p < a.n_tiles) tile_coords(t_p);
 #pragma unroll
   for (int d = 0; d < kDepth; ++d) produce(d);
+  // the V image has been landing behind the dependency wait and the first data copies
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
 
   // ---- per-lane fragment addresses --------------------------------------------------------------------
   // A fragment (M[m][k]) of (stage s, k-step kk, row tile mt): image row 16s + 4kk + q, column 8mt + g.
@@ -265,7 +285,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
 
   int slot = 0;
   unsigned parity = 0;
-  for (unsigned t = tfirst; t < a.n_tiles; t += tstride) {
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
     double acc[MTOT][NT][2];
 #pragma unroll
     for (int mt = 0; mt < MTOT; ++mt)
@@ -376,6 +397,12 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
         }
       }
     }
+    // next tile: the oldest one the producer has claimed (it always has: it claimed the successor when it
+    // issued this tile's last stage)
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
   }
 }
 
@@ -416,20 +443,34 @@ struct TmaState {
   std::vector<MapEntry> cache;
 };
 
-// supported classes of ceil(n/8), the columns-per-warp choice and the warps per CTA for each
+// supported classes of ceil(n/8); per class the columns-per-warp choice (NT), the warps per CTA and the CTAs
+// per SM, for the plain and for the two-stream (TWO) kernels.
+//   lanes == 1: one persistent CTA per SM, as many warps as the register file allows.
+//   lanes == 2 (exx_apply runs two batches at a time on two streams): where the V image is small enough
+//     (n <= 64) a CTA takes half an SM (8 warps, <= 128 registers, <= 113 KB) so that kernels of the two lanes
+//     are co-resident and each fills the other's launch gaps, ramps, tails and epilogues; larger axes keep
+//     one CTA per SM and leave a few thousand registers free for the other lane's accumulate kernel.
 struct ClassCfg {
-  int mtot, nt, warps, warps_two;
+  int mtot;
+  int nt, warps, minb;
+  int nt_two, warps_two, minb_two;
 };
-inline bool pick_class(int n, ClassCfg* c) {
+inline bool pick_class(int n, int lanes, ClassCfg* c) {
   const int need = (n + 7) / 8;
-  if (need <= 2) *c = {2, 4, 16, 12};
-  else if (need <= 4) *c = {4, 4, 16, 12};
-  else if (need <= 6) *c = {6, 4, 16, 12};
-  else if (need <= 8) *c = {8, 4, 12, 8};
-  else if (need <= 12) *c = {12, 2, 12, 12};
-  else if (need <= 15) *c = {15, 2, 12, 12};
-  else if (need <= 16) *c = {16, 2, 12, 8};
-  else return false;
+  if (need > 16) return false;
+  if (lanes == 2 && need <= 8) {
+    const int m = need <= 2 ? 2 : need <= 4 ? 4 : need <= 6 ? 6 : 8;
+    if (m == 8) *c = {8, 2, 8, 2, 2, 8, 2};
+    else *c = {m, 4, 8, 2, 2, 8, 2};
+    return true;
+  }
+  if (need <= 2) *c = {2, 4, 16, 1, 4, 12, 1};
+  else if (need <= 4) *c = {4, 4, 16, 1, 4, 12, 1};
+  else if (need <= 6) *c = {6, 4, 16, 1, 4, 12, 1};
+  else if (need <= 8) *c = {8, 4, 12, 1, 4, 8, 1};
+  else if (need <= 12) *c = {12, 2, 12, 1, 2, 12, 1};
+  else if (need <= 15) *c = {15, 2, 12, 1, 2, 12, 1};
+  else *c = {16, 2, 12, 1, 2, 8, 1};
   return true;
 }
 
@@ -468,18 +509,32 @@ inline bool use_pdl() {
   return on;
 }
 
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS>
+inline bool pdl_half() {
+  static const bool on = [] {
+    const char* e = getenv("EXX_PDL_HALF");
+    return e && e[0] == '1';
+  }();
+  return on;
+}
+
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB>
 cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, cudaStream_t s) {
   constexpr int LDV = 8 * MTOT + 4;
   const size_t img = sizeof(double) * 16 * (size_t)a.S * LDV;
-  // image | (alignment slack) | rings | mbarriers.  The request always exceeds half of the SM's shared memory
-  // so that exactly one CTA is resident: the tile split assumes one persistent CTA per SM.
-  size_t smem = img + 1024 + (size_t)WARPS * kDepth * (TWO ? 2 : 1) * 1024 * NT + (size_t)WARPS * kDepth * 8;
-  if (smem < 117 * 1024) smem = 117 * 1024;
-  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS>;
+  // image | (alignment slack) | rings | mbarriers.  The request is padded so that exactly MINB CTAs fit an SM
+  // (above 1/(MINB+1) of its shared memory): the tile split assumes one CTA of this launch per SM.
+  size_t smem = img + 1024 + (size_t)WARPS * kDepth * (TWO ? 2 : 1) * 1024 * NT + (size_t)WARPS * kDepth * 8 + 16;
+  const size_t floor_bytes = MINB == 1 ? 117 * 1024 : 77 * 1024;
+  if (MINB == 2 && smem > 113 * 1024) return cudaErrorInvalidConfiguration;
+  if (smem < floor_bytes) smem = floor_bytes;
+  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB>;
   static size_t attr_smem = 0;  // per instantiation
   if (smem > attr_smem) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // always the largest shared-memory carveout: kernels of the two lanes must agree on the SM's L1/shared
+    // split to be resident together (and a switch between launches drains the SM)
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     attr_smem = smem;
   }
@@ -493,19 +548,21 @@ cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
-  cfg.numAttrs = use_pdl() ? 1 : 0;
+  // Half-SM kernels (MINB == 2) are launched without programmatic serialization: an early-launched successor
+  // would sit in griddepcontrol.wait in the very slot the other lane's kernel is meant to use.
+  cfg.numAttrs = (use_pdl() && (MINB == 1 || pdl_half())) ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
 }
 
-template <int MTOT, int NT, int WARPS, int WARPS_TWO>
+template <int MTOT, int NT, int WARPS, int MINB, int NT2, int WARPS2, int MINB2>
 cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a,
                          int sm_count, cudaStream_t s) {
   if (xmode) {
-    if (two) return launch_one<MTOT, NT, true, true, WARPS_TWO>(m0, m1, a, sm_count, s);
-    return launch_one<MTOT, NT, true, false, WARPS>(m0, m1, a, sm_count, s);
+    if (two) return launch_one<MTOT, NT2, true, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
+    return launch_one<MTOT, NT, true, false, WARPS, MINB>(m0, m1, a, sm_count, s);
   }
-  if (two) return launch_one<MTOT, NT, false, true, WARPS_TWO>(m0, m1, a, sm_count, s);
-  return launch_one<MTOT, NT, false, false, WARPS>(m0, m1, a, sm_count, s);
+  if (two) return launch_one<MTOT, NT2, false, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
+  return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, s);
 }
 
 inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
@@ -523,7 +580,7 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   if (!st) return cudaErrorNotSupported;
   const int n = p->n[axis];
   ClassCfg cc;
-  if (!pick_class(n, &cc)) return cudaErrorNotSupported;
+  if (!pick_class(n, p->lanes, &cc)) return cudaErrorNotSupported;
   const double* img = st->d_img[axis][forward ? 0 : 1];
   if (!img) return cudaErrorNotSupported;
   if ((p->n[0] & 1) || !aligned16(out) || (in && !aligned16(in))) return cudaErrorNotSupported;
@@ -532,7 +589,7 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   if (apply_mult && !(axis == 2 && !forward)) return cudaErrorInvalidValue;
   if (pd && (!aligned16(pd->psi) || !aligned16(pd->tgt))) return cudaErrorNotSupported;
   const bool two = pd != nullptr || apply_mult;
-  const int NT = cc.nt;
+  const int NT = two ? cc.nt_two : cc.nt;
 
   TArgs a{};
   a.out = out;
@@ -588,14 +645,22 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   }
   if (a.n_tiles == 0) return cudaSuccess;
   ++p->tma_launches;
+  if (cc.minb == 2) {
+    switch (cc.mtot) {
+      case 2: return launch_class<2, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
+      case 4: return launch_class<4, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
+      case 6: return launch_class<6, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
+      default: return launch_class<8, 2, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
+    }
+  }
   switch (cc.mtot) {
-    case 2: return launch_class<2, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 4: return launch_class<4, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 6: return launch_class<6, 4, 16, 12>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 8: return launch_class<8, 4, 12, 8>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 12: return launch_class<12, 2, 12, 12>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 15: return launch_class<15, 2, 12, 12>(xmode, two, m0, m1, a, p->sm_count, s);
-    default: return launch_class<16, 2, 12, 8>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 2: return launch_class<2, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 4: return launch_class<4, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 6: return launch_class<6, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 8: return launch_class<8, 4, 12, 1, 4, 8, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 12: return launch_class<12, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 15: return launch_class<15, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    default: return launch_class<16, 2, 12, 1, 2, 8, 1>(xmode, two, m0, m1, a, p->sm_count, s);
   }
 }
 
@@ -615,7 +680,7 @@ cudaError_t tma_init(exx_plan* p) {
   p->tma_state = st;
   for (int ax = 0; ax < 3; ++ax) {
     ClassCfg cc;
-    if (!pick_class(p->n[ax], &cc)) continue;  // this axis runs on the plain kernel
+    if (!pick_class(p->n[ax], 1, &cc)) continue;  // this axis runs on the plain kernel (mtot does not depend on lanes)
     const bool xmode = ax == 0;
     // axes 1 and 2 are both L-mode: identical matrices share the images
     if (ax == 2 && p->d_V[2] == p->d_V[1] && st->d_img[1][0]) {

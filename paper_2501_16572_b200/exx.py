@@ -66,6 +66,10 @@ def load_library():
     lib.exx_plan_last_launch_count.argtypes = [vp]
     lib.exx_plan_tma_launch_count.restype = C.c_longlong
     lib.exx_plan_tma_launch_count.argtypes = [vp]
+    lib.exx_plan_set_lanes.restype = C.c_int
+    lib.exx_plan_set_lanes.argtypes = [vp, C.c_int]
+    lib.exx_plan_get_lanes.restype = C.c_int
+    lib.exx_plan_get_lanes.argtypes = [vp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
     lib.exx_plan_set_profiling.restype = C.c_int
@@ -150,6 +154,13 @@ class Plan:
 
     def set_variant(self, variant: int):
         _check(self._lib.exx_plan_set_variant(self._h, variant), "exx_plan_set_variant")
+
+    def set_lanes(self, lanes: int):
+        _check(self._lib.exx_plan_set_lanes(self._h, lanes), "exx_plan_set_lanes")
+
+    @property
+    def lanes(self) -> int:
+        return int(self._lib.exx_plan_get_lanes(self._h))
 
     def workspace_bytes(self, n_c: int = 0) -> int:
         return int(self._lib.exx_plan_workspace_bytes(self._h, n_c))

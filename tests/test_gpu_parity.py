@@ -207,3 +207,27 @@ def test_fast_variant_agrees_with_reference_variant_bitwise_close():
     assert float((a[0] - b[0]).abs().max() / a[0].abs().max()) < 1e-12
     assert abs(a[1] - b[1]) < 1e-12 * abs(a[1])
     plan.close()
+
+
+@pytest.mark.parametrize("cfg,n_orb,n_tgt,n_c", [(2, 12, 6, 4), (3, 6, 5, 3), (1, 8, 8, 8)])
+def test_two_lanes_bitwise_equal_to_one_lane(cfg, n_orb, n_tgt, n_c):
+    # include/exx.h exx_plan_set_lanes: target blocks alternate between two streams; every vx_k is still
+    # accumulated in ascending j by one lane only, so the result must not change by a single bit
+    w = wl.scaled(wl.WORKLOADS[cfg], n_orb, n_tgt, 0)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cuda")
+    plan = exx.Plan.for_workload(w, max_batch=16, device=0)
+    assert plan.lanes == 1
+    v1, e1, x1 = plan.apply(psi, occ, tgt, occ_t, n_c=n_c)
+    v1, e1, x1 = v1.clone(), e1.clone(), x1.clone()
+    plan.set_lanes(2)
+    assert plan.lanes == 2
+    for _ in range(3):
+        v2, e2, x2 = plan.apply(psi, occ, tgt, occ_t, n_c=n_c)
+        torch.cuda.synchronize()
+        assert torch.equal(v1, v2) and torch.equal(e1, e2) and torch.equal(x1, x2)
+    o = _oracle_plan(w)
+    vo, eo, xo = orc.exx_apply(o, psi.cpu().numpy(), occ.cpu().numpy(), tgt.cpu().numpy(), occ_t.cpu().numpy())
+    assert _rel(v2.cpu().numpy(), vo) < TOL and abs(x2.item() - xo) < TOL * abs(xo)
+    with pytest.raises(exx.ExxError):
+        plan.set_lanes(3)
+    plan.close()
