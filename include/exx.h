@@ -10,6 +10,7 @@
  *   phi_jk = f(L) (psi_j .* tgt_k)                                   Eqs. 2-5
  *   vx_k   = - sum_j occ_j * psi_j .* phi_jk                          Eq. 1 / Eq. 19b
  *   e_k    = h^3 * <tgt_k, vx_k>,   E_x = 1/2 sum_k occ_tgt_k e_k     BASELINE.json north_star (R7)
+ *   xi = W R^-T, V~ Phi = -xi (h^3 xi^T Phi)                          ACE, Eqs. 17-20, 26-29
  *
  * f(L) is evaluated with the batch Kronecker-product formalism (Eqs. 6-7, 9-11, 16; PAPER.md:66-70,
  * 86-98, 134): L = I(x)I(x)Kx + I(x)Ky(x)I + Kz(x)I(x)I, K_a = V_a diag(lam_a) V_a^T, three mode products
@@ -134,6 +135,31 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
 exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_occ, int n_occ,
                           const double* h_tgt, int tgt_start, const double* h_occ_tgt, int n_tgt,
                           double* h_vx, double* h_ex, double* h_ex_k, int n_c);
+
+/*
+ * ACE tail (Section III.A, Eqs. 17-20 and 26), the step right after exx_apply with the
+ * orbitals themselves as targets (then W^(n) = vx_n, Eq. 19):
+ *   M  = h^3 Psi^T W                  [n_orb][n_orb]   Eq. 20 (grid inner product, R15)
+ *   R R^T = -(M + M^T)/2              R lower triangular; the paper's "Cholesky factor of M": M is negative
+ *                                     definite because Vx is, so -M is what is factored (R16, R17)
+ *   xi = W R^-T                       [n_orb][N]       Eqs. 18, 26
+ * d_psi, d_w [n_orb][N]; d_xi [n_orb][N] may equal d_w (in place) but must not partially overlap it, nor d_psi.
+ * d_M (optional, NULL): receives M, n_orb*n_orb doubles, row-major.  d_info (optional, NULL): device int, set to
+ * 0 on success or to the 1-based index of the first non-positive pivot (then xi holds NaNs); the call itself
+ * never synchronises, so the caller reads d_info after synchronising the stream.
+ * Workspace: exx_ace_workspace_bytes(plan, n_orb, n_trial) bytes (n_trial = 0 if only building).
+ */
+size_t exx_ace_workspace_bytes(const exx_plan* plan, int n_orb, int n_trial);
+exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w, int n_orb, double* d_xi,
+                         double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * ACE application (Section III.B, Eqs. 27-29) to n_trial trial functions:
+ *   chi = h^3 xi^T Phi  [n_orb][n_trial] (Eq. 28),   d_out = -xi chi  [n_trial][N] (Eqs. 27, 29; sign per R17).
+ * d_out must not overlap d_xi or d_phi (EXX_ERR_ALIAS).  With Phi = Psi the result equals W.
+ */
+exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
+                         double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);

@@ -475,4 +475,53 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
   return EXX_OK;
 }
 
+size_t exx_ace_workspace_bytes(const exx_plan* plan, int n_orb, int n_trial) {
+  if (!plan || n_orb < 1 || n_trial < 0) return 0;
+  const size_t b = exx::ace_build_workspace_doubles(plan, n_orb);
+  const size_t a = n_trial > 0 ? exx::ace_apply_workspace_doubles(plan, n_orb, n_trial) : 0;
+  return sizeof(double) * (a > b ? a : b);
+}
+
+exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w, int n_orb, double* d_xi,
+                         double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_orb < 1 || n_orb > 32768 || !d_psi || !d_w || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  const size_t need = sizeof(double) * exx::ace_build_workspace_doubles(plan, n_orb);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if (((uintptr_t)d_workspace) & 15) return EXX_ERR_INVALID_ARG;
+  const size_t fn = sizeof(double) * (size_t)plan->N * (size_t)n_orb;
+  const size_t mm = sizeof(double) * (size_t)n_orb * n_orb;
+  if ((d_xi != d_w && overlaps(d_xi, fn, d_w, fn)) || overlaps(d_xi, fn, d_psi, fn) ||
+      overlaps(d_xi, fn, d_workspace, need) || overlaps(d_workspace, need, d_psi, fn) ||
+      overlaps(d_workspace, need, d_w, fn) || overlaps(d_M, mm, d_workspace, need) || overlaps(d_M, mm, d_xi, fn) ||
+      overlaps(d_info, sizeof(int), d_workspace, need) || overlaps(d_info, sizeof(int), d_xi, fn))
+    return EXX_ERR_ALIAS;
+  long long launches = 0;
+  EXX_CUDA(exx::ace_build(plan, d_psi, d_w, n_orb, d_xi, d_M, d_info, (double*)d_workspace,
+                          (cudaStream_t)cuda_stream, &launches));
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
+                         double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_orb < 1 || n_orb > 32768 || n_trial < 0 || n_trial > 32768 || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (n_trial > 0 && (!d_phi || !d_out)) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  if (n_trial == 0) { plan->last_launches = 0; return EXX_OK; }
+  const size_t need = sizeof(double) * exx::ace_apply_workspace_doubles(plan, n_orb, n_trial);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if (((uintptr_t)d_workspace) & 15) return EXX_ERR_INVALID_ARG;
+  const size_t fx = sizeof(double) * (size_t)plan->N * (size_t)n_orb;
+  const size_t fp = sizeof(double) * (size_t)plan->N * (size_t)n_trial;
+  if (overlaps(d_out, fp, d_xi, fx) || overlaps(d_out, fp, d_phi, fp) || overlaps(d_out, fp, d_workspace, need) ||
+      overlaps(d_workspace, need, d_xi, fx) || overlaps(d_workspace, need, d_phi, fp))
+    return EXX_ERR_ALIAS;
+  long long launches = 0;
+  EXX_CUDA(exx::ace_apply(plan, d_xi, n_orb, d_phi, n_trial, d_out, (double*)d_workspace,
+                          (cudaStream_t)cuda_stream, &launches));
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
 }  // extern "C"

@@ -119,6 +119,13 @@ cudaError_t tma_init(exx_plan* p);
 void tma_destroy(exx_plan* p);
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
                              bool apply_mult, const FastArgs* pd, cudaStream_t s);
+// ---- ACE tail and application (kernels_ace.cu) ----
+size_t ace_build_workspace_doubles(const exx_plan* p, int n);
+size_t ace_apply_workspace_doubles(const exx_plan* p, int n, int m);
+cudaError_t ace_build(exx_plan* p, const double* psi, const double* w, int n, double* xi, double* M_out, int* info,
+                      double* ws, cudaStream_t s, long long* launches);
+cudaError_t ace_apply(exx_plan* p, const double* xi, int n, const double* phi, int m, double* out, double* ws,
+                      cudaStream_t s, long long* launches);
 cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,
                              const FastArgs* fa, cudaStream_t s, long long* launches);
 

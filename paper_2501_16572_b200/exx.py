@@ -70,6 +70,12 @@ def load_library():
     lib.exx_plan_set_lanes.argtypes = [vp, C.c_int]
     lib.exx_plan_get_lanes.restype = C.c_int
     lib.exx_plan_get_lanes.argtypes = [vp]
+    lib.exx_ace_workspace_bytes.restype = C.c_size_t
+    lib.exx_ace_workspace_bytes.argtypes = [vp, C.c_int, C.c_int]
+    lib.exx_ace_build.restype = C.c_int
+    lib.exx_ace_build.argtypes = [vp, dp, dp, C.c_int, dp, dp, vp, vp, C.c_size_t, vp]
+    lib.exx_ace_apply.restype = C.c_int
+    lib.exx_ace_apply.argtypes = [vp, dp, C.c_int, dp, C.c_int, dp, vp, C.c_size_t, vp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
     lib.exx_plan_set_profiling.restype = C.c_int
@@ -145,6 +151,7 @@ class Plan:
             self._lib.exx_plan_destroy(self._h)
             self._h = C.c_void_p()
         self._ws = None
+        self._aws = None
 
     def __del__(self):
         try:
@@ -243,6 +250,52 @@ class Plan:
                                  C.c_void_p(s.cuda_stream))
         _check(st, "exx_apply")
         return vx, ex_k, ex
+
+    def ace_workspace_bytes(self, n_orb: int, n_trial: int = 0) -> int:
+        return int(self._lib.exx_ace_workspace_bytes(self._h, n_orb, n_trial))
+
+    def _ace_ws(self, n_orb: int, n_trial: int) -> torch.Tensor:
+        need = self.ace_workspace_bytes(n_orb, n_trial)
+        if getattr(self, "_aws", None) is None or self._aws.numel() < need:
+            self._aws = None
+            self._aws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._aws
+
+    def ace_build(self, psi: torch.Tensor, w: torch.Tensor, xi: torch.Tensor | None = None, want_M: bool = True,
+                  stream: torch.cuda.Stream | None = None):
+        """exx_ace_build (PAPER.md:163-230, Eqs. 17-20, 26): returns (xi [n, nz, ny, nx], M [n, n] or None,
+        info int32 0-dim device tensor).  ``xi`` may be ``w`` (in place)."""
+        n = psi.shape[0]
+        if psi.numel() != n * self.N or w.numel() != n * self.N:
+            raise ValueError("psi/w must be [n, nz, ny, nx]")
+        if xi is None:
+            xi = torch.empty_like(w)
+        M = torch.empty((n, n), dtype=torch.float64, device=self.device) if want_M else None
+        info = torch.zeros((), dtype=torch.int32, device=self.device)
+        ws = self._ace_ws(n, 0)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_ace_build(self._h, _dev_ptr(psi, self.device, "psi"), _dev_ptr(w, self.device, "w"), n,
+                                     _dev_ptr(xi, self.device, "xi"), _dev_ptr(M, self.device, "M"),
+                                     C.c_void_p(info.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(),
+                                     C.c_void_p(s.cuda_stream))
+        _check(st, "exx_ace_build")
+        return xi, M, info
+
+    def ace_apply(self, xi: torch.Tensor, phi: torch.Tensor, out: torch.Tensor | None = None,
+                  stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+        """exx_ace_apply (Eqs. 27-29): out = -xi (h^3 xi^T phi), [m, nz, ny, nx]."""
+        n, m = xi.shape[0], phi.shape[0]
+        if xi.numel() != n * self.N or phi.numel() != m * self.N:
+            raise ValueError("xi/phi must be [n, nz, ny, nx]")
+        if out is None:
+            out = torch.empty_like(phi)
+        ws = self._ace_ws(n, m)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_ace_apply(self._h, _dev_ptr(xi, self.device, "xi"), n, _dev_ptr(phi, self.device, "phi"), m,
+                                     _dev_ptr(out, self.device, "out"), C.c_void_p(ws.data_ptr()), ws.numel(),
+                                     C.c_void_p(s.cuda_stream))
+        _check(st, "exx_ace_apply")
+        return out
 
     def apply_host(self, psi, occ, tgt=None, tgt_start: int = -1, n_tgt: int | None = None, occ_tgt=None,
                    vx=None, n_c: int = 0):
