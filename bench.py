@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--n-tgt", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-ace", action="store_true", help="skip the ACE tail/apply measurement (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -299,6 +300,45 @@ def run_b200(args):
                "d2h_bytes_per_step": int(h_vx.numel() * 8 + w.n_tgt * 8 + 8), "ms_per_step": dt * 1e3,
                "api": "exx_apply_host (pinned host buffers; synchronous; wall clock)", "ex": ex_h}
 
+    # ---- ACE tail and application, when the targets are the orbitals themselves ---
+    ace = None
+    if not args.no_ace and world == 1 and w.n_tgt == w.n_orb and w.tgt_start == 0:
+        n = w.n_orb
+        xi = torch.empty_like(vx)
+        out = torch.empty_like(vx)
+
+        def timed(fn, reps=5):
+            for _ in range(2):
+                fn()
+            ts = []
+            for _ in range(reps):
+                flush.fill_(1)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                fn()
+                b.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            return statistics.median(ts)
+
+        info_box = []
+        ms_build = timed(lambda: info_box.append(plan.ace_build(d_psi, vx, xi=xi, want_M=False, stream=stream)[2]))
+        n_launch_build = plan.last_launch_count
+        ms_apply = timed(lambda: plan.ace_apply(xi, d_psi, out=out, stream=stream))
+        n_launch_apply = plan.last_launch_count
+        fl_build = 2.0 * n * n * w.N + sum(2.0 * min(64, n - kb) * (kb + min(64, n - kb)) * w.N
+                                           for kb in range(0, n, 64)) + n ** 3 / 3.0
+        fl_apply = 4.0 * n * n * w.N
+        ace = {"build_ms": ms_build, "apply_ms": ms_apply, "info": int(info_box[-1].item()),
+               "build_tflops": fl_build / ms_build / 1e9, "apply_tflops": fl_apply / ms_apply / 1e9,
+               "build_frac_of_dmma_peak": fl_build / ms_build / 1e9 / peak_dmma,
+               "apply_frac_of_dmma_peak": fl_apply / ms_apply / 1e9 / peak_dmma,
+               "apply_columns_per_s": n / (ms_apply * 1e-3), "launches": [int(n_launch_build), int(n_launch_apply)],
+               "max_abs_err_ace_psi_minus_vx": float((out - vx).abs().max().item()),
+               "max_abs_vx": float(vx.abs().max().item()),
+               "what": "exx_ace_build(psi, W=vx) and exx_ace_apply(xi, psi): median of 5, L2 flushed, CUDA events; "
+                       "share of the exchange step = (build_ms) / ms_per_step"}
+
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         cpu_baseline, _, _ = time_oracle(w, psi.cpu(), occ.cpu(), tgt.cpu(), occ_t.cpu(), args.cpu_seconds)
@@ -309,7 +349,7 @@ def run_b200(args):
             "config": config_dict(w, n_c, {"parallelism": f"targets sharded over {world} rank(s), orbitals replicated"}),
             "applies_per_s": world * w.n_tgt / (ms_per_step * 1e-3), "E_x": ex_val,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches_per_step * args.steps),
-            "roofline": roofline, "cpu_baseline": cpu_baseline}
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "ace": ace}
     print(json.dumps(line), flush=True)
     plan.close()
     if world > 1:

@@ -127,6 +127,22 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
                      size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * Pair-symmetric exchange apply for the case targets == orbitals: phi_jk = phi_kj
+ * (Eq. 2, is symmetric in the pair for real orbitals), so only the pairs j <= k are solved and each
+ * solution feeds both vx_k (-= occ_j psi_j phi_jk) and, for j != k, vx_j (-= occ_k psi_k phi_jk).  Same result as
+ * exx_apply(psi, occ, n, psi, occ, n, ...) up to the order of the sum over j (not bitwise: the terms arrive in a
+ * different order), with about half the Poisson solves: exx_plan_last_solve_count reports how many were executed
+ * (n(n+1)/2 plus the few j > k pairs inside the diagonal blocks of the rectangular batches).
+ * d_vx [n_orb][N] is overwritten; d_ex / d_ex_k as in exx_apply with occ_tgt = occ.  Same workspace and errors.
+ */
+exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double* d_occ, int n_orb, double* d_vx,
+                               double* d_ex, double* d_ex_k, int n_c, void* d_workspace, size_t workspace_bytes,
+                               void* cuda_stream);
+
+/* Pair solves executed by the last exx_apply (n_occ*n_tgt) / exx_apply_symmetric call on this plan. */
+long long exx_plan_last_solve_count(const exx_plan* plan);
+
+/*
  * Convenience end-to-end call with HOST buffers (pageable or pinned): uploads psi/occ (and tgt unless
  * tgt_start >= 0 selects the block h_psi[tgt_start .. tgt_start+n_tgt) as targets), runs exx_apply on an
  * internal stream, downloads vx / e_k / E_x and synchronises.  Device buffers are allocated and freed

@@ -110,7 +110,7 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->h = h; p->order = fd_order; p->omega = omega; p->max_batch = max_batch; p->device = device;
   p->variant = EXX_VARIANT_FUSED_DMMA;
   p->N = (long long)nx * ny * nz;
-  p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->tma_launches = 0;
+  p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; }
@@ -237,6 +237,8 @@ exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult) {
 }
 
 long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }
+
+long long exx_plan_last_solve_count(const exx_plan* plan) { return plan ? plan->last_solves : 0; }
 
 long long exx_plan_tma_launch_count(const exx_plan* plan) { return plan ? plan->tma_launches : 0; }
 
@@ -385,7 +387,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
           }
           launches += 2;
         } else {
-          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0};
+          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0, false};
           EXX_CUDA(exx::fast_solve_batch(plan, nullptr, lane1 ? buf1 : buf0, two_lanes ? nullptr : buf1, nb, &fa, ls,
                                          &launches));
         }
@@ -415,6 +417,93 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     }
   }
   plan->last_launches = launches;
+  plan->last_solves = (long long)n_occ * n_tgt;
+  return EXX_OK;
+}
+
+exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double* d_occ, int n_orb, double* d_vx,
+                               double* d_ex, double* d_ex_k, int n_c, void* d_workspace, size_t workspace_bytes,
+                               void* cuda_stream) {
+  if (!plan || n_orb < 0) return EXX_ERR_INVALID_ARG;
+  if (n_orb > 0 && (!d_psi || !d_occ || !d_vx)) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
+  const size_t need = exx_plan_workspace_bytes(plan, n_c);
+  if (n_orb > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
+  if (overlaps(d_vx, fn * n_orb, d_psi, fn * n_orb) || overlaps(d_vx, fn * n_orb, d_workspace, need) ||
+      overlaps(d_workspace, need, d_psi, fn * n_orb))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  long long launches = 0, solves = 0;
+  PlanExtras* ex = extras_of(plan);
+  double* buf0 = (double*)d_workspace;
+  double* buf1 = buf0 + N * (size_t)n_c;
+  if (n_orb > 0) {
+    // contributions are scattered to vx_k and vx_j: start from zero, every batch accumulates
+    EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_orb, s));
+    ++launches;
+  }
+  auto run_batch = [&](int j0, int nj, int k0, int nk) -> exx_status {
+    const exx::BatchDesc bd{j0, nj, k0, nk};
+    const int nb = nj * nk;
+    solves += nb;
+    if (plan->variant == EXX_VARIANT_REFERENCE) {
+      {
+        exx::ProfScope ps(plan, exx::KC_PAIR_DENSITY, s);
+        EXX_CUDA(exx::ref_pair_density(plan, d_psi, d_psi, bd, buf0, s));
+      }
+      EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
+      {
+        exx::ProfScope ps(plan, exx::KC_ACCUMULATE, s);
+        EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, false, d_vx, s, true));
+        EXX_CUDA(exx::sym_accumulate_transposed(plan, d_psi, d_occ, buf0, bd, d_vx, s));
+      }
+      launches += 3;
+    } else {
+      const exx::FastArgs fa{d_psi, d_psi, d_occ, d_vx, bd, n_orb, n_orb, false, true};
+      EXX_CUDA(exx::fast_solve_batch(plan, nullptr, buf0, buf1, nb, &fa, s, &launches));
+    }
+    return EXX_OK;
+  };
+  // Batches are rectangles of the (j,k) plane that cover the triangle j <= k: a block of nk consecutive targets
+  // against the orbitals 0 .. k0+nk-1 (the nk(nk-1)/2 pairs with j > k inside the diagonal block are solved and
+  // ignored), nk as large as n_c allows; a target with more than n_c partners is cut into j-chunks.
+  for (int k0 = 0; k0 < n_orb;) {
+    int nk = 1;
+    while (k0 + nk + 1 <= n_orb && (long long)(nk + 1) * (k0 + nk + 1) <= n_c) ++nk;
+    if (k0 + nk > n_c) {
+      nk = 1;
+      for (int j0 = 0; j0 <= k0; j0 += n_c) {
+        const int nj = k0 + 1 - j0 < n_c ? k0 + 1 - j0 : n_c;
+        exx_status st = run_batch(j0, nj, k0, 1);
+        if (st != EXX_OK) return st;
+      }
+    } else {
+      exx_status st = run_batch(0, k0 + nk, k0, nk);
+      if (st != EXX_OK) return st;
+    }
+    k0 += nk;
+  }
+  if (d_ex && n_orb == 0) {
+    EXX_CUDA(exx::zero_fill(d_ex, 1, s));
+    ++launches;
+  }
+  if ((d_ex || d_ex_k) && n_orb > 0) {
+    for (int k0 = 0; k0 < n_orb; k0 += kEnergyChunk) {
+      const int nk = n_orb - k0 < kEnergyChunk ? n_orb - k0 : kEnergyChunk;
+      if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
+      {
+        exx::ProfScope ps(plan, exx::KC_OTHER, s);
+        EXX_CUDA(exx::energy(plan, d_psi + N * (size_t)k0, d_vx + N * (size_t)k0, d_occ + k0, nk,
+                             ex->d_energy_scratch, d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
+      }
+      launches += 2;
+    }
+  }
+  plan->last_launches = launches;
+  plan->last_solves = solves;
   return EXX_OK;
 }
 

@@ -51,6 +51,7 @@ struct exx_plan {
   int sm_count;
   int smem_optin;
   long long last_launches;
+  long long last_solves;   // pair solves the last exx_apply / exx_apply_symmetric call executed
   long long tma_launches;  // cumulative count of TMA-staged mode-product launches (test hook)
   // exx_apply runs `lanes` batches at a time (1 or 2): lane 0 on the caller's stream, lane 1 on lane_stream,
   // forked and joined with the two events
@@ -75,7 +76,10 @@ cudaError_t ref_pair_density(const exx_plan* p, const double* psi, const double*
 cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const double* in, double* out,
                              int nb, bool apply_mult, cudaStream_t s);
 cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
-                           BatchDesc bd, bool first, double* vx, cudaStream_t s);
+                           BatchDesc bd, bool first, double* vx, cudaStream_t s, bool sym = false);
+// pair-symmetric apply: vx_j -= sum_{k in batch, k > j} occ_k psi_k phi_jk for every j of the batch
+cudaError_t sym_accumulate_transposed(const exx_plan* p, const double* psi, const double* occ, const double* phi,
+                                      BatchDesc bd, double* vx, cudaStream_t s);
 // shared by both variants: e_k = h^3 <tgt_k, vx_k>, then E_x
 cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
                    int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s);
@@ -113,6 +117,7 @@ struct FastArgs {
   BatchDesc bd;
   int n_occ, n_tgt;  // extents of psi / tgt (tensor maps cover the whole arrays)
   bool first;  // first batch for these targets: vx is overwritten, not accumulated into
+  bool sym;    // pair-symmetric apply (tgt == psi): only j <= k contributes to vx_k, and phi_jk also feeds vx_j
 };
 // ---- TMA-staged mode products (kernels_tma.cu), the default; cudaErrorNotSupported -> cp.async kernels ----
 cudaError_t tma_init(exx_plan* p);

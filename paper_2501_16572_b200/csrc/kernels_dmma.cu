@@ -547,7 +547,11 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   if (fa) {
     {
       ProfScope ps(p, KC_ACCUMULATE, s);
-      e = ref_accumulate(p, fa->psi, fa->occ, cur, fa->bd, fa->first, fa->vx, s);
+      e = ref_accumulate(p, fa->psi, fa->occ, cur, fa->bd, fa->first, fa->vx, s, fa->sym);
+      if (e == cudaSuccess && fa->sym) {
+        e = sym_accumulate_transposed(p, fa->psi, fa->occ, cur, fa->bd, fa->vx, s);
+        ++*launches;
+      }
     }
     if (e != cudaSuccess) return e;
     ++*launches;

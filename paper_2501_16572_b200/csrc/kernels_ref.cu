@@ -55,13 +55,15 @@ __global__ void k_mode_product(const double* __restrict__ in, double* __restrict
 template <int VEC, int UNROLL>
 __global__ void __launch_bounds__(256) k_accumulate(const double* __restrict__ psi, const double* __restrict__ occ,
                                                     const double* __restrict__ phi, BatchDesc bd, bool first,
-                                                    unsigned N, double* __restrict__ vx) {
+                                                    unsigned N, double* __restrict__ vx, bool sym) {
   const int kk = blockIdx.y;
-  const int nj = bd.nj;
+  // sym (pair-symmetric apply): only the pairs j <= k of the rectangular batch contribute to vx_k
+  const int nj = sym ? min(bd.nj, bd.k0 + kk - bd.j0 + 1) : bd.nj;
+  if (nj <= 0) return;
   double* v = vx + (size_t)(bd.k0 + kk) * N;
   const double* oc = occ + bd.j0;
   const double* psi0 = psi + (size_t)bd.j0 * N;
-  const double* phi0 = phi + (size_t)kk * nj * N;
+  const double* phi0 = phi + (size_t)kk * bd.nj * N;
   const unsigned stride = gridDim.x * blockDim.x * VEC;
   for (unsigned i = (blockIdx.x * blockDim.x + threadIdx.x) * VEC; i < N; i += stride) {
     double acc[VEC];
@@ -98,6 +100,42 @@ __global__ void __launch_bounds__(256) k_accumulate(const double* __restrict__ p
       for (int e = 0; e < VEC; ++e) acc[e] -= o * pj[e] * ph[e];
       pj += N;
       ph += N;
+    }
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) v[i + e] = acc[e];
+  }
+}
+
+// Pair-symmetric apply, the transposed contribution (phi_jk = phi_kj): for every j of the
+// batch, vx_j(r) -= sum_{k in batch, k > j} occ_k psi_k(r) phi_jk(r), k ascending.  grid.y = nj.
+template <int VEC>
+__global__ void __launch_bounds__(256) k_accumulate_transposed(const double* __restrict__ psi,
+                                                               const double* __restrict__ occ,
+                                                               const double* __restrict__ phi, BatchDesc bd,
+                                                               unsigned N, double* __restrict__ vx) {
+  const int jj = blockIdx.y;
+  const int j = bd.j0 + jj;
+  int kk0 = j + 1 - bd.k0;  // first target of the batch with k > j
+  if (kk0 < 0) kk0 = 0;
+  if (kk0 >= bd.nk) return;
+  double* v = vx + (size_t)j * N;
+  const unsigned stride = gridDim.x * blockDim.x * VEC;
+  for (unsigned i = (blockIdx.x * blockDim.x + threadIdx.x) * VEC; i < N; i += stride) {
+    double acc[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) acc[e] = v[i + e];
+    for (int kk = kk0; kk < bd.nk; ++kk) {
+      const double o = occ[bd.k0 + kk];
+      const double* pk = psi + (size_t)(bd.k0 + kk) * N + i;
+      const double* ph = phi + ((size_t)kk * bd.nj + jj) * N + i;
+      if (VEC == 2) {
+        const double2 x = *reinterpret_cast<const double2*>(pk);
+        const double2 y = *reinterpret_cast<const double2*>(ph);
+        acc[0] -= o * x.x * y.x;
+        acc[VEC - 1] -= o * x.y * y.y;
+      } else {
+        acc[0] -= o * pk[0] * ph[0];
+      }
     }
 #pragma unroll
     for (int e = 0; e < VEC; ++e) v[i + e] = acc[e];
@@ -191,18 +229,32 @@ cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const do
 }
 
 cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
-                           BatchDesc bd, bool first, double* vx, cudaStream_t s) {
+                           BatchDesc bd, bool first, double* vx, cudaStream_t s, bool sym) {
   static const int variant = [] { const char* e = getenv("EXX_ACC"); return e ? atoi(e) : 1; }();
   const unsigned N = (unsigned)p->N;
   const bool vec2 = (N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
   if (vec2 && variant >= 2) {
     dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nk);
-    if (variant == 3) k_accumulate<2, 8><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
-    else k_accumulate<2, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+    if (variant == 3) k_accumulate<2, 8><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
+    else k_accumulate<2, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
   } else {
     dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
-    if (variant == 0) k_accumulate<1, 2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
-    else k_accumulate<1, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx);
+    if (variant == 0) k_accumulate<1, 2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
+    else k_accumulate<1, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t sym_accumulate_transposed(const exx_plan* p, const double* psi, const double* occ, const double* phi,
+                                      BatchDesc bd, double* vx, cudaStream_t s) {
+  const unsigned N = (unsigned)p->N;
+  const bool vec2 = (N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
+  if (vec2) {
+    dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nj);
+    k_accumulate_transposed<2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, N, vx);
+  } else {
+    dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nj);
+    k_accumulate_transposed<1><<<grid, 256, 0, s>>>(psi, occ, phi, bd, N, vx);
   }
   return cudaGetLastError();
 }

@@ -60,6 +60,10 @@ def load_library():
     lib.exx_poisson_solve.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
     lib.exx_apply.restype = C.c_int
     lib.exx_apply.argtypes = [vp, dp, dp, C.c_int, dp, dp, C.c_int, dp, dp, dp, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_apply_symmetric.restype = C.c_int
+    lib.exx_apply_symmetric.argtypes = [vp, dp, dp, C.c_int, dp, dp, dp, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_plan_last_solve_count.restype = C.c_longlong
+    lib.exx_plan_last_solve_count.argtypes = [vp]
     lib.exx_apply_host.restype = C.c_int
     lib.exx_apply_host.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, dp, C.c_int, dp, dp, dp, C.c_int]
     lib.exx_plan_last_launch_count.restype = C.c_longlong
@@ -250,6 +254,29 @@ class Plan:
                                  C.c_void_p(s.cuda_stream))
         _check(st, "exx_apply")
         return vx, ex_k, ex
+
+    def apply_symmetric(self, psi: torch.Tensor, occ: torch.Tensor, vx: torch.Tensor | None = None, n_c: int = 0,
+                        want_ex_k: bool = True, stream: torch.cuda.Stream | None = None):
+        """exx_apply_symmetric: targets == orbitals, only the pairs j <= k are solved.  Returns (vx, e_k, E_x)."""
+        n = psi.shape[0]
+        if psi.numel() != n * self.N:
+            raise ValueError("psi must be [n, nz, ny, nx]")
+        if vx is None:
+            vx = torch.empty((n, self.nz, self.ny, self.nx), dtype=torch.float64, device=self.device)
+        ex = torch.empty((), dtype=torch.float64, device=self.device)
+        ex_k = torch.empty(n, dtype=torch.float64, device=self.device) if want_ex_k else None
+        ws = self._workspace(n_c)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_apply_symmetric(self._h, _dev_ptr(psi, self.device, "psi"), _dev_ptr(occ, self.device, "occ"),
+                                           n, _dev_ptr(vx, self.device, "vx"), _dev_ptr(ex, self.device, "ex"),
+                                           _dev_ptr(ex_k, self.device, "ex_k"), n_c, C.c_void_p(ws.data_ptr()),
+                                           ws.numel(), C.c_void_p(s.cuda_stream))
+        _check(st, "exx_apply_symmetric")
+        return vx, ex_k, ex
+
+    @property
+    def last_solve_count(self) -> int:
+        return int(self._lib.exx_plan_last_solve_count(self._h))
 
     def ace_workspace_bytes(self, n_orb: int, n_trial: int = 0) -> int:
         return int(self._lib.exx_ace_workspace_bytes(self._h, n_orb, n_trial))
