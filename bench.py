@@ -28,6 +28,10 @@ import torch  # noqa: E402
 
 from paper_2501_16572_b200 import workloads as wl  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per k_mode_t launch (average over the six passes of a batch) from the
+# `ncu --set full` captures summarised in profiles/r1_final_summary.md, keyed by (config, n_c); other shapes: null.
+NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (5, 128): 3.545e9}
+
 METRIC = "poisson_pair_solves_per_s"
 UNIT = "solves/s"
 
@@ -270,7 +274,9 @@ def run_b200(args):
     achieved = flops_step * prof_steps / (mp_ms * 1e-3) / 1e12 if mp_ms > 0 else 0.0
     roofline = {"bound": "tensor", "kernel": "k_mode_dmma (six mode products per batch, FP64 mma.sync -> DMMA.8x8x4)",
                 "achieved": achieved, "peak": peak_dmma, "unit": "TFLOP/s", "frac": achieved / peak_dmma,
-                "traffic": None,
+                "traffic": NCU_TRAFFIC_BYTES.get((w.cfg, n_c)),
+                "traffic_note": "bytes per k_mode_t launch, profiles/r1_final_summary.md (cold-cache ncu replay); "
+                                f"algorithmic bytes per launch = {2 * 8 * w.N * min(n_c, w.pair_solves):.4g} (batch read + written in place)",
                 "peak_source": "measured live: exx_probe_fp64_peak DMMA issue loop (MEASURED_PEAKS.json has no FP64 entry); "
                                f"DFMA loop {peak_dfma:.2f} TF",
                 "avg_launch_ms": mp_ms / max(mp_cnt, 1), "launches": mp_cnt // prof_steps,
@@ -339,6 +345,32 @@ def run_b200(args):
                "what": "exx_ace_build(psi, W=vx) and exx_ace_apply(xi, psi): median of 5, L2 flushed, CUDA events; "
                        "share of the exchange step = (build_ms) / ms_per_step"}
 
+    # ---- pair-symmetric apply: same result from about half the solves --------------
+    symmetric = None
+    if not args.no_ace and world == 1 and w.n_tgt == w.n_orb and w.tgt_start == 0:
+        vx_s = torch.empty_like(vx)
+        for _ in range(2):
+            plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c, stream=stream)
+        ts = []
+        for _ in range(min(args.steps, 5)):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            _, _, ex_s = plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ms_s = statistics.median(ts)
+        executed = plan.last_solve_count
+        symmetric = {"ms_per_step": ms_s, "executed_solves_per_step": int(executed),
+                     "executed_solves_per_s": executed / (ms_s * 1e-3),
+                     "pair_equivalent_solves_per_s": w.pair_solves / (ms_s * 1e-3),
+                     "applies_per_s": w.n_tgt / (ms_s * 1e-3), "speedup_vs_full": ms_per_step / ms_s,
+                     "step_frac_executed": executed * w.flops_per_solve / (ms_s * 1e-3) / 1e12 / peak_dmma,
+                     "E_x": float(ex_s.item()),
+                     "max_rel_diff_vs_full": float(((vx_s - vx).abs().max() / vx.abs().max()).item()),
+                     "what": "exx_apply_symmetric: only pairs j <= k solved; roofline credit only for executed solves"}
+
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         cpu_baseline, _, _ = time_oracle(w, psi.cpu(), occ.cpu(), tgt.cpu(), occ_t.cpu(), args.cpu_seconds)
@@ -349,7 +381,7 @@ def run_b200(args):
             "config": config_dict(w, n_c, {"parallelism": f"targets sharded over {world} rank(s), orbitals replicated"}),
             "applies_per_s": world * w.n_tgt / (ms_per_step * 1e-3), "E_x": ex_val,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches_per_step * args.steps),
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "ace": ace}
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "ace": ace, "symmetric": symmetric}
     print(json.dumps(line), flush=True)
     plan.close()
     if world > 1:
