@@ -231,3 +231,26 @@ def test_two_lanes_bitwise_equal_to_one_lane(cfg, n_orb, n_tgt, n_c):
     with pytest.raises(exx.ExxError):
         plan.set_lanes(3)
     plan.close()
+
+
+def test_apply_is_cuda_graph_capturable():
+    """include/exx.h: "The calls are CUDA-graph capturable" -- capture one exx_apply (PDL launches included) on a
+    side stream, replay it twice, and compare bitwise with the eager result."""
+    w = wl.scaled(wl.WORKLOADS[1], 8)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    plan = exx.Plan.for_workload(w, device=0)
+    d_psi, d_occ = psi.cuda(), occ.cuda()
+    vx_eager, ek_eager, ex_eager = plan.apply(d_psi, d_occ, d_psi, d_occ, n_c=4)   # also warms up attributes / tensor maps
+    torch.cuda.synchronize()
+    vx = torch.zeros_like(vx_eager)
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.graph(g, stream=s):
+        _, ek, ex = plan.apply(d_psi, d_occ, d_psi, d_occ, vx=vx, n_c=4, stream=torch.cuda.current_stream())
+    for _ in range(2):
+        vx.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(vx, vx_eager) and torch.equal(ek, ek_eager) and torch.equal(ex, ex_eager)
+    plan.close()
