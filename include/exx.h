@@ -177,6 +177,35 @@ exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w,
 exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
                          double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * Bloch-periodic (k-point) variant, complex FP64 (Eqs. 1-3 "subject to Bloch
+ * boundary conditions at the wavevector k-q in the directions that the system is extended"; :159, :218 complex
+ * arithmetic).  Readings R18-R20:
+ *   - theta[a] = (k-q)_a * n_a * h is the Bloch phase across the cell along periodic axis a (ignored on Dirichlet
+ *     axes): u(x + n_a h) = exp(i theta[a]) u(x); the 1-D FD matrix is Hermitian, K = V diag(lam) V^H.
+ *   - one call handles ONE (k,q) pair: every d_psi[j] carries the phase of q, every d_tgt[k] that of k, the plan is
+ *     built for theta = theta_k - theta_q; the caller loops over q with `accumulate` != 0 and passes
+ *     d_occ[j] = w_q * g_jq (used verbatim).
+ *   - a complex grid function is two real planes [2][N] (real part, then imaginary part); a set is [n][2][N].
+ *       d_vx[k] (+)= - sum_j d_occ[j] * d_psi[j] .* f(L_theta)( conj(d_psi[j]) .* d_tgt[k] )
+ *       d_ex_k[k] = h^3 Re <d_tgt[k], d_vx[k]>            (optional, NULL; computed after the update)
+ * exx_plan_create_bloch validates like exx_plan_create (theta must be finite).  Workspace:
+ * exx_plan_workspace_bytes_bloch(plan, n_c) (three buffers of n_c complex functions).  A complex mode product runs
+ * as two launches of the real tensor-core kernel (real and imaginary part of V) plus a combine; axes whose matrix is
+ * real (Dirichlet, theta = 0) take one.  exx_apply / exx_poisson_solve / exx_ace_* on a plan with a nonzero phase
+ * return EXX_ERR_INVALID_ARG.  Errors and aliasing rules as for exx_apply.
+ */
+exx_status exx_plan_create_bloch(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
+                                 double omega, const double theta[3], int max_batch, int device);
+size_t exx_plan_workspace_bytes_bloch(const exx_plan* plan, int n_c);
+exx_status exx_poisson_solve_bloch(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
+                                   void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+exx_status exx_apply_bloch(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ, const double* d_tgt,
+                           int n_tgt, double* d_vx, int accumulate, double* d_ex_k, int n_c, void* d_workspace,
+                           size_t workspace_bytes, void* cuda_stream);
+/* Test hook: eigenpairs of one axis of a Bloch plan; h_V_re / h_V_im column-major like exx_plan_get_axis. */
+exx_status exx_plan_get_axis_bloch(const exx_plan* plan, int axis, double* h_lambda, double* h_V_re, double* h_V_im);
+
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);
 

@@ -52,6 +52,10 @@ inline int default_lanes(const exx_plan* p) {
   return 1;
 }
 
+// a plan with a nonzero Bloch phase has complex eigenvectors: only the *_bloch entry points may use it
+inline bool is_complex_plan(const exx_plan* p) { return p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
+                                                         !p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty(); }
+
 inline int resolve_nc(const exx_plan* p, int n_c) {
   if (n_c == 0) n_c = p->max_batch < kDefaultBatch ? p->max_batch : kDefaultBatch;
   return n_c;
@@ -93,8 +97,11 @@ const char* exx_status_string(exx_status s) {
   return "unknown exx_status";
 }
 
-exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3],
-                           int fd_order, double omega, int max_batch, int device) {
+}  // extern "C"
+
+// exx_plan_create / exx_plan_create_bloch (theta == nullptr: real plan)
+static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
+                              double omega, const double* theta, int max_batch, int device) {
   if (!out) return EXX_ERR_INVALID_ARG;
   *out = nullptr;
   if (nx < 1 || ny < 1 || nz < 1 || !(h > 0.0) || !std::isfinite(h) || !bc || fd_order < 2 ||
@@ -113,17 +120,30 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
-  for (int a = 0; a < 3; ++a) { p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; }
+  for (int a = 0; a < 3; ++a) {
+    p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
+    // a Bloch phase only exists on a periodic axis; theta == 0 there is the real periodic matrix
+    p->theta[a] = (theta && bc[a] == EXX_BC_PERIODIC) ? theta[a] : 0.0;
+    if (theta && !std::isfinite(theta[a])) { delete p; return EXX_ERR_INVALID_ARG; }
+  }
 
   try {
     for (int a = 0; a < 3; ++a) {
       // identical axes share the eigendecomposition (and, on the device, the matrix)
       int same = -1;
       for (int b = 0; b < a; ++b)
-        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a]) same = b;
+        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a] && p->theta[b] == p->theta[a]) same = b;
       if (same >= 0) {
         p->h_lam[a] = p->h_lam[same];
         p->h_V[a] = p->h_V[same];
+        p->h_Vi[a] = p->h_Vi[same];
+        continue;
+      }
+      if (p->theta[a] != 0.0) {
+        if (!exx::bloch_eigh(p->n[a], h, fd_order, p->theta[a], p->h_lam[a], p->h_V[a], p->h_Vi[a])) {
+          delete p;
+          return EXX_ERR_EIGENSOLVE;
+        }
         continue;
       }
       std::vector<double> K = exx::second_derivative_matrix(p->n[a], h, bc[a], fd_order);
@@ -147,11 +167,15 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
     for (int a = 0; a < 3 && e == cudaSuccess; ++a) {
       int same = -1;
       for (int b = 0; b < a; ++b)
-        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a]) same = b;
-      if (same >= 0) { p->d_V[a] = p->d_V[same]; continue; }
+        if (p->n[b] == p->n[a] && p->bc[b] == p->bc[a] && p->theta[b] == p->theta[a]) same = b;
+      if (same >= 0) { p->d_V[a] = p->d_V[same]; p->d_Vi[a] = p->d_Vi[same]; continue; }
       const size_t bytes = sizeof(double) * p->h_V[a].size();
       e = cudaMalloc(&p->d_V[a], bytes);
       if (e == cudaSuccess) e = cudaMemcpy(p->d_V[a], p->h_V[a].data(), bytes, cudaMemcpyHostToDevice);
+      if (e == cudaSuccess && !p->h_Vi[a].empty()) {
+        e = cudaMalloc(&p->d_Vi[a], bytes);
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_Vi[a], p->h_Vi[a].data(), bytes, cudaMemcpyHostToDevice);
+      }
     }
     if (e == cudaSuccess) e = cudaMalloc(&p->d_mult, sizeof(double) * p->N);
     if (e == cudaSuccess)
@@ -173,6 +197,19 @@ exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, con
   return EXX_OK;
 }
 
+extern "C" {
+
+exx_status exx_plan_create(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3],
+                           int fd_order, double omega, int max_batch, int device) {
+  return create_plan(out, nx, ny, nz, h, bc, fd_order, omega, nullptr, max_batch, device);
+}
+
+exx_status exx_plan_create_bloch(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
+                                 double omega, const double theta[3], int max_batch, int device) {
+  if (!theta) return EXX_ERR_INVALID_ARG;
+  return create_plan(out, nx, ny, nz, h, bc, fd_order, omega, theta, max_batch, device);
+}
+
 exx_status exx_plan_destroy(exx_plan* plan) {
   if (!plan) return EXX_OK;
   exx_plan_full* p = static_cast<exx_plan_full*>(plan);
@@ -187,6 +224,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
       bool shared = false;
       for (int b = 0; b < a; ++b) shared |= (p->d_V[b] == p->d_V[a]);
       if (!shared && p->d_V[a]) cudaFree(p->d_V[a]);
+      if (!shared && p->d_Vi[a]) cudaFree(p->d_Vi[a]);
     }
     if (p->d_mult) cudaFree(p->d_mult);
     if (p->ex.d_energy_scratch) cudaFree(p->ex.d_energy_scratch);
@@ -294,6 +332,7 @@ extern "C" {
 exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
                              void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!plan || n_rhs < 0 || (n_rhs > 0 && (!d_rhs || !d_phi))) return EXX_ERR_INVALID_ARG;
+  if (is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
@@ -330,6 +369,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
                      double* d_ex, double* d_ex_k, int n_c, void* d_workspace,
                      size_t workspace_bytes, void* cuda_stream) {
   if (!plan || n_occ < 0 || n_tgt < 0) return EXX_ERR_INVALID_ARG;
+  if (is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   if (n_occ > 0 && (!d_psi || !d_occ)) return EXX_ERR_INVALID_ARG;
   if (n_tgt > 0 && (!d_tgt || !d_vx)) return EXX_ERR_INVALID_ARG;
   if (d_ex && !d_occ_tgt && n_tgt > 0) return EXX_ERR_INVALID_ARG;
@@ -424,7 +464,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
 exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double* d_occ, int n_orb, double* d_vx,
                                double* d_ex, double* d_ex_k, int n_c, void* d_workspace, size_t workspace_bytes,
                                void* cuda_stream) {
-  if (!plan || n_orb < 0) return EXX_ERR_INVALID_ARG;
+  if (!plan || n_orb < 0 || is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   if (n_orb > 0 && (!d_psi || !d_occ || !d_vx)) return EXX_ERR_INVALID_ARG;
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
@@ -573,7 +613,7 @@ size_t exx_ace_workspace_bytes(const exx_plan* plan, int n_orb, int n_trial) {
 
 exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w, int n_orb, double* d_xi,
                          double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
-  if (!plan || n_orb < 1 || n_orb > 32768 || !d_psi || !d_w || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (!plan || n_orb < 1 || n_orb > 32768 || !d_psi || !d_w || !d_xi || is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
   const size_t need = sizeof(double) * exx::ace_build_workspace_doubles(plan, n_orb);
   if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
@@ -594,7 +634,8 @@ exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w,
 
 exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
                          double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
-  if (!plan || n_orb < 1 || n_orb > 32768 || n_trial < 0 || n_trial > 32768 || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (!plan || n_orb < 1 || n_orb > 32768 || n_trial < 0 || n_trial > 32768 || !d_xi || is_complex_plan(plan))
+    return EXX_ERR_INVALID_ARG;
   if (n_trial > 0 && (!d_phi || !d_out)) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
   if (n_trial == 0) { plan->last_launches = 0; return EXX_OK; }
@@ -610,6 +651,115 @@ exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const do
   EXX_CUDA(exx::ace_apply(plan, d_xi, n_orb, d_phi, n_trial, d_out, (double*)d_workspace,
                           (cudaStream_t)cuda_stream, &launches));
   plan->last_launches = launches;
+  return EXX_OK;
+}
+
+size_t exx_plan_workspace_bytes_bloch(const exx_plan* plan, int n_c) {
+  if (!plan) return 0;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return 0;
+  return 6 * sizeof(double) * (size_t)plan->N * (size_t)n_c;  // three buffers of n_c complex functions
+}
+
+exx_status exx_plan_get_axis_bloch(const exx_plan* plan, int axis, double* h_lambda, double* h_V_re, double* h_V_im) {
+  if (!plan || axis < 0 || axis > 2) return EXX_ERR_INVALID_ARG;
+  const int n = plan->n[axis];
+  if (h_lambda) std::memcpy(h_lambda, plan->h_lam[axis].data(), sizeof(double) * n);
+  for (int i = 0; i < n; ++i)
+    for (int m = 0; m < n; ++m) {
+      if (h_V_re) h_V_re[i + (size_t)n * m] = plan->h_V[axis][(size_t)i * n + m];
+      if (h_V_im) h_V_im[i + (size_t)n * m] = plan->h_Vi[axis].empty() ? 0.0 : plan->h_Vi[axis][(size_t)i * n + m];
+    }
+  return EXX_OK;
+}
+
+exx_status exx_poisson_solve_bloch(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
+                                   void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_rhs < 0 || (n_rhs > 0 && (!d_rhs || !d_phi))) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  if (n_rhs == 0) { plan->last_launches = 0; return EXX_OK; }
+  const size_t need = exx_plan_workspace_bytes_bloch(plan, n_c);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if (((uintptr_t)d_workspace) & 15) return EXX_ERR_INVALID_ARG;
+  const size_t N = (size_t)plan->N, fn = 2 * sizeof(double) * N;
+  if (d_rhs != d_phi && overlaps(d_rhs, fn * n_rhs, d_phi, fn * n_rhs)) return EXX_ERR_ALIAS;
+  if (overlaps(d_workspace, need, d_phi, fn * n_rhs) || overlaps(d_workspace, need, d_rhs, fn * n_rhs))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  double* b0 = (double*)d_workspace;
+  double* const buf[3] = {b0, b0 + 2 * N * (size_t)n_c, b0 + 4 * N * (size_t)n_c};
+  long long launches = 0;
+  for (int r0 = 0; r0 < n_rhs; r0 += n_c) {
+    const int nb = n_rhs - r0 < n_c ? n_rhs - r0 : n_c;
+    EXX_CUDA(cudaMemcpyAsync(buf[0], d_rhs + 2 * N * (size_t)r0, fn * nb, cudaMemcpyDeviceToDevice, s));
+    double* res = nullptr;
+    EXX_CUDA(exx::bloch_solve_batch(plan, buf, nb, s, &launches, &res));
+    EXX_CUDA(cudaMemcpyAsync(d_phi + 2 * N * (size_t)r0, res, fn * nb, cudaMemcpyDeviceToDevice, s));
+  }
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+exx_status exx_apply_bloch(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ, const double* d_tgt,
+                           int n_tgt, double* d_vx, int accumulate, double* d_ex_k, int n_c, void* d_workspace,
+                           size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_occ < 0 || n_tgt < 0) return EXX_ERR_INVALID_ARG;
+  if (n_occ > 0 && (!d_psi || !d_occ)) return EXX_ERR_INVALID_ARG;
+  if (n_tgt > 0 && (!d_tgt || !d_vx)) return EXX_ERR_INVALID_ARG;
+  n_c = resolve_nc(plan, n_c);
+  if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  const size_t N = (size_t)plan->N, fn = 2 * sizeof(double) * N;
+  const size_t need = exx_plan_workspace_bytes_bloch(plan, n_c);
+  if (n_occ > 0 && n_tgt > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
+  if (d_workspace && (((uintptr_t)d_workspace) & 15)) return EXX_ERR_INVALID_ARG;
+  if (overlaps(d_vx, fn * n_tgt, d_psi, fn * n_occ) || overlaps(d_vx, fn * n_tgt, d_tgt, fn * n_tgt) ||
+      overlaps(d_vx, fn * n_tgt, d_workspace, need) || overlaps(d_workspace, need, d_psi, fn * n_occ) ||
+      overlaps(d_workspace, need, d_tgt, fn * n_tgt))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  long long launches = 0;
+  PlanExtras* ex = extras_of(plan);
+  if (n_tgt > 0 && n_occ == 0) {
+    if (!accumulate) { EXX_CUDA(exx::zero_fill(d_vx, 2 * (long long)N * n_tgt, s)); ++launches; }
+  } else if (n_tgt > 0) {
+    double* b0 = (double*)d_workspace;
+    double* const buf[3] = {b0, b0 + 2 * N * (size_t)n_c, b0 + 4 * N * (size_t)n_c};
+    const int nj_max = n_occ < n_c ? n_occ : n_c;
+    const int nk_max = n_c / nj_max;
+    for (int k0 = 0; k0 < n_tgt; k0 += nk_max) {
+      const int nk = n_tgt - k0 < nk_max ? n_tgt - k0 : nk_max;
+      for (int j0 = 0; j0 < n_occ; j0 += nj_max) {
+        const int nj = n_occ - j0 < nj_max ? n_occ - j0 : nj_max;
+        const exx::BatchDesc bd{j0, nj, k0, nk};
+        {
+          exx::ProfScope ps(plan, exx::KC_PAIR_DENSITY, s);
+          EXX_CUDA(exx::bloch_pair_density(plan, d_psi, d_tgt, bd, buf[0], s));
+        }
+        double* res = nullptr;
+        EXX_CUDA(exx::bloch_solve_batch(plan, buf, nj * nk, s, &launches, &res));
+        {
+          exx::ProfScope ps(plan, exx::KC_ACCUMULATE, s);
+          EXX_CUDA(exx::bloch_accumulate(plan, d_psi, d_occ, res, bd, j0 == 0 && !accumulate, d_vx, s));
+        }
+        launches += 2;
+      }
+    }
+  }
+  if (d_ex_k && n_tgt > 0) {
+    // e_k = h^3 Re <tgt_k, vx_k> = h^3 times the real dot product of the two planar arrays of length 2N (R20)
+    for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
+      const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
+      exx::ProfScope ps(plan, exx::KC_OTHER, s);
+      EXX_CUDA(exx::energy(plan, d_tgt + 2 * N * (size_t)k0, d_vx + 2 * N * (size_t)k0, nullptr, nk,
+                           ex->d_energy_scratch, d_ex_k + k0, nullptr, s, 2 * (long long)N));
+      launches += 2;
+    }
+  }
+  plan->last_launches = launches;
+  plan->last_solves = (long long)n_occ * n_tgt;
   return EXX_OK;
 }
 

@@ -16,6 +16,9 @@ std::vector<double> second_derivative_matrix(int n, double h, int bc, int order)
 // Cyclic Jacobi: A (row-major, symmetric, destroyed) -> eigenvalues ascending in lam, eigenvectors in
 // V row-major V[i*n + m] = component i of eigenvector m.  Returns false if not converged.
 bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::vector<double>& V);
+// Hermitian Bloch-periodic axis (R18): K(theta) = V diag(lam) V^H, V = Vr + i Vi row-major [i][m].
+bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& Vr,
+                std::vector<double>& Vi);
 // f(Lambda~) table (PAPER.md:61 Eq. 5, :134 Eq. 16; R1-R3), entry [a + nx*(b + ny*c)].
 std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
                                      const std::vector<double>& lz, double omega, double zero_tol);
@@ -42,8 +45,13 @@ struct exx_plan {
   long long N;
   std::vector<double> h_lam[3];
   std::vector<double> h_V[3];  // row-major [i][m]
+  // Bloch-periodic plans (exx_plan_create_bloch): imaginary parts of the eigenvectors; empty for an axis whose
+  // matrix is real (Dirichlet, or theta == 0)
+  double theta[3];
+  std::vector<double> h_Vi[3];
   std::vector<double> h_mult;
   // device copies
+  double* d_Vi[3];   // Bloch plans: imaginary parts, same layout; nullptr for a real axis
   double* d_V[3];    // row-major [i][m], n*n (axes with identical matrices share one allocation)
   double* d_Vpad[3]; // zero-padded shared-memory images of V for the DMMA kernels (kernels_dmma.cu)
   double* d_mult;    // N
@@ -82,7 +90,7 @@ cudaError_t sym_accumulate_transposed(const exx_plan* p, const double* psi, cons
                                       BatchDesc bd, double* vx, cudaStream_t s);
 // shared by both variants: e_k = h^3 <tgt_k, vx_k>, then E_x
 cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
-                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s);
+                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s, long long len = 0);
 cudaError_t zero_fill(double* p, long long n, cudaStream_t s);
 
 // RAII event pair around one launch when profiling is on (no-op otherwise).
@@ -123,7 +131,7 @@ struct FastArgs {
 cudaError_t tma_init(exx_plan* p);
 void tma_destroy(exx_plan* p);
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
-                             bool apply_mult, const FastArgs* pd, cudaStream_t s);
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part = 0);
 // ---- ACE tail and application (kernels_ace.cu) ----
 size_t ace_build_workspace_doubles(const exx_plan* p, int n);
 size_t ace_apply_workspace_doubles(const exx_plan* p, int n, int m);
@@ -131,6 +139,13 @@ cudaError_t ace_build(exx_plan* p, const double* psi, const double* w, int n, do
                       double* ws, cudaStream_t s, long long* launches);
 cudaError_t ace_apply(exx_plan* p, const double* xi, int n, const double* phi, int m, double* out, double* ws,
                       cudaStream_t s, long long* launches);
+// ---- Bloch-periodic complex variant (kernels_bloch.cu) ----
+cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd, double* out,
+                               cudaStream_t s);
+cudaError_t bloch_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi, BatchDesc bd,
+                             bool first, double* vx, cudaStream_t s);
+cudaError_t bloch_solve_batch(exx_plan* p, double* const buf[3], int nb, cudaStream_t s, long long* launches,
+                              double** result);
 cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,
                              const FastArgs* fa, cudaStream_t s, long long* launches);
 

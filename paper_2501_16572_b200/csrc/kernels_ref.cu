@@ -261,10 +261,11 @@ cudaError_t sym_accumulate_transposed(const exx_plan* p, const double* psi, cons
 
 // ex_k_scratch: n_tgt * kEnergyBlocks doubles (carved from the caller's workspace)
 cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
-                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s) {
+                   int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s, long long len) {
   if (n_tgt <= 0) return cudaSuccess;
   dim3 grid(kEnergyBlocks, n_tgt);
-  k_energy_partial<<<grid, kEnergyThreads, 0, s>>>(tgt, vx, p->N, ex_k_scratch);
+  // len: doubles per function (0 = N; the complex variant passes 2N for its two planes)
+  k_energy_partial<<<grid, kEnergyThreads, 0, s>>>(tgt, vx, len > 0 ? len : p->N, ex_k_scratch);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   k_energy_final<<<1, 256, 0, s>>>(ex_k_scratch, kEnergyBlocks, n_tgt, p->h * p->h * p->h, occ_tgt,

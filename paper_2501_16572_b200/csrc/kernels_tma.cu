@@ -440,6 +440,7 @@ struct MapEntry {
 struct TmaState {
   double* d_img[3][2];  // [axis][0 = forward (V^T), 1 = backward (V)]
   bool img_owned[3][2];
+  double* d_img_im[3][2];  // Bloch plans: images of the imaginary parts, forward = Im(V^H) = -Vi^T, backward = Vi
   std::vector<MapEntry> cache;
 };
 
@@ -575,13 +576,13 @@ inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 // cudaErrorNotSupported: sizes or alignment outside what TMA can address (odd nx, n > 128, unaligned
 // buffers, no driver entry point); the caller then uses the cp.async kernels of kernels_dmma.cu.
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
-                             bool apply_mult, const FastArgs* pd, cudaStream_t s) {
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st) return cudaErrorNotSupported;
   const int n = p->n[axis];
   ClassCfg cc;
   if (!pick_class(n, p->lanes, &cc)) return cudaErrorNotSupported;
-  const double* img = st->d_img[axis][forward ? 0 : 1];
+  const double* img = part ? st->d_img_im[axis][forward ? 0 : 1] : st->d_img[axis][forward ? 0 : 1];
   if (!img) return cudaErrorNotSupported;
   if ((p->n[0] & 1) || !aligned16(out) || (in && !aligned16(in))) return cudaErrorNotSupported;
   const bool xmode = axis == 0;
@@ -676,6 +677,7 @@ cudaError_t tma_init(exx_plan* p) {
     for (int d = 0; d < 2; ++d) {
       st->d_img[ax][d] = nullptr;
       st->img_owned[ax][d] = false;
+      st->d_img_im[ax][d] = nullptr;
     }
   p->tma_state = st;
   for (int ax = 0; ax < 3; ++ax) {
@@ -686,9 +688,28 @@ cudaError_t tma_init(exx_plan* p) {
     if (ax == 2 && p->d_V[2] == p->d_V[1] && st->d_img[1][0]) {
       st->d_img[2][0] = st->d_img[1][0];
       st->d_img[2][1] = st->d_img[1][1];
+      st->d_img_im[2][0] = st->d_img_im[1][0];
+      st->d_img_im[2][1] = st->d_img_im[1][1];
       continue;
     }
     const int n = p->n[ax], S = (n + 15) / 16, ldv = 8 * cc.mtot + 4;
+    for (int d = 0; d < 2 && !p->h_Vi[ax].empty(); ++d) {  // Bloch axis: forward M = V^H, Im = -Vi^T; backward Im = Vi
+      std::vector<double> img((size_t)16 * S * ldv, 0.0);
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int within = xmode ? ((q & 1) + 8 * (q >> 1) + 2 * kk) : (2 * q + (kk & 1) + 8 * (kk >> 1));
+            const int k = 16 * s + within;
+            if (k >= n) continue;
+            double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];
+            for (int m = 0; m < n; ++m)
+              row[m] = d == 0 ? -p->h_Vi[ax][(size_t)k * n + m] : p->h_Vi[ax][(size_t)m * n + k];
+          }
+      cudaError_t e = cudaMalloc(&st->d_img_im[ax][d], sizeof(double) * img.size());
+      if (e != cudaSuccess) return e;
+      e = cudaMemcpy(st->d_img_im[ax][d], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+    }
     for (int d = 0; d < 2; ++d) {
       std::vector<double> img((size_t)16 * S * ldv, 0.0);
       for (int s = 0; s < S; ++s)
@@ -716,7 +737,10 @@ void tma_destroy(exx_plan* p) {
   if (!st) return;
   for (int ax = 0; ax < 3; ++ax)
     for (int d = 0; d < 2; ++d)
+    {
       if (st->img_owned[ax][d] && st->d_img[ax][d]) cudaFree(st->d_img[ax][d]);
+      if (st->d_img_im[ax][d] && !(ax == 2 && st->d_img_im[2][d] == st->d_img_im[1][d])) cudaFree(st->d_img_im[ax][d]);
+    }
   delete st;
   p->tma_state = nullptr;
 }

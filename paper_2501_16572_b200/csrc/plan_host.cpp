@@ -121,6 +121,72 @@ bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::v
   return true;
 }
 
+// Bloch-periodic axis (R18): K = A + iB Hermitian, A symmetric, B antisymmetric; every wrapped stencil
+// entry carries exp(i theta wraps).  Solved through the real symmetric embedding S = [[A, -B], [B, A]] (2n x 2n):
+// each complex eigenvector u + iv appears twice, as (u; v) and as (-v; u) = i (u + iv).  Going through the 2n
+// real eigenvectors in ascending order and keeping those that survive a complex modified Gram-Schmidt against
+// the ones already kept leaves exactly n orthonormal complex eigenvectors (any orthonormal basis of a
+// degenerate eigenspace serves: f(L) does not depend on it).
+bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& Vr,
+                std::vector<double>& Vi) {
+  const std::vector<double> w = fd_weights(order, h);
+  const int n0 = order / 2, m2 = 2 * n;
+  std::vector<double> S((size_t)m2 * m2, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int q = -n0; q <= n0; ++q) {
+      int j = i + q, wraps = 0;
+      while (j < 0) { j += n; --wraps; }
+      while (j >= n) { j -= n; ++wraps; }
+      const double a = w[std::abs(q)] * std::cos(theta * wraps), b = w[std::abs(q)] * std::sin(theta * wraps);
+      S[(size_t)i * m2 + j] += a;              // A
+      S[(size_t)(n + i) * m2 + n + j] += a;    // A
+      S[(size_t)i * m2 + n + j] -= b;          // -B
+      S[(size_t)(n + i) * m2 + j] += b;        // B
+    }
+  for (int i = 0; i < m2; ++i)                 // remove the rounding-level asymmetry of cos/sin sums
+    for (int j = i + 1; j < m2; ++j) {
+      const double v = 0.5 * (S[(size_t)i * m2 + j] + S[(size_t)j * m2 + i]);
+      S[(size_t)i * m2 + j] = S[(size_t)j * m2 + i] = v;
+    }
+  std::vector<double> l2, V2;
+  if (!jacobi_eigh(m2, S, l2, V2)) return false;
+  lam.assign(n, 0.0);
+  Vr.assign((size_t)n * n, 0.0);
+  Vi.assign((size_t)n * n, 0.0);
+  int kept = 0;
+  std::vector<double> zr(n), zi(n);
+  for (int c = 0; c < m2 && kept < n; ++c) {
+    for (int i = 0; i < n; ++i) {
+      zr[i] = V2[(size_t)i * m2 + c];
+      zi[i] = V2[(size_t)(n + i) * m2 + c];
+    }
+    for (int pass = 0; pass < 2; ++pass)       // MGS twice
+      for (int m = 0; m < kept; ++m) {
+        double pr = 0.0, pi = 0.0;             // <v_m, z> = sum conj(v_m) z
+        for (int i = 0; i < n; ++i) {
+          const double vr = Vr[(size_t)i * n + m], vi = Vi[(size_t)i * n + m];
+          pr += vr * zr[i] + vi * zi[i];
+          pi += vr * zi[i] - vi * zr[i];
+        }
+        for (int i = 0; i < n; ++i) {
+          const double vr = Vr[(size_t)i * n + m], vi = Vi[(size_t)i * n + m];
+          zr[i] -= pr * vr - pi * vi;
+          zi[i] -= pr * vi + pi * vr;
+        }
+      }
+    double nrm = 0.0;
+    for (int i = 0; i < n; ++i) nrm += zr[i] * zr[i] + zi[i] * zi[i];
+    if (nrm < 0.25) continue;                  // the partner i*(u+iv) of a vector already kept
+    nrm = std::sqrt(nrm);
+    for (int i = 0; i < n; ++i) {
+      Vr[(size_t)i * n + kept] = zr[i] / nrm;
+      Vi[(size_t)i * n + kept] = zi[i] / nrm;
+    }
+    lam[kept++] = l2[c];
+  }
+  return kept == n;
+}
+
 std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
                                      const std::vector<double>& lz, double omega, double zero_tol) {
   const size_t nx = lx.size(), ny = ly.size(), nz = lz.size();

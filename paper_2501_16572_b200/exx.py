@@ -80,6 +80,17 @@ def load_library():
     lib.exx_ace_build.argtypes = [vp, dp, dp, C.c_int, dp, dp, vp, vp, C.c_size_t, vp]
     lib.exx_ace_apply.restype = C.c_int
     lib.exx_ace_apply.argtypes = [vp, dp, C.c_int, dp, C.c_int, dp, vp, C.c_size_t, vp]
+    lib.exx_plan_create_bloch.restype = C.c_int
+    lib.exx_plan_create_bloch.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, ip, C.c_int,
+                                          C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int]
+    lib.exx_plan_workspace_bytes_bloch.restype = C.c_size_t
+    lib.exx_plan_workspace_bytes_bloch.argtypes = [vp, C.c_int]
+    lib.exx_poisson_solve_bloch.restype = C.c_int
+    lib.exx_poisson_solve_bloch.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_apply_bloch.restype = C.c_int
+    lib.exx_apply_bloch.argtypes = [vp, dp, dp, C.c_int, dp, C.c_int, dp, C.c_int, dp, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_plan_get_axis_bloch.restype = C.c_int
+    lib.exx_plan_get_axis_bloch.argtypes = [vp, C.c_int, dp, dp, dp]
     lib.exx_status_string.restype = C.c_char_p
     lib.exx_status_string.argtypes = [C.c_int]
     lib.exx_plan_set_profiling.restype = C.c_int
@@ -131,7 +142,7 @@ def probe_fp64_peak(kind: int, device: int = 0, seconds: float = 1.0) -> float:
 class Plan:
     """exx_plan_create / exx_plan_destroy (the per-axis eigendecompositions, once)."""
 
-    def __init__(self, nx, ny, nz, h, bc=(0, 0, 0), fd_order=12, omega=0.0, max_batch=64, device=0):
+    def __init__(self, nx, ny, nz, h, bc=(0, 0, 0), fd_order=12, omega=0.0, max_batch=64, device=0, theta=None):
         lib = load_library()
         self._lib = lib
         self._h = C.c_void_p()
@@ -141,8 +152,13 @@ class Plan:
         self.device_index = int(device)
         self.device = torch.device("cuda", device) if device >= 0 else torch.device("cpu")
         bc_arr = (C.c_int * 3)(*[int(b) for b in bc])
-        st = lib.exx_plan_create(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, max_batch, device)
-        _check(st, "exx_plan_create")
+        if theta is None:
+            st = lib.exx_plan_create(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, max_batch, device)
+            _check(st, "exx_plan_create")
+        else:   # Bloch-periodic plan: theta[a] = (k-q)_a * n_a * h (exx_plan_create_bloch)
+            th = (C.c_double * 3)(*[float(t) for t in theta])
+            st = lib.exx_plan_create_bloch(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, th, max_batch, device)
+            _check(st, "exx_plan_create_bloch")
         self._ws = None
 
     @classmethod
@@ -277,6 +293,59 @@ class Plan:
     @property
     def last_solve_count(self) -> int:
         return int(self._lib.exx_plan_last_solve_count(self._h))
+
+    # ---- Bloch-periodic complex variant: complex functions are two real planes [n, 2, nz, ny, nx] --------------
+    def get_axis_bloch(self, axis: int):
+        n = (self.nx, self.ny, self.nz)[axis]
+        lam, Vr, Vi = np.empty(n), np.empty((n, n), order="F"), np.empty((n, n), order="F")
+        _check(self._lib.exx_plan_get_axis_bloch(self._h, axis, C.c_void_p(lam.ctypes.data), C.c_void_p(Vr.ctypes.data),
+                                                 C.c_void_p(Vi.ctypes.data)), "exx_plan_get_axis_bloch")
+        return lam, Vr + 1j * Vi
+
+    def _workspace_bloch(self, n_c: int) -> torch.Tensor:
+        need = int(self._lib.exx_plan_workspace_bytes_bloch(self._h, n_c))
+        if need == 0:
+            raise ValueError(f"n_c={n_c} outside 1..max_batch={self.max_batch}")
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._ws
+
+    def poisson_solve_bloch(self, rhs: torch.Tensor, out: torch.Tensor | None = None, n_c: int = 0,
+                            stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+        """exx_poisson_solve_bloch: rhs / out are [n_rhs, 2, nz, ny, nx] (real and imaginary planes)."""
+        n_rhs = rhs.shape[0]
+        if rhs.numel() != n_rhs * 2 * self.N:
+            raise ValueError("rhs must be [n_rhs, 2, nz, ny, nx]")
+        if out is None:
+            out = torch.empty_like(rhs)
+        ws = self._workspace_bloch(n_c)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_poisson_solve_bloch(self._h, _dev_ptr(rhs, self.device, "rhs"), _dev_ptr(out, self.device, "out"),
+                                               n_rhs, n_c, C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(s.cuda_stream))
+        _check(st, "exx_poisson_solve_bloch")
+        return out
+
+    def apply_bloch(self, psi: torch.Tensor, occ: torch.Tensor, tgt: torch.Tensor, vx: torch.Tensor | None = None,
+                    accumulate: bool = False, want_ex_k: bool = True, n_c: int = 0,
+                    stream: torch.cuda.Stream | None = None):
+        """exx_apply_bloch for one (k,q) pair: psi [n_occ, 2, nz, ny, nx], tgt [n_tgt, 2, ...]; returns (vx, e_k)."""
+        n_occ, n_tgt = psi.shape[0], tgt.shape[0]
+        if psi.numel() != n_occ * 2 * self.N or tgt.numel() != n_tgt * 2 * self.N:
+            raise ValueError("psi/tgt must be [n, 2, nz, ny, nx]")
+        if vx is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs vx")
+            vx = torch.empty_like(tgt)
+        ex_k = torch.empty(n_tgt, dtype=torch.float64, device=self.device) if want_ex_k else None
+        ws = self._workspace_bloch(n_c)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_apply_bloch(self._h, _dev_ptr(psi, self.device, "psi"), _dev_ptr(occ, self.device, "occ"), n_occ,
+                                       _dev_ptr(tgt, self.device, "tgt"), n_tgt, _dev_ptr(vx, self.device, "vx"),
+                                       1 if accumulate else 0, _dev_ptr(ex_k, self.device, "ex_k"), n_c,
+                                       C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(s.cuda_stream))
+        _check(st, "exx_apply_bloch")
+        return vx, ex_k
 
     def ace_workspace_bytes(self, n_orb: int, n_trial: int = 0) -> int:
         return int(self._lib.exx_ace_workspace_bytes(self._h, n_orb, n_trial))

@@ -89,3 +89,30 @@ def test_library_planner_agrees_with_oracle_planner(lib, dims, bc, omega, h):
     if all(b == 0 for b in bc):
         assert m[-1, -1, -1] == (0.0 if omega <= 0 else pytest.approx(np.pi / omega ** 2, rel=1e-14))
     p.close()
+
+
+@pytest.mark.parametrize("dims,bc,theta", [((16, 12, 9), (0, 0, 1), (0.7, -2.1, 0.5)), ((48, 48, 48), (0, 0, 0), (np.pi, 0.0, 1.0)),
+                                           ((7, 60, 5), (1, 0, 0), (0.3, np.pi / 2, -np.pi))])
+def test_bloch_planner_agrees_with_bloch_oracle(lib, dims, bc, theta):
+    """exx_plan_create_bloch (real-symmetric embedding + Jacobi + complex Gram-Schmidt) against numpy's Hermitian
+    eigh on the oracle's matrix: eigenvalues, unitarity, K V = V Lambda, and the multiplier table."""
+    from oracle import bloch_oracle as blo
+    nx, ny, nz = dims
+    h, omega = 0.3, 0.106
+    p = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=4, device=-1, theta=theta)
+    o = blo.make_plan(nx, ny, nz, h, bc, 12, omega, theta)
+    scale = abs(blo.fd_weights(12, h)[0])
+    for ax, n in enumerate(dims):
+        lam, V = p.get_axis_bloch(ax)
+        assert np.allclose(lam, o.lam[ax], rtol=0, atol=5e-13 * scale)
+        assert np.allclose(V.conj().T @ V, np.eye(n), atol=1e-12)
+        K = blo.bloch_second_derivative_matrix(n, h, bc[ax], 12, theta[ax])
+        assert np.allclose(K @ V, V * lam[None, :], rtol=0, atol=2e-12 * scale)
+        if bc[ax] == 1 or theta[ax] == 0.0:
+            assert np.all(V.imag == 0.0)           # real axis: the real planner was used
+    assert np.allclose(p.get_multiplier(), o.mult, rtol=1e-10, atol=0)
+    # the real entry points refuse a complex plan
+    dummy = C.c_void_p(1 << 20)
+    assert lib.exx_poisson_solve(p._h, dummy, dummy, 1, 1, dummy, 1 << 30, None) == 1
+    assert p._lib.exx_plan_workspace_bytes_bloch(p._h, 4) == 6 * 8 * nx * ny * nz * 4
+    p.close()
