@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--n-tgt", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--bloch", action="store_true",
+                    help="measure the Bloch-periodic complex variant (SURVEY 8(f) NEXT-3) on the config's grid instead")
     ap.add_argument("--no-ace", action="store_true", help="skip the ACE tail/apply measurement (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -388,9 +390,74 @@ def run_b200(args):
         dist.destroy_process_group()
 
 
+def run_bloch(args):
+    """One (k,q) pair of the complex variant on the config's grid and orbital count: phases pi/2, pi/3, pi/5 on the
+    periodic axes, complex orbitals from workloads.make_complex_orbitals.  Roofline credit = executed real flops:
+    per pass 2*N*n per plane product, 4 plane products on a complex axis (P and Q over two planes), 2 on a real one."""
+    import math
+    from paper_2501_16572_b200 import exx
+    import __graft_entry__ as ge
+    ge.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    w = workload_from_args(args)
+    n_c = args.nc or 16
+    theta = tuple(t if b == wl.PERIODIC else 0.0 for t, b in zip((math.pi / 2, math.pi / 3, math.pi / 5), w.bc))
+    psi = wl.make_complex_orbitals(w, dev if w.cfg >= 4 else "cpu").to(dev)
+    occ = torch.from_numpy(wl.occupations(w)).to(dev)
+    tgt = psi[w.tgt_start:w.tgt_start + w.n_tgt]
+    plan = exx.Plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, max_batch=max(128, n_c), device=0, theta=theta)
+    plan.set_variant(args.variant)
+    vx = torch.empty_like(tgt)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        return plan.apply_bloch(psi, occ, tgt, vx=vx, n_c=n_c, stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    launches = plan.last_launch_count
+    sampler = ClockSampler(0)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for e0, e1 in ev:
+        flush.fill_(1)
+        e0.record(stream)
+        _, e_k = step()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+    peak = exx.probe_fp64_peak(1, 0, 1.5)
+    plan.set_profiling(True)
+    flush.fill_(1)
+    step()
+    prof = plan.get_profile()
+    plan.set_profiling(False)
+    flops = sum(2 * (4 if t != 0.0 else 2) * 2.0 * w.N * n for t, n in zip(theta, (w.nx, w.ny, w.nz))) * w.pair_solves
+    mp_ms = prof["mode_product"][0]
+    line = {"metric": "bloch_pair_solves_per_s", "value": w.pair_solves / (ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c128 (two f64 planes)", "data": "synthetic",
+            "config": config_dict(w, n_c, {"theta": list(theta), "variant": "Bloch-periodic complex (one k-q pair)"}),
+            "clocks": clocks, "gpu_launches": int(launches * args.steps), "e_k0": float(e_k[0].item()),
+            "roofline": {"bound": "tensor", "kernel": "k_mode_t (real and imaginary part of V) + k_combine",
+                         "achieved": flops / (mp_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                         "frac": flops / (mp_ms * 1e-3) / 1e12 / peak,
+                         "step_frac": flops / (ms * 1e-3) / 1e12 / peak, "flops_per_step": flops,
+                         "class_ms_per_step": {k: v[0] for k, v in prof.items()},
+                         "note": "mode_product class includes the combine kernels; executed real flops (4x a real solve on complex axes)"}}
+    print(json.dumps(line), flush=True)
+    plan.close()
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.bloch and args.impl != "reference":
+        run_bloch(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_b200(args)

@@ -168,6 +168,14 @@ def make_inputs(w: Workload, device: str | torch.device = "cpu"):
     return psi, occ, tgt, occ_tgt
 
 
+def make_complex_orbitals(w: Workload, device: str | torch.device = "cpu") -> torch.Tensor:
+    """[n_orb, 2, nz, ny, nx] complex orbitals as two real planes for the Bloch-periodic variant: real part = the
+    workload's orbitals, imaginary part = half of the previous orbital (deterministic; data only, no arithmetic of
+    the method)."""
+    re = make_orbitals(w, device)
+    return torch.stack([re, 0.5 * torch.roll(re, shifts=1, dims=0)], dim=1).contiguous()
+
+
 def make_rhs(w: Workload, n_rhs: int, device: str | torch.device = "cpu", seed_offset: int = 1000) -> torch.Tensor:
     """[n_rhs, nz, ny, nx] seeded N(0,1) right-hand sides for the bare solver (Fig. 1-style sweeps)."""
     device = torch.device(device)
