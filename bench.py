@@ -30,7 +30,7 @@ from paper_2501_16572_b200 import workloads as wl  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_mode_t launch (average over the six passes of a batch) from the
 # `ncu --set full` captures summarised in profiles/r1_final_summary.md, keyed by (config, n_c); other shapes: null.
-NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (5, 128): 3.545e9}
+NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (5, 128): 3.545e9}   # refreshed when a new capture is committed
 
 METRIC = "poisson_pair_solves_per_s"
 UNIT = "solves/s"
@@ -49,8 +49,13 @@ def parse_args():
     ap.add_argument("--n-tgt", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--solver-sweep", action="store_true",
+                    help="bare exx_poisson_solve over n_c = 1..512 on the config's grid (the paper's Figs. 1-2 in shape)")
     ap.add_argument("--bloch", action="store_true",
                     help="measure the Bloch-periodic complex variant (SURVEY 8(f) NEXT-3) on the config's grid instead")
+    ap.add_argument("--nc-sym", type=int, default=0,
+                    help="batch size of the pair-symmetric apply (0 = min(n_c, 4 n_orb): larger rectangles waste more "
+                         "j > k pairs inside their diagonal blocks)")
     ap.add_argument("--no-ace", action="store_true", help="skip the ACE tail/apply measurement (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -351,20 +356,21 @@ def run_b200(args):
     symmetric = None
     if not args.no_ace and world == 1 and w.n_tgt == w.n_orb and w.tgt_start == 0:
         vx_s = torch.empty_like(vx)
+        n_c_sym = args.nc_sym or min(n_c, 4 * w.n_orb)
         for _ in range(2):
-            plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c, stream=stream)
+            plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
         ts = []
         for _ in range(min(args.steps, 5)):
             flush.fill_(1)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
-            _, _, ex_s = plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c, stream=stream)
+            _, _, ex_s = plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
             b.record(stream)
             torch.cuda.synchronize()
             ts.append(a.elapsed_time(b))
         ms_s = statistics.median(ts)
         executed = plan.last_solve_count
-        symmetric = {"ms_per_step": ms_s, "executed_solves_per_step": int(executed),
+        symmetric = {"ms_per_step": ms_s, "n_c": n_c_sym, "executed_solves_per_step": int(executed),
                      "executed_solves_per_s": executed / (ms_s * 1e-3),
                      "pair_equivalent_solves_per_s": w.pair_solves / (ms_s * 1e-3),
                      "applies_per_s": w.n_tgt / (ms_s * 1e-3), "speedup_vs_full": ms_per_step / ms_s,
@@ -453,9 +459,66 @@ def run_bloch(args):
     plan.close()
 
 
+def run_solver_sweep(args):
+    """The paper's Fig. 1 (time per linear system against the batch size n_c) and Fig. 2 (batch solver, GPU against
+    CPU) in shape, on the config's grid: seeded N(0,1) right-hand sides, exx_poisson_solve,
+    CUDA events, median of 5 after 2 warm-ups; n_c = 1 is the non-batch limit (Eq. 8: one system per set of
+    products).  The CPU column is the oracle's poisson_solve (numpy) on batches of 20 (the paper's n_c)."""
+    from paper_2501_16572_b200 import exx
+    import __graft_entry__ as ge
+    ge.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    w = workload_from_args(args)
+    n_rhs = int(max(32, min(512, (3 << 30) // (w.N * 8))))
+    rhs = wl.make_rhs(w, n_rhs, dev)
+    out = torch.empty_like(rhs)
+    plan = exx.Plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, max_batch=512, device=0)
+    peak = exx.probe_fp64_peak(1, 0, 1.0)
+    stream = torch.cuda.current_stream(dev)
+    rows = []
+    for n_c in (1, 2, 4, 8, 16, 20, 32, 64, 128, 256, 512):
+        if n_c > n_rhs:
+            break
+        m = n_rhs if n_c >= 16 else max(n_c, min(n_rhs, 16 * n_c))     # fewer systems for the tiny batches
+        for _ in range(2):
+            plan.poisson_solve(rhs[:m], out=out[:m], n_c=n_c, stream=stream)
+        ts = []
+        for _ in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            plan.poisson_solve(rhs[:m], out=out[:m], n_c=n_c, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ms = statistics.median(ts)
+        rows.append({"n_c": n_c, "systems": m, "us_per_solve": 1e3 * ms / m, "solves_per_s": m / (ms * 1e-3),
+                     "frac_of_dmma_peak": m * w.flops_per_solve / (ms * 1e-3) / 1e12 / peak})
+    from oracle import exx_oracle as orc   # cpu_baseline leg
+    oplan = orc.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega)
+    c = rhs[:20].cpu().numpy()
+    orc.poisson_solve(oplan, c[:2])
+    t0 = time.perf_counter()
+    reps = 0
+    while time.perf_counter() - t0 < min(args.cpu_seconds, 10.0):
+        orc.poisson_solve(oplan, c)
+        reps += 1
+    cpu_us = 1e6 * (time.perf_counter() - t0) / (20 * reps)
+    best = min(rows, key=lambda r: r["us_per_solve"])
+    print(json.dumps({"metric": "poisson_solve_sweep", "config": config_dict(w, 0), "peak_tflops": peak, "rows": rows,
+                      "speedup_batch_vs_nc1": rows[0]["us_per_solve"] / best["us_per_solve"], "best_n_c": best["n_c"],
+                      "cpu_baseline": {"us_per_solve": cpu_us, "cores": _oracle_threads(), "kind": "oracle",
+                                       "sample": f"oracle poisson_solve, batches of 20, {reps} repetitions"},
+                      "gpu_over_cpu_at_nc20": cpu_us / next(r["us_per_solve"] for r in rows if r["n_c"] == 20)}), flush=True)
+    plan.close()
+
+
 def main():
     args = parse_args()
-    if args.bloch and args.impl != "reference":
+    if args.solver_sweep and args.impl != "reference":
+        run_solver_sweep(args)
+    elif args.bloch and args.impl != "reference":
         run_bloch(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -93,6 +93,14 @@ exx_status exx_plan_set_variant(exx_plan* plan, int variant);
 exx_status exx_plan_set_lanes(exx_plan* plan, int lanes);
 int exx_plan_get_lanes(const exx_plan* plan);
 
+/*
+ * Accumulate mode (off by default): while on, exx_apply ADDS its result into d_vx instead of overwriting it, so the
+ * sum over the occupied orbitals of Eq. 1 can be split over several calls -- the orbital ring of
+ * SURVEY.md 8(e), where each rank holds one block of orbitals at a time (paper_2501_16572_b200/sharding.py).  d_ex /
+ * d_ex_k are computed from the d_vx found after the call, so request them on the last call only.
+ */
+exx_status exx_plan_set_accumulate(exx_plan* plan, int on);
+
 /* Bytes of device workspace exx_apply / exx_poisson_solve need for batches of n_c right-hand sides
  * (0 if plan is NULL or n_c is outside 1..max_batch). */
 size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c);

@@ -118,7 +118,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->variant = EXX_VARIANT_FUSED_DMMA;
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
-  p->prof_on = false;
+  p->prof_on = false; p->accumulate = false;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
     p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
@@ -250,6 +250,12 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes) {
 }
 
 int exx_plan_get_lanes(const exx_plan* plan) { return plan ? plan->lanes : 0; }
+
+exx_status exx_plan_set_accumulate(exx_plan* plan, int on) {
+  if (!plan) return EXX_ERR_INVALID_ARG;
+  plan->accumulate = on != 0;
+  return EXX_OK;
+}
 
 size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c) {
   if (!plan) return 0;
@@ -388,8 +394,10 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
   PlanExtras* ex = extras_of(plan);
 
   if (n_tgt > 0 && n_occ == 0) {
-    EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_tgt, s));
-    ++launches;
+    if (!plan->accumulate) {
+      EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_tgt, s));
+      ++launches;
+    }
   } else if (n_tgt > 0) {
     double* buf0 = (double*)d_workspace;
     double* buf1 = buf0 + N * (size_t)n_c;
@@ -423,11 +431,11 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
           EXX_CUDA(ref_solve_batch(plan, buf0, buf1, nb, s, &launches));
           {
             exx::ProfScope ps(plan, exx::KC_ACCUMULATE, s);
-            EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, j0 == 0, d_vx, s));
+            EXX_CUDA(exx::ref_accumulate(plan, d_psi, d_occ, buf0, bd, j0 == 0 && !plan->accumulate, d_vx, s));
           }
           launches += 2;
         } else {
-          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0, false};
+          const exx::FastArgs fa{d_psi, d_tgt, d_occ, d_vx, bd, n_occ, n_tgt, j0 == 0 && !plan->accumulate, false};
           EXX_CUDA(exx::fast_solve_batch(plan, nullptr, lane1 ? buf1 : buf0, two_lanes ? nullptr : buf1, nb, &fa, ls,
                                          &launches));
         }

@@ -67,6 +67,7 @@ struct exx_plan {
   cudaStream_t lane_stream;
   cudaEvent_t ev_fork, ev_join;
   // optional per-kernel-class CUDA-event timing (exx_plan_set_profiling)
+  bool accumulate;  // exx_plan_set_accumulate: exx_apply adds into d_vx instead of overwriting it
   bool prof_on;
   std::vector<exx::ProfRec> prof;
 };

@@ -72,6 +72,8 @@ def load_library():
     lib.exx_plan_tma_launch_count.argtypes = [vp]
     lib.exx_plan_set_lanes.restype = C.c_int
     lib.exx_plan_set_lanes.argtypes = [vp, C.c_int]
+    lib.exx_plan_set_accumulate.restype = C.c_int
+    lib.exx_plan_set_accumulate.argtypes = [vp, C.c_int]
     lib.exx_plan_get_lanes.restype = C.c_int
     lib.exx_plan_get_lanes.argtypes = [vp]
     lib.exx_ace_workspace_bytes.restype = C.c_size_t
@@ -184,6 +186,10 @@ class Plan:
 
     def set_lanes(self, lanes: int):
         _check(self._lib.exx_plan_set_lanes(self._h, lanes), "exx_plan_set_lanes")
+
+    def set_accumulate(self, on: bool):
+        """exx_plan_set_accumulate: exx_apply adds into vx instead of overwriting it."""
+        _check(self._lib.exx_plan_set_accumulate(self._h, 1 if on else 0), "exx_plan_set_accumulate")
 
     @property
     def lanes(self) -> int:

@@ -35,3 +35,41 @@ def reduce_energy(e_k_local: torch.Tensor, occ_tgt_local: torch.Tensor, k0: int,
         dist.all_reduce(e_k, op=dist.ReduceOp.SUM, group=group)
         dist.all_reduce(ex, op=dist.ReduceOp.SUM, group=group)
     return e_k, ex[0]
+
+
+def shard_orbitals(n_orb: int, rank: int, world: int) -> tuple[int, int, int]:
+    """Orbital block [j0, j1) held by `rank` at the start of the ring, and the common padded block length
+    (blocks are padded with zero-occupation orbitals so every ring message has the same size)."""
+    j0, j1 = shard_targets(n_orb, rank, world)
+    return j0, j1, -(-n_orb // world) if n_orb else 0
+
+
+def ring_apply(apply_block, psi_block: torch.Tensor, occ_block: torch.Tensor, rank: int, world: int, group=None):
+    """Orbital ring of SURVEY.md 8(e) for orbitals that do not fit one GPU (the paper's suggestion (i),
+    PAPER.md:285: move orbitals, not right-hand sides).
+
+    Every rank keeps its targets and ONE block of occupied orbitals at a time; in `world` steps each block
+    visits every rank.  Step s: start sending the held block to rank+1 and receiving the next one from rank-1
+    (NCCL P2P over NVLink on GPUs, gloo in the CPU tests), call ``apply_block(psi, occ, accumulate=s > 0,
+    last=s == world - 1)`` on the held block -- the transfer overlaps the compute -- then wait and swap.
+    ``apply_block`` runs exx_apply with the plan's accumulate mode (exx_plan_set_accumulate), asking for the
+    energy on the last step only.  psi_block [nb, ...] / occ_block [nb] must have the same (padded) shape on
+    every rank; padding orbitals carry occ = 0 and contribute nothing.  Host logic only.
+    """
+    import torch.distributed as dist
+    cur_psi, cur_occ = psi_block, occ_block
+    nxt_psi, nxt_occ = torch.empty_like(psi_block), torch.empty_like(occ_block)
+    for step in range(world):
+        last = step == world - 1
+        reqs = []
+        if not last and world > 1:
+            dst, src = (rank + 1) % world, (rank - 1) % world
+            ops = [dist.P2POp(dist.isend, cur_psi, dst, group), dist.P2POp(dist.irecv, nxt_psi, src, group),
+                   dist.P2POp(dist.isend, cur_occ, dst, group), dist.P2POp(dist.irecv, nxt_occ, src, group)]
+            reqs = dist.batch_isend_irecv(ops)
+        apply_block(cur_psi, cur_occ, accumulate=step > 0, last=last)
+        for r in reqs:
+            r.wait()
+        if not last:
+            cur_psi, nxt_psi = nxt_psi, cur_psi
+            cur_occ, nxt_occ = nxt_occ, cur_occ

@@ -254,3 +254,37 @@ def test_apply_is_cuda_graph_capturable():
         torch.cuda.synchronize()
         assert torch.equal(vx, vx_eager) and torch.equal(ek, ek_eager) and torch.equal(ex, ex_eager)
     plan.close()
+
+
+def test_accumulate_mode_splits_the_orbital_sum():
+    """exx_plan_set_accumulate: the sum over occupied orbitals (Eq. 1) split over two calls -- what one rank does in
+    the orbital ring (sharding.ring_apply) -- equals the oracle and the one-shot apply."""
+    from paper_2501_16572_b200 import sharding
+    w = wl.scaled(wl.WORKLOADS[1], 8)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    occ = torch.linspace(2.0, 0.1, 8, dtype=torch.float64)
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ.numpy())
+    plan = exx.Plan.for_workload(w, device=0)
+    d_psi, d_occ = psi.cuda(), occ.cuda()
+    vx_full, _, _ = plan.apply(d_psi, d_occ, d_psi, d_occ, n_c=4)
+    vx = torch.full_like(vx_full, 7.0)                      # garbage: the first call must overwrite it
+    out = {}
+
+    def apply_block(p, o, accumulate, last):
+        plan.set_accumulate(accumulate)
+        out["r"] = plan.apply(p, o, d_psi, d_occ if last else None, vx=vx, n_c=4, want_ex_k=last)
+        plan.set_accumulate(False)
+
+    apply_block(d_psi[:5].contiguous(), d_occ[:5].contiguous(), False, False)
+    apply_block(d_psi[5:].contiguous(), d_occ[5:].contiguous(), True, True)
+    torch.cuda.synchronize()
+    _, e_k, ex = out["r"]
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL
+    assert _rel(vx.cpu().numpy(), vx_full.cpu().numpy()) < 1e-13
+    assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
+    # the ring driver with one rank is a single plain call
+    vx2 = torch.empty_like(vx)
+    sharding.ring_apply(lambda p, o, accumulate, last: plan.apply(p, o, d_psi, d_occ, vx=vx2, n_c=4), d_psi, d_occ, 0, 1)
+    torch.cuda.synchronize()
+    assert torch.equal(vx2, vx_full)
+    plan.close()

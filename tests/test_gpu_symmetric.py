@@ -83,9 +83,9 @@ def test_symmetric_on_config2_full_size():
     o = orc.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega)
     vx_o, e_o, ex_o = orc.exx_apply(o, psi.numpy(), occ.numpy(), psi.numpy(), occ.numpy())
     plan = exx.Plan.for_workload(w, device=0)
-    vx, e_k, ex = plan.apply_symmetric(psi.cuda(), occ.cuda(), n_c=w.default_nc)
+    vx, e_k, ex = plan.apply_symmetric(psi.cuda(), occ.cuda(), n_c=128)
     torch.cuda.synchronize()
-    assert plan.last_solve_count == _expected_solves(w.n_orb, w.default_nc) < 0.55 * w.n_orb ** 2
+    assert plan.last_solve_count == _expected_solves(w.n_orb, 128) < 0.55 * w.n_orb ** 2
     assert _rel(vx.cpu().numpy(), vx_o) < TOL
     assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
     plan.close()
