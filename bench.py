@@ -29,8 +29,8 @@ import torch  # noqa: E402
 from paper_2501_16572_b200 import workloads as wl  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per k_mode_t launch (average over the six passes of a batch) from the
-# `ncu --set full` captures summarised in profiles/r1_final_summary.md, keyed by (config, n_c); other shapes: null.
-NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (5, 128): 3.545e9}   # refreshed when a new capture is committed
+# `ncu --set full` captures summarised in profiles/r1_final2_summary.md and r1_final_summary.md, keyed by (config, n_c); other shapes: null.
+NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (2, 1024): 1.739e9, (5, 128): 3.545e9}
 
 METRIC = "poisson_pair_solves_per_s"
 UNIT = "solves/s"
@@ -282,7 +282,7 @@ def run_b200(args):
     roofline = {"bound": "tensor", "kernel": "k_mode_dmma (six mode products per batch, FP64 mma.sync -> DMMA.8x8x4)",
                 "achieved": achieved, "peak": peak_dmma, "unit": "TFLOP/s", "frac": achieved / peak_dmma,
                 "traffic": NCU_TRAFFIC_BYTES.get((w.cfg, n_c)),
-                "traffic_note": "bytes per k_mode_t launch, profiles/r1_final_summary.md (cold-cache ncu replay); "
+                "traffic_note": "bytes per k_mode_t launch, profiles/r1_final2_summary.md / r1_final_summary.md (cold-cache ncu replay); "
                                 f"algorithmic bytes per launch = {2 * 8 * w.N * min(n_c, w.pair_solves):.4g} (batch read + written in place)",
                 "peak_source": "measured live: exx_probe_fp64_peak DMMA issue loop (MEASURED_PEAKS.json has no FP64 entry); "
                                f"DFMA loop {peak_dfma:.2f} TF",

@@ -18,10 +18,13 @@ constexpr int kDefaultBatch = 32;
 constexpr int kEnergyChunk = 1024;  // targets per energy launch (bounds the plan-owned scratch)
 constexpr int kEnergyBlocks = 64;   // must match kernels_ref.cu
 
+constexpr int kHostChunks = 4;  // exx_apply_host: target chunks whose download overlaps the next chunk's compute
 struct HostApiBuffers {
   double* base = nullptr;
   size_t bytes = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t done[kHostChunks] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 inline exx_status cuda_fail(cudaError_t e) {
@@ -230,6 +233,9 @@ exx_status exx_plan_destroy(exx_plan* plan) {
     if (p->ex.d_energy_scratch) cudaFree(p->ex.d_energy_scratch);
     if (p->ex.hb.base) cudaFree(p->ex.hb.base);
     if (p->ex.hb.stream) cudaStreamDestroy(p->ex.hb.stream);
+    if (p->ex.hb.copy_stream) cudaStreamDestroy(p->ex.hb.copy_stream);
+    for (int c = 0; c < kHostChunks; ++c)
+      if (p->ex.hb.done[c]) cudaEventDestroy(p->ex.hb.done[c]);
   }
   delete p;
   return EXX_OK;
@@ -332,6 +338,24 @@ cudaError_t ref_solve_batch(exx_plan* p, double* buf0, double* buf1, int nb, cud
 }
 
 }  // namespace
+
+// a6 for n_tgt targets: e_k = h^3 <tgt_k, vx_k>, *d_ex = 1/2 sum_k occ_tgt_k e_k (chunked: bounded plan-owned scratch)
+static exx_status run_energy(exx_plan* plan, const double* d_tgt, const double* d_vx, const double* d_occ_tgt, int n_tgt,
+                             double* d_ex, double* d_ex_k, cudaStream_t s, long long* launches) {
+  PlanExtras* ex = extras_of(plan);
+  const size_t N = (size_t)plan->N;
+  for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
+    const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
+    if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++*launches; }   // the first chunk overwrites *d_ex
+    {
+      exx::ProfScope ps(plan, exx::KC_OTHER, s);
+      EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0, d_occ_tgt ? d_occ_tgt + k0 : nullptr,
+                           nk, ex->d_energy_scratch, d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
+    }
+    *launches += 2;
+  }
+  return EXX_OK;
+}
 
 extern "C" {
 
@@ -451,18 +475,8 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     ++launches;
   }
   if ((d_ex || d_ex_k) && n_tgt > 0) {
-    // E_x is accumulated chunk by chunk; the first chunk overwrites *d_ex
-    for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
-      const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
-      if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
-      {
-        exx::ProfScope ps(plan, exx::KC_OTHER, s);
-        EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0,
-                             d_occ_tgt ? d_occ_tgt + k0 : nullptr, nk, ex->d_energy_scratch,
-                             d_ex_k ? d_ex_k + k0 : nullptr, d_ex, s));
-      }
-      launches += 2;
-    }
+    exx_status st = run_energy(plan, d_tgt, d_vx, d_occ_tgt, n_tgt, d_ex, d_ex_k, s, &launches);
+    if (st != EXX_OK) return st;
   }
   plan->last_launches = launches;
   plan->last_solves = (long long)n_occ * n_tgt;
@@ -600,15 +614,47 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
     EXX_CUDA(cudaMemcpyAsync(d_tgt, h_tgt, sizeof(double) * N * n_tgt, cudaMemcpyHostToDevice, s));
   if (h_occ_tgt && n_tgt > 0)
     EXX_CUDA(cudaMemcpyAsync(d_occ_tgt, h_occ_tgt, sizeof(double) * n_tgt, cudaMemcpyHostToDevice, s));
-  exx_status st = exx_apply(plan, d_psi, d_occ, n_occ, d_tgt, h_occ_tgt ? d_occ_tgt : nullptr, n_tgt, d_vx,
-                            h_ex ? d_ex : nullptr, h_ex_k ? d_ex_k : nullptr, n_c, d_ws, ws, s);
-  if (st != EXX_OK) return st;
-  if (h_vx && n_tgt > 0)
-    EXX_CUDA(cudaMemcpyAsync(h_vx, d_vx, sizeof(double) * N * n_tgt, cudaMemcpyDeviceToHost, s));
+  // The targets are applied in up to kHostChunks blocks (multiples of the k-block of a batch, so every batch and
+  // hence every bit of the result is that of a single exx_apply); the download of a block's vx runs on a second
+  // stream while the next block computes.  The energy is taken over all targets at the end.
+  if (!ex->hb.copy_stream) {
+    EXX_CUDA(cudaStreamCreateWithFlags(&ex->hb.copy_stream, cudaStreamNonBlocking));
+    for (int c = 0; c < kHostChunks; ++c) EXX_CUDA(cudaEventCreateWithFlags(&ex->hb.done[c], cudaEventDisableTiming));
+  }
+  const int nj_max = n_occ < n_c ? (n_occ > 0 ? n_occ : 1) : n_c;
+  const int kblock = n_c / nj_max > 0 ? n_c / nj_max : 1;
+  int chunk = (n_tgt + kHostChunks - 1) / kHostChunks;
+  chunk = (chunk + kblock - 1) / kblock * kblock;
+  if (chunk < 1) chunk = 1;
+  long long launches = 0, solves = 0;
+  int c = 0;
+  for (int k0 = 0; k0 < n_tgt; k0 += chunk, ++c) {
+    const int nk = n_tgt - k0 < chunk ? n_tgt - k0 : chunk;
+    exx_status st = exx_apply(plan, d_psi, d_occ, n_occ, d_tgt + N * (size_t)k0, nullptr, nk, d_vx + N * (size_t)k0,
+                              nullptr, nullptr, n_c, d_ws, ws, s);
+    if (st != EXX_OK) return st;
+    launches += plan->last_launches;
+    solves += plan->last_solves;
+    if (h_vx) {
+      EXX_CUDA(cudaEventRecord(ex->hb.done[c], s));
+      EXX_CUDA(cudaStreamWaitEvent(ex->hb.copy_stream, ex->hb.done[c], 0));
+      EXX_CUDA(cudaMemcpyAsync(h_vx + N * (size_t)k0, d_vx + N * (size_t)k0, sizeof(double) * N * nk,
+                               cudaMemcpyDeviceToHost, ex->hb.copy_stream));
+    }
+  }
+  if (n_tgt == 0 && h_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
+  if ((h_ex || h_ex_k) && n_tgt > 0) {
+    exx_status st = run_energy(plan, d_tgt, d_vx, h_occ_tgt ? d_occ_tgt : nullptr, n_tgt, h_ex ? d_ex : nullptr,
+                               h_ex_k ? d_ex_k : nullptr, s, &launches);
+    if (st != EXX_OK) return st;
+  }
+  plan->last_launches = launches;
+  plan->last_solves = solves;
   if (h_ex_k && n_tgt > 0)
     EXX_CUDA(cudaMemcpyAsync(h_ex_k, d_ex_k, sizeof(double) * n_tgt, cudaMemcpyDeviceToHost, s));
   if (h_ex) EXX_CUDA(cudaMemcpyAsync(h_ex, d_ex, sizeof(double), cudaMemcpyDeviceToHost, s));
   EXX_CUDA(cudaStreamSynchronize(s));
+  EXX_CUDA(cudaStreamSynchronize(ex->hb.copy_stream));
   return EXX_OK;
 }
 
