@@ -408,7 +408,7 @@ def run_bloch(args):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     dev = torch.device("cuda", 0)
     w = workload_from_args(args)
-    n_c = args.nc or 16
+    n_c = args.nc or (512 if w.N <= 200000 else 256)
     theta = tuple(t if b == wl.PERIODIC else 0.0 for t, b in zip((math.pi / 2, math.pi / 3, math.pi / 5), w.bc))
     psi = wl.make_complex_orbitals(w, dev if w.cfg >= 4 else "cpu").to(dev)
     occ = torch.from_numpy(wl.occupations(w)).to(dev)

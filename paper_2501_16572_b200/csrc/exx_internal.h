@@ -132,7 +132,7 @@ struct FastArgs {
 cudaError_t tma_init(exx_plan* p);
 void tma_destroy(exx_plan* p);
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
-                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part = 0);
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part = 0, bool rmw = false);
 // ---- ACE tail and application (kernels_ace.cu) ----
 size_t ace_build_workspace_doubles(const exx_plan* p, int n);
 size_t ace_apply_workspace_doubles(const exx_plan* p, int n, int m);

@@ -5,7 +5,9 @@
 // right-hand sides is 2 nb real ones and a complex mode product out = M in, M = Mr + i Mi (V^H forward, V backward),
 // is two launches of the REAL tensor-core kernel k_mode_t over those 2 nb planes,
 //     P = Mr [in_re | in_im],   Q = Mi [in_re | in_im],
-// followed by the streaming combine out_re = P_re - Q_im, out_im = P_im + Q_re (k_combine, in place over P).
+// combined as out_re = P_re - Q_im, out_im = P_im + Q_re: the Q launch adds its result straight into P's planes in its
+// epilogue (read-modify-write, k_mode_t `rmw`); only the z-backward product, whose launches carry the multiplier as a
+// second TMA stream, writes Q out and runs the streaming k_combine.
 // That is the 4x real flops of a Zgemm on the FP64 tensor pipe with no new MMA kernel.  An axis whose matrix is
 // real (Dirichlet, or theta = 0) needs neither Q nor the combine: one in-place launch.  The eigen-space multiplier
 // is real and rides as the second TMA stream of the z-backward launches, exactly as in the real path.
@@ -144,11 +146,18 @@ cudaError_t bloch_solve_batch(exx_plan* p, double* const buf[3], int nb, cudaStr
       } else {
         e = tma_mode_product(p, ax, fwd, cur, other, 2 * nb, mult, nullptr, s, 0);
         if (e == cudaSuccess) {
-          if ((e = tma_mode_product(p, ax, fwd, cur, q, 2 * nb, mult, nullptr, s, 1)) != cudaSuccess) return e;
-          dim3 grid(grid_for(N, 256, p->sm_count), nb);
-          k_combine<<<grid, 256, 0, s>>>(other, q, N);
-          if ((e = cudaGetLastError()) != cudaSuccess) return e;
-          *launches += 3;
+          if (!mult) {
+            // second launch adds Q into P's planes in its epilogue (read-modify-write): no Q buffer, no combine pass
+            if ((e = tma_mode_product(p, ax, fwd, cur, other, 2 * nb, false, nullptr, s, 1, true)) != cudaSuccess) return e;
+            *launches += 2;
+          } else {
+            // the two-stream (multiplier) kernel has no read-modify-write epilogue: separate Q, then the combine
+            if ((e = tma_mode_product(p, ax, fwd, cur, q, 2 * nb, mult, nullptr, s, 1)) != cudaSuccess) return e;
+            dim3 grid(grid_for(N, 256, p->sm_count), nb);
+            k_combine<<<grid, 256, 0, s>>>(other, q, N);
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
+            *launches += 3;
+          }
           double* t = cur; cur = other; other = t;
           done = true;
         } else if (e != cudaErrorNotSupported) {

@@ -130,6 +130,12 @@ struct TArgs {
   FastDiv div_nj;  // pair density only
   int exact;       // no ragged edge in this launch: the epilogue stores without predicates
   BatchDesc bd;    // pair density only
+  // Complex (Bloch) products, second launch: the result Q = Mi [in_re | in_im] is not stored but added into the first
+  // launch's output P with the planes swapped, out_re = P_re - Q_im, out_im = P_im + Q_re (planes alternate re, im;
+  // plane_stride = N doubles).  per_plane: rows (X-mode) / outer indices (L-mode) of one plane.
+  int rmw;
+  long long plane_stride;
+  FastDiv div_plane;
 };
 
 __device__ __forceinline__ bool elect_one() {
@@ -142,7 +148,7 @@ __device__ __forceinline__ void stg_v2(double* p, double x, double y) {
 }
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB>
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
     k_mode_t(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const TArgs a) {
   static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
@@ -344,7 +350,29 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         limit = a.rows_total;
       }
       double* base = a.out + ((long long)(row0 + 2 * q) * n + g);
-      if (a.exact) {
+      if (RMW) {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int r = row0 + 8 * nt + 2 * q + e;
+            if (r < limit) {
+              const bool odd = fast_div((unsigned)r, a.div_plane) & 1u;  // this row belongs to an imaginary plane
+              const double sgn = odd ? -1.0 : 1.0;
+              double* dst = base + (long long)(8 * nt + e) * n + (odd ? -a.plane_stride : a.plane_stride);
+#pragma unroll
+              for (int m0 = 0; m0 < MTOT; m0 += 4) {
+                double old[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                  if (m0 + u < MTOT && 8 * (m0 + u) + g < n) old[u] = dst[8 * (m0 + u)];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                  if (m0 + u < MTOT && 8 * (m0 + u) + g < n) dst[8 * (m0 + u)] = fma(sgn, acc[m0 + u][nt][e], old[u]);
+              }
+            }
+          }
+      } else if (a.exact) {
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
@@ -375,7 +403,29 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           const unsigned o = fast_div(cc, a.div_cpo);
           const int col0 = 16 * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
           double* ptr = a.out + ((long long)o * n + g) * a.inner + col0;
-          if (a.exact) {
+          if (RMW) {
+            const bool odd = fast_div(o, a.div_plane) & 1u;
+            const double sgn = odd ? -1.0 : 1.0;
+            double* pr = ptr + (odd ? -a.plane_stride : a.plane_stride);
+            const bool in0 = col0 < a.inner, in1 = col0 + 8 < a.inner;
+#pragma unroll
+            for (int m0 = 0; m0 < MTOT; m0 += 2) {
+              double2 o0[2], o1[2];
+#pragma unroll
+              for (int u = 0; u < 2; ++u)
+                if (m0 + u < MTOT && 8 * (m0 + u) + g < n) {
+                  if (in0) o0[u] = *reinterpret_cast<const double2*>(pr + u * mstep);
+                  if (in1) o1[u] = *reinterpret_cast<const double2*>(pr + u * mstep + 8);
+                }
+#pragma unroll
+              for (int u = 0; u < 2; ++u)
+                if (m0 + u < MTOT && 8 * (m0 + u) + g < n) {
+                  if (in0) stg_v2(pr + u * mstep, fma(sgn, acc[m0 + u][2 * ch][0], o0[u].x), fma(sgn, acc[m0 + u][2 * ch][1], o0[u].y));
+                  if (in1) stg_v2(pr + u * mstep + 8, fma(sgn, acc[m0 + u][2 * ch + 1][0], o1[u].x), fma(sgn, acc[m0 + u][2 * ch + 1][1], o1[u].y));
+                }
+              pr += 2 * mstep;
+            }
+          } else if (a.exact) {
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
               stg_v2(ptr, acc[mt][2 * ch][0], acc[mt][2 * ch][1]);
@@ -518,7 +568,7 @@ inline bool pdl_half() {
   return on;
 }
 
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB>
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
 cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, cudaStream_t s) {
   constexpr int LDV = 8 * MTOT + 4;
   const size_t img = sizeof(double) * 16 * (size_t)a.S * LDV;
@@ -528,7 +578,7 @@ cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs
   const size_t floor_bytes = MINB == 1 ? 117 * 1024 : 77 * 1024;
   if (MINB == 2 && smem > 113 * 1024) return cudaErrorInvalidConfiguration;
   if (smem < floor_bytes) smem = floor_bytes;
-  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB>;
+  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW>;
   static size_t attr_smem = 0;  // per instantiation
   if (smem > attr_smem) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -560,9 +610,11 @@ cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUte
                          int sm_count, cudaStream_t s) {
   if (xmode) {
     if (two) return launch_one<MTOT, NT2, true, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
+    if (a.rmw) return launch_one<MTOT, NT, true, false, WARPS, MINB, true>(m0, m1, a, sm_count, s);
     return launch_one<MTOT, NT, true, false, WARPS, MINB>(m0, m1, a, sm_count, s);
   }
   if (two) return launch_one<MTOT, NT2, false, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
+  if (a.rmw) return launch_one<MTOT, NT, false, false, WARPS, MINB, true>(m0, m1, a, sm_count, s);
   return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, s);
 }
 
@@ -576,7 +628,7 @@ inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 // cudaErrorNotSupported: sizes or alignment outside what TMA can address (odd nx, n > 128, unaligned
 // buffers, no driver entry point); the caller then uses the cp.async kernels of kernels_dmma.cu.
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
-                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part) {
+                             bool apply_mult, const FastArgs* pd, cudaStream_t s, int part, bool rmw) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st) return cudaErrorNotSupported;
   const int n = p->n[axis];
@@ -643,6 +695,12 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
     } else {
       m1 = m0;
     }
+  }
+  if (rmw) {  // only the plain (one-stream) kernels have the read-modify-write epilogue; planes come in (re, im) pairs
+    if (two || (nb & 1)) return cudaErrorInvalidValue;
+    a.rmw = 1;
+    a.plane_stride = p->N;
+    a.div_plane = make_fastdiv((unsigned)(xmode ? a.rows_per_rhs : (int)(p->N / ((long long)n * a.inner))));
   }
   if (a.n_tiles == 0) return cudaSuccess;
   ++p->tma_launches;
