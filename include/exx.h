@@ -127,7 +127,8 @@ exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi,
  *   *d_ex    = 1/2 sum_k d_occ_tgt[k] d_ex_k[k]                                     optional (NULL); needs d_occ_tgt
  * d_psi [n_occ][N], d_occ [n_occ]; d_tgt [n_tgt][N] may alias a block of d_psi.  d_vx must not overlap
  * d_psi / d_tgt / the workspace (EXX_ERR_ALIAS).  n_c = right-hand sides per batch, 1..max_batch,
- * 0 = library default.  Every (j,k) pair is solved (no symmetry shortcut, R12).  n_occ == 0 gives vx = 0.
+ * 0 = library default (about 1 GB of right-hand sides per
+ * batch, at least 32, at most max_batch).  Every (j,k) pair is solved (no symmetry shortcut, R12).  n_occ == 0 gives vx = 0.
  */
 exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ,
                      const double* d_tgt, const double* d_occ_tgt, int n_tgt, double* d_vx,

@@ -48,7 +48,7 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
 inline bool all_axes_fast(const exx_plan* p) { return p->d_Vpad[0] && p->d_Vpad[1] && p->d_Vpad[2]; }
 
 // One lane by default: two lanes measured +1.5 % .. +2.7 % on the 96^3 / 120^3 configs (the other lane's
-// accumulate overlaps the mode products) and -2 % .. -6 % at 48^3, see DESIGN.md 6.3.  EXX_LANES overrides.
+// accumulate overlaps the mode products) and -2 % .. -6 % at 48^3, see DESIGN.md 6.4.  EXX_LANES overrides.
 inline int default_lanes(const exx_plan* p) {
   if (const char* e = getenv("EXX_LANES"))
     if (e[0] == '2') return all_axes_fast(p) ? 2 : 1;
@@ -59,8 +59,14 @@ inline int default_lanes(const exx_plan* p) {
 inline bool is_complex_plan(const exx_plan* p) { return p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
                                                          !p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty(); }
 
+// n_c == 0: about 1 GB of right-hand sides per batch (measured: larger batches only amortise launch ramps and tails,
+// DESIGN.md section 9), at least kDefaultBatch, at most max_batch
 inline int resolve_nc(const exx_plan* p, int n_c) {
-  if (n_c == 0) n_c = p->max_batch < kDefaultBatch ? p->max_batch : kDefaultBatch;
+  if (n_c == 0) {
+    long long want = (1LL << 30) / (8 * p->N);
+    if (want < kDefaultBatch) want = kDefaultBatch;
+    n_c = want < p->max_batch ? (int)want : p->max_batch;
+  }
   return n_c;
 }
 

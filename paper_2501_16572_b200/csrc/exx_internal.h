@@ -62,7 +62,7 @@ struct exx_plan {
   long long last_solves;   // pair solves the last exx_apply / exx_apply_symmetric call executed
   long long tma_launches;  // cumulative count of TMA-staged mode-product launches (test hook)
   // exx_apply runs `lanes` batches at a time (1 or 2): lane 0 on the caller's stream, lane 1 on lane_stream,
-  // forked and joined with the two events (DESIGN.md 6.3)
+  // forked and joined with the two events (DESIGN.md 6.4)
   int lanes;
   cudaStream_t lane_stream;
   cudaEvent_t ev_fork, ev_join;
