@@ -154,8 +154,10 @@ long long exx_plan_last_solve_count(const exx_plan* plan);
 /*
  * Convenience end-to-end call with HOST buffers (pageable or pinned): uploads psi/occ (and tgt unless
  * tgt_start >= 0 selects the block h_psi[tgt_start .. tgt_start+n_tgt) as targets), runs exx_apply on an
- * internal stream, downloads vx / e_k / E_x and synchronises.  Device buffers are allocated and freed
- * inside the call.  Any of h_vx, h_ex, h_ex_k may be NULL.
+ * internal stream, downloads vx / e_k / E_x and synchronises.  The targets are applied in up to four blocks
+ * (multiples of a batch's target block, so the result is bitwise that of one exx_apply) and a finished block's vx
+ * is downloaded on a second stream while the next block computes.  The device buffers are owned by the plan, grown
+ * on demand and released by exx_plan_destroy.  Any of h_vx, h_ex, h_ex_k may be NULL.  Not thread safe per plan.
  */
 exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_occ, int n_occ,
                           const double* h_tgt, int tgt_start, const double* h_occ_tgt, int n_tgt,
