@@ -5,13 +5,23 @@
 
 A "step" is one full exchange apply (all SURVEY 8(a) rows: pair density, 3+3 mode products with the
 eigen-space multiply, accumulate, energy) of one BASELINE.json config over synthetic orbitals.
-Default workload: BASELINE.json configs[1] (48^3 HSE bulk, 64 orbitals, 4,096 pair solves).
-N > 1 (torchrun): targets are sharded across ranks, orbitals replicated, no data-path collective
-(weak scaling: every rank applies Vx to its own block of n_tgt targets); rank 0 prints the line.
+
+Default workload: BASELINE.json configs[4] (120^3 HSE bulk, 3,200 orbitals = 44 GB, 128 targets, 409,600 pair solves
+per step) -- the largest single-GPU configuration, the stand-in for the paper's 6,000-electron case.  The same line
+carries `roofline` (FP64 tensor pipe, measured live), `e2e` (exx_apply_host from host buffers, the orbitals streamed
+in blocks), `cpu_baseline` (the oracle on a bounded sample) and, as extra objects, short measurements of configs 2-4
+(`configs`) and the batch-size sweep of config 4 (`sweep_cfg4`, BASELINE.json configs[3], the paper's Fig. 1 in shape).
+
+N > 1 (torchrun): targets are sharded across ranks, orbitals replicated; the one collective of the path (all-reduce
+of the per-target energies, sharding.reduce_energy) is inside the timed region; rank 0 prints the line.
+--scaling weak (default): every rank applies Vx to its own block of n_tgt targets; --scaling strong: the config's
+n_tgt targets are split over the ranks.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import glob
 import json
 import os
 import statistics
@@ -28,27 +38,28 @@ import torch  # noqa: E402
 
 from paper_2501_16572_b200 import workloads as wl  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum per k_mode_t launch (average over the six passes of a batch) from the
-# `ncu --set full` captures summarised in profiles/r1_final2_summary.md and r1_final_summary.md, keyed by (config, n_c); other shapes: null.
-NCU_TRAFFIC_BYTES = {(2, 128): 167.9e6, (2, 1024): 1.739e9, (5, 128): 3.545e9}
-
 METRIC = "poisson_pair_solves_per_s"
 UNIT = "solves/s"
+DEFAULT_CONFIG = 5
+DEFAULT_STEPS = {1: 20, 2: 20, 3: 10, 4: 5, 5: 3}
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=0, help="timed steps (0 = a per-config default that finishes in minutes)")
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); default 2 = configs[1]")
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG,
+                    help="BASELINE.json config number (1-based); default 5 = configs[4], the largest single-GPU one")
     ap.add_argument("--nc", type=int, default=0, help="right-hand sides per batch (0 = workload default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--variant", type=int, default=0, help="0 = DMMA path (default), 1 = plain-kernel cross-check variant")
     ap.add_argument("--n-orb", type=int, default=0, help="override orbital count (debug; invalidates the headline)")
     ap.add_argument("--n-tgt", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the configs 2-4 / sweep_cfg4 extra objects")
     ap.add_argument("--solver-sweep", action="store_true",
                     help="bare exx_poisson_solve over n_c = 1..512 on the config's grid (the paper's Figs. 1-2 in shape)")
     ap.add_argument("--bloch", action="store_true",
@@ -56,9 +67,12 @@ def parse_args():
     ap.add_argument("--nc-sym", type=int, default=0,
                     help="batch size of the pair-symmetric apply (0 = min(n_c, 4 n_orb): larger rectangles waste more "
                          "j > k pairs inside their diagonal blocks)")
-    ap.add_argument("--no-ace", action="store_true", help="skip the ACE tail/apply measurement (SURVEY 8(f) NEXT-1)")
+    ap.add_argument("--no-ace", action="store_true", help="skip the ACE / pair-symmetric measurements (SURVEY 8(f) NEXT-1/2)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.steps <= 0:
+        args.steps = DEFAULT_STEPS.get(args.config, 5)
+    return args
 
 
 def workload_from_args(args) -> wl.Workload:
@@ -95,16 +109,26 @@ def _oracle_threads() -> int:
     return len(os.sched_getaffinity(0))
 
 
-def time_oracle(w: wl.Workload, psi, occ, tgt, occ_t, budget_s: float, steps: int = 1, warmup: int = 0):
-    """Oracle exx_apply on a bounded sample of the workload's targets (all occupied orbitals, the first
-    n_s targets, n_s sized from a one-target calibration so a step takes about `budget_s`)."""
+def oracle_sample_workload(w: wl.Workload) -> wl.Workload:
+    """The bounded sample the oracle is timed on: the config's own grid, operator and input recipe with at most 64
+    (grids up to 500k points) / 16 (larger) host-generated orbitals, all of them targets.  The cost of a pair solve
+    does not depend on the orbital count, so solves/s on the sample is the oracle's rate on the workload."""
+    m = min(w.n_orb, 64 if w.N <= 500_000 else 16)
+    return wl.scaled(w, m, m, 0)
+
+
+def time_oracle(w: wl.Workload, budget_s: float, steps: int = 1, warmup: int = 0):
+    """Oracle exx_apply on the bounded sample: all sample orbitals against the first n_s sample targets, n_s sized
+    from a one-target calibration so that one step takes about `budget_s` seconds of CPU."""
     from oracle import exx_oracle as orc   # the one place bench.py executes oracle/ (cpu_baseline / --impl reference)
-    plan = orc.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega)
+    ws = oracle_sample_workload(w)
+    psi, occ, tgt, occ_t = wl.make_inputs(ws, "cpu")
+    plan = orc.make_plan(ws.nx, ws.ny, ws.nz, ws.h, ws.bc, ws.order, ws.omega)
     psi_n, occ_n, tgt_n, occ_t_n = psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy()
     t0 = time.perf_counter()
     orc.exx_apply(plan, psi_n, occ_n, tgt_n[:1], occ_t_n[:1])
     t1 = time.perf_counter() - t0
-    n_s = int(max(1, min(w.n_tgt, budget_s / max(t1, 1e-6))))
+    n_s = int(max(1, min(ws.n_tgt, budget_s / max(t1, 1e-6))))
     times = []
     for i in range(warmup + steps):
         t0 = time.perf_counter()
@@ -113,10 +137,11 @@ def time_oracle(w: wl.Workload, psi, occ, tgt, occ_t, budget_s: float, steps: in
         if i >= warmup:
             times.append(dt)
     dt = sum(times) / len(times)
-    solves = w.n_orb * n_s
+    solves = ws.n_orb * n_s
     return {"value": solves / dt, "unit": UNIT, "cores": _oracle_threads(), "kind": "oracle",
-            "sample": f"oracle/exx_oracle.exx_apply (numpy FP64) on {n_s} of {w.n_tgt} targets x {w.n_orb} occupied "
-                      f"= {solves} pair solves, {dt:.2f} s per step"}, dt, solves
+            "sample": f"oracle/exx_oracle.exx_apply (numpy FP64) on the grid, operator and input recipe of {w.name} with "
+                      f"{ws.n_orb} host-generated orbitals x {n_s} targets = {solves} pair solves, {dt:.2f} s per step "
+                      f"(the workload itself: {w.n_orb} x {w.n_tgt} = {w.pair_solves})"}, dt, solves
 
 
 def run_reference(args):
@@ -124,13 +149,13 @@ def run_reference(args):
     if rank != 0:
         return
     w = workload_from_args(args)
-    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
     steps = max(1, min(args.steps, 3))
-    budget = min(args.cpu_seconds, 120.0 / (steps + 1))
-    cb, dt, solves = time_oracle(w, psi, occ, tgt, occ_t, budget, steps=steps, warmup=min(args.warmup, 1))
+    warmup = min(args.warmup, 1)
+    budget = min(args.cpu_seconds, 120.0 / (steps + warmup + 1))
+    cb, dt, solves = time_oracle(w, budget, steps=steps, warmup=warmup)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "steps": steps, "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_dict(w, args.nc or w.default_nc, {"l2": "n/a (CPU)"}),
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -147,11 +172,11 @@ class ClockSampler:
              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
              "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, period_ms: int = 20):
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.QUERY}",
-                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                          "--format=csv,noheader,nounits", "-lms", str(period_ms)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
@@ -162,7 +187,7 @@ class ClockSampler:
             return out
         try:
             self.proc.terminate()
-            text, _ = self.proc.communicate(timeout=5)
+            text, _ = self.proc.communicate(timeout=10)
         except Exception:
             return out
         sm, mx, reasons, power = [], [], set(), []
@@ -187,10 +212,165 @@ class ClockSampler:
         return out
 
 
+def load_ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` captures: the newest profiles/r*_ncu_traffic.csv (columns cfg,n_c,kernel,dram_read_bytes,
+    dram_write_bytes,...).  {(cfg, n_c): (bytes, file)}; shapes that were not captured report null."""
+    out = {}
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_ncu_traffic.csv")))
+    if not files:
+        return out
+    with open(files[-1], newline="") as fh:
+        for row in csv.DictReader(r for r in fh if not r.startswith("#")):
+            try:
+                key = (int(row["cfg"]), int(row["n_c"]))
+                out[key] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), os.path.basename(files[-1]))
+            except (KeyError, ValueError):
+                continue
+    return out
+
+
+def timed_apply(step, steps: int, warmup: int, flush, stream, barrier=None):
+    """`warmup` untimed steps, then exactly `steps` steps, each inside its own CUDA-event pair on `stream` with an L2
+    flush (256 MiB write) before it; returns the summed milliseconds and the last step's result."""
+    res = None
+    for _ in range(warmup):
+        res = step()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for e0, e1 in ev:
+        flush.fill_(1)             # evict L2 between timed steps (outside the event pair)
+        e0.record(stream)
+        res = step()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return sum(e0.elapsed_time(e1) for e0, e1 in ev), res
+
+
+def instrumented(plan, step, flush, prof_steps: int, flops_step: float, peak: float):
+    """Per-kernel-class durations from separate instrumented steps (a CUDA-event pair around every launch on the
+    caller's stream; this defeats the overlap of consecutive launches, so these steps are slightly slower than the
+    timed ones).  Returns the mode-product class's achieved TFLOP/s and the per-class table."""
+    plan.set_profiling(True)
+    for _ in range(prof_steps):
+        flush.fill_(1)
+        step()
+    prof = plan.get_profile()
+    plan.set_profiling(False)
+    mp_ms, mp_cnt = prof["mode_product"]
+    all_ms = sum(v[0] for v in prof.values())
+    achieved = flops_step * prof_steps / (mp_ms * 1e-3) / 1e12 if mp_ms > 0 else 0.0
+    return {"achieved": achieved, "frac": achieved / peak, "avg_launch_ms": mp_ms / max(mp_cnt, 1),
+            "launches": mp_cnt // prof_steps, "share_of_step": mp_ms / all_ms if all_ms > 0 else None,
+            "class_ms_per_step": {k: v[0] / prof_steps for k, v in prof.items()}}
+
+
+def measure_extra(exx, cfg: int, dev, local: int, peak: float, flush, stream, n_tgt: int = 0, n_c: int = 0,
+                  steps: int = 3, want_ace: bool = False, psi=None):
+    """A short measurement of another BASELINE.json config (same method as the headline: L2 flush, CUDA events),
+    optionally on a reduced target block (stated in the result)."""
+    w0 = wl.WORKLOADS[cfg]
+    w = w0 if not n_tgt or n_tgt >= w0.n_tgt else wl.scaled(w0, w0.n_orb, n_tgt, w0.tgt_start)
+    n_c = n_c or w.default_nc
+    if psi is None:
+        psi, occ, _, _ = wl.make_inputs(w, dev)
+    else:
+        occ = torch.from_numpy(wl.occupations(w)).to(dev)
+    tgt = psi[w.tgt_start:w.tgt_start + w.n_tgt]
+    occ_t = occ[w.tgt_start:w.tgt_start + w.n_tgt]
+    plan = exx.Plan.for_workload(w, max_batch=max(128, n_c), device=local)
+    vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64, device=dev)
+
+    def step():
+        return plan.apply(psi, occ, tgt, occ_t, vx=vx, n_c=n_c, stream=stream)
+
+    total_ms, (_, _, ex) = timed_apply(step, steps, 2, flush, stream)
+    ms = total_ms / steps
+    flops = w.pair_solves * w.flops_per_solve
+    out = {"workload": f"BASELINE.json configs[{cfg - 1}]: {w0.name}", "n_occ": w.n_orb, "n_tgt": w.n_tgt,
+           "targets": "all" if w.n_tgt == w0.n_tgt else f"reduced block: {w.n_tgt} of {w0.n_tgt} targets from {w.tgt_start}",
+           "n_c": n_c, "pair_solves_per_step": w.pair_solves, "steps": steps, "ms_per_step": ms,
+           "value": w.pair_solves / (ms * 1e-3), "unit": UNIT, "applies_per_s": w.n_tgt / (ms * 1e-3),
+           "step_frac": flops / (ms * 1e-3) / 1e12 / peak, "E_x": float(ex.item()),
+           "launches_per_step": plan.last_launch_count}
+    if want_ace and w.n_tgt == w.n_orb and w.tgt_start == 0:
+        out.update(measure_ace_and_symmetric(plan, w, psi, occ, vx, ms, n_c, 0, peak, flush, stream, steps))
+    plan.close()
+    return out, psi
+
+
+def measure_ace_and_symmetric(plan, w, d_psi, d_occ, vx, ms_per_step, n_c, nc_sym, peak_dmma, flush, stream, steps):
+    """SURVEY 8(f) NEXT-1 (ACE tail and application on the step's own vx) and NEXT-2 (pair-symmetric apply)."""
+    n = w.n_orb
+    xi = torch.empty_like(vx)
+    out = torch.empty_like(vx)
+
+    def timed(fn, reps=5):
+        for _ in range(2):
+            fn()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts)
+
+    info_box = []
+    ms_build = timed(lambda: info_box.append(plan.ace_build(d_psi, vx, xi=xi, want_M=False, stream=stream)[2]))
+    n_launch_build = plan.last_launch_count
+    ms_apply = timed(lambda: plan.ace_apply(xi, d_psi, out=out, stream=stream))
+    n_launch_apply = plan.last_launch_count
+    fl_build = 2.0 * n * n * w.N + sum(2.0 * min(64, n - kb) * (kb + min(64, n - kb)) * w.N
+                                       for kb in range(0, n, 64)) + n ** 3 / 3.0
+    fl_apply = 4.0 * n * n * w.N
+    ace = {"build_ms": ms_build, "apply_ms": ms_apply, "info": int(info_box[-1].item()),
+           "build_tflops": fl_build / ms_build / 1e9, "apply_tflops": fl_apply / ms_apply / 1e9,
+           "build_frac_of_dmma_peak": fl_build / ms_build / 1e9 / peak_dmma,
+           "apply_frac_of_dmma_peak": fl_apply / ms_apply / 1e9 / peak_dmma,
+           "apply_columns_per_s": n / (ms_apply * 1e-3), "launches": [int(n_launch_build), int(n_launch_apply)],
+           "max_abs_err_ace_psi_minus_vx": float((out - vx).abs().max().item()),
+           "max_abs_vx": float(vx.abs().max().item()),
+           "what": "exx_ace_build(psi, W=vx) and exx_ace_apply(xi, psi): median of 5, L2 flushed, CUDA events"}
+    vx_s = torch.empty_like(vx)
+    n_c_sym = nc_sym or min(n_c, 4 * w.n_orb)
+    for _ in range(2):
+        plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
+    ts = []
+    for _ in range(min(steps, 5)):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        _, _, ex_s = plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    ms_s = statistics.median(ts)
+    executed = plan.last_solve_count
+    symmetric = {"ms_per_step": ms_s, "n_c": n_c_sym, "executed_solves_per_step": int(executed),
+                 "executed_solves_per_s": executed / (ms_s * 1e-3),
+                 "pair_equivalent_solves_per_s": w.pair_solves / (ms_s * 1e-3),
+                 "applies_per_s": w.n_tgt / (ms_s * 1e-3), "speedup_vs_full": ms_per_step / ms_s,
+                 "step_frac_executed": executed * w.flops_per_solve / (ms_s * 1e-3) / 1e12 / peak_dmma,
+                 "E_x": float(ex_s.item()),
+                 "max_rel_diff_vs_full": float(((vx_s - vx).abs().max() / vx.abs().max()).item()),
+                 "what": "exx_apply_symmetric: only pairs j <= k solved; roofline credit only for executed solves"}
+    return {"ace": ace, "symmetric": symmetric}
+
+
 def run_b200(args):
     import torch.distributed as dist
-    from paper_2501_16572_b200 import exx
+    from paper_2501_16572_b200 import exx, sharding
 
+    t_start = time.perf_counter()
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -211,53 +391,53 @@ def run_b200(args):
     n_c = args.nc or w.default_nc
     # inputs: generated on the GPU for the large configs, on the host (numpy) for configs 1-3
     gen_dev = dev if w.cfg >= 4 else "cpu"
-    psi, occ, tgt, occ_t = wl.make_inputs(w, gen_dev)
+    psi, occ, _, _ = wl.make_inputs(w, gen_dev)
     d_psi, d_occ = psi.to(dev), occ.to(dev)
-    # weak scaling: rank r applies Vx to n_tgt targets starting at tgt_start + r*n_tgt (wrapping)
-    from paper_2501_16572_b200 import sharding
-    idx = sharding.weak_scaling_targets(w.tgt_start, w.n_tgt, w.n_orb, rank)
-    if world == 1:
+    del psi
+    t_gen = time.perf_counter() - t_start
+    # weak scaling: rank r applies Vx to n_tgt targets starting at tgt_start + r*n_tgt (wrapping);
+    # strong scaling: the config's n_tgt targets are split over the ranks (sharding.shard_targets)
+    if args.scaling == "strong":
+        k0, k1 = sharding.shard_targets(w.n_tgt, rank, world)
+        d_tgt = d_psi[w.tgt_start + k0:w.tgt_start + k1]
+        d_occ_t = d_occ[w.tgt_start + k0:w.tgt_start + k1]
+        n_tgt_union, k_off = w.n_tgt, k0
+    elif world == 1:
         d_tgt = d_psi[w.tgt_start:w.tgt_start + w.n_tgt]
         d_occ_t = d_occ[w.tgt_start:w.tgt_start + w.n_tgt]
+        n_tgt_union, k_off = w.n_tgt, 0
     else:
-        d_tgt = d_psi[idx.to(dev)].contiguous()
-        d_occ_t = d_occ[idx.to(dev)].contiguous()
+        idx = sharding.weak_scaling_targets(w.tgt_start, w.n_tgt, w.n_orb, rank).to(dev)
+        d_tgt = d_psi[idx].contiguous()
+        d_occ_t = d_occ[idx].contiguous()
+        n_tgt_union, k_off = world * w.n_tgt, rank * w.n_tgt
+    n_tgt_local = d_tgt.shape[0]
+    solves_all_ranks = w.n_orb * n_tgt_union
 
     plan = exx.Plan.for_workload(w, max_batch=max(128, n_c), device=local)
     plan.set_variant(args.variant)
-    vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64, device=dev)
+    vx = torch.empty((n_tgt_local, w.nz, w.ny, w.nx), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream(dev)
 
     def step():
-        return plan.apply(d_psi, d_occ, d_tgt, d_occ_t, vx=vx, n_c=n_c, stream=stream)
+        vx_, e_k, ex = plan.apply(d_psi, d_occ, d_tgt, d_occ_t, vx=vx, n_c=n_c, stream=stream)
+        if world > 1:   # the path's one collective: per-target energies of the union, E_x of the union
+            e_k, ex = sharding.reduce_energy(e_k, d_occ_t, k_off, n_tgt_union)
+        return vx_, e_k, ex
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
+    warmup = max(args.warmup, 3)
+    period = 20 if w.pair_solves * w.flops_per_solve < 5e13 else 250
+    sampler = ClockSampler(local, period) if rank == 0 else None
+    total_ms, (_, e_k, ex) = timed_apply(step, args.steps, warmup, flush, stream, dist.barrier if world > 1 else None)
     launches_per_step = plan.last_launch_count
-
-    sampler = ClockSampler(local) if rank == 0 else None
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for e0, e1 in ev:
-        flush.fill_(1)             # evict L2 between timed steps (outside the event pair)
-        e0.record(stream)
-        _, e_k, ex = step()
-        e1.record(stream)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    total_ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
     t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms = float(t.item())
     clocks = sampler.stop() if sampler else None
     ms_per_step = total_ms / args.steps
-    value = world * w.pair_solves / (ms_per_step * 1e-3)
+    value = solves_all_ranks / (ms_per_step * 1e-3)
     ex_val = float(ex.item())
 
     if rank != 0:
@@ -268,132 +448,113 @@ def run_b200(args):
     # ---- roofline of the dominant kernel class (mode products on the FP64 tensor pipe) -----------------
     peak_dmma = exx.probe_fp64_peak(1, local, 1.5)
     peak_dfma = exx.probe_fp64_peak(0, local, 0.5)
-    plan.set_profiling(True)
-    prof_steps = min(2, args.steps)
-    for _ in range(prof_steps):
-        flush.fill_(1)
-        step()
-    prof = plan.get_profile()
-    plan.set_profiling(False)
-    mp_ms, mp_cnt = prof["mode_product"]
-    all_ms = sum(v[0] for v in prof.values())
-    flops_step = w.pair_solves * w.flops_per_solve
-    achieved = flops_step * prof_steps / (mp_ms * 1e-3) / 1e12 if mp_ms > 0 else 0.0
-    roofline = {"bound": "tensor", "kernel": "k_mode_dmma (six mode products per batch, FP64 mma.sync -> DMMA.8x8x4)",
-                "achieved": achieved, "peak": peak_dmma, "unit": "TFLOP/s", "frac": achieved / peak_dmma,
-                "traffic": NCU_TRAFFIC_BYTES.get((w.cfg, n_c)),
-                "traffic_note": "bytes per k_mode_t launch, profiles/r1_final2_summary.md / r1_final_summary.md (cold-cache ncu replay); "
-                                f"algorithmic bytes per launch = {2 * 8 * w.N * min(n_c, w.pair_solves):.4g} (batch read + written in place)",
-                "peak_source": "measured live: exx_probe_fp64_peak DMMA issue loop (MEASURED_PEAKS.json has no FP64 entry); "
-                               f"DFMA loop {peak_dfma:.2f} TF",
-                "avg_launch_ms": mp_ms / max(mp_cnt, 1), "launches": mp_cnt // prof_steps,
-                "share_of_step": mp_ms / all_ms if all_ms > 0 else None,
+    flops_step = w.n_orb * n_tgt_local * w.flops_per_solve
+    prof_steps = 1 if ms_per_step > 2000 else min(2, args.steps)
+    inst = instrumented(plan, step, flush, prof_steps, flops_step, peak_dmma)
+    traffic = load_ncu_traffic().get((w.cfg, n_c))
+    n_batch = min(n_c, w.n_orb * n_tgt_local)
+    roofline = {"bound": "tensor",
+                "kernel": "k_mode_t (the mode products of a batch, FP64 mma.sync -> DMMA.8x8x4, operands by TMA)",
+                "achieved": inst["achieved"], "peak": peak_dmma, "unit": "TFLOP/s", "frac": inst["frac"],
+                "traffic": traffic[0] if traffic else None,
+                "traffic_note": (f"dram bytes per launch from the committed ncu --set full capture profiles/{traffic[1]}"
+                                 if traffic else "no committed ncu capture for this (config, n_c)")
+                                + f"; algorithmic bytes of an in-place pass over one batch = {2 * 8 * w.N * n_batch:.4g}",
+                "peak_source": "measured live by this repo's own probe (exx_probe_fp64_peak, a register-resident DMMA issue "
+                               "loop, 1.5 s): MEASURED_PEAKS.json has no FP64 entry and the profiling guide states no FP64 "
+                               f"fallback; 148 SMs x 128 flop/clk x 1.965 GHz = 37.2; DFMA loop {peak_dfma:.2f} TF",
+                "avg_launch_ms": inst["avg_launch_ms"], "launches": inst["launches"],
+                "share_of_step": inst["share_of_step"],
                 "step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
-                "class_ms_per_step": {k: v[0] / prof_steps for k, v in prof.items()},
-                "measured": "separate instrumented steps (CUDA-event pair around every launch, caller's stream)"}
+                "class_ms_per_step": inst["class_ms_per_step"],
+                "measured": f"{prof_steps} separate instrumented step(s) (CUDA-event pair around every launch, caller's stream)"}
 
     # ---- end to end through the C-ABI with host buffers (H2D + D2H inside the timed region) ------------
     e2e = None
-    if not args.no_e2e and world == 1 and w.n_orb * w.N * 8 <= (24 << 30):
-        h_psi = torch.empty(psi.shape, dtype=torch.float64, pin_memory=True)
-        h_psi.copy_(psi)
-        h_occ = occ.cpu().contiguous()
-        h_occ_t = occ_t.cpu().contiguous()
-        h_vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64, pin_memory=True)
-        k = max(3, min(args.steps, 5))
-        for _ in range(2):
-            plan.apply_host(h_psi, h_occ, tgt_start=w.tgt_start, n_tgt=w.n_tgt, occ_tgt=h_occ_t, vx=h_vx, n_c=n_c)
-        t0 = time.perf_counter()
-        for _ in range(k):
-            _, _, ex_h = plan.apply_host(h_psi, h_occ, tgt_start=w.tgt_start, n_tgt=w.n_tgt, occ_tgt=h_occ_t,
-                                         vx=h_vx, n_c=n_c)
-        dt = (time.perf_counter() - t0) / k
-        e2e = {"value": w.pair_solves / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(h_psi.numel() * 8 + h_occ.numel() * 8 + h_occ_t.numel() * 8),
-               "d2h_bytes_per_step": int(h_vx.numel() * 8 + w.n_tgt * 8 + 8), "ms_per_step": dt * 1e3,
-               "api": "exx_apply_host (pinned host buffers; synchronous; wall clock)", "ex": ex_h}
+    if not args.no_e2e and world == 1:
+        e2e = measure_e2e(plan, w, d_psi, d_occ, n_c, ms_per_step)
 
-    # ---- ACE tail and application, when the targets are the orbitals themselves ---
-    ace = None
+    extra = {}
     if not args.no_ace and world == 1 and w.n_tgt == w.n_orb and w.tgt_start == 0:
-        n = w.n_orb
-        xi = torch.empty_like(vx)
-        out = torch.empty_like(vx)
+        extra.update(measure_ace_and_symmetric(plan, w, d_psi, d_occ, vx, ms_per_step, n_c, args.nc_sym, peak_dmma,
+                                               flush, stream, args.steps))
+    plan.close()
 
-        def timed(fn, reps=5):
-            for _ in range(2):
-                fn()
-            ts = []
-            for _ in range(reps):
-                flush.fill_(1)
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(stream)
-                fn()
-                b.record(stream)
-                torch.cuda.synchronize()
-                ts.append(a.elapsed_time(b))
-            return statistics.median(ts)
-
-        info_box = []
-        ms_build = timed(lambda: info_box.append(plan.ace_build(d_psi, vx, xi=xi, want_M=False, stream=stream)[2]))
-        n_launch_build = plan.last_launch_count
-        ms_apply = timed(lambda: plan.ace_apply(xi, d_psi, out=out, stream=stream))
-        n_launch_apply = plan.last_launch_count
-        fl_build = 2.0 * n * n * w.N + sum(2.0 * min(64, n - kb) * (kb + min(64, n - kb)) * w.N
-                                           for kb in range(0, n, 64)) + n ** 3 / 3.0
-        fl_apply = 4.0 * n * n * w.N
-        ace = {"build_ms": ms_build, "apply_ms": ms_apply, "info": int(info_box[-1].item()),
-               "build_tflops": fl_build / ms_build / 1e9, "apply_tflops": fl_apply / ms_apply / 1e9,
-               "build_frac_of_dmma_peak": fl_build / ms_build / 1e9 / peak_dmma,
-               "apply_frac_of_dmma_peak": fl_apply / ms_apply / 1e9 / peak_dmma,
-               "apply_columns_per_s": n / (ms_apply * 1e-3), "launches": [int(n_launch_build), int(n_launch_apply)],
-               "max_abs_err_ace_psi_minus_vx": float((out - vx).abs().max().item()),
-               "max_abs_vx": float(vx.abs().max().item()),
-               "what": "exx_ace_build(psi, W=vx) and exx_ace_apply(xi, psi): median of 5, L2 flushed, CUDA events; "
-                       "share of the exchange step = (build_ms) / ms_per_step"}
-
-    # ---- pair-symmetric apply: same result from about half the solves --------------
-    symmetric = None
-    if not args.no_ace and world == 1 and w.n_tgt == w.n_orb and w.tgt_start == 0:
-        vx_s = torch.empty_like(vx)
-        n_c_sym = args.nc_sym or min(n_c, 4 * w.n_orb)
-        for _ in range(2):
-            plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
-        ts = []
-        for _ in range(min(args.steps, 5)):
-            flush.fill_(1)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            _, _, ex_s = plan.apply_symmetric(d_psi, d_occ, vx=vx_s, n_c=n_c_sym, stream=stream)
-            b.record(stream)
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        ms_s = statistics.median(ts)
-        executed = plan.last_solve_count
-        symmetric = {"ms_per_step": ms_s, "n_c": n_c_sym, "executed_solves_per_step": int(executed),
-                     "executed_solves_per_s": executed / (ms_s * 1e-3),
-                     "pair_equivalent_solves_per_s": w.pair_solves / (ms_s * 1e-3),
-                     "applies_per_s": w.n_tgt / (ms_s * 1e-3), "speedup_vs_full": ms_per_step / ms_s,
-                     "step_frac_executed": executed * w.flops_per_solve / (ms_s * 1e-3) / 1e12 / peak_dmma,
-                     "E_x": float(ex_s.item()),
-                     "max_rel_diff_vs_full": float(((vx_s - vx).abs().max() / vx.abs().max()).item()),
-                     "what": "exx_apply_symmetric: only pairs j <= k solved; roofline credit only for executed solves"}
+    # ---- the other configs and the config-4 batch sweep, short runs (extra objects, not the headline) --
+    if not args.no_extras and world == 1 and w.cfg == DEFAULT_CONFIG and not (args.n_orb or args.n_tgt):
+        del d_psi, d_tgt, vx
+        torch.cuda.empty_cache()
+        configs = {}
+        configs["cfg2"], _ = measure_extra(exx, 2, dev, local, peak_dmma, flush, stream, steps=10, want_ace=not args.no_ace)
+        configs["cfg3"], _ = measure_extra(exx, 3, dev, local, peak_dmma, flush, stream, steps=3, want_ace=not args.no_ace)
+        configs["cfg4"], psi4 = measure_extra(exx, 4, dev, local, peak_dmma, flush, stream, n_tgt=32, steps=3)
+        sweep = []
+        for nc in (16, 32, 64, 128, 256, 512):
+            r, _ = measure_extra(exx, 4, dev, local, peak_dmma, flush, stream, n_tgt=8, n_c=nc, steps=3, psi=psi4)
+            sweep.append({k: r[k] for k in ("n_c", "n_tgt", "pair_solves_per_step", "ms_per_step", "value", "step_frac")})
+        del psi4
+        torch.cuda.empty_cache()
+        extra["configs"] = configs
+        extra["sweep_cfg4"] = {"what": "BASELINE.json configs[3] batch-size sweep (the paper's Fig. 1 in shape): all 1,536 "
+                                       "orbitals against a reduced block of 8 targets (896..903), 3 timed steps each",
+                               "unit": UNIT, "rows": sweep}
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
-        cpu_baseline, _, _ = time_oracle(w, psi.cpu(), occ.cpu(), tgt.cpu(), occ_t.cpu(), args.cpu_seconds)
+        cpu_baseline, _, _ = time_oracle(w, args.cpu_seconds)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(w, n_c, {"parallelism": f"targets sharded over {world} rank(s), orbitals replicated"}),
-            "applies_per_s": world * w.n_tgt / (ms_per_step * 1e-3), "E_x": ex_val,
+            "config": config_dict(w, n_c, {"parallelism": f"targets sharded over {world} rank(s) ({args.scaling} scaling), "
+                                                           "orbitals replicated; one all-reduce of the per-target energies",
+                                           "pair_solves_all_ranks": solves_all_ranks}),
+            "applies_per_s": n_tgt_union / (ms_per_step * 1e-3), "E_x": ex_val,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches_per_step * args.steps),
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "ace": ace, "symmetric": symmetric}
+            "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "vs_cpu_baseline": value / cpu_baseline["value"] if cpu_baseline else None,
+            "seconds": {"inputs": t_gen, "total": time.perf_counter() - t_start}}
+    line.update(extra)
     print(json.dumps(line), flush=True)
-    plan.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def measure_e2e(plan, w, d_psi, d_occ, n_c, ms_per_step):
+    """The same step through exx_apply_host: HOST buffers in, HOST results out, H2D of the orbitals (streamed in blocks,
+    two resident at a time) and D2H of vx / e_k / E_x inside the timed region; wall clock around the synchronous call."""
+    shape = tuple(d_psi.shape)
+    pinned = True
+    try:
+        h_psi = torch.empty(shape, dtype=torch.float64, pin_memory=True)
+    except RuntimeError:
+        pinned = False
+        h_psi = torch.empty(shape, dtype=torch.float64)
+    chunk = max(1, (1 << 30) // (w.N * 8))
+    for j0 in range(0, w.n_orb, chunk):      # the bytes the device path used, copied out in 1 GiB pieces
+        h_psi[j0:j0 + chunk].copy_(d_psi[j0:j0 + chunk])
+    h_occ = d_occ.cpu().contiguous()
+    h_occ_t = h_occ[w.tgt_start:w.tgt_start + w.n_tgt].contiguous()
+    try:
+        h_vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64, pin_memory=pinned)
+    except RuntimeError:
+        h_vx = torch.empty((w.n_tgt, w.nz, w.ny, w.nx), dtype=torch.float64)
+    k = int(max(2, min(5, 90e3 / max(ms_per_step, 1e-3))))
+    wu = 1 if ms_per_step > 2000 else 2
+    for _ in range(wu):
+        plan.apply_host(h_psi, h_occ, tgt_start=w.tgt_start, n_tgt=w.n_tgt, occ_tgt=h_occ_t, vx=h_vx, n_c=n_c)
+    t0 = time.perf_counter()
+    for _ in range(k):
+        _, _, ex_h = plan.apply_host(h_psi, h_occ, tgt_start=w.tgt_start, n_tgt=w.n_tgt, occ_tgt=h_occ_t,
+                                     vx=h_vx, n_c=n_c)
+    dt = (time.perf_counter() - t0) / k
+    return {"value": w.pair_solves / dt, "unit": UNIT,
+            "h2d_bytes_per_step": int((h_psi.numel() + w.n_tgt * w.N + h_occ.numel() + h_occ_t.numel()) * 8),
+            "d2h_bytes_per_step": int(h_vx.numel() * 8 + w.n_tgt * 8 + 8), "ms_per_step": dt * 1e3,
+            "steps": k, "warmup": wu,
+            "api": "exx_apply_host (" + ("pinned" if pinned else "pageable: pinning failed on this box") +
+                   " host buffers; orbitals uploaded in blocks while the previous block computes; synchronous; wall clock)",
+            "ex": ex_h}
 
 
 def run_bloch(args):
@@ -422,20 +583,11 @@ def run_bloch(args):
     def step():
         return plan.apply_bloch(psi, occ, tgt, vx=vx, n_c=n_c, stream=stream)
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-    launches = plan.last_launch_count
     sampler = ClockSampler(0)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for e0, e1 in ev:
-        flush.fill_(1)
-        e0.record(stream)
-        _, e_k = step()
-        e1.record(stream)
-    torch.cuda.synchronize()
+    total_ms, (_, e_k) = timed_apply(step, args.steps, max(args.warmup, 3), flush, stream)
+    launches = plan.last_launch_count
     clocks = sampler.stop()
-    ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+    ms = total_ms / args.steps
     peak = exx.probe_fp64_peak(1, 0, 1.5)
     plan.set_profiling(True)
     flush.fill_(1)
@@ -449,21 +601,22 @@ def run_bloch(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "c128 (two f64 planes)", "data": "synthetic",
             "config": config_dict(w, n_c, {"theta": list(theta), "variant": "Bloch-periodic complex (one k-q pair)"}),
             "clocks": clocks, "gpu_launches": int(launches * args.steps), "e_k0": float(e_k[0].item()),
-            "roofline": {"bound": "tensor", "kernel": "k_mode_t (real and imaginary part of V) + k_combine",
+            "roofline": {"bound": "tensor", "kernel": "k_mode_t (complex mode products)",
                          "achieved": flops / (mp_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
                          "frac": flops / (mp_ms * 1e-3) / 1e12 / peak,
                          "step_frac": flops / (ms * 1e-3) / 1e12 / peak, "flops_per_step": flops,
                          "class_ms_per_step": {k: v[0] for k, v in prof.items()},
-                         "note": "mode_product class includes the combine kernels; executed real flops (4x a real solve on complex axes)"}}
+                         "note": "executed real flops (4x a real solve on complex axes)"}}
     print(json.dumps(line), flush=True)
     plan.close()
 
 
 def run_solver_sweep(args):
-    """The paper's Fig. 1 (time per linear system against the batch size n_c) and Fig. 2 (batch solver, GPU against
-    CPU) in shape, on the config's grid: seeded N(0,1) right-hand sides, exx_poisson_solve,
-    CUDA events, median of 5 after 2 warm-ups; n_c = 1 is the non-batch limit (Eq. 8: one system per set of
-    products).  The CPU column is the oracle's poisson_solve (numpy) on batches of 20 (the paper's n_c)."""
+    """The paper's Fig. 1 (time per linear system against the batch size n_c) and Fig. 2 (batch against non-batch
+    solver, GPU against CPU) in shape, on the config's grid: seeded N(0,1) right-hand sides,
+    exx_poisson_solve, CUDA events, median of 5 after 2 warm-ups.  `nonbatch_eq8` is the per-slice algorithm of Eq. 8
+    (V1^T B_k V2 for every frontal slice, then the product with V3; exx_poisson_solve_nonbatch), one
+    system at a time.  The CPU column is the oracle's poisson_solve (numpy) on batches of 20 (the paper's n_c)."""
     from paper_2501_16572_b200 import exx
     import __graft_entry__ as ge
     ge.build()
@@ -477,24 +630,36 @@ def run_solver_sweep(args):
     plan = exx.Plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, max_batch=512, device=0)
     peak = exx.probe_fp64_peak(1, 0, 1.0)
     stream = torch.cuda.current_stream(dev)
+
+    def med(fn, reps=5):
+        for _ in range(2):
+            fn()
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts)
+
     rows = []
     for n_c in (1, 2, 4, 8, 16, 20, 32, 64, 128, 256, 512):
         if n_c > n_rhs:
             break
         m = n_rhs if n_c >= 16 else max(n_c, min(n_rhs, 16 * n_c))     # fewer systems for the tiny batches
-        for _ in range(2):
-            plan.poisson_solve(rhs[:m], out=out[:m], n_c=n_c, stream=stream)
-        ts = []
-        for _ in range(5):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            plan.poisson_solve(rhs[:m], out=out[:m], n_c=n_c, stream=stream)
-            b.record(stream)
-            torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        ms = statistics.median(ts)
+        ms = med(lambda: plan.poisson_solve(rhs[:m], out=out[:m], n_c=n_c, stream=stream))
         rows.append({"n_c": n_c, "systems": m, "us_per_solve": 1e3 * ms / m, "solves_per_s": m / (ms * 1e-3),
                      "frac_of_dmma_peak": m * w.flops_per_solve / (ms * 1e-3) / 1e12 / peak})
+    nonbatch = None
+    if hasattr(plan, "poisson_solve_nonbatch"):
+        m = min(n_rhs, 16)
+        ms = med(lambda: plan.poisson_solve_nonbatch(rhs[:m], out=out[:m], stream=stream))
+        nonbatch = {"systems": m, "us_per_solve": 1e3 * ms / m, "solves_per_s": m / (ms * 1e-3),
+                    "launches_per_system": plan.last_launch_count / m,
+                    "what": "Eq. 8 (PAPER.md:74-78): one launch per frontal slice for V1^T B_k V2, one for the product "
+                            "with V3, the multiplier, and the same back"}
     from oracle import exx_oracle as orc   # cpu_baseline leg
     oplan = orc.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega)
     c = rhs[:20].cpu().numpy()
@@ -507,7 +672,9 @@ def run_solver_sweep(args):
     cpu_us = 1e6 * (time.perf_counter() - t0) / (20 * reps)
     best = min(rows, key=lambda r: r["us_per_solve"])
     print(json.dumps({"metric": "poisson_solve_sweep", "config": config_dict(w, 0), "peak_tflops": peak, "rows": rows,
+                      "nonbatch_eq8": nonbatch,
                       "speedup_batch_vs_nc1": rows[0]["us_per_solve"] / best["us_per_solve"], "best_n_c": best["n_c"],
+                      "speedup_batch_vs_nonbatch_eq8": nonbatch["us_per_solve"] / best["us_per_solve"] if nonbatch else None,
                       "cpu_baseline": {"us_per_solve": cpu_us, "cores": _oracle_threads(), "kind": "oracle",
                                        "sample": f"oracle poisson_solve, batches of 20, {reps} repetitions"},
                       "gpu_over_cpu_at_nc20": cpu_us / next(r["us_per_solve"] for r in rows if r["n_c"] == 20)}), flush=True)

@@ -11,6 +11,8 @@
 
 namespace {
 
+using exx::DeviceScope;
+
 thread_local cudaError_t g_last_cuda = cudaSuccess;
 thread_local char g_msg[256];
 
@@ -25,6 +27,8 @@ struct HostApiBuffers {
   cudaStream_t stream = nullptr;
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t done[kHostChunks] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t up[2] = {nullptr, nullptr};    // orbital block b uploaded into ring buffer b % 2
+  cudaEvent_t used[2] = {nullptr, nullptr};  // the compute that read ring buffer b % 2 has finished
 };
 
 inline exx_status cuda_fail(cudaError_t e) {
@@ -46,14 +50,6 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
 
 // the DMMA kernels serve every axis (n <= 128): no pass needs the second workspace half as scratch
 inline bool all_axes_fast(const exx_plan* p) { return p->d_Vpad[0] && p->d_Vpad[1] && p->d_Vpad[2]; }
-
-// One lane by default: two lanes measured +1.5 % .. +2.7 % on the 96^3 / 120^3 configs (the other lane's
-// accumulate overlaps the mode products) and -2 % .. -6 % at 48^3, see DESIGN.md 6.4.  EXX_LANES overrides.
-inline int default_lanes(const exx_plan* p) {
-  if (const char* e = getenv("EXX_LANES"))
-    if (e[0] == '2') return all_axes_fast(p) ? 2 : 1;
-  return 1;
-}
 
 // a plan with a nonzero Bloch phase has complex eigenvectors: only the *_bloch entry points may use it
 inline bool is_complex_plan(const exx_plan* p) { return p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
@@ -169,7 +165,8 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   }
 
   if (device >= 0) {  // device < 0: host-only plan (planner tests); compute calls return EXX_ERR_CUDA
-    cudaError_t e = cudaSetDevice(device);
+    DeviceScope dev_scope(device);  // the caller's current device is restored on return
+    cudaError_t e = dev_scope.err;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, device);
     if (e == cudaSuccess)
       e = cudaDeviceGetAttribute(&p->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -196,7 +193,6 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->lane_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
-    if (e == cudaSuccess) p->lanes = default_lanes(p);
     if (e != cudaSuccess) {
       exx_plan_destroy(p);
       return e == cudaErrorMemoryAllocation ? EXX_ERR_ALLOC : cuda_fail(e);
@@ -223,7 +219,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
   if (!plan) return EXX_OK;
   exx_plan_full* p = static_cast<exx_plan_full*>(plan);
   if (p->device >= 0) {
-    cudaSetDevice(p->device);
+    DeviceScope dev_scope(p->device);
     exx::fast_destroy(p);
     exx::tma_destroy(p);
     if (p->lane_stream) cudaStreamDestroy(p->lane_stream);
@@ -242,6 +238,10 @@ exx_status exx_plan_destroy(exx_plan* plan) {
     if (p->ex.hb.copy_stream) cudaStreamDestroy(p->ex.hb.copy_stream);
     for (int c = 0; c < kHostChunks; ++c)
       if (p->ex.hb.done[c]) cudaEventDestroy(p->ex.hb.done[c]);
+    for (int c = 0; c < 2; ++c) {
+      if (p->ex.hb.up[c]) cudaEventDestroy(p->ex.hb.up[c]);
+      if (p->ex.hb.used[c]) cudaEventDestroy(p->ex.hb.used[c]);
+    }
   }
   delete p;
   return EXX_OK;
@@ -352,7 +352,7 @@ static exx_status run_energy(exx_plan* plan, const double* d_tgt, const double* 
   const size_t N = (size_t)plan->N;
   for (int k0 = 0; k0 < n_tgt; k0 += kEnergyChunk) {
     const int nk = n_tgt - k0 < kEnergyChunk ? n_tgt - k0 : kEnergyChunk;
-    if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++*launches; }   // the first chunk overwrites *d_ex
+    if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(plan, d_ex, 1, s)); ++*launches; }   // the first chunk overwrites *d_ex
     {
       exx::ProfScope ps(plan, exx::KC_OTHER, s);
       EXX_CUDA(exx::energy(plan, d_tgt + N * (size_t)k0, d_vx + N * (size_t)k0, d_occ_tgt ? d_occ_tgt + k0 : nullptr,
@@ -372,6 +372,8 @@ exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi,
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   if (n_rhs == 0) { plan->last_launches = 0; return EXX_OK; }
   const size_t need = exx_plan_workspace_bytes(plan, n_c);
   if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
@@ -412,6 +414,8 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
   const size_t need = exx_plan_workspace_bytes(plan, n_c);
   if (n_occ > 0 && n_tgt > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
@@ -425,7 +429,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
 
   if (n_tgt > 0 && n_occ == 0) {
     if (!plan->accumulate) {
-      EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_tgt, s));
+      EXX_CUDA(exx::zero_fill(plan, d_vx, (long long)N * n_tgt, s));
       ++launches;
     }
   } else if (n_tgt > 0) {
@@ -477,7 +481,7 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     }
   }
   if (d_ex && n_tgt == 0) {
-    EXX_CUDA(exx::zero_fill(d_ex, 1, s));
+    EXX_CUDA(exx::zero_fill(plan, d_ex, 1, s));
     ++launches;
   }
   if ((d_ex || d_ex_k) && n_tgt > 0) {
@@ -497,6 +501,8 @@ exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
   const size_t need = exx_plan_workspace_bytes(plan, n_c);
   if (n_orb > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
@@ -510,7 +516,7 @@ exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double
   double* buf1 = buf0 + N * (size_t)n_c;
   if (n_orb > 0) {
     // contributions are scattered to vx_k and vx_j: start from zero, every batch accumulates
-    EXX_CUDA(exx::zero_fill(d_vx, (long long)N * n_orb, s));
+    EXX_CUDA(exx::zero_fill(plan, d_vx, (long long)N * n_orb, s));
     ++launches;
   }
   auto run_batch = [&](int j0, int nj, int k0, int nk) -> exx_status {
@@ -555,13 +561,13 @@ exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double
     k0 += nk;
   }
   if (d_ex && n_orb == 0) {
-    EXX_CUDA(exx::zero_fill(d_ex, 1, s));
+    EXX_CUDA(exx::zero_fill(plan, d_ex, 1, s));
     ++launches;
   }
   if ((d_ex || d_ex_k) && n_orb > 0) {
     for (int k0 = 0; k0 < n_orb; k0 += kEnergyChunk) {
       const int nk = n_orb - k0 < kEnergyChunk ? n_orb - k0 : kEnergyChunk;
-      if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
+      if (k0 == 0 && d_ex) { EXX_CUDA(exx::zero_fill(plan, d_ex, 1, s)); ++launches; }
       {
         exx::ProfScope ps(plan, exx::KC_OTHER, s);
         EXX_CUDA(exx::energy(plan, d_psi + N * (size_t)k0, d_vx + N * (size_t)k0, d_occ + k0, nk,
@@ -583,15 +589,24 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
   if (tgt_in_psi && tgt_start + n_tgt > n_occ) return EXX_ERR_INVALID_ARG;
   if (!tgt_in_psi && n_tgt > 0 && !h_tgt) return EXX_ERR_INVALID_ARG;
   if (h_ex && !h_occ_tgt && n_tgt > 0) return EXX_ERR_INVALID_ARG;
+  if (is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
-  EXX_CUDA(cudaSetDevice(plan->device));
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   PlanExtras* ex = extras_of(plan);
   const size_t N = (size_t)plan->N;
   const size_t ws = exx_plan_workspace_bytes(plan, n_c);
-  // carve: psi | tgt (if separate) | vx | occ | occ_tgt | ex_k | ex | workspace
-  size_t n_dbl = N * n_occ + (tgt_in_psi ? 0 : N * n_tgt) + N * n_tgt + n_occ + 2 * (size_t)n_tgt + 8;
+  // Orbital blocks (Eq. 1's sum over j split with the plan's accumulate mode): with more orbitals than a batch holds,
+  // a block is one batch's worth of orbitals (n_c); otherwise the set is cut into kHostChunks blocks so that the
+  // upload of block b+1 still overlaps the compute of block b.  Only two blocks are resident at a time.
+  int blk = n_occ > n_c ? n_c : (n_occ + kHostChunks - 1) / kHostChunks;
+  if (blk < 1) blk = 1;
+  const int n_blocks = n_occ > 0 ? (n_occ + blk - 1) / blk : 0;
+  const int n_buf = n_blocks > 1 ? 2 : 1;
+  // carve: tgt | vx | psi block ring | occ | occ_tgt | ex_k | ex | workspace
+  size_t n_dbl = 2 * N * n_tgt + (size_t)n_buf * N * blk + n_occ + 2 * (size_t)n_tgt + 8;
   size_t bytes = sizeof(double) * n_dbl + ws + 512;
   if (ex->hb.bytes < bytes) {
     if (ex->hb.base) cudaFree(ex->hb.base);
@@ -601,54 +616,96 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
     ex->hb.bytes = bytes;
   }
   if (!ex->hb.stream) EXX_CUDA(cudaStreamCreateWithFlags(&ex->hb.stream, cudaStreamNonBlocking));
-  cudaStream_t s = ex->hb.stream;
+  if (!ex->hb.copy_stream) {
+    EXX_CUDA(cudaStreamCreateWithFlags(&ex->hb.copy_stream, cudaStreamNonBlocking));
+    for (int c = 0; c < kHostChunks; ++c) EXX_CUDA(cudaEventCreateWithFlags(&ex->hb.done[c], cudaEventDisableTiming));
+    for (int c = 0; c < 2; ++c) {
+      EXX_CUDA(cudaEventCreateWithFlags(&ex->hb.up[c], cudaEventDisableTiming));
+      EXX_CUDA(cudaEventCreateWithFlags(&ex->hb.used[c], cudaEventDisableTiming));
+    }
+  }
+  cudaStream_t s = ex->hb.stream, cs = ex->hb.copy_stream;
   double* q = ex->hb.base;
-  double* d_psi = q; q += N * n_occ;
-  double* d_tgt = tgt_in_psi ? d_psi + N * (size_t)tgt_start : q;
-  if (!tgt_in_psi) q += N * n_tgt;
+  double* d_tgt = q; q += N * n_tgt;
   double* d_vx = q; q += N * n_tgt;
+  double* d_blk[2] = {q, q + (n_buf > 1 ? N * (size_t)blk : 0)}; q += (size_t)n_buf * N * blk;
   double* d_occ = q; q += n_occ;
   double* d_occ_tgt = q; q += n_tgt;
   double* d_ex_k = q; q += n_tgt;
   double* d_ex = q; q += 8;
   void* d_ws = (void*)(((uintptr_t)q + 255) & ~(uintptr_t)255);
-  if (n_occ > 0) {
-    EXX_CUDA(cudaMemcpyAsync(d_psi, h_psi, sizeof(double) * N * n_occ, cudaMemcpyHostToDevice, s));
-    EXX_CUDA(cudaMemcpyAsync(d_occ, h_occ, sizeof(double) * n_occ, cudaMemcpyHostToDevice, s));
-  }
-  if (!tgt_in_psi && n_tgt > 0)
-    EXX_CUDA(cudaMemcpyAsync(d_tgt, h_tgt, sizeof(double) * N * n_tgt, cudaMemcpyHostToDevice, s));
+
+  auto upload_block = [&](int b) -> exx_status {  // on the copy stream, once the buffer's previous user is done
+    const int j0 = b * blk, nj = n_occ - j0 < blk ? n_occ - j0 : blk;
+    if (b >= 2) EXX_CUDA(cudaStreamWaitEvent(cs, ex->hb.used[b & 1], 0));
+    EXX_CUDA(cudaMemcpyAsync(d_blk[b & 1], h_psi + N * (size_t)j0, sizeof(double) * N * nj, cudaMemcpyHostToDevice, cs));
+    EXX_CUDA(cudaEventRecord(ex->hb.up[b & 1], cs));
+    return EXX_OK;
+  };
+  if (n_blocks > 0) { exx_status st = upload_block(0); if (st != EXX_OK) return st; }
+  if (n_tgt > 0)
+    EXX_CUDA(cudaMemcpyAsync(d_tgt, tgt_in_psi ? h_psi + N * (size_t)tgt_start : h_tgt, sizeof(double) * N * n_tgt,
+                             cudaMemcpyHostToDevice, s));
+  if (n_occ > 0) EXX_CUDA(cudaMemcpyAsync(d_occ, h_occ, sizeof(double) * n_occ, cudaMemcpyHostToDevice, s));
   if (h_occ_tgt && n_tgt > 0)
     EXX_CUDA(cudaMemcpyAsync(d_occ_tgt, h_occ_tgt, sizeof(double) * n_tgt, cudaMemcpyHostToDevice, s));
-  // The targets are applied in up to kHostChunks blocks (multiples of the k-block of a batch, so every batch and
-  // hence every bit of the result is that of a single exx_apply); the download of a block's vx runs on a second
-  // stream while the next block computes.  The energy is taken over all targets at the end.
-  if (!ex->hb.copy_stream) {
-    EXX_CUDA(cudaStreamCreateWithFlags(&ex->hb.copy_stream, cudaStreamNonBlocking));
-    for (int c = 0; c < kHostChunks; ++c) EXX_CUDA(cudaEventCreateWithFlags(&ex->hb.done[c], cudaEventDisableTiming));
-  }
-  const int nj_max = n_occ < n_c ? (n_occ > 0 ? n_occ : 1) : n_c;
-  const int kblock = n_c / nj_max > 0 ? n_c / nj_max : 1;
-  int chunk = (n_tgt + kHostChunks - 1) / kHostChunks;
-  chunk = (chunk + kblock - 1) / kblock * kblock;
-  if (chunk < 1) chunk = 1;
+
+  // the call owns d_vx: the plan's accumulate mode (meant for exx_apply on caller buffers) is overridden per block
+  const bool saved_accumulate = plan->accumulate;
   long long launches = 0, solves = 0;
-  int c = 0;
-  for (int k0 = 0; k0 < n_tgt; k0 += chunk, ++c) {
-    const int nk = n_tgt - k0 < chunk ? n_tgt - k0 : chunk;
-    exx_status st = exx_apply(plan, d_psi, d_occ, n_occ, d_tgt + N * (size_t)k0, nullptr, nk, d_vx + N * (size_t)k0,
-                              nullptr, nullptr, n_c, d_ws, ws, s);
-    if (st != EXX_OK) return st;
+  exx_status result = EXX_OK;
+  auto apply_block = [&](int b, int k0, int nk) -> exx_status {
+    const int j0 = b * blk, nj = n_occ - j0 < blk ? n_occ - j0 : blk;
+    plan->accumulate = b > 0;
+    exx_status st = exx_apply(plan, d_blk[b & 1], d_occ + j0, nj, d_tgt + N * (size_t)k0, nullptr, nk,
+                              d_vx + N * (size_t)k0, nullptr, nullptr, n_c, d_ws, ws, s);
     launches += plan->last_launches;
     solves += plan->last_solves;
-    if (h_vx) {
-      EXX_CUDA(cudaEventRecord(ex->hb.done[c], s));
-      EXX_CUDA(cudaStreamWaitEvent(ex->hb.copy_stream, ex->hb.done[c], 0));
-      EXX_CUDA(cudaMemcpyAsync(h_vx + N * (size_t)k0, d_vx + N * (size_t)k0, sizeof(double) * N * nk,
-                               cudaMemcpyDeviceToHost, ex->hb.copy_stream));
+    return st;
+  };
+  if (n_blocks == 0 && n_tgt > 0) {
+    plan->accumulate = false;
+    result = exx_apply(plan, nullptr, nullptr, 0, d_tgt, nullptr, n_tgt, d_vx, nullptr, nullptr, n_c, d_ws, ws, s);
+    launches += plan->last_launches;
+    if (result == EXX_OK && h_vx)
+      result = cudaMemcpyAsync(h_vx, d_vx, sizeof(double) * N * n_tgt, cudaMemcpyDeviceToHost, s) == cudaSuccess
+                   ? EXX_OK : cuda_fail(cudaGetLastError());
+  }
+  for (int b = 0; b < n_blocks && result == EXX_OK && n_tgt > 0; ++b) {
+    cudaError_t ce = cudaStreamWaitEvent(s, ex->hb.up[b & 1], 0);
+    if (ce != cudaSuccess) { result = cuda_fail(ce); break; }
+    if (b + 1 < n_blocks) {
+      if ((result = apply_block(b, 0, n_tgt)) != EXX_OK) break;
+      if ((ce = cudaEventRecord(ex->hb.used[b & 1], s)) != cudaSuccess) { result = cuda_fail(ce); break; }
+      // enqueued after this block's kernels: a pageable h_psi makes the copy call block the host, and the GPU then
+      // already has its work (with pinned memory the order does not matter)
+      if ((result = upload_block(b + 1)) != EXX_OK) break;
+    } else {
+      // last block: the targets go in up to kHostChunks chunks and a finished chunk's vx is downloaded on the copy
+      // stream (idle by now) while the next chunk computes
+      int chunk = (n_tgt + kHostChunks - 1) / kHostChunks;
+      if (chunk < 1) chunk = 1;
+      int c = 0;
+      for (int k0 = 0; k0 < n_tgt && result == EXX_OK; k0 += chunk, ++c) {
+        const int nk = n_tgt - k0 < chunk ? n_tgt - k0 : chunk;
+        if ((result = apply_block(b, k0, nk)) != EXX_OK) break;
+        if (h_vx) {
+          if ((ce = cudaEventRecord(ex->hb.done[c], s)) == cudaSuccess) ce = cudaStreamWaitEvent(cs, ex->hb.done[c], 0);
+          if (ce == cudaSuccess)
+            ce = cudaMemcpyAsync(h_vx + N * (size_t)k0, d_vx + N * (size_t)k0, sizeof(double) * N * nk,
+                                 cudaMemcpyDeviceToHost, cs);
+          if (ce != cudaSuccess) result = cuda_fail(ce);
+        }
+      }
     }
   }
-  if (n_tgt == 0 && h_ex) { EXX_CUDA(exx::zero_fill(d_ex, 1, s)); ++launches; }
+  plan->accumulate = saved_accumulate;
+  if (result != EXX_OK) {
+    cudaStreamSynchronize(s);
+    cudaStreamSynchronize(cs);
+    return result;
+  }
+  if (n_tgt == 0 && h_ex) { EXX_CUDA(exx::zero_fill(plan, d_ex, 1, s)); ++launches; }
   if ((h_ex || h_ex_k) && n_tgt > 0) {
     exx_status st = run_energy(plan, d_tgt, d_vx, h_occ_tgt ? d_occ_tgt : nullptr, n_tgt, h_ex ? d_ex : nullptr,
                                h_ex_k ? d_ex_k : nullptr, s, &launches);
@@ -660,7 +717,7 @@ exx_status exx_apply_host(exx_plan* plan, const double* h_psi, const double* h_o
     EXX_CUDA(cudaMemcpyAsync(h_ex_k, d_ex_k, sizeof(double) * n_tgt, cudaMemcpyDeviceToHost, s));
   if (h_ex) EXX_CUDA(cudaMemcpyAsync(h_ex, d_ex, sizeof(double), cudaMemcpyDeviceToHost, s));
   EXX_CUDA(cudaStreamSynchronize(s));
-  EXX_CUDA(cudaStreamSynchronize(ex->hb.copy_stream));
+  EXX_CUDA(cudaStreamSynchronize(cs));
   return EXX_OK;
 }
 
@@ -675,6 +732,8 @@ exx_status exx_ace_build(exx_plan* plan, const double* d_psi, const double* d_w,
                          double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!plan || n_orb < 1 || n_orb > 32768 || !d_psi || !d_w || !d_xi || is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   const size_t need = sizeof(double) * exx::ace_build_workspace_doubles(plan, n_orb);
   if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
   if (((uintptr_t)d_workspace) & 15) return EXX_ERR_INVALID_ARG;
@@ -698,6 +757,8 @@ exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const do
     return EXX_ERR_INVALID_ARG;
   if (n_trial > 0 && (!d_phi || !d_out)) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   if (n_trial == 0) { plan->last_launches = 0; return EXX_OK; }
   const size_t need = sizeof(double) * exx::ace_apply_workspace_doubles(plan, n_orb, n_trial);
   if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
@@ -739,6 +800,8 @@ exx_status exx_poisson_solve_bloch(exx_plan* plan, const double* d_rhs, double* 
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   if (n_rhs == 0) { plan->last_launches = 0; return EXX_OK; }
   const size_t need = exx_plan_workspace_bytes_bloch(plan, n_c);
   if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
@@ -771,6 +834,8 @@ exx_status exx_apply_bloch(exx_plan* plan, const double* d_psi, const double* d_
   n_c = resolve_nc(plan, n_c);
   if (n_c < 1 || n_c > plan->max_batch) return EXX_ERR_INVALID_ARG;
   if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
   const size_t N = (size_t)plan->N, fn = 2 * sizeof(double) * N;
   const size_t need = exx_plan_workspace_bytes_bloch(plan, n_c);
   if (n_occ > 0 && n_tgt > 0 && (!d_workspace || workspace_bytes < need)) return EXX_ERR_WORKSPACE;
@@ -783,7 +848,7 @@ exx_status exx_apply_bloch(exx_plan* plan, const double* d_psi, const double* d_
   long long launches = 0;
   PlanExtras* ex = extras_of(plan);
   if (n_tgt > 0 && n_occ == 0) {
-    if (!accumulate) { EXX_CUDA(exx::zero_fill(d_vx, 2 * (long long)N * n_tgt, s)); ++launches; }
+    if (!accumulate) { EXX_CUDA(exx::zero_fill(plan, d_vx, 2 * (long long)N * n_tgt, s)); ++launches; }
   } else if (n_tgt > 0) {
     double* b0 = (double*)d_workspace;
     double* const buf[3] = {b0, b0 + 2 * N * (size_t)n_c, b0 + 4 * N * (size_t)n_c};

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <vector>
 
 #include "exx.h"
@@ -92,7 +93,43 @@ cudaError_t sym_accumulate_transposed(const exx_plan* p, const double* psi, cons
 // shared by both variants: e_k = h^3 <tgt_k, vx_k>, then E_x
 cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const double* occ_tgt,
                    int n_tgt, double* ex_k_scratch, double* ex_k, double* ex, cudaStream_t s, long long len = 0);
-cudaError_t zero_fill(double* p, long long n, cudaStream_t s);
+cudaError_t zero_fill(const exx_plan* p, double* ptr, long long n, cudaStream_t s);
+
+// Opt-in to more than 48 KB of dynamic shared memory, remembered per kernel instantiation AND per device
+// (cudaFuncSetAttribute applies to the current device only; a plan may live on any device of the process).  One static
+// instance per launch site.  Concurrent callers race benignly: the attribute call is idempotent.
+struct SmemOptIn {
+  static constexpr int kMaxDevices = 64;
+  std::atomic<size_t> bytes[kMaxDevices];
+  template <typename K>
+  cudaError_t ensure(K kern, int device, size_t need, bool max_carveout = false) {
+    const bool tracked = device >= 0 && device < kMaxDevices;
+    if (tracked && bytes[device].load(std::memory_order_acquire) >= need) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need);
+    if (e != cudaSuccess) return e;
+    if (max_carveout) {
+      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+      if (e != cudaSuccess) return e;
+    }
+    if (tracked) bytes[device].store(need, std::memory_order_release);
+    return cudaSuccess;
+  }
+};
+
+// Makes the plan's device current for the duration of an entry point and restores the caller's device afterwards.
+struct DeviceScope {
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceScope(int device) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+    else if (err == cudaSuccess) prev = -1;  // nothing to restore
+  }
+  ~DeviceScope() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+  bool ok() const { return err == cudaSuccess; }
+};
 
 // RAII event pair around one launch when profiling is on (no-op otherwise).
 struct ProfScope {

@@ -389,10 +389,6 @@ inline bool vec2_ok(long long N, const void* a, const void* b, const void* c) {
 constexpr size_t kGramSmem = sizeof(double) * kStages * 2 * kTile * kLdA;
 constexpr size_t kExpandSmem = sizeof(double) * kStages * (kTile * kLdA + kKC * kLdB);
 
-template <typename K>
-cudaError_t opt_in(K kern, size_t bytes) {
-  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-}
 
 // C[ni][nj] = alpha * A B^T over the grid index; part: ksplit*ni*nj doubles
 cudaError_t gram(exx_plan* p, const double* A, int ni, const double* B, int nj, double alpha, double* part,
@@ -405,12 +401,12 @@ cudaError_t gram(exx_plan* p, const double* A, int ni, const double* B, int nj, 
   {
     ProfScope ps(p, KC_OTHER, s);
     if (vec2_ok(N, A, B, nullptr)) {
-      static const cudaError_t once = opt_in(k_gram<2>, kGramSmem);
-      if (once != cudaSuccess) return once;
+      static SmemOptIn opt;
+      if ((e = opt.ensure(k_gram<2>, p->device, kGramSmem)) != cudaSuccess) return e;
       k_gram<2><<<grid, 128, kGramSmem, s>>>(A, B, ni, nj, N, gs.slice, tiles_j, part);
     } else {
-      static const cudaError_t once = opt_in(k_gram<1>, kGramSmem);
-      if (once != cudaSuccess) return once;
+      static SmemOptIn opt;
+      if ((e = opt.ensure(k_gram<1>, p->device, kGramSmem)) != cudaSuccess) return e;
       k_gram<1><<<grid, 128, kGramSmem, s>>>(A, B, ni, nj, N, gs.slice, tiles_j, part);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -427,14 +423,15 @@ cudaError_t expand(exx_plan* p, const double* T, int ldt, int mi, int nk, const 
                    int ksel, double alpha, double* Out, cudaStream_t s, long long* launches) {
   const long long N = p->N;
   dim3 grid((unsigned)((N + kTile - 1) / kTile), (mi + kTile - 1) / kTile);
+  cudaError_t e;
   ProfScope ps(p, KC_OTHER, s);
   if (vec2_ok(N, in_lo, in_hi, Out)) {
-    static const cudaError_t once = opt_in(k_expand<2>, kExpandSmem);
-    if (once != cudaSuccess) return once;
+    static SmemOptIn opt;
+    if ((e = opt.ensure(k_expand<2>, p->device, kExpandSmem)) != cudaSuccess) return e;
     k_expand<2><<<grid, 128, kExpandSmem, s>>>(T, ldt, mi, nk, in_lo, in_hi, ksel, N, alpha, Out);
   } else {
-    static const cudaError_t once = opt_in(k_expand<1>, kExpandSmem);
-    if (once != cudaSuccess) return once;
+    static SmemOptIn opt;
+    if ((e = opt.ensure(k_expand<1>, p->device, kExpandSmem)) != cudaSuccess) return e;
     k_expand<1><<<grid, 128, kExpandSmem, s>>>(T, ldt, mi, nk, in_lo, in_hi, ksel, N, alpha, Out);
   }
   *launches += 1;

@@ -334,17 +334,8 @@ inline bool pick_class(int n, int* mtot, int* nt) {
   return true;
 }
 
-// EXX_NO_PDL=1 disables programmatic dependent launch (debug / A-B measurements)
-inline bool use_pdl() {
-  static const bool on = [] {
-    const char* e = getenv("EXX_NO_PDL");
-    return !(e && e[0] == '1');
-  }();
-  return on;
-}
-
 template <int MTOT, int NT>
-cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int grid, cudaStream_t s) {
+cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int grid, int device, cudaStream_t s) {
   constexpr size_t smem_v = sizeof(double) * 8 * MTOT * (8 * MTOT + 4);
 #define EXX_LAUNCH(XM, FW, PDD)                                                                         \
   do {                                                                                                  \
@@ -354,11 +345,10 @@ cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int gri
     const size_t smem_need = smem_v + (size_t)kWarps * kRing * NT * ((PDD) ? 2 : 1) * 256;              \
     const size_t smem = smem_need > kMinSmem ? smem_need : kMinSmem;                                    \
     auto kern = k_mode_w<MTOT, NT, XM, FW, PDD>;                                                        \
-    static bool attr_set = false; /* per instantiation; plans on one device share it */                \
-    if (!attr_set) {                                                                                    \
-      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    static SmemOptIn opt; /* per instantiation and device */                                           \
+    {                                                                                                   \
+      cudaError_t e = opt.ensure(kern, device, smem);                                                   \
       if (e != cudaSuccess) return e;                                                                   \
-      attr_set = true;                                                                                  \
     }                                                                                                   \
     cudaLaunchConfig_t cfg = {};                                                                        \
     cfg.gridDim = dim3(grid);                                                                           \
@@ -369,7 +359,7 @@ cudaError_t launch_class(bool xmode, bool fwd, bool two, const WArgs& a, int gri
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                      \
     at[0].val.programmaticStreamSerializationAllowed = 1;                                               \
     cfg.attrs = at;                                                                                     \
-    cfg.numAttrs = use_pdl() ? 1 : 0;                                                                   \
+    cfg.numAttrs = 1;                                                                                   \
     return cudaLaunchKernelEx(&cfg, kern, a);                                                           \
   } while (0)
   if (xmode) {
@@ -433,13 +423,13 @@ cudaError_t fast_mode_product(const exx_plan* p, int axis, bool forward, const d
   const long long ctas = (a.n_tiles + kWarps - 1) / kWarps;
   const int grid = (int)(ctas < p->sm_count ? ctas : p->sm_count);
   switch (mtot) {
-    case 2: return launch_class<2, 4>(xmode, forward, two, a, grid, s);
-    case 4: return launch_class<4, 4>(xmode, forward, two, a, grid, s);
-    case 6: return launch_class<6, 4>(xmode, forward, two, a, grid, s);
-    case 8: return launch_class<8, 2>(xmode, forward, two, a, grid, s);
-    case 12: return launch_class<12, 2>(xmode, forward, two, a, grid, s);
-    case 15: return launch_class<15, 2>(xmode, forward, two, a, grid, s);
-    default: return launch_class<16, 2>(xmode, forward, two, a, grid, s);
+    case 2: return launch_class<2, 4>(xmode, forward, two, a, grid, p->device, s);
+    case 4: return launch_class<4, 4>(xmode, forward, two, a, grid, p->device, s);
+    case 6: return launch_class<6, 4>(xmode, forward, two, a, grid, p->device, s);
+    case 8: return launch_class<8, 2>(xmode, forward, two, a, grid, p->device, s);
+    case 12: return launch_class<12, 2>(xmode, forward, two, a, grid, p->device, s);
+    case 15: return launch_class<15, 2>(xmode, forward, two, a, grid, p->device, s);
+    default: return launch_class<16, 2>(xmode, forward, two, a, grid, p->device, s);
   }
 }
 

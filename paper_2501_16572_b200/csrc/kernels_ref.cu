@@ -230,17 +230,14 @@ cudaError_t ref_mode_product(const exx_plan* p, int axis, bool forward, const do
 
 cudaError_t ref_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi,
                            BatchDesc bd, bool first, double* vx, cudaStream_t s, bool sym) {
-  static const int variant = [] { const char* e = getenv("EXX_ACC"); return e ? atoi(e) : 1; }();
   const unsigned N = (unsigned)p->N;
   const bool vec2 = (N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
-  if (vec2 && variant >= 2) {
+  if (vec2) {  // 16-byte loads and stores (the normal case: N even, buffers 16-byte aligned)
     dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nk);
-    if (variant == 3) k_accumulate<2, 8><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
-    else k_accumulate<2, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
+    k_accumulate<2, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
   } else {
     dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
-    if (variant == 0) k_accumulate<1, 2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
-    else k_accumulate<1, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
+    k_accumulate<1, 4><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, N, vx, sym);
   }
   return cudaGetLastError();
 }
@@ -273,9 +270,9 @@ cudaError_t energy(const exx_plan* p, const double* tgt, const double* vx, const
   return cudaGetLastError();
 }
 
-cudaError_t zero_fill(double* ptr, long long n, cudaStream_t s) {
+cudaError_t zero_fill(const exx_plan* p, double* ptr, long long n, cudaStream_t s) {
   if (n <= 0) return cudaSuccess;
-  k_zero<<<grid_for(n, 256, 148), 256, 0, s>>>(ptr, n);
+  k_zero<<<grid_for(n, 256, p->sm_count), 256, 0, s>>>(ptr, n);
   return cudaGetLastError();
 }
 

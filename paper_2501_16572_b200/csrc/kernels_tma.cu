@@ -552,24 +552,9 @@ cudaError_t get_map(TmaState* st, const void* base, unsigned long long d0, unsig
   return cudaSuccess;
 }
 
-inline bool use_pdl() {
-  static const bool on = [] {
-    const char* e = getenv("EXX_NO_PDL");
-    return !(e && e[0] == '1');
-  }();
-  return on;
-}
-
-inline bool pdl_half() {
-  static const bool on = [] {
-    const char* e = getenv("EXX_PDL_HALF");
-    return e && e[0] == '1';
-  }();
-  return on;
-}
-
 template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
-cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, cudaStream_t s) {
+cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, int device,
+                       cudaStream_t s) {
   constexpr int LDV = 8 * MTOT + 4;
   const size_t img = sizeof(double) * 16 * (size_t)a.S * LDV;
   // image | (alignment slack) | rings | mbarriers.  The request is padded so that exactly MINB CTAs fit an SM
@@ -579,15 +564,12 @@ cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs
   if (MINB == 2 && smem > 113 * 1024) return cudaErrorInvalidConfiguration;
   if (smem < floor_bytes) smem = floor_bytes;
   auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW>;
-  static size_t attr_smem = 0;  // per instantiation
-  if (smem > attr_smem) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // always the largest shared-memory carveout: kernels of the two lanes must agree on the SM's L1/shared
+  // split to be resident together (and a switch between launches drains the SM)
+  static SmemOptIn opt;  // per instantiation and device
+  {
+    cudaError_t e = opt.ensure(kern, device, smem, true);
     if (e != cudaSuccess) return e;
-    // always the largest shared-memory carveout: kernels of the two lanes must agree on the SM's L1/shared
-    // split to be resident together (and a switch between launches drains the SM)
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    attr_smem = smem;
   }
   cudaLaunchConfig_t cfg = {};
   const unsigned grid = a.n_tiles < (unsigned)sm_count ? a.n_tiles : (unsigned)sm_count;
@@ -601,21 +583,21 @@ cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs
   cfg.attrs = at;
   // Half-SM kernels (MINB == 2) are launched without programmatic serialization: an early-launched successor
   // would sit in griddepcontrol.wait in the very slot the other lane's kernel is meant to use.
-  cfg.numAttrs = (use_pdl() && (MINB == 1 || pdl_half())) ? 1 : 0;
+  cfg.numAttrs = MINB == 1 ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
 }
 
 template <int MTOT, int NT, int WARPS, int MINB, int NT2, int WARPS2, int MINB2>
 cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a,
-                         int sm_count, cudaStream_t s) {
+                         int sm_count, int device, cudaStream_t s) {
   if (xmode) {
-    if (two) return launch_one<MTOT, NT2, true, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
-    if (a.rmw) return launch_one<MTOT, NT, true, false, WARPS, MINB, true>(m0, m1, a, sm_count, s);
-    return launch_one<MTOT, NT, true, false, WARPS, MINB>(m0, m1, a, sm_count, s);
+    if (two) return launch_one<MTOT, NT2, true, true, WARPS2, MINB2>(m0, m1, a, sm_count, device, s);
+    if (a.rmw) return launch_one<MTOT, NT, true, false, WARPS, MINB, true>(m0, m1, a, sm_count, device, s);
+    return launch_one<MTOT, NT, true, false, WARPS, MINB>(m0, m1, a, sm_count, device, s);
   }
-  if (two) return launch_one<MTOT, NT2, false, true, WARPS2, MINB2>(m0, m1, a, sm_count, s);
-  if (a.rmw) return launch_one<MTOT, NT, false, false, WARPS, MINB, true>(m0, m1, a, sm_count, s);
-  return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, s);
+  if (two) return launch_one<MTOT, NT2, false, true, WARPS2, MINB2>(m0, m1, a, sm_count, device, s);
+  if (a.rmw) return launch_one<MTOT, NT, false, false, WARPS, MINB, true>(m0, m1, a, sm_count, device, s);
+  return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, device, s);
 }
 
 inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
@@ -706,20 +688,20 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   ++p->tma_launches;
   if (cc.minb == 2) {
     switch (cc.mtot) {
-      case 2: return launch_class<2, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
-      case 4: return launch_class<4, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
-      case 6: return launch_class<6, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
-      default: return launch_class<8, 2, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, s);
+      case 2: return launch_class<2, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+      case 4: return launch_class<4, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+      case 6: return launch_class<6, 4, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+      default: return launch_class<8, 2, 8, 2, 2, 8, 2>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
     }
   }
   switch (cc.mtot) {
-    case 2: return launch_class<2, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 4: return launch_class<4, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 6: return launch_class<6, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 8: return launch_class<8, 4, 12, 1, 4, 8, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 12: return launch_class<12, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    case 15: return launch_class<15, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, s);
-    default: return launch_class<16, 2, 12, 1, 2, 8, 1>(xmode, two, m0, m1, a, p->sm_count, s);
+    case 2: return launch_class<2, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    case 4: return launch_class<4, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    case 6: return launch_class<6, 4, 16, 1, 4, 12, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    case 8: return launch_class<8, 4, 12, 1, 4, 8, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    case 12: return launch_class<12, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    case 15: return launch_class<15, 2, 12, 1, 2, 12, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
+    default: return launch_class<16, 2, 12, 1, 2, 8, 1>(xmode, two, m0, m1, a, p->sm_count, p->device, s);
   }
 }
 

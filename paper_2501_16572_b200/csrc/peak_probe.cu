@@ -3,7 +3,7 @@
 // denominator with these (sustained over `seconds`), as SURVEY.md 8(d) requires.
 #include <cuda_runtime.h>
 
-#include "exx.h"
+#include "exx_internal.h"
 
 namespace {
 
@@ -47,7 +47,8 @@ __global__ void __launch_bounds__(256) k_dmma(double* out, int iters, double a, 
 
 extern "C" exx_status exx_probe_fp64_peak(int kind, int device, double seconds, double* tflops) {
   if (!tflops || (kind != 0 && kind != 1) || !(seconds > 0.0) || seconds > 30.0) return EXX_ERR_INVALID_ARG;
-  if (cudaSetDevice(device) != cudaSuccess) return EXX_ERR_CUDA;
+  exx::DeviceScope dev_scope(device);  // the caller's current device is restored on return
+  if (!dev_scope.ok()) return EXX_ERR_CUDA;
   int sms = 0;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return EXX_ERR_CUDA;
   const int threads = 256, blocks = sms * 8;

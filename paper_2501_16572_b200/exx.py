@@ -231,12 +231,25 @@ class Plan:
     def tma_launch_count(self) -> int:
         return int(self._lib.exx_plan_tma_launch_count(self._h))
 
+    def _release_workspaces(self):
+        """Drop the cached workspace.  Work queued on a non-current stream may still be using it and the caching
+        allocator only knows the allocation stream, so the device is synchronised first (a rare event: only when a
+        larger n_c arrives)."""
+        if self._ws is not None:
+            torch.cuda.synchronize(self.device)
+        self._ws = None
+
+    @staticmethod
+    def _expect(t, n: int, what: str):
+        if t is not None and t.numel() != n:
+            raise ValueError(f"{what}: expected {n} elements, got {t.numel()}")
+
     def _workspace(self, n_c: int) -> torch.Tensor:
         need = self.workspace_bytes(n_c)
         if need == 0:
             raise ValueError(f"n_c={n_c} outside 1..max_batch={self.max_batch}")
         if self._ws is None or self._ws.numel() < need:
-            self._ws = None
+            self._release_workspaces()
             self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
         return self._ws
 
@@ -248,6 +261,7 @@ class Plan:
             raise ValueError("rhs must be [n_rhs, nz, ny, nx]")
         if out is None:
             out = torch.empty_like(rhs)
+        self._expect(out, n_rhs * self.N, "out")
         ws = self._workspace(n_c)
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
         st = self._lib.exx_poisson_solve(self._h, _dev_ptr(rhs, self.device, "rhs"), _dev_ptr(out, self.device, "out"),
@@ -265,6 +279,9 @@ class Plan:
             raise ValueError("psi/tgt must be [n, nz, ny, nx]")
         if vx is None:
             vx = torch.empty((n_tgt, self.nz, self.ny, self.nx), dtype=torch.float64, device=self.device)
+        self._expect(occ, n_occ, "occ")
+        self._expect(occ_tgt, n_tgt, "occ_tgt")
+        self._expect(vx, n_tgt * self.N, "vx")
         ex = torch.empty((), dtype=torch.float64, device=self.device) if occ_tgt is not None else None
         ex_k = torch.empty(n_tgt, dtype=torch.float64, device=self.device) if want_ex_k else None
         ws = self._workspace(n_c)
@@ -285,6 +302,8 @@ class Plan:
             raise ValueError("psi must be [n, nz, ny, nx]")
         if vx is None:
             vx = torch.empty((n, self.nz, self.ny, self.nx), dtype=torch.float64, device=self.device)
+        self._expect(occ, n, "occ")
+        self._expect(vx, n * self.N, "vx")
         ex = torch.empty((), dtype=torch.float64, device=self.device)
         ex_k = torch.empty(n, dtype=torch.float64, device=self.device) if want_ex_k else None
         ws = self._workspace(n_c)
@@ -313,7 +332,7 @@ class Plan:
         if need == 0:
             raise ValueError(f"n_c={n_c} outside 1..max_batch={self.max_batch}")
         if self._ws is None or self._ws.numel() < need:
-            self._ws = None
+            self._release_workspaces()
             self._ws = torch.empty(need, dtype=torch.uint8, device=self.device)
         return self._ws
 
@@ -343,6 +362,8 @@ class Plan:
             if accumulate:
                 raise ValueError("accumulate=True needs vx")
             vx = torch.empty_like(tgt)
+        self._expect(occ, n_occ, "occ")
+        self._expect(vx, n_tgt * 2 * self.N, "vx")
         ex_k = torch.empty(n_tgt, dtype=torch.float64, device=self.device) if want_ex_k else None
         ws = self._workspace_bloch(n_c)
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
@@ -359,6 +380,8 @@ class Plan:
     def _ace_ws(self, n_orb: int, n_trial: int) -> torch.Tensor:
         need = self.ace_workspace_bytes(n_orb, n_trial)
         if getattr(self, "_aws", None) is None or self._aws.numel() < need:
+            if getattr(self, "_aws", None) is not None:
+                torch.cuda.synchronize(self.device)   # kernels queued on any stream may still use the old block
             self._aws = None
             self._aws = torch.empty(need, dtype=torch.uint8, device=self.device)
         return self._aws
@@ -372,6 +395,7 @@ class Plan:
             raise ValueError("psi/w must be [n, nz, ny, nx]")
         if xi is None:
             xi = torch.empty_like(w)
+        self._expect(xi, n * self.N, "xi")
         M = torch.empty((n, n), dtype=torch.float64, device=self.device) if want_M else None
         info = torch.zeros((), dtype=torch.int32, device=self.device)
         ws = self._ace_ws(n, 0)
@@ -391,6 +415,7 @@ class Plan:
             raise ValueError("xi/phi must be [n, nz, ny, nx]")
         if out is None:
             out = torch.empty_like(phi)
+        self._expect(out, m * self.N, "out")
         ws = self._ace_ws(n, m)
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
         st = self._lib.exx_ace_apply(self._h, _dev_ptr(xi, self.device, "xi"), n, _dev_ptr(phi, self.device, "phi"), m,
@@ -411,6 +436,10 @@ class Plan:
             n_tgt, tgt_start = tgt.shape[0], -1
         if vx is None:
             vx = np.empty((n_tgt, self.nz, self.ny, self.nx))
+        for t, n, what in ((psi, n_occ * self.N, "psi"), (occ, n_occ, "occ"), (occ_tgt, n_tgt, "occ_tgt"),
+                           (vx, n_tgt * self.N, "vx"), (tgt, n_tgt * self.N, "tgt")):
+            if t is not None and (t.size if isinstance(t, np.ndarray) else t.numel()) != n:
+                raise ValueError(f"{what}: expected {n} elements")
         ex = np.zeros(1)
         ex_k = np.empty(n_tgt)
         st = self._lib.exx_apply_host(self._h, _host_ptr(psi, "psi"), _host_ptr(occ, "occ"), n_occ,

@@ -42,6 +42,12 @@ SOLVE_CASES = [
     (1, 1, 40, 0.25, (0, 0, 1), 0.106, 2, 2),
     (96, 96, 96, 0.2, (0, 0, 0), 0.106, 2, 2),
     (120, 120, 120, 0.2, (0, 0, 0), 0.106, 1, 1),
+    # one axis longer than 128 points in each position: that axis runs on the plain kernel (per-axis fallback,
+    # buffer swap, pending multiplier), the other two stay on the tensor-core path
+    (130, 8, 6, 0.3, (0, 0, 0), 0.106, 3, 2),
+    (8, 132, 6, 0.3, (1, 0, 1), 0.0, 3, 2),
+    (6, 8, 136, 0.3, (0, 0, 1), 0.106, 3, 3),
+    (6, 8, 136, 0.3, (0, 0, 0), 0.0, 2, 1),
 ]
 
 
@@ -63,10 +69,71 @@ def test_poisson_solve_matches_oracle(case, variant):
     out2 = plan.poisson_solve(d, out=d, n_c=n_c)                 # in place
     torch.cuda.synchronize()
     assert torch.equal(out2, out)
-    if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0 and max(nx, ny, nz) <= 128:
-        assert plan.tma_launch_count == 12 * ((n_rhs + n_c - 1) // n_c)   # every pass went through the TMA kernels
+    if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0:
+        # two calls; per batch two passes through the TMA kernels for every axis of at most 128 points
+        n_fast = sum(1 for n in (nx, ny, nz) if n <= 128)
+        assert plan.tma_launch_count == 4 * n_fast * ((n_rhs + n_c - 1) // n_c)
     else:
         assert plan.tma_launch_count == 0
+    plan.close()
+
+
+@pytest.mark.parametrize("dims,bc,omega", [((130, 8, 6), (0, 0, 0), 0.106), ((8, 132, 6), (0, 1, 0), 0.0),
+                                           ((6, 8, 136), (0, 0, 1), 0.106)])
+def test_apply_with_an_axis_longer_than_128(dims, bc, omega):
+    """exx.h: an axis longer than 128 points falls back, per axis, to the plain kernel -- the only user of the second
+    workspace half (canary-guarded here) and of the pending-multiplier hand-over."""
+    nx, ny, nz = dims
+    rng = np.random.default_rng(11)
+    n = 5
+    psi = rng.standard_normal((n, nz, ny, nx))
+    occ = np.linspace(2.0, 0.2, n)
+    plan = exx.Plan(nx, ny, nz, 0.3, bc, 12, omega, max_batch=8, device=0)
+    o = orc.make_plan(nx, ny, nz, 0.3, bc, 12, omega)
+    vx_o, e_o, ex_o = orc.exx_apply(o, psi, occ, psi[1:4], occ[1:4])
+    d_psi, d_occ = torch.from_numpy(psi).cuda(), torch.from_numpy(occ).cuda()
+    nbytes = plan.workspace_bytes(3)
+    raw = torch.full((nbytes // 8 + 2 * 512,), -7.25e300, dtype=torch.float64, device="cuda")
+    plan._ws = raw[512:512 + nbytes // 8].view(torch.uint8)
+    vx, e_k, ex = plan.apply(d_psi, d_occ, d_psi[1:4], d_occ[1:4], n_c=3)
+    torch.cuda.synchronize()
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL and abs(ex.item() - ex_o) < TOL * abs(ex_o)
+    assert bool((raw[:512] == -7.25e300).all() and (raw[-512:] == -7.25e300).all())
+    assert 0 < plan.tma_launch_count < plan.last_launch_count      # both kinds of kernels ran
+    # in-place solve on the same plan: the result must come back into the caller's buffer after the swaps
+    C = rng.standard_normal((2, nz, ny, nx))
+    d = torch.from_numpy(C).cuda()
+    plan.poisson_solve(d, out=d, n_c=2)
+    torch.cuda.synchronize()
+    assert _rel(d.cpu().numpy(), orc.poisson_solve(o, C)) < TOL
+    assert bool((raw[:512] == -7.25e300).all() and (raw[-512:] == -7.25e300).all())
+    plan.close()
+
+
+def test_buffers_offset_by_8_bytes_take_the_cpasync_path():
+    """TMA needs 16-byte aligned bases: with even nx but psi / vx / rhs offset by one double every product must fall
+    back to the cp.async tensor-core kernels (exx_plan_tma_launch_count stays 0) and still match the oracle."""
+    w = wl.scaled(wl.WORKLOADS[2], 6, 3, 1)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    plan = exx.Plan.for_workload(w, max_batch=8, device=0)
+    N = w.N
+    raw_psi = torch.zeros(6 * N + 1, dtype=torch.float64, device="cuda")
+    d_psi = raw_psi[1:].view(6, w.nz, w.ny, w.nx)
+    d_psi.copy_(psi)
+    raw_vx = torch.zeros(3 * N + 1, dtype=torch.float64, device="cuda")
+    d_vx = raw_vx[1:].view(3, w.nz, w.ny, w.nx)
+    assert d_psi.data_ptr() % 16 == 8 and d_vx.data_ptr() % 16 == 8
+    ws = torch.empty(plan.workspace_bytes(4) + 8, dtype=torch.uint8, device="cuda")
+    plan._ws = ws[8:]
+    vx, e_k, ex = plan.apply(d_psi, occ.cuda(), d_psi[1:4], occ_t.cuda(), vx=d_vx, n_c=4)
+    torch.cuda.synchronize()
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy())
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL and abs(ex.item() - ex_o) < TOL * abs(ex_o)
+    assert plan.tma_launch_count == 0 and plan.last_launch_count > 0
+    out = plan.poisson_solve(d_psi[:2], out=d_vx[:2], n_c=2)
+    torch.cuda.synchronize()
+    assert _rel(out.cpu().numpy(), orc.poisson_solve(_oracle_plan(w), psi[:2].numpy())) < TOL
+    assert plan.tma_launch_count == 0
     plan.close()
 
 
@@ -191,6 +258,30 @@ def test_apply_host_end_to_end(variant):
     # separate target block
     vx_h2, _, _ = plan.apply_host(psi.numpy(), occ.numpy(), tgt=np.ascontiguousarray(tgt.numpy()), occ_tgt=occ_t.numpy())
     assert _rel(vx_h2, vx_o) < TOL
+    plan.close()
+
+
+@pytest.mark.parametrize("n_orb,n_c", [(11, 4), (11, 16), (3, 2), (1, 1)])
+def test_apply_host_streams_the_orbitals_in_blocks(n_orb, n_c):
+    """exx_apply_host uploads the orbitals block by block (two resident) and accumulates block after block: more
+    orbitals than a batch (blocks of n_c, ragged last block), fewer (four blocks), and the plan's own accumulate mode
+    must not leak into the call.  Bitwise equal to the device-buffer exx_apply (same order of the sum over j)."""
+    w = wl.scaled(wl.WORKLOADS[1], n_orb, min(n_orb, 5), 0)
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cpu")
+    occ = torch.linspace(2.0, 0.3, n_orb, dtype=torch.float64)
+    occ_t = occ[:w.n_tgt]
+    plan = exx.Plan.for_workload(w, max_batch=16, device=0)
+    vx_o, e_o, ex_o = orc.exx_apply(_oracle_plan(w), psi.numpy(), occ.numpy(), tgt.numpy(), occ_t.numpy())
+    plan.set_accumulate(True)          # must be ignored by the host call and restored afterwards
+    for _ in range(2):                 # second call reuses the plan-owned buffers (stale vx inside)
+        vx_h, e_h, ex_h = plan.apply_host(psi.numpy(), occ.numpy(), tgt_start=0, n_tgt=w.n_tgt, occ_tgt=occ_t.numpy(), n_c=n_c)
+        assert _rel(vx_h, vx_o) < TOL and abs(ex_h - ex_o) < TOL * abs(ex_o)
+        assert np.abs(e_h - e_o).max() < TOL * np.abs(e_o).max()
+    plan.set_accumulate(False)
+    d_psi = psi.cuda()
+    vx_d, _, _ = plan.apply(d_psi, occ.cuda(), d_psi[:w.n_tgt], occ_t.cuda(), n_c=n_c)
+    torch.cuda.synchronize()
+    assert np.array_equal(vx_d.cpu().numpy(), vx_h)
     plan.close()
 
 
