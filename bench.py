@@ -57,6 +57,9 @@ def parse_args():
     ap.add_argument("--variant", type=int, default=0, help="0 = DMMA path (default), 1 = plain-kernel cross-check variant")
     ap.add_argument("--n-orb", type=int, default=0, help="override orbital count (debug; invalidates the headline)")
     ap.add_argument("--n-tgt", type=int, default=0)
+    ap.add_argument("--fusion", type=int, default=-1,
+                    help="exx_plan_set_fusion mask (measurement hook; -1 = library default 3: fused z pass and fused "
+                         "x-backward + accumulate)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the configs 2-4 / sweep_cfg4 extra objects")
@@ -416,6 +419,8 @@ def run_b200(args):
 
     plan = exx.Plan.for_workload(w, max_batch=max(128, n_c), device=local)
     plan.set_variant(args.variant)
+    if args.fusion >= 0:
+        plan.set_fusion(args.fusion)
     vx = torch.empty((n_tgt_local, w.nz, w.ny, w.nx), dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream(dev)

@@ -94,6 +94,18 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes);
 int exx_plan_get_lanes(const exx_plan* plan);
 
 /*
+ * Pass fusion of the default variant (test and measurement hook; default 3 = both on).  Bit 0: the z-forward product,
+ * the eigen-space multiply and the z-backward product of a batch (Eq. 11's third and fourth GEMM and Eq. 16,
+ * PAPER.md:96-98, :134) run as ONE kernel, the intermediate staying in registers.  Bit 1: the x-backward product and
+ * the accumulate of Eq. 1 run as one kernel; phi_jk is never written to memory and exx_apply shapes its
+ * batches as nj occupied orbitals x nk targets with nk large enough to keep every SM busy.  With a bit off (or where
+ * TMA cannot address the buffers, or an axis has more than 128 points) the separate passes run.  The result does not
+ * depend on the mask beyond rounding (the sum over j is taken in ascending order either way).
+ */
+exx_status exx_plan_set_fusion(exx_plan* plan, int mask);
+int exx_plan_get_fusion(const exx_plan* plan);
+
+/*
  * Accumulate mode (off by default): while on, exx_apply ADDS its result into d_vx instead of overwriting it, so the
  * sum over the occupied orbitals of Eq. 1 can be split over several calls -- the orbital ring of
  * SURVEY.md 8(e), where each rank holds one block of orbitals at a time (paper_2501_16572_b200/sharding.py).  d_ex /

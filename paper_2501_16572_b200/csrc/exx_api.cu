@@ -124,6 +124,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false; p->accumulate = false;
+  p->fusion = 3;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
     p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
@@ -190,6 +191,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
       e = cudaMalloc(&p->ex.d_energy_scratch, sizeof(double) * kEnergyChunk * kEnergyBlocks);
     if (e == cudaSuccess) e = exx::fast_init(p);
     if (e == cudaSuccess) e = exx::tma_init(p);
+    if (e == cudaSuccess) e = exx::fused_init(p);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->lane_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
@@ -221,6 +223,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
   if (p->device >= 0) {
     DeviceScope dev_scope(p->device);
     exx::fast_destroy(p);
+    exx::fused_destroy(p);
     exx::tma_destroy(p);
     if (p->lane_stream) cudaStreamDestroy(p->lane_stream);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
@@ -262,6 +265,14 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes) {
 }
 
 int exx_plan_get_lanes(const exx_plan* plan) { return plan ? plan->lanes : 0; }
+
+exx_status exx_plan_set_fusion(exx_plan* plan, int mask) {
+  if (!plan || mask < 0 || mask > 3) return EXX_ERR_INVALID_ARG;
+  plan->fusion = mask;
+  return EXX_OK;
+}
+
+int exx_plan_get_fusion(const exx_plan* plan) { return plan ? plan->fusion : 0; }
 
 exx_status exx_plan_set_accumulate(exx_plan* plan, int on) {
   if (!plan) return EXX_ERR_INVALID_ARG;
@@ -436,7 +447,21 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     double* buf0 = (double*)d_workspace;
     double* buf1 = buf0 + N * (size_t)n_c;
     // Batch = nk targets x nj occupied orbitals, nj*nk <= n_c.  With n_occ >= n_c one target per batch.
-    const int nj_max = n_occ < n_c ? n_occ : n_c;
+    int nj_max = n_occ < n_c ? n_occ : n_c;
+    // Fused x-backward + accumulate (k_mode_xacc): a work item is (row tile, target) and loops over the batch's j, so a
+    // batch needs enough targets to give every warp several items; nj only has to amortise the read-modify-write of
+    // vx_k (16/nj bytes per point and pair).  The sum over j is ascending whatever the shape.
+    const int xacc_rows = plan->variant == EXX_VARIANT_FUSED_DMMA && (plan->fusion & 2) ? exx::fused_xacc_tile_rows(plan) : 0;
+    if (xacc_rows > 0 && !(plan->n[0] & 1)) {
+      const long long tiles_per_rhs = (N / plan->n[0] + xacc_rows - 1) / xacc_rows;
+      long long nk_want = (96LL * plan->sm_count + tiles_per_rhs - 1) / tiles_per_rhs;
+      if (nk_want > n_tgt) nk_want = n_tgt;
+      if (nk_want > n_c) nk_want = n_c;
+      int nj = (int)(n_c / nk_want);
+      const int nj_floor = n_occ < 8 ? n_occ : 8;
+      if (nj < nj_floor) nj = nj_floor < n_c ? nj_floor : n_c;
+      if (nj < nj_max) nj_max = nj;
+    }
     const int nk_max = n_c / nj_max;
     // Two lanes: target block kb runs on lane kb % 2 (all its j-batches in order, so vx_k is accumulated in
     // the same order as with one lane and no vx_k is touched by both lanes); lane 1 works in the second half

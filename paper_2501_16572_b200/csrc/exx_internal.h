@@ -65,6 +65,9 @@ struct exx_plan {
   // exx_apply runs `lanes` batches at a time (1 or 2): lane 0 on the caller's stream, lane 1 on lane_stream,
   // forked and joined with the two events
   int lanes;
+  // bit 0: z-forward + multiplier + z-backward in one pass (k_mode_zz); bit 1: x-backward + accumulate in one pass
+  // (k_mode_xacc).  Default 3; exx_plan_set_fusion (test / measurement hook)
+  int fusion;
   cudaStream_t lane_stream;
   cudaEvent_t ev_fork, ev_join;
   // optional per-kernel-class CUDA-event timing (exx_plan_set_profiling)
@@ -147,6 +150,13 @@ struct ProfScope {
   ~ProfScope() {
     if (e1) cudaEventRecord(e1, s);
   }
+  void cancel() {  // nothing was launched inside this scope: drop the record
+    if (!e1) return;
+    cudaEventDestroy(p->prof.back().e0);
+    cudaEventDestroy(e1);
+    p->prof.pop_back();
+    e1 = nullptr;
+  }
 };
 
 // ---- fast variant (kernels_dmma.cu) ----------------------------------------------------------
@@ -170,6 +180,12 @@ cudaError_t tma_init(exx_plan* p);
 void tma_destroy(exx_plan* p);
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
                              bool apply_mult, const FastArgs* pd, cudaStream_t s, int part = 0, bool rmw = false);
+// ---- fused passes (kernels_fused.cu); cudaErrorNotSupported -> the unfused passes above ----
+cudaError_t fused_init(exx_plan* p);   // after tma_init
+void fused_destroy(exx_plan* p);       // before tma_destroy
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s);
+cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
+int fused_xacc_tile_rows(const exx_plan* p);
 // ---- ACE tail and application (kernels_ace.cu) ----
 size_t ace_build_workspace_doubles(const exx_plan* p, int n);
 size_t ace_apply_workspace_doubles(const exx_plan* p, int n, int m);

@@ -528,12 +528,41 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   }
   if (!first_done && (e = one_product(p, 0, true, src, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
   if ((e = one_product(p, 1, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 2, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 2, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  // z-forward + multiplier + z-backward: one fused pass where k_mode_zz can run, else two passes
+  e = cudaErrorNotSupported;
+  if (p->variant == EXX_VARIANT_FUSED_DMMA) {
+    ProfScope ps(p, KC_MODE_PRODUCT, s);
+    e = fused_zz(p, cur, cur, nb, s);
+    if (e != cudaSuccess) ps.cancel();
+  }
+  if (e == cudaSuccess) {
+    mult_pending = false;
+    *launches += 1;
+  } else if (e == cudaErrorNotSupported) {
+    if ((e = one_product(p, 2, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+    if ((e = one_product(p, 2, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+    *launches += 2;
+  } else {
+    return e;
+  }
   if (mult_pending) return cudaErrorUnknown;  // cannot happen: same axis, same support decision
   if ((e = one_product(p, 1, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  *launches += 3;
+  // x-backward + accumulate: one fused pass where k_mode_xacc can run
+  if (fa && p->variant == EXX_VARIANT_FUSED_DMMA) {
+    {
+      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      e = fused_xacc(p, cur, nb, fa, s);
+      if (e != cudaSuccess) ps.cancel();
+    }
+    if (e == cudaSuccess) {
+      *launches += 1;
+      return e;
+    }
+    if (e != cudaErrorNotSupported) return e;
+  }
   if ((e = one_product(p, 0, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
-  *launches += 6;
+  *launches += 1;
   if (fa) {
     {
       ProfScope ps(p, KC_ACCUMULATE, s);

@@ -1,0 +1,740 @@
+// Fused passes of the default variant: fewer trips of a batch through HBM than the six in-place products of
+// kernels_tma.cu.  Same machinery as k_mode_t -- FP64 tensor cores (DMMA.8x8x4),
+// operands staged by TMA into per-warp mbarrier rings, persistent CTAs, programmatic dependent launch -- plus two
+// things k_mode_t does not have:
+//
+//   * k_mode_zz: z-forward product, eigen-space multiply and z-backward product in ONE pass (Eq. 11's third and
+//     fourth GEMM and the Hadamard product of Eq. 16).  The forward product is issued with
+//     the MMA operands swapped, C^T = B^T A^T, so that its accumulator fragment (lane (g,q): T[m = 8mt+2q+e][column
+//     8nt+g]) IS the A fragment of the backward product written as Y^T = T'^T Vz^T: the intermediate T never leaves
+//     the registers, no shuffle, no shared-memory bounce.  The multiplier tile follows the data tile through the same
+//     TMA ring and is read in accumulator layout.  One shared-memory image of Vz serves both products (its columns are
+//     permuted so that both access patterns are bank-conflict free).
+//   * k_mode_xacc: x-backward product and accumulate (a5) in one pass.  A work item is (row tile, target k); the
+//     warp loops over the occupied orbitals j of the batch, keeps vx_k's tile in a second set of accumulators and
+//     reads the psi_j tile, which follows the data tile through the TMA ring, in accumulator layout:
+//     vx_k -= occ_j psi_j phi_jk with j ascending, exactly the order of k_accumulate (bitwise run-to-run
+//     reproducible, independent of the batch shape).  phi is never written to memory.
+#include "tma_common.cuh"
+
+namespace exx {
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_mode_zz
+// ---------------------------------------------------------------------------------------------------------------
+struct ZArgs {
+  double* out;
+  const double* V;  // image [16*S][8*MTOT+4]: row 16s+4kk+q = z index read by lane q in k-step kk, column sigma(m)
+  int n;
+  int S;        // stages of 16 contraction indices per product
+  int kk_last;  // 0: n % 16 == 0; else k-steps of the ragged last stage
+  unsigned n_tiles;
+  int inner;              // nx*ny
+  int cpo;                // chunks of 16 columns per right-hand side
+  unsigned total_chunks;  // cpo * nb
+  int outer;              // nb
+  FastDiv div_cpo;
+};
+
+template <int MTOT, int NT, int WARPS, int IC>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_zz(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const ZArgs a) {
+  static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
+  static_assert(MTOT % IC == 0, "output row tiles are processed IC at a time");
+  constexpr int LDV = 8 * MTOT + 4;
+  constexpr unsigned kStage = 1024u * NT;
+  constexpr int CH = NT / 2;
+  constexpr int SMAX = (MTOT + 1) / 2;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, S = a.S;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * S) * LDV;
+
+  for (unsigned i = 2 * tid; i < 16u * S * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kStage);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kStage) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kStage) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+
+  // ---- producer: a tile is S data stages (tm0) followed by S multiplier stages (tm1, same columns) ------------
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pc0[CH], pc2[CH];
+  auto tile_coords = [&](unsigned t) {
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        pc2[ch] = (int)o;
+        pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
+      } else {  // past the end: an all-out-of-bounds data box (zeros), never stored
+        pc2[ch] = a.outer;
+        pc0[ch] = 0;
+      }
+    }
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kStage;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kStage);
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) {
+        if (s_p < S) tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
+        else tma_load_3d(dst + 2048u * ch, &tm1, pc0[ch], 16 * (s_p - S), 0, bar);
+      }
+    }
+    if (++s_p == 2 * S) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  // ---- per-lane fragment addresses --------------------------------------------------------------------------
+  const unsigned b1 = (unsigned)(q >> 1);
+  // forward product, Vz fragment: image row 16s + 4kk + q, column sigma(8mt + g), sigma(c) = c ^ ((c >> 2) & 1)
+  unsigned v1_lane = smem0 + 8u * (q * LDV + (g ^ ((g >> 2) & 1)));
+  // data fragment inside a stage (as k_mode_t's L-mode): box row 2q + (kk&1) + 8(kk>>1), column 8(nt&1)+g
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const unsigned row = 2u * q + (i & 1);
+    xo[i] = 128u * row + 16u * ((4u * (i >> 1) + (g >> 1)) ^ row) + 8u * (g & 1);
+  }
+  // multiplier fragment in accumulator layout: box row 8h + 2q + e (the eigen index m within its 16), column 8(nt&1)+g
+  unsigned tq[2][2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e)
+#pragma unroll
+    for (int np = 0; np < 2; ++np) {
+      const unsigned row = 2u * q + e;
+      tq[e][np] = 128u * row + 16u * ((4u * np + (g >> 1)) ^ row) + 8u * (g & 1);
+    }
+  // backward product, Vz fragment: image row 8it + g (an output index), column sigma(8mt + 2q + e) = 8mt + 2q + (e ^ b1)
+  unsigned v2_lane[2];
+  v2_lane[0] = smem0 + 8u * (g * LDV + 2u * q + b1);
+  v2_lane[1] = smem0 + 8u * (g * LDV + 2u * q + (1u ^ b1));
+  // z index of output row 8it + 2q + e: the index image row 8it + 2q + e holds (standard stage / ragged last stage)
+  const int zo_std[2] = {4 * (q & 1) + (q >> 1), 4 * (q & 1) + 2 + (q >> 1)};
+  const int zo_lin[2] = {2 * q, 2 * q + 1};
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  const int s_std = a.kk_last ? S - 1 : S;
+  while (t < a.n_tiles) {
+    double acc[MTOT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+    // ---- forward product, operands swapped: acc[mt][nt][e] = T[m = 8mt + 2q + e][column 8nt + g] -------------
+    for (int s = 0; s < S; ++s) {
+      asm volatile("" : "+r"(v1_lane), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kStage;
+      const unsigned aa = v1_lane + (unsigned)s * (16u * LDV * 8u);
+      if (s < s_std) {
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          double bf[NT];
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt)
+            bf[nt] = lds64(sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1));
+          double af[MTOT];
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], bf[nt], af[mt]);
+        }
+      } else {
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          if (kk < a.kk_last) {
+            double bf[NT];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              const unsigned row = 4u * kk + q;
+              bf[nt] = lds64(sb + 2048u * (nt >> 1) + 128u * row + 16u * ((4u * (nt & 1) + (g >> 1)) ^ (row & 7u)) +
+                             8u * (g & 1));
+            }
+            double af[MTOT];
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], bf[nt], af[mt]);
+          }
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+
+    // ---- eigen-space multiply (a3): the multiplier tile arrives in S more stages, read in accumulator layout ---
+#pragma unroll
+    for (int sp = 0; sp < SMAX; ++sp) {
+      if (sp < S) {
+        mbar_wait(my_bar + 8u * slot, parity);
+        const unsigned sb = my_ring + slot * kStage;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          constexpr int kDummy = 0;
+          (void)kDummy;
+          if (2 * sp + h < MTOT) {
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+              for (int e = 0; e < 2; ++e)
+                acc[2 * sp + h < MTOT ? 2 * sp + h : 0][nt][e] *=
+                    lds64(sb + 2048u * (nt >> 1) + 1024u * h + tq[e][nt & 1]);
+          }
+        }
+        __syncwarp();
+        produce(slot);
+        if (++slot == kDepth) {
+          slot = 0;
+          parity ^= 1u;
+        }
+      }
+    }
+
+    // ---- backward product Y^T = T'^T Vz^T, IC output row tiles at a time; A fragments are the accumulators ------
+    int o_ch[CH], col_ch[CH];
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        o_ch[ch] = (int)o;
+        col_ch[ch] = 16 * (int)(cc - o * (unsigned)a.cpo) + g;
+      } else {
+        o_ch[ch] = 0;
+        col_ch[ch] = a.inner;  // nothing stored
+      }
+    }
+#pragma unroll 1
+    for (int it0 = 0; it0 < MTOT; it0 += IC) {
+      double acc2[IC][NT][2];
+#pragma unroll
+      for (int ic = 0; ic < IC; ++ic)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) acc2[ic][nt][0] = acc2[ic][nt][1] = 0.0;
+      const unsigned wrow = (unsigned)it0 * (8u * LDV * 8u);
+#pragma unroll
+      for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          double w[IC];
+#pragma unroll
+          for (int ic = 0; ic < IC; ++ic) w[ic] = lds64(v2_lane[e] + wrow + (8u * ic * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int ic = 0; ic < IC; ++ic)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc2[ic][nt], acc[mt][nt][e], w[ic]);
+        }
+      // store: lane (g,q) holds Y[z(8it + 2q + e)][column 8nt + g]
+#pragma unroll
+      for (int ic = 0; ic < IC; ++ic) {
+        const int it = it0 + ic;
+        const bool lin = a.kk_last && (it >> 1) == S - 1;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int z = 8 * it + (lin ? zo_lin[e] : zo_std[e]);
+          if (z < n) {
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              const int col = col_ch[nt >> 1] + 8 * (nt & 1);
+              if (col < a.inner)
+                a.out[((long long)o_ch[nt >> 1] * n + z) * a.inner + col] = acc2[ic][nt][e];
+            }
+          }
+        }
+      }
+    }
+
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_mode_xacc
+// ---------------------------------------------------------------------------------------------------------------
+struct XArgs {
+  const double* V;    // X-mode image of Vx (backward), as k_mode_t stages it
+  const double* occ;  // occ + j0
+  double* vx;         // vx + k0 * N
+  int n;
+  int S;
+  int kk_last;
+  unsigned n_tiles;  // work items: tiles_per_rhs * nk
+  int rows_per_rhs;  // N / nx
+  int nj, nk, j0;
+  int first;  // vx_k is overwritten (first batch of these targets), not accumulated into
+  FastDiv div_nk;
+};
+
+template <int MTOT, int NT, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_xacc(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XArgs a) {
+  static_assert(NT == 1 || NT == 2 || NT == 4, "a tile is 8, 16 or 32 rows");
+  constexpr int LDV = 8 * MTOT + 4;
+  constexpr unsigned kStage = 1024u * NT;  // a {16 x, 8 NT rows} box
+  constexpr int SMAX = (MTOT + 1) / 2;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, S = a.S;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * S) * LDV;
+
+  for (unsigned i = 2 * tid; i < 16u * S * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kStage);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kStage) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kStage) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+
+  // ---- producer: item (row tile rb, target kq) = nj steps; a step is S stages of the batch's right-hand side
+  //      (jj, kq) from tm0 followed by S stages of psi_{j0+jj} from tm1, same rows -----------------------------
+  unsigned t_p = tfirst;
+  int s_p = 0, jj_p = 0;
+  int prow_d = 0, prow_p = 0;
+  auto tile_coords = [&](unsigned t) {
+    const int rb = (int)fast_div(t, a.div_nk);
+    const int kq = (int)t - rb * a.nk;
+    prow_d = (a.nj * kq) * a.rows_per_rhs + rb * (8 * NT);
+    prow_p = a.j0 * a.rows_per_rhs + rb * (8 * NT);
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kStage;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kStage);
+      if (s_p < S) tma_load_2d(dst, &tm0, 16 * s_p, prow_d, bar);
+      else tma_load_2d(dst, &tm1, 16 * (s_p - S), prow_p, bar);
+    }
+    if (++s_p == 2 * S) {
+      s_p = 0;
+      if (++jj_p == a.nj) {
+        jj_p = 0;
+        t_p = claim_tile();
+#pragma unroll
+        for (int i = 0; i < kDepth + 1; ++i)
+          if (i == fifo_n) fifo[i] = t_p;
+        ++fifo_n;
+        if (t_p < a.n_tiles) tile_coords(t_p);
+      } else {
+        prow_d += a.rows_per_rhs;
+        prow_p += a.rows_per_rhs;
+      }
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  // ---- per-lane fragment addresses --------------------------------------------------------------------------
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) xo[i] = 128u * g + 16u * ((4u * (q >> 1) + i) ^ (unsigned)g) + 8u * (q & 1);
+  // psi fragment in accumulator layout: box row 8nt + 2q + e (a data row), x = 8h + g within the stage's 16
+  unsigned pq[2][2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const unsigned row = 2u * q + e;
+      pq[e][h] = 128u * row + 16u * ((4u * h + (g >> 1)) ^ row) + 8u * (g & 1);
+    }
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  const int s_std = a.kk_last ? S - 1 : S;
+  while (t < a.n_tiles) {
+    const int rb = (int)fast_div(t, a.div_nk);
+    const int kq = (int)t - rb * a.nk;
+    const int row0 = rb * (8 * NT);  // within the target's rows
+    double* vbase = a.vx + ((long long)kq * a.rows_per_rhs + row0 + 2 * q) * n + g;
+    double vacc[MTOT][NT][2];
+    if (a.first) {
+#pragma unroll
+      for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) vacc[mt][nt][0] = vacc[mt][nt][1] = 0.0;
+    } else {
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const bool rok = row0 + 8 * nt + 2 * q + e < a.rows_per_rhs;
+          const double* src = vbase + (long long)(8 * nt + e) * n;
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) vacc[mt][nt][e] = (rok && 8 * mt + g < n) ? src[8 * mt] : 0.0;
+        }
+    }
+
+    for (int jj = 0; jj < a.nj; ++jj) {
+      const double oc = __ldg(a.occ + jj);
+      double acc[MTOT][NT][2];
+#pragma unroll
+      for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+      // phi_jk tile: acc[mt][nt][e] = phi[row 8nt + 2q + e][x = 8mt + g]
+      for (int s = 0; s < S; ++s) {
+        asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+        mbar_wait(my_bar + 8u * slot, parity);
+        const unsigned sb = my_ring + slot * kStage;
+        const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+        if (s < s_std) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk) {
+            double bf[NT];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) bf[nt] = lds64(sb + xo[kk] + 1024u * nt);
+            double af[MTOT];
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+          }
+        } else {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk) {
+            if (kk < a.kk_last) {
+              double bf[NT];
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt)
+                bf[nt] = lds64(sb + 1024u * nt + 128u * g + 16u * ((2u * kk + (q >> 1)) ^ (unsigned)g) + 8u * (q & 1));
+              double af[MTOT];
+#pragma unroll
+              for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+              for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+            }
+          }
+        }
+        __syncwarp();
+        produce(slot);
+        if (++slot == kDepth) {
+          slot = 0;
+          parity ^= 1u;
+        }
+      }
+
+      // a5: vx_k -= occ_j psi_j phi_jk; the psi_j tile arrives in S more stages, read in accumulator layout
+#pragma unroll
+      for (int sp = 0; sp < SMAX; ++sp) {
+        if (sp < S) {
+          mbar_wait(my_bar + 8u * slot, parity);
+          const unsigned sb = my_ring + slot * kStage;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            if (2 * sp + h < MTOT) {
+              constexpr int kZero = 0;
+              const int mt = 2 * sp + h < MTOT ? 2 * sp + h : kZero;
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const double ps = lds64(sb + 1024u * nt + pq[e][h]);
+                  vacc[mt][nt][e] -= oc * ps * acc[mt][nt][e];
+                }
+            }
+          }
+          __syncwarp();
+          produce(slot);
+          if (++slot == kDepth) {
+            slot = 0;
+            parity ^= 1u;
+          }
+        }
+      }
+    }
+
+    // vx_k tile back to memory
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        if (row0 + 8 * nt + 2 * q + e < a.rows_per_rhs) {
+          double* dst = vbase + (long long)(8 * nt + e) * n;
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt)
+            if (8 * mt + g < n) dst[8 * mt] = vacc[mt][nt][e];
+        }
+      }
+
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+
+template <typename Kern, typename Args>
+cudaError_t launch_persistent(Kern kern, SmemOptIn& opt, size_t smem, int warps, unsigned n_tiles, const exx_plan* p,
+                              const CUtensorMap& m0, const CUtensorMap& m1, const Args& a, cudaStream_t s) {
+  // padded above half an SM's shared memory: exactly one CTA per SM (the tile split assumes it)
+  const size_t floor_bytes = 117 * 1024;
+  if (smem < floor_bytes) smem = floor_bytes;
+  if (smem > (size_t)p->smem_optin) return cudaErrorNotSupported;
+  cudaError_t e = opt.ensure(kern, p->device, smem, true);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  const unsigned grid = n_tiles < (unsigned)p->sm_count ? n_tiles : (unsigned)p->sm_count;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * warps);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
+}
+
+inline size_t smem_need(int S, int mtot, int warps, int nt) {
+  const size_t img = sizeof(double) * 16 * (size_t)S * (8 * mtot + 4);
+  return img + 1024 + (size_t)warps * kDepth * 1024 * nt + (size_t)warps * kDepth * 8 + 16;
+}
+
+template <int MTOT, int NT, int WARPS, int IC>
+cudaError_t launch_zz(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const ZArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  return launch_persistent(k_mode_zz<MTOT, NT, WARPS, IC>, opt, smem_need(a.S, MTOT, WARPS, NT), WARPS, a.n_tiles, p, m0,
+                           m1, a, s);
+}
+
+template <int MTOT, int NT, int WARPS>
+cudaError_t launch_xacc(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  return launch_persistent(k_mode_xacc<MTOT, NT, WARPS>, opt, smem_need(a.S, MTOT, WARPS, NT), WARPS, a.n_tiles, p, m0, m1,
+                           a, s);
+}
+
+// class of ceil(n/8), as kernels_tma.cu's pick_class (the images are shared with it)
+inline int mtot_class(int n) {
+  const int need = (n + 7) / 8;
+  if (need > 16) return 0;
+  return need <= 2 ? 2 : need <= 4 ? 4 : need <= 6 ? 6 : need <= 8 ? 8 : need <= 12 ? 12 : need <= 15 ? 15 : 16;
+}
+
+// rows per warp tile (in units of 8) of k_mode_xacc: two accumulator sets have to fit the register file
+inline int xacc_nt(int mtot) { return mtot <= 8 ? 2 : 1; }
+
+}  // namespace
+
+// Rows of a k_mode_xacc work item (exx_apply sizes its batches with it).
+int fused_xacc_tile_rows(const exx_plan* p) {
+  const int mtot = mtot_class(p->n[0]);
+  return mtot ? 8 * xacc_nt(mtot) : 0;
+}
+
+// The image k_mode_zz stages: row 16s + 4kk + q holds the z index the lane with that q reads in k-step kk of stage
+// s (k_mode_t's L-mode order), column sigma(m) = m ^ ((m >> 2) & 1) holds eigenvector m: image[row(z)][sigma(m)] =
+// Vz[z][m].  The forward product reads it as V^T (lane (g,q): row by q, column by g), the backward product as V (row
+// by g, column by q); the column permutation makes both patterns bank-conflict free.
+cudaError_t fused_init(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return cudaSuccess;
+  st->d_img_zz = nullptr;
+  const int n = p->n[2], mtot = mtot_class(n);
+  if (!mtot || !p->h_Vi[2].empty()) return cudaSuccess;
+  const int S = (n + 15) / 16, ldv = 8 * mtot + 4;
+  std::vector<double> img((size_t)16 * S * ldv, 0.0);
+  for (int s = 0; s < S; ++s)
+    for (int kk = 0; kk < 4; ++kk)
+      for (int q = 0; q < 4; ++q) {
+        const int z = 16 * s + within_stage(false, n, s, kk, q);
+        if (z >= n) continue;
+        double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];
+        for (int m = 0; m < n; ++m) row[m ^ ((m >> 2) & 1)] = p->h_V[2][(size_t)z * n + m];
+      }
+  cudaError_t e = cudaMalloc(&st->d_img_zz, sizeof(double) * img.size());
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(st->d_img_zz, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+}
+
+void fused_destroy(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return;
+  if (st->d_img_zz) cudaFree(st->d_img_zz);
+  st->d_img_zz = nullptr;
+}
+
+// z-forward product, multiplier and z-backward product of nb right-hand sides in one pass, in place or out of place.
+// cudaErrorNotSupported: the caller runs the two k_mode_t passes instead.
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st || !st->d_img_zz || !(p->fusion & 1)) return cudaErrorNotSupported;
+  const int n = p->n[2], mtot = mtot_class(n);
+  if (!mtot) return cudaErrorNotSupported;
+  if ((p->n[0] & 1) || !aligned16(out) || !aligned16(in) || !aligned16(p->d_mult)) return cudaErrorNotSupported;
+  const long long inner = (long long)p->n[0] * p->n[1];
+  ZArgs a{};
+  a.out = out;
+  a.V = st->d_img_zz;
+  a.n = n;
+  a.S = (n + 15) / 16;
+  a.kk_last = tail_ksteps(n);
+  a.inner = (int)inner;
+  a.cpo = (int)((inner + 15) / 16);
+  const long long chunks = (long long)a.cpo * nb;
+  if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.total_chunks = (unsigned)chunks;
+  a.outer = nb;
+  a.div_cpo = make_fastdiv((unsigned)a.cpo);
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if ((e = get_map(st, in, inner, n, nb, 16, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, p->d_mult, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+  const int NT = mtot <= 8 ? 4 : 2;
+  const int CH = NT / 2;
+  a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+  if (a.n_tiles == 0) return cudaSuccess;
+  ++p->tma_launches;
+  switch (mtot) {
+    case 2: return launch_zz<2, 4, 16, 2>(p, m0, m1, a, s);
+    case 4: return launch_zz<4, 4, 16, 1>(p, m0, m1, a, s);
+    case 6: return launch_zz<6, 4, 12, 1>(p, m0, m1, a, s);
+    case 8: return launch_zz<8, 4, 8, 2>(p, m0, m1, a, s);
+    case 12: return launch_zz<12, 2, 12, 3>(p, m0, m1, a, s);
+    case 15: return launch_zz<15, 2, 12, 1>(p, m0, m1, a, s);
+    default: return launch_zz<16, 2, 12, 1>(p, m0, m1, a, s);
+  }
+}
+
+// x-backward product of the batch in `in` (nb = nj*nk right-hand sides, pair (j0 + b % nj, k0 + b / nj)) fused with the
+// accumulate into vx.  cudaErrorNotSupported: the caller runs k_mode_t and k_accumulate instead.
+cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st || !(p->fusion & 2) || !fa || fa->sym) return cudaErrorNotSupported;
+  const int n = p->n[0], mtot = mtot_class(n);
+  if (!mtot || !st->d_img[0][1]) return cudaErrorNotSupported;
+  if ((n & 1) || !aligned16(in) || !aligned16(fa->psi) || !aligned16(fa->vx)) return cudaErrorNotSupported;
+  if (nb != fa->bd.nj * fa->bd.nk) return cudaErrorInvalidValue;
+  const int NT = xacc_nt(mtot);
+  XArgs a{};
+  a.V = st->d_img[0][1];
+  a.occ = fa->occ + fa->bd.j0;
+  a.vx = fa->vx + (size_t)fa->bd.k0 * (size_t)p->N;
+  a.n = n;
+  a.S = (n + 15) / 16;
+  a.kk_last = tail_ksteps(n);
+  a.rows_per_rhs = (int)(p->N / n);
+  a.nj = fa->bd.nj;
+  a.nk = fa->bd.nk;
+  a.j0 = fa->bd.j0;
+  a.first = fa->first ? 1 : 0;
+  a.div_nk = make_fastdiv((unsigned)a.nk);
+  const long long rows_total = (long long)a.rows_per_rhs * nb, rows_psi = (long long)a.rows_per_rhs * fa->n_occ;
+  if (rows_total >= (1LL << 31) - 64 || rows_psi >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  const long long tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+  if (tiles_per_rhs * a.nk >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.n_tiles = (unsigned)(tiles_per_rhs * a.nk);
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if ((e = get_map(st, in, n, rows_total, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, fa->psi, n, rows_psi, 0, 8 * NT, &m1)) != cudaSuccess) return e;
+  ++p->tma_launches;
+  switch (mtot) {
+    case 2: return launch_xacc<2, 2, 16>(p, m0, m1, a, s);
+    case 4: return launch_xacc<4, 2, 16>(p, m0, m1, a, s);
+    case 6: return launch_xacc<6, 2, 12>(p, m0, m1, a, s);
+    case 8: return launch_xacc<8, 2, 12>(p, m0, m1, a, s);
+    case 12: return launch_xacc<12, 1, 12>(p, m0, m1, a, s);
+    case 15: return launch_xacc<15, 1, 12>(p, m0, m1, a, s);
+    default: return launch_xacc<16, 1, 12>(p, m0, m1, a, s);
+  }
+}
+
+}  // namespace exx

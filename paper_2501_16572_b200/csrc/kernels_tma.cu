@@ -31,90 +31,17 @@
 //
 // The paper's four data reorganisations (Eqs. 12-15) do not exist here: they are
 // artefacts of calling a 2-D GEMM library and are replaced by tensor-map strides.
-#include <cuda.h>  // CUtensorMap and its enums only; cuTensorMapEncodeTiled is resolved at run time
-
-#include <cstdint>
-#include <cstdlib>
-#include <cstring>
-
-#include "exx_internal.h"
+#include "tma_common.cuh"
 
 namespace exx {
 namespace {
-
-constexpr int kDepth = 2;  // ring depth in stages of 16 contraction indices (4 k-steps, >= 96 DMMAs each)
-
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-      : "+d"(c[0]), "+d"(c[1])
-      : "d"(a), "d"(b));
-}
-__device__ __forceinline__ double lds64(unsigned addr) {
-  double v;
-  asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
-}
-// Blocks until the phase with the given parity has completed.  A bounded spin turns a lost transaction (a
-// bug) into a trap instead of a hung GPU.
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-  unsigned done = 0;
-  for (unsigned spin = 0; !done; ++spin) {
-    asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
-        : "=r"(done)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    if (spin > (1u << 24)) __trap();
-  }
-}
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
-      "l"(tm), "r"(c0), "r"(c1), "r"(bar)
-      : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int c0, int c1, int c2,
-                                            unsigned bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(
-          dst),
-      "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
-      : "memory");
-}
-
-// Exact n / d for n < 2^31 with a host-computed multiplier (d = 2^shift when mul == 0).
-struct FastDiv {
-  unsigned mul;
-  int shift;
-};
-inline FastDiv make_fastdiv(unsigned d) {
-  FastDiv f{0u, 0};
-  if ((d & (d - 1)) == 0) {
-    while ((1u << f.shift) < d) ++f.shift;
-    return f;
-  }
-  int L = 0;
-  while ((1ull << L) < d) ++L;
-  f.mul = (unsigned)(((1ull << (31 + L)) / d) + 1ull);
-  f.shift = L - 1;
-  return f;
-}
-__device__ __forceinline__ unsigned fast_div(unsigned n, const FastDiv& f) {
-  return f.mul ? (__umulhi(n, f.mul) >> f.shift) : (n >> f.shift);
-}
 
 struct TArgs {
   double* out;
   const double* V;  // permuted, zero-padded image [16*S][8*MTOT+4] (tma_init)
   int n;
   int S;        // stages per tile = ceil(n/16)
-  int kk_last;  // k-steps of the last stage that touch indices < n
+  int kk_last;  // 0: n is a multiple of 16; else ceil((n % 16) / 4), the k-steps of the ragged last stage
   unsigned n_tiles;
   // L-mode
   int inner;              // contiguous run below the contracted axis
@@ -137,15 +64,6 @@ struct TArgs {
   long long plane_stride;
   FastDiv div_plane;
 };
-
-__device__ __forceinline__ bool elect_one() {
-  unsigned pred;
-  asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
-  return pred != 0;
-}
-__device__ __forceinline__ void stg_v2(double* p, double x, double y) {
-  asm volatile("st.global.v2.f64 [%0], {%1, %2};\n" ::"l"(p), "d"(x), "d"(y) : "memory");
-}
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
 template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
@@ -292,6 +210,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   int slot = 0;
   unsigned parity = 0;
   unsigned t = tfirst;
+  const int s_std = a.kk_last ? S - 1 : S;  // stages of four standard k-steps
   while (t < a.n_tiles) {
     double acc[MTOT][NT][2];
 #pragma unroll
@@ -306,10 +225,9 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * (NS * kStage);
       const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
-      const int nk = (s == S - 1) ? a.kk_last : 4;
+      if (s < s_std) {
 #pragma unroll
-      for (int kk = 0; kk < 4; ++kk) {
-        if (kk < nk) {
+        for (int kk = 0; kk < 4; ++kk) {
           double bf[NT];
 #pragma unroll
           for (int nt = 0; nt < NT; ++nt) {
@@ -325,6 +243,35 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           for (int mt = 0; mt < MTOT; ++mt)
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+        }
+      } else {
+        // ragged last stage (n % 16 != 0): contraction index 4 kk + q in k-step kk, so that ceil(rem / 4) k-steps
+        // cover the rem valid indices (60 -> 3 instead of 4, X-mode 120 -> 2 instead of 4); tma_init lays the
+        // image rows of this stage out in the same order
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          if (kk < a.kk_last) {
+            double bf[NT];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              unsigned off;
+              if (XMODE) {
+                off = sb + 1024u * nt + 128u * g + 16u * ((2u * kk + (q >> 1)) ^ (unsigned)g) + 8u * (q & 1);
+              } else {
+                const unsigned row = 4u * kk + q;
+                off = sb + 2048u * (nt >> 1) + 128u * row + 16u * ((4u * (nt & 1) + (g >> 1)) ^ (row & 7u)) + 8u * (g & 1);
+              }
+              bf[nt] = lds64(off);
+              if (TWO) bf[nt] *= lds64(off + kStage);
+            }
+            double af[MTOT];
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+            for (int mt = 0; mt < MTOT; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+          }
         }
       }
       // every lane's reads of this stage have completed (their values fed the DMMAs above): refill it
@@ -458,42 +405,6 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
 
 // ---- host side ----------------------------------------------------------------------------------------
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-  static EncodeTiledFn fn = [] {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult qr;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess ||
-        qr != cudaDriverEntryPointSuccess)
-      p = nullptr;
-    return (EncodeTiledFn)p;
-  }();
-  return fn;
-}
-
-struct MapKey {
-  const void* base;
-  unsigned long long d0, d1, d2;
-  unsigned b1;  // box rows (box is always 16 wide; third box dimension 1)
-  bool operator==(const MapKey& o) const {
-    return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b1 == o.b1;
-  }
-};
-struct MapEntry {
-  MapKey key;
-  CUtensorMap map;
-};
-
-struct TmaState {
-  double* d_img[3][2];  // [axis][0 = forward (V^T), 1 = backward (V)]
-  bool img_owned[3][2];
-  double* d_img_im[3][2];  // Bloch plans: images of the imaginary parts, forward = Im(V^H) = -Vi^T, backward = Vi
-  std::vector<MapEntry> cache;
-};
-
 // supported classes of ceil(n/8); per class the columns-per-warp choice (NT), the warps per CTA and the CTAs
 // per SM, for the plain and for the two-stream (TWO) kernels.
 //   lanes == 1: one persistent CTA per SM, as many warps as the register file allows.
@@ -523,33 +434,6 @@ inline bool pick_class(int n, int lanes, ClassCfg* c) {
   else if (need <= 15) *c = {15, 2, 12, 1, 2, 12, 1};
   else *c = {16, 2, 12, 1, 2, 8, 1};
   return true;
-}
-
-// 2-D ([d1][d0]) or 3-D ([d2][d1][d0]) FP64 tensor, box {16, box_rows(, 1)}, 128-byte swizzle, zero fill.
-cudaError_t get_map(TmaState* st, const void* base, unsigned long long d0, unsigned long long d1,
-                    unsigned long long d2, unsigned box_rows, CUtensorMap* out) {
-  const MapKey key{base, d0, d1, d2, box_rows};
-  for (const auto& e : st->cache)
-    if (e.key == key) {
-      *out = e.map;
-      return cudaSuccess;
-    }
-  EncodeTiledFn fn = encode_fn();
-  if (!fn) return cudaErrorNotSupported;
-  const cuuint32_t rank = d2 ? 3 : 2;
-  cuuint64_t gdim[3] = {d0, d1, d2 ? d2 : 1};
-  cuuint64_t gstr[2] = {d0 * 8ull, d0 * d1 * 8ull};
-  cuuint32_t box[3] = {16u, box_rows, 1u};
-  cuuint32_t estr[3] = {1u, 1u, 1u};
-  alignas(64) CUtensorMap m;
-  const CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, const_cast<void*>(base), gdim, gstr, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  if (st->cache.size() >= 64) st->cache.clear();
-  st->cache.push_back(MapEntry{key, m});
-  *out = m;
-  return cudaSuccess;
 }
 
 template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
@@ -600,8 +484,6 @@ cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUte
   return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, device, s);
 }
 
-inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
-
 }  // namespace
 
 // One mode product along `axis` for nb right-hand sides; in == out is allowed (and is the normal case).
@@ -634,8 +516,7 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   CUtensorMap m0, m1;
   cudaError_t e;
   if (xmode) {
-    const int rem = n - 16 * (a.S - 1);
-    a.kk_last = rem > 0 ? 4 : 0;  // every k-step of an X-mode stage touches both halves of the 16-block
+    a.kk_last = tail_ksteps(n);
     a.rows_per_rhs = (int)(p->N / n);
     const long long rows_total = (long long)a.rows_per_rhs * nb;
     if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
@@ -659,8 +540,7 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   } else {
     const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
     const long long outer = p->N / (n * inner) * nb;
-    const int rem = n - 16 * (a.S - 1);
-    a.kk_last = rem > 8 ? 4 : 2;  // k-steps 0,1 cover rows 0..7 of a stage, k-steps 2,3 rows 8..15
+    a.kk_last = tail_ksteps(n);
     a.inner = (int)inner;
     a.cpo = (int)((inner + 15) / 16);
     const long long chunks = (long long)a.cpo * outer;
@@ -738,7 +618,7 @@ cudaError_t tma_init(exx_plan* p) {
       for (int s = 0; s < S; ++s)
         for (int kk = 0; kk < 4; ++kk)
           for (int q = 0; q < 4; ++q) {
-            const int within = xmode ? ((q & 1) + 8 * (q >> 1) + 2 * kk) : (2 * q + (kk & 1) + 8 * (kk >> 1));
+            const int within = within_stage(xmode, n, s, kk, q);
             const int k = 16 * s + within;
             if (k >= n) continue;
             double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];
@@ -755,7 +635,7 @@ cudaError_t tma_init(exx_plan* p) {
       for (int s = 0; s < S; ++s)
         for (int kk = 0; kk < 4; ++kk)
           for (int q = 0; q < 4; ++q) {
-            const int within = xmode ? ((q & 1) + 8 * (q >> 1) + 2 * kk) : (2 * q + (kk & 1) + 8 * (kk >> 1));
+            const int within = within_stage(xmode, n, s, kk, q);
             const int k = 16 * s + within;
             if (k >= n) continue;
             double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];

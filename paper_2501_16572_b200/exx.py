@@ -76,6 +76,10 @@ def load_library():
     lib.exx_plan_set_accumulate.argtypes = [vp, C.c_int]
     lib.exx_plan_get_lanes.restype = C.c_int
     lib.exx_plan_get_lanes.argtypes = [vp]
+    lib.exx_plan_set_fusion.restype = C.c_int
+    lib.exx_plan_set_fusion.argtypes = [vp, C.c_int]
+    lib.exx_plan_get_fusion.restype = C.c_int
+    lib.exx_plan_get_fusion.argtypes = [vp]
     lib.exx_ace_workspace_bytes.restype = C.c_size_t
     lib.exx_ace_workspace_bytes.argtypes = [vp, C.c_int, C.c_int]
     lib.exx_ace_build.restype = C.c_int
@@ -186,6 +190,14 @@ class Plan:
 
     def set_lanes(self, lanes: int):
         _check(self._lib.exx_plan_set_lanes(self._h, lanes), "exx_plan_set_lanes")
+
+    def set_fusion(self, mask: int):
+        """exx_plan_set_fusion: bit 0 = fused z products, bit 1 = fused x-backward + accumulate (default 3)."""
+        _check(self._lib.exx_plan_set_fusion(self._h, mask), "exx_plan_set_fusion")
+
+    @property
+    def fusion(self) -> int:
+        return int(self._lib.exx_plan_get_fusion(self._h))
 
     def set_accumulate(self, on: bool):
         """exx_plan_set_accumulate: exx_apply adds into vx instead of overwriting it."""

@@ -70,9 +70,10 @@ def test_poisson_solve_matches_oracle(case, variant):
     torch.cuda.synchronize()
     assert torch.equal(out2, out)
     if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0:
-        # two calls; per batch two passes through the TMA kernels for every axis of at most 128 points
-        n_fast = sum(1 for n in (nx, ny, nz) if n <= 128)
-        assert plan.tma_launch_count == 4 * n_fast * ((n_rhs + n_c - 1) // n_c)
+        # two calls; per batch two passes through the TMA kernels for an x or y axis of at most 128 points and one
+        # fused pass (forward + multiplier + backward) for such a z axis
+        per_batch = 2 * (nx <= 128) + 2 * (ny <= 128) + 1 * (nz <= 128)
+        assert plan.tma_launch_count == 2 * per_batch * ((n_rhs + n_c - 1) // n_c)
     else:
         assert plan.tma_launch_count == 0
     plan.close()
@@ -134,6 +135,63 @@ def test_buffers_offset_by_8_bytes_take_the_cpasync_path():
     torch.cuda.synchronize()
     assert _rel(out.cpu().numpy(), orc.poisson_solve(_oracle_plan(w), psi[:2].numpy())) < TOL
     assert plan.tma_launch_count == 0
+    plan.close()
+
+
+FUSION_GRIDS = [
+    # (nx, ny, nz, bc, omega): every ceil(n/8) class of the fused kernels, ragged last stages (n % 16 in 1..15), ragged
+    # row tiles and column chunks, periodic and Dirichlet
+    (16, 16, 16, (0, 0, 0), 0.0),
+    (20, 12, 9, (0, 1, 0), 0.106),
+    (26, 14, 30, (1, 0, 0), 0.106),
+    (44, 6, 50, (0, 0, 1), 0.0),
+    (60, 10, 60, (0, 0, 1), 0.106),
+    (72, 6, 90, (0, 0, 0), 0.106),
+    (100, 4, 114, (1, 1, 1), 0.106),
+    (126, 4, 128, (0, 0, 0), 0.0),
+    (8, 132, 6, (0, 0, 0), 0.106),      # y axis on the plain kernel, x and z fused
+]
+
+
+@pytest.mark.parametrize("grid", FUSION_GRIDS, ids=lambda c: f"{c[0]}x{c[1]}x{c[2]}")
+def test_fused_passes_match_oracle_and_unfused(grid):
+    """exx_plan_set_fusion: k_mode_zz (z-forward + multiplier + z-backward) and k_mode_xacc (x-backward + accumulate)
+    against the oracle and against the separate passes, for every mask, solver and apply, accumulate mode included."""
+    nx, ny, nz, bc, omega = grid
+    rng = np.random.default_rng(5)
+    n_orb, n_tgt, t0 = 7, 3, 2
+    psi = rng.standard_normal((n_orb, nz, ny, nx))
+    occ = np.linspace(2.0, 0.1, n_orb)
+    C = rng.standard_normal((5, nz, ny, nx))
+    o = orc.make_plan(nx, ny, nz, 0.3, bc, 12, omega)
+    phi_o = orc.poisson_solve(o, C)
+    vx_o, e_o, ex_o = orc.exx_apply(o, psi, occ, psi[t0:t0 + n_tgt], occ[t0:t0 + n_tgt])
+    plan = exx.Plan(nx, ny, nz, 0.3, bc, 12, omega, max_batch=32, device=0)
+    d_psi, d_occ, d_C = torch.from_numpy(psi).cuda(), torch.from_numpy(occ).cuda(), torch.from_numpy(C).cuda()
+    results = {}
+    for mask in (0, 1, 2, 3):
+        plan.set_fusion(mask)
+        assert plan.fusion == mask
+        for n_c in (3, 32):
+            phi = plan.poisson_solve(d_C, n_c=n_c)
+            assert _rel(phi.cpu().numpy(), phi_o) < TOL
+            vx, e_k, ex = plan.apply(d_psi, d_occ, d_psi[t0:t0 + n_tgt], d_occ[t0:t0 + n_tgt], n_c=n_c)
+            torch.cuda.synchronize()
+            assert _rel(vx.cpu().numpy(), vx_o) < TOL, (mask, n_c)
+            assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
+            results[(mask, n_c)] = vx.clone()
+        # accumulate mode: two calls over a split of the orbitals give the full sum
+        plan.set_accumulate(False)
+        vx2, _, _ = plan.apply(d_psi[:4], d_occ[:4], d_psi[t0:t0 + n_tgt], n_c=32)
+        plan.set_accumulate(True)
+        plan.apply(d_psi[4:], d_occ[4:], d_psi[t0:t0 + n_tgt], vx=vx2, n_c=32)
+        plan.set_accumulate(False)
+        torch.cuda.synchronize()
+        assert _rel(vx2.cpu().numpy(), vx_o) < TOL
+    # the sum over j is ascending whatever the batch shape and the mask: rounding-level agreement between all of them
+    ref = results[(0, 32)]
+    for key, v in results.items():
+        assert float((v - ref).abs().max() / ref.abs().max()) < 1e-12, key
     plan.close()
 
 
