@@ -25,7 +25,7 @@ exactness), periodic spectrum closed form, order-2 Dirichlet sine spectrum, dens
 solve / dense matrix function of a brute-force assembled 3-D Laplacian on tiny grids,
 plane-wave analytic solution, screened kernel against the numerically integrated radial
 Fourier transform of erfc(w r)/r, Hermiticity / negativity / linearity / pair symmetry,
-E_x double-loop identity, naive triple-loop solve.  Nothing here is "parity unpinned".
+E_x double-loop identity, naive triple-loop solve, Eq. 8 per-slice solve against the batch solve.  Nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -190,6 +190,30 @@ def poisson_solve_loops(plan: OraclePlan, c: np.ndarray) -> np.ndarray:
                         for a_ in range(nx):
                             s += Vz[z, c_] * Vy[y, b_] * Vx[x, a_] * t[c_, b_, a_]
                 out[z, y, x] = s
+    return out
+
+
+def poisson_solve_eq8(plan: OraclePlan, b: np.ndarray) -> np.ndarray:
+    """The NON-batch Kronecker solve of ONE right-hand side, PAPER.md:74-78 (Eq. 8a/8b), step by step in the
+    paper's order: for every frontal slice B_k = B(:,:,k) (an n1 x n2 matrix, here b[k].T since arrays are
+    [z, y, x]) the two small products V1^T B_k V2; the slices stacked into an (n1 n2) x n3 matrix times V3; the
+    Hadamard product with f(Lambda~); then the same back: times V3^T, and V1 X~_k V2^T per slice.  That is the
+    paper's 4 n3 + 2 dense products.  Pinned by equality with :func:`poisson_solve` (itself pinned to the dense
+    direct solve) and with :func:`poisson_solve_loops`; the Fig. 2 comparison line of SURVEY.md 8(f) NEXT-4."""
+    b = np.asarray(b, dtype=np.float64)
+    V1, V2, V3 = plan.V                                      # x, y, z
+    n1, n2, n3 = plan.nx, plan.ny, plan.nz
+    T = np.empty((n1 * n2, n3))
+    for k in range(n3):                                      # 2 n3 products
+        Bk = b[k].T                                          # B(:,:,k): [x, y]
+        T[:, k] = ((V1.T @ Bk) @ V2).reshape(n1 * n2, order="F")   # vec over (x fastest, then y)
+    Xt = T @ V3                                              # 1 product: [(a,b), c]
+    Xt = Xt * plan.mult.reshape(n3, n2 * n1).T               # f(Lambda~) (.) ..., table entry [c, b, a]
+    Y = Xt @ V3.T                                            # 1 product: [(a,b), k]
+    out = np.empty((n3, n2, n1))
+    for k in range(n3):                                      # 2 n3 products
+        Xk = Y[:, k].reshape(n1, n2, order="F")
+        out[k] = ((V1 @ Xk) @ V2.T).T
     return out
 
 

@@ -134,6 +134,29 @@ def test_vectorised_solve_equals_naive_loops():
         assert np.allclose(a, b, rtol=0, atol=1e-13 * np.abs(b).max())
 
 
+def test_eq8_per_slice_solve_equals_batch_solve_and_dense_function(golden_dir):
+    """PAPER.md:74-78 (Eq. 8): the non-batch per-slice algorithm is the same linear map as the batch formalism
+    (Eq. 11) and as the dense matrix function of the assembled Laplacian (Eq. 4) -- unequal axis lengths and mixed
+    boundary conditions, so that a transposed slice or a swapped V1/V2 fails."""
+    for dims, bc, omega in (((5, 4, 6), (P, P, P), 0.0), ((4, 6, 5), (P, D, P), 0.106), ((6, 5, 4), (D, P, D), 0.106)):
+        nx, ny, nz = dims
+        plan = orc.make_plan(nx, ny, nz, 0.3, bc, 12, omega)
+        c = np.random.default_rng(8).standard_normal((nz, ny, nx))
+        a = orc.poisson_solve_eq8(plan, c)
+        assert np.allclose(a, orc.poisson_solve(plan, c), rtol=0, atol=1e-13 * np.abs(a).max())
+        assert np.allclose(a, orc.poisson_solve_loops(plan, c), rtol=0, atol=1e-13 * np.abs(a).max())
+        if omega == 0.0:
+            continue
+        # dense matrix function of the point-by-point assembled Laplacian (no Kronecker structure), screened kernel
+        L = dense_laplacian(golden_dir, nx, ny, nz, 0.3, bc, 12)
+        lam, U = np.linalg.eigh(L)
+        small = np.abs(lam) < 1e-9
+        mu = np.where(small, 1.0, -lam)
+        f = np.where(small, np.pi / omega ** 2, 4 * np.pi * (1 - np.exp(-mu / (4 * omega ** 2))) / mu)
+        ref = (U * f[None, :]) @ U.T @ c.ravel()
+        assert np.allclose(a.ravel(), ref, rtol=0, atol=5e-12 * np.abs(ref).max())
+
+
 def test_batch_invariance():
     # PAPER.md:137: the batch formalism is the same linear map for any n_c and any batch composition
     plan = orc.make_plan(9, 8, 7, 0.3, (P, P, D), 12, 0.106)
