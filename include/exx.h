@@ -133,6 +133,17 @@ exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi,
                              void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * The NON-batch Kronecker solver of PAPER.md:74-78 (Eq. 8a/8b), the comparison line of the paper's Fig. 2 (not the
+ * product path): the right-hand sides are solved one at a time; for each, every frontal slice B(:,:,k) is multiplied
+ * by V1^T and V2, the stacked slices by V3, then by f(Lambda~), and the same back -- 4 nz + 2 small dense products,
+ * one kernel launch each (exx_plan_last_launch_count reports them).  Same result as exx_poisson_solve.  Real plans
+ * only.  d_workspace: at least 2 N doubles (exx_plan_workspace_bytes(plan, 1)); d_phi may equal d_rhs.  Errors as
+ * exx_poisson_solve.
+ */
+exx_status exx_poisson_solve_nonbatch(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, void* d_workspace,
+                                      size_t workspace_bytes, void* cuda_stream);
+
+/*
  * Exchange apply (Eq. 1, 42 Eq. 2, 178 Eq. 19b):
  *   d_vx[k]  = - sum_{j<n_occ} d_occ[j] * d_psi[j] .* f(L)(d_psi[j] .* d_tgt[k])     [n_tgt][N], overwritten
  *   d_ex_k[k] = h^3 <d_tgt[k], d_vx[k]>                                            [n_tgt], optional (NULL)

@@ -413,6 +413,29 @@ exx_status exx_poisson_solve(exx_plan* plan, const double* d_rhs, double* d_phi,
   return EXX_OK;
 }
 
+exx_status exx_poisson_solve_nonbatch(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, void* d_workspace,
+                                      size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_rhs < 0 || (n_rhs > 0 && (!d_rhs || !d_phi))) return EXX_ERR_INVALID_ARG;
+  if (is_complex_plan(plan)) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
+  if (n_rhs == 0) { plan->last_launches = 0; return EXX_OK; }
+  const size_t N = (size_t)plan->N, fn = sizeof(double) * N;
+  const size_t need = 2 * fn;
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if (d_rhs != d_phi && overlaps(d_rhs, fn * n_rhs, d_phi, fn * n_rhs)) return EXX_ERR_ALIAS;
+  if (overlaps(d_workspace, need, d_phi, fn * n_rhs) || overlaps(d_workspace, need, d_rhs, fn * n_rhs))
+    return EXX_ERR_ALIAS;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  double* buf0 = (double*)d_workspace;
+  long long launches = 0;
+  for (int b = 0; b < n_rhs; ++b)
+    EXX_CUDA(exx::nonbatch_solve_one(plan, d_rhs + N * (size_t)b, d_phi + N * (size_t)b, buf0, buf0 + N, s, &launches));
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
 exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ,
                      const double* d_tgt, const double* d_occ_tgt, int n_tgt, double* d_vx,
                      double* d_ex, double* d_ex_k, int n_c, void* d_workspace,

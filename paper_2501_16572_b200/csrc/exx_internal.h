@@ -186,6 +186,9 @@ void fused_destroy(exx_plan* p);       // before tma_destroy
 cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s);
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);
+// ---- non-batch Eq. 8 solver, the Fig. 2 comparison line (kernels_nonbatch.cu) ----
+cudaError_t nonbatch_solve_one(exx_plan* p, const double* rhs, double* phi, double* buf0, double* buf1, cudaStream_t s,
+                               long long* launches);
 // ---- ACE tail and application (kernels_ace.cu) ----
 size_t ace_build_workspace_doubles(const exx_plan* p, int n);
 size_t ace_apply_workspace_doubles(const exx_plan* p, int n, int m);

@@ -58,6 +58,8 @@ def load_library():
     lib.exx_plan_get_multiplier.argtypes = [vp, dp]
     lib.exx_poisson_solve.restype = C.c_int
     lib.exx_poisson_solve.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
+    lib.exx_poisson_solve_nonbatch.restype = C.c_int
+    lib.exx_poisson_solve_nonbatch.argtypes = [vp, dp, dp, C.c_int, vp, C.c_size_t, vp]
     lib.exx_apply.restype = C.c_int
     lib.exx_apply.argtypes = [vp, dp, dp, C.c_int, dp, dp, C.c_int, dp, dp, dp, C.c_int, vp, C.c_size_t, vp]
     lib.exx_apply_symmetric.restype = C.c_int
@@ -279,6 +281,23 @@ class Plan:
         st = self._lib.exx_poisson_solve(self._h, _dev_ptr(rhs, self.device, "rhs"), _dev_ptr(out, self.device, "out"),
                                          n_rhs, n_c, C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(s.cuda_stream))
         _check(st, "exx_poisson_solve")
+        return out
+
+    def poisson_solve_nonbatch(self, rhs: torch.Tensor, out: torch.Tensor | None = None,
+                               stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+        """exx_poisson_solve_nonbatch: the per-slice algorithm of PAPER.md:74-78 (Eq. 8), one system at a time."""
+        n_rhs = rhs.shape[0] if rhs.dim() > 3 else 1
+        if rhs.numel() != n_rhs * self.N:
+            raise ValueError("rhs must be [n_rhs, nz, ny, nx]")
+        if out is None:
+            out = torch.empty_like(rhs)
+        self._expect(out, n_rhs * self.N, "out")
+        ws = self._workspace(1)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_poisson_solve_nonbatch(self._h, _dev_ptr(rhs, self.device, "rhs"),
+                                                  _dev_ptr(out, self.device, "out"), n_rhs, C.c_void_p(ws.data_ptr()),
+                                                  ws.numel(), C.c_void_p(s.cuda_stream))
+        _check(st, "exx_poisson_solve_nonbatch")
         return out
 
     def apply(self, psi: torch.Tensor, occ: torch.Tensor, tgt: torch.Tensor, occ_tgt: torch.Tensor | None = None,

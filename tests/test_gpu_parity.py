@@ -138,6 +138,28 @@ def test_buffers_offset_by_8_bytes_take_the_cpasync_path():
     plan.close()
 
 
+@pytest.mark.parametrize("dims,bc,omega", [((16, 16, 16), (0, 0, 0), 0.0), ((20, 12, 9), (0, 1, 0), 0.106),
+                                           ((13, 17, 11), (1, 1, 1), 0.106), ((48, 48, 48), (0, 0, 0), 0.106)])
+def test_nonbatch_eq8_solver_matches_oracle(dims, bc, omega):
+    """exx_poisson_solve_nonbatch (Eq. 8; the Fig. 2 comparison line) against the oracle's per-slice
+    solve and against the batch solver; 4 nz + 2 launches per system."""
+    nx, ny, nz = dims
+    C = np.random.default_rng(21).standard_normal((3, nz, ny, nx))
+    o = orc.make_plan(nx, ny, nz, 0.3, bc, 12, omega)
+    ref = np.stack([orc.poisson_solve_eq8(o, C[b]) for b in range(3)])
+    plan = exx.Plan(nx, ny, nz, 0.3, bc, 12, omega, max_batch=8, device=0)
+    d = torch.from_numpy(C).cuda()
+    out = plan.poisson_solve_nonbatch(d)
+    torch.cuda.synchronize()
+    assert plan.last_launch_count == 3 * (4 * nz + 2)
+    assert _rel(out.cpu().numpy(), ref) < TOL
+    assert _rel(out.cpu().numpy(), plan.poisson_solve(d, n_c=3).cpu().numpy()) < TOL
+    plan.poisson_solve_nonbatch(d, out=d)          # in place
+    torch.cuda.synchronize()
+    assert torch.equal(d, out)
+    plan.close()
+
+
 FUSION_GRIDS = [
     # (nx, ny, nz, bc, omega): every ceil(n/8) class of the fused kernels, ragged last stages (n % 16 in 1..15), ragged
     # row tiles and column chunks, periodic and Dirichlet
