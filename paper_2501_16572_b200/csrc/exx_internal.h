@@ -180,10 +180,12 @@ cudaError_t tma_init(exx_plan* p);
 void tma_destroy(exx_plan* p);
 cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* in, double* out, int nb,
                              bool apply_mult, const FastArgs* pd, cudaStream_t s, int part = 0, bool rmw = false);
+cudaError_t tma_mode_product_c(exx_plan* p, int axis, bool forward, double* buf, int nb, cudaStream_t s);
 // ---- fused passes (kernels_fused.cu); cudaErrorNotSupported -> the unfused passes above ----
 cudaError_t fused_init(exx_plan* p);   // after tma_init
 void fused_destroy(exx_plan* p);       // before tma_destroy
 cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s);
+cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);
 // ---- non-batch Eq. 8 solver, the Fig. 2 comparison line (kernels_nonbatch.cu) ----

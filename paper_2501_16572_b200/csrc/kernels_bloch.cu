@@ -137,12 +137,30 @@ cudaError_t bloch_solve_batch(exx_plan* p, double* const buf[3], int nb, cudaStr
     const int ax = axis[i];
     const bool fwd = i < 3, mult = i == 3, cplx = p->d_Vi[ax] != nullptr;
     bool done = false;
+    if (i == 2 && p->variant != EXX_VARIANT_REFERENCE) {
+      // z-forward + multiplier + z-backward in one pass (kernels_fused.cu): the real kernel over the 2 nb planes for a
+      // real z axis, the embedded complex one for a complex z axis with n <= 64
+      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      e = cplx ? fused_zz_c(p, cur, nb, s) : fused_zz(p, cur, cur, 2 * nb, s);
+      if (e == cudaSuccess) {
+        ++*launches;
+        ++i;  // the z-backward product is done too
+        continue;
+      }
+      ps.cancel();
+      if (e != cudaErrorNotSupported) return e;
+    }
     if (p->variant != EXX_VARIANT_REFERENCE) {
       ProfScope ps(p, KC_MODE_PRODUCT, s);
       if (!cplx) {
         e = tma_mode_product(p, ax, fwd, cur, cur, 2 * nb, mult, nullptr, s, 0);
         if (e == cudaSuccess) { ++*launches; done = true; }
         else if (e != cudaErrorNotSupported) return e;
+      } else if (!mult && (e = tma_mode_product_c(p, ax, fwd, cur, nb, s)) != cudaErrorNotSupported) {
+        // n <= 64: one in-place launch on the real embedding [[Mr, -Mi], [Mi, Mr]] (kernels_tma.cu, CPLX)
+        if (e != cudaSuccess) return e;
+        ++*launches;
+        done = true;
       } else {
         e = tma_mode_product(p, ax, fwd, cur, other, 2 * nb, mult, nullptr, s, 0);
         if (e == cudaSuccess) {

@@ -37,11 +37,17 @@ struct ZArgs {
   FastDiv div_cpo;
 };
 
-template <int MTOT, int NT, int WARPS, int IC>
+// CPLX (Bloch plans, complex z axis with n <= 64): a function is a (re, im) pair of planes and V the real embedding
+// E = [[Vr, -Vi], [Vi, Vr]] of the complex eigenvector matrix (forward product with E^T = embedding of V^H, backward
+// with E): the same kernel with 2 S stages and 2 MH row tiles, the second half of each belonging to the im plane; the
+// (real) multiplier tile is fetched once per plane.
+template <int MTOT, int NT, int WARPS, int IC, bool CPLX = false>
 __global__ void __launch_bounds__(32 * WARPS, 1)
     k_mode_zz(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const ZArgs a) {
   static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
   static_assert(MTOT % IC == 0, "output row tiles are processed IC at a time");
+  static_assert(!CPLX || MTOT % 2 == 0, "row tiles of the re plane, then of the im plane");
+  constexpr int MH = CPLX ? MTOT / 2 : MTOT;
   constexpr int LDV = 8 * MTOT + 4;
   constexpr unsigned kStage = 1024u * NT;
   constexpr int CH = NT / 2;
@@ -51,10 +57,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int g = lane >> 2, q = lane & 3;
   const int n = a.n, S = a.S;
+  const int S2 = CPLX ? 2 * S : S;  // stages per product
   const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
-  const unsigned img_bytes = 8u * (16u * S) * LDV;
+  const unsigned img_bytes = 8u * (16u * S2) * LDV;
 
-  for (unsigned i = 2 * tid; i < 16u * S * LDV; i += 2 * 32 * WARPS)
+  for (unsigned i = 2 * tid; i < 16u * S2 * LDV; i += 2 * 32 * WARPS)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
   asm volatile("cp.async.commit_group;\n" ::: "memory");
 
@@ -83,7 +90,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned fifo[kDepth + 1];
   int fifo_n = 0;
 
-  // ---- producer: a tile is S data stages (tm0) followed by S multiplier stages (tm1, same columns) ------------
+  // ---- producer: a tile is S2 data stages (tm0) followed by S2 multiplier stages (tm1, same columns) -----------
   unsigned t_p = tfirst;
   int s_p = 0;
   int pc0[CH], pc2[CH];
@@ -93,7 +100,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       const unsigned cc = t * CH + ch;
       if (cc < a.total_chunks) {
         const unsigned o = fast_div(cc, a.div_cpo);
-        pc2[ch] = (int)o;
+        pc2[ch] = CPLX ? 2 * (int)o : (int)o;  // CPLX: o counts complex functions, plane 2o is the re plane
         pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
       } else {  // past the end: an all-out-of-bounds data box (zeros), never stored
         pc2[ch] = a.outer;
@@ -109,11 +116,16 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       mbar_expect_tx(bar, kStage);
 #pragma unroll
       for (int ch = 0; ch < CH; ++ch) {
-        if (s_p < S) tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
-        else tma_load_3d(dst + 2048u * ch, &tm1, pc0[ch], 16 * (s_p - S), 0, bar);
+        if (s_p < S2) {
+          const bool im = CPLX && s_p >= S;
+          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * (im ? s_p - S : s_p), pc2[ch] + (im ? 1 : 0), bar);
+        } else {
+          const int tl = s_p - S2;
+          tma_load_3d(dst + 2048u * ch, &tm1, pc0[ch], 16 * (CPLX && tl >= S ? tl - S : tl), 0, bar);
+        }
       }
     }
-    if (++s_p == 2 * S) {
+    if (++s_p == 2 * S2) {
       s_p = 0;
       t_p = claim_tile();
 #pragma unroll
@@ -160,7 +172,6 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   int slot = 0;
   unsigned parity = 0;
   unsigned t = tfirst;
-  const int s_std = a.kk_last ? S - 1 : S;
   while (t < a.n_tiles) {
     double acc[MTOT][NT][2];
 #pragma unroll
@@ -169,12 +180,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
     // ---- forward product, operands swapped: acc[mt][nt][e] = T[m = 8mt + 2q + e][column 8nt + g] -------------
-    for (int s = 0; s < S; ++s) {
+    for (int s = 0; s < S2; ++s) {
       asm volatile("" : "+r"(v1_lane), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kStage;
       const unsigned aa = v1_lane + (unsigned)s * (16u * LDV * 8u);
-      if (s < s_std) {
+      const bool ragged = a.kk_last && (s == S - 1 || (CPLX && s == S2 - 1));
+      if (!ragged) {
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
           double bf[NT];
@@ -221,13 +233,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     // ---- eigen-space multiply (a3): the multiplier tile arrives in S more stages, read in accumulator layout ---
 #pragma unroll
     for (int sp = 0; sp < SMAX; ++sp) {
-      if (sp < S) {
+      if (sp < S2) {
         mbar_wait(my_bar + 8u * slot, parity);
         const unsigned sb = my_ring + slot * kStage;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-          constexpr int kDummy = 0;
-          (void)kDummy;
           if (2 * sp + h < MTOT) {
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
@@ -253,7 +263,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       const unsigned cc = t * CH + ch;
       if (cc < a.total_chunks) {
         const unsigned o = fast_div(cc, a.div_cpo);
-        o_ch[ch] = (int)o;
+        o_ch[ch] = CPLX ? 2 * (int)o : (int)o;
         col_ch[ch] = 16 * (int)(cc - o * (unsigned)a.cpo) + g;
       } else {
         o_ch[ch] = 0;
@@ -284,16 +294,18 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
 #pragma unroll
       for (int ic = 0; ic < IC; ++ic) {
         const int it = it0 + ic;
-        const bool lin = a.kk_last && (it >> 1) == S - 1;
+        const int im = (CPLX && it >= MH) ? 1 : 0;  // row tiles MH.. belong to the im plane
+        const int itp = it - im * MH;
+        const bool lin = a.kk_last && (itp >> 1) == S - 1;
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          const int z = 8 * it + (lin ? zo_lin[e] : zo_std[e]);
+          const int z = 8 * itp + (lin ? zo_lin[e] : zo_std[e]);
           if (z < n) {
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) {
               const int col = col_ch[nt >> 1] + 8 * (nt & 1);
               if (col < a.inner)
-                a.out[((long long)o_ch[nt >> 1] * n + z) * a.inner + col] = acc2[ic][nt][e];
+                a.out[((long long)(o_ch[nt >> 1] + im) * n + z) * a.inner + col] = acc2[ic][nt][e];
             }
           }
         }
@@ -581,6 +593,9 @@ cudaError_t launch_persistent(Kern kern, SmemOptIn& opt, size_t smem, int warps,
   return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
 }
 
+template <int MTOT, int NT, int WARPS, int IC>
+cudaError_t launch_zz_c(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const ZArgs& a, cudaStream_t s);
+
 inline size_t smem_need(int S, int mtot, int warps, int nt) {
   const size_t img = sizeof(double) * 16 * (size_t)S * (8 * mtot + 4);
   return img + 1024 + (size_t)warps * kDepth * 1024 * nt + (size_t)warps * kDepth * 8 + 16;
@@ -591,6 +606,13 @@ cudaError_t launch_zz(const exx_plan* p, const CUtensorMap& m0, const CUtensorMa
   static SmemOptIn opt;
   return launch_persistent(k_mode_zz<MTOT, NT, WARPS, IC>, opt, smem_need(a.S, MTOT, WARPS, NT), WARPS, a.n_tiles, p, m0,
                            m1, a, s);
+}
+
+template <int MTOT, int NT, int WARPS, int IC>
+cudaError_t launch_zz_c(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const ZArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  return launch_persistent(k_mode_zz<MTOT, NT, WARPS, IC, true>, opt, smem_need(2 * a.S, MTOT, WARPS, NT), WARPS, a.n_tiles,
+                           p, m0, m1, a, s);
 }
 
 template <int MTOT, int NT, int WARPS>
@@ -626,9 +648,35 @@ cudaError_t fused_init(exx_plan* p) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st) return cudaSuccess;
   st->d_img_zz = nullptr;
+  st->d_img_zz_c = nullptr;
   const int n = p->n[2], mtot = mtot_class(n);
-  if (!mtot || !p->h_Vi[2].empty()) return cudaSuccess;
+  if (!mtot) return cudaSuccess;
   const int S = (n + 15) / 16, ldv = 8 * mtot + 4;
+  if (!p->h_Vi[2].empty()) {
+    // complex z axis: E = [[Vr, -Vi], [Vi, Vr]], rows (plane, z) and columns (plane, m), same permutations per block
+    if (mtot > 8) return cudaSuccess;
+    const int ldc = 16 * mtot + 4;
+    std::vector<double> img((size_t)32 * S * ldc, 0.0);
+    for (int s = 0; s < S; ++s)
+      for (int kk = 0; kk < 4; ++kk)
+        for (int q = 0; q < 4; ++q) {
+          const int z = 16 * s + within_stage(false, n, s, kk, q);
+          if (z >= n) continue;
+          double* row_re = &img[(size_t)(16 * s + 4 * kk + q) * ldc];
+          double* row_im = &img[(size_t)(16 * S + 16 * s + 4 * kk + q) * ldc];
+          for (int m = 0; m < n; ++m) {
+            const int c = m ^ ((m >> 2) & 1);
+            const double vr = p->h_V[2][(size_t)z * n + m], vi = p->h_Vi[2][(size_t)z * n + m];
+            row_re[c] = vr;
+            row_re[8 * mtot + c] = -vi;
+            row_im[c] = vi;
+            row_im[8 * mtot + c] = vr;
+          }
+        }
+    cudaError_t e = cudaMalloc(&st->d_img_zz_c, sizeof(double) * img.size());
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(st->d_img_zz_c, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+  }
   std::vector<double> img((size_t)16 * S * ldv, 0.0);
   for (int s = 0; s < S; ++s)
     for (int kk = 0; kk < 4; ++kk)
@@ -647,7 +695,9 @@ void fused_destroy(exx_plan* p) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st) return;
   if (st->d_img_zz) cudaFree(st->d_img_zz);
+  if (st->d_img_zz_c) cudaFree(st->d_img_zz_c);
   st->d_img_zz = nullptr;
+  st->d_img_zz_c = nullptr;
 }
 
 // z-forward product, multiplier and z-backward product of nb right-hand sides in one pass, in place or out of place.
@@ -689,6 +739,44 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
     case 12: return launch_zz<12, 2, 12, 3>(p, m0, m1, a, s);
     case 15: return launch_zz<15, 2, 12, 1>(p, m0, m1, a, s);
     default: return launch_zz<16, 2, 12, 1>(p, m0, m1, a, s);
+  }
+}
+
+// The same for nb complex functions ([nb][2][N] planes) of a Bloch plan whose z axis is complex with n <= 64, in place.
+cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st || !st->d_img_zz_c || !(p->fusion & 1)) return cudaErrorNotSupported;
+  const int n = p->n[2], mh = mtot_class(n);
+  if (!mh || mh > 8) return cudaErrorNotSupported;
+  if ((p->n[0] & 1) || !aligned16(buf) || !aligned16(p->d_mult)) return cudaErrorNotSupported;
+  const long long inner = (long long)p->n[0] * p->n[1];
+  ZArgs a{};
+  a.out = buf;
+  a.V = st->d_img_zz_c;
+  a.n = n;
+  a.S = (n + 15) / 16;
+  a.kk_last = tail_ksteps(n);
+  a.inner = (int)inner;
+  a.cpo = (int)((inner + 15) / 16);
+  const long long chunks = (long long)a.cpo * nb;
+  if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.total_chunks = (unsigned)chunks;
+  a.outer = 2 * nb;
+  a.div_cpo = make_fastdiv((unsigned)a.cpo);
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if ((e = get_map(st, buf, inner, n, 2LL * nb, 16, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, p->d_mult, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+  const int NT = mh <= 4 ? 4 : 2;
+  const int CH = NT / 2;
+  a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+  if (a.n_tiles == 0) return cudaSuccess;
+  ++p->tma_launches;
+  switch (mh) {
+    case 2: return launch_zz_c<4, 4, 16, 1>(p, m0, m1, a, s);
+    case 4: return launch_zz_c<8, 4, 8, 2>(p, m0, m1, a, s);
+    case 6: return launch_zz_c<12, 2, 12, 3>(p, m0, m1, a, s);
+    default: return launch_zz_c<16, 2, 12, 1>(p, m0, m1, a, s);
   }
 }
 

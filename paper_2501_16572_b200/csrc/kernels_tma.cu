@@ -40,7 +40,7 @@ struct TArgs {
   double* out;
   const double* V;  // permuted, zero-padded image [16*S][8*MTOT+4] (tma_init)
   int n;
-  int S;        // stages per tile = ceil(n/16)
+  int S;        // stages per tile = ceil(n/16); CPLX: per plane (a tile is 2 S stages, re plane then im plane)
   int kk_last;  // 0: n is a multiple of 16; else ceil((n % 16) / 4), the k-steps of the ragged last stage
   unsigned n_tiles;
   // L-mode
@@ -60,16 +60,23 @@ struct TArgs {
   // Complex (Bloch) products, second launch: the result Q = Mi [in_re | in_im] is not stored but added into the first
   // launch's output P with the planes swapped, out_re = P_re - Q_im, out_im = P_im + Q_re (planes alternate re, im;
   // plane_stride = N doubles).  per_plane: rows (X-mode) / outer indices (L-mode) of one plane.
+  // Complex (Bloch) products, single launch (CPLX): a function is a (re, im) pair of planes and the product is the real
+  // embedding [[Mr, -Mi], [Mi, Mr]] of M: contraction over 2 S stages, output row tiles 0..MTOT/2-1 go to the re plane,
+  // the rest to the im plane.  plane_rows: rows (X-mode) / plane_outer: outer indices (L-mode) between the two planes.
+  int plane_rows;
+  int plane_outer;
   int rmw;
   long long plane_stride;
   FastDiv div_plane;
 };
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
     k_mode_t(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const TArgs a) {
   static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
+  static_assert(!CPLX || (!TWO && !RMW && MTOT % 2 == 0), "the embedded complex product is a plain one-stream pass");
+  constexpr int MH = CPLX ? MTOT / 2 : MTOT;  // row tiles per plane
   constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): the A-fragment reads are bank-conflict free
   constexpr int NS = TWO ? 2 : 1;    // two streams are staged separately and multiplied on consumption
   constexpr unsigned kStage = 1024u * NT;  // bytes per stage and stream: 16 x (8*NT) doubles
@@ -81,11 +88,12 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int g = lane >> 2, q = lane & 3;
   const int n = a.n, S = a.S;
+  const int S2 = CPLX ? 2 * S : S;  // stages per tile
   const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
-  const unsigned img_bytes = 8u * (16u * S) * LDV;
+  const unsigned img_bytes = 8u * (16u * S2) * LDV;
 
   // ---- stage the V image once per CTA (one burst of 16-byte asynchronous copies) -------------------------
-  for (unsigned i = 2 * tid; i < 16u * S * LDV; i += 2 * 32 * WARPS)
+  for (unsigned i = 2 * tid; i < 16u * S2 * LDV; i += 2 * 32 * WARPS)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
   asm volatile("cp.async.commit_group;\n" ::: "memory");
 
@@ -137,6 +145,10 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
         pr0 = j * a.rows_per_rhs + rb * (8 * NT);
         pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+      } else if (CPLX) {
+        const int fn = (int)fast_div(t, a.div_tiles);
+        const int rb = (int)t - fn * a.tiles_per_rhs;
+        pr0 = 2 * fn * a.rows_per_rhs + rb * (8 * NT);
       } else {
         pr0 = (int)t * (8 * NT);
       }
@@ -146,7 +158,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         const unsigned cc = t * CH + ch;
         if (cc < a.total_chunks) {
           const unsigned o = fast_div(cc, a.div_cpo);
-          pc2[ch] = (int)o;
+          // CPLX: o counts the outer indices of the re planes only; the re plane of function b starts 2 b planes in
+          pc2[ch] = CPLX ? (int)(o + fast_div(o, a.div_plane) * (unsigned)a.plane_outer) : (int)o;
           pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
         } else {  // past the end: an all-out-of-bounds box (zeros), never stored
           pc2[ch] = a.outer;
@@ -161,18 +174,20 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
     const unsigned dst = my_ring + slot * (NS * kStage);
     if (elect_one()) {
       mbar_expect_tx(bar, NS * kStage);
+      const bool im = CPLX && s_p >= S;  // second half of a complex tile: the im plane
+      const int sl = im ? s_p - S : s_p;
       if (XMODE) {
-        tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
-        if (TWO) tma_load_2d(dst + kStage, &tm1, 16 * s_p, pr1, bar);
+        tma_load_2d(dst, &tm0, 16 * sl, pr0 + (im ? a.plane_rows : 0), bar);
+        if (TWO) tma_load_2d(dst + kStage, &tm1, 16 * sl, pr1, bar);
       } else {
 #pragma unroll
         for (int ch = 0; ch < CH; ++ch) {
-          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
-          if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * s_p, 0, bar);
+          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * sl, pc2[ch] + (im ? a.plane_outer : 0), bar);
+          if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * sl, 0, bar);
         }
       }
     }
-    if (++s_p == S) {
+    if (++s_p == S2) {
       s_p = 0;
       t_p = claim_tile();
 #pragma unroll
@@ -210,7 +225,6 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   int slot = 0;
   unsigned parity = 0;
   unsigned t = tfirst;
-  const int s_std = a.kk_last ? S - 1 : S;  // stages of four standard k-steps
   while (t < a.n_tiles) {
     double acc[MTOT][NT][2];
 #pragma unroll
@@ -218,14 +232,15 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
-    for (int s = 0; s < S; ++s) {
+    for (int s = 0; s < S2; ++s) {
       // opaque uses: keep the per-lane fragment offsets in registers (at the register cap the compiler
       // otherwise rebuilds them from %tid in every k-step, ~20 instructions ahead of the first LDS)
       asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * (NS * kStage);
       const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
-      if (s < s_std) {
+      const bool ragged = a.kk_last && (s == S - 1 || (CPLX && s == S2 - 1));  // last stage of a plane, n % 16 != 0
+      if (!ragged) {
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
           double bf[NT];
@@ -292,11 +307,18 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
         const int rb = (int)t - rhs * a.tiles_per_rhs;
         row0 = rhs * a.rows_per_rhs + rb * (8 * NT);
         limit = (rhs + 1) * a.rows_per_rhs;
+      } else if (CPLX) {  // rows of the re plane of function fn; the im plane lies plane_rows rows further
+        const int fn = (int)fast_div(t, a.div_tiles);
+        const int rb = (int)t - fn * a.tiles_per_rhs;
+        row0 = 2 * fn * a.rows_per_rhs + rb * (8 * NT);
+        limit = (2 * fn + 1) * a.rows_per_rhs;
       } else {
         row0 = (int)t * (8 * NT);
         limit = a.rows_total;
       }
       double* base = a.out + ((long long)(row0 + 2 * q) * n + g);
+      // CPLX: row tile mt >= MH is row tile mt - MH of the im plane
+      const long long xim = CPLX ? (long long)a.plane_rows * n - 8 * MH : 0;
       if (RMW) {
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
@@ -326,7 +348,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           for (int e = 0; e < 2; ++e) {
             double* dst = base + (long long)(8 * nt + e) * n;
 #pragma unroll
-            for (int mt = 0; mt < MTOT; ++mt) dst[8 * mt] = acc[mt][nt][e];
+            for (int mt = 0; mt < MTOT; ++mt) dst[8 * mt + (mt >= MH ? xim : 0)] = acc[mt][nt][e];
           }
       } else {
 #pragma unroll
@@ -337,7 +359,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
               double* dst = base + (long long)(8 * nt + e) * n;
 #pragma unroll
               for (int mt = 0; mt < MTOT; ++mt)
-                if (8 * mt + g < n) dst[8 * mt] = acc[mt][nt][e];
+                if (8 * (mt >= MH ? mt - MH : mt) + g < n) dst[8 * mt + (mt >= MH ? xim : 0)] = acc[mt][nt][e];
             }
           }
       }
@@ -347,9 +369,12 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       for (int ch = 0; ch < CH; ++ch) {
         const unsigned cc = t * CH + ch;
         if (cc < a.total_chunks) {
-          const unsigned o = fast_div(cc, a.div_cpo);
-          const int col0 = 16 * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
+          const unsigned o_t = fast_div(cc, a.div_cpo);
+          const int col0 = 16 * (int)(cc - o_t * (unsigned)a.cpo) + 2 * q;
+          const unsigned o = CPLX ? o_t + fast_div(o_t, a.div_plane) * (unsigned)a.plane_outer : o_t;
           double* ptr = a.out + ((long long)o * n + g) * a.inner + col0;
+          // CPLX: row tile mt >= MH is row tile mt - MH of the im plane, plane_outer outer indices further
+          const long long lim = CPLX ? ((long long)a.plane_outer * n - 8 * MH) * a.inner : 0;
           if (RMW) {
             const bool odd = fast_div(o, a.div_plane) & 1u;
             const double sgn = odd ? -1.0 : 1.0;
@@ -375,6 +400,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           } else if (a.exact) {
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
+              if (CPLX && mt == MH) ptr += lim;
               stg_v2(ptr, acc[mt][2 * ch][0], acc[mt][2 * ch][1]);
               stg_v2(ptr + 8, acc[mt][2 * ch + 1][0], acc[mt][2 * ch + 1][1]);
               ptr += mstep;
@@ -384,7 +410,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
             const bool in0 = col0 < a.inner, in1 = col0 + 8 < a.inner;
 #pragma unroll
             for (int mt = 0; mt < MTOT; ++mt) {
-              if (8 * mt + g < n) {
+              if (CPLX && mt == MH) ptr += lim;
+              if (8 * (mt >= MH ? mt - MH : mt) + g < n) {
                 if (in0) stg_v2(ptr, acc[mt][2 * ch][0], acc[mt][2 * ch][1]);
                 if (in1) stg_v2(ptr + 8, acc[mt][2 * ch + 1][0], acc[mt][2 * ch + 1][1]);
               }
@@ -436,18 +463,18 @@ inline bool pick_class(int n, int lanes, ClassCfg* c) {
   return true;
 }
 
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false>
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false>
 cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, int device,
                        cudaStream_t s) {
   constexpr int LDV = 8 * MTOT + 4;
-  const size_t img = sizeof(double) * 16 * (size_t)a.S * LDV;
+  const size_t img = sizeof(double) * 16 * (size_t)a.S * (CPLX ? 2 : 1) * LDV;
   // image | (alignment slack) | rings | mbarriers.  The request is padded so that exactly MINB CTAs fit an SM
   // (above 1/(MINB+1) of its shared memory): the tile split assumes one CTA of this launch per SM.
   size_t smem = img + 1024 + (size_t)WARPS * kDepth * (TWO ? 2 : 1) * 1024 * NT + (size_t)WARPS * kDepth * 8 + 16;
   const size_t floor_bytes = MINB == 1 ? 117 * 1024 : 77 * 1024;
   if (MINB == 2 && smem > 113 * 1024) return cudaErrorInvalidConfiguration;
   if (smem < floor_bytes) smem = floor_bytes;
-  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW>;
+  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW, CPLX>;
   // always the largest shared-memory carveout: kernels of the two lanes must agree on the SM's L1/shared
   // split to be resident together (and a switch between launches drains the SM)
   static SmemOptIn opt;  // per instantiation and device
@@ -585,6 +612,70 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   }
 }
 
+// Complex (Bloch) mode product in ONE launch, in place: nb complex functions = 2 nb planes (re, im) in `buf`, the product
+// with M = V^H (forward) or V (backward) taken as the real embedding [[Mr, -Mi], [Mi, Mr]] (contraction over both
+// planes, output rows for both planes; 4x the real flops, the same as a Zgemm).  Needs 2 ceil(n/8) <= 16, i.e. n <= 64;
+// cudaErrorNotSupported otherwise (the caller then runs the two-launch read-modify-write path).
+cudaError_t tma_mode_product_c(exx_plan* p, int axis, bool forward, double* buf, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return cudaErrorNotSupported;
+  const int n = p->n[axis];
+  const double* img = st->d_img_c[axis][forward ? 0 : 1];
+  if (!img || (p->n[0] & 1) || !aligned16(buf)) return cudaErrorNotSupported;
+  const int need = (n + 7) / 8;
+  const int mh = need <= 2 ? 2 : need <= 4 ? 4 : need <= 6 ? 6 : 8;
+  const bool xmode = axis == 0;
+  const int NT = mh <= 4 ? 4 : 2;
+  TArgs a{};
+  a.out = buf;
+  a.V = img;
+  a.n = n;
+  a.S = (n + 15) / 16;
+  a.kk_last = tail_ksteps(n);
+  CUtensorMap m0;
+  cudaError_t e;
+  if (xmode) {
+    a.rows_per_rhs = (int)(p->N / n);
+    a.plane_rows = a.rows_per_rhs;
+    const long long rows_total = 2LL * a.rows_per_rhs * nb;
+    if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    a.rows_total = (int)rows_total;
+    a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+    a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+    a.exact = (n == 8 * mh) && (a.rows_per_rhs % (8 * NT) == 0);
+    a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
+    if ((e = get_map(st, buf, n, rows_total, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  } else {
+    const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
+    const long long P = p->N / (n * inner);  // outer indices per plane
+    a.inner = (int)inner;
+    a.cpo = (int)((inner + 15) / 16);
+    const long long chunks = (long long)a.cpo * P * nb;
+    if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    a.total_chunks = (unsigned)chunks;
+    a.outer = (int)(2 * P * nb);
+    a.plane_outer = (int)P;
+    a.div_plane = make_fastdiv((unsigned)P);
+    a.div_cpo = make_fastdiv((unsigned)a.cpo);
+    a.exact = (n == 8 * mh) && (inner % 16 == 0);
+    const int CH = NT / 2;
+    a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+    if ((e = get_map(st, buf, inner, n, 2 * P * nb, 16, &m0)) != cudaSuccess) return e;
+  }
+  if (a.n_tiles == 0) return cudaSuccess;
+  ++p->tma_launches;
+#define EXX_LAUNCH_C(MT, NTT, W)                                                                            \
+  (xmode ? launch_one<MT, NTT, true, false, W, 1, false, true>(m0, m0, a, p->sm_count, p->device, s)       \
+         : launch_one<MT, NTT, false, false, W, 1, false, true>(m0, m0, a, p->sm_count, p->device, s))
+  switch (mh) {
+    case 2: return EXX_LAUNCH_C(4, 4, 16);
+    case 4: return EXX_LAUNCH_C(8, 4, 12);
+    case 6: return EXX_LAUNCH_C(12, 2, 12);
+    default: return EXX_LAUNCH_C(16, 2, 12);
+  }
+#undef EXX_LAUNCH_C
+}
+
 // Upload, per axis and direction, the shared-memory image of M (M[m][k] = V[k][m] forward, V[m][k] backward)
 // that k_mode_t stages verbatim: row 16s + 4kk + q holds the contraction index the lane with that q reads in
 // k-step kk of stage s (see the fragment-address comment in the kernel), zero beyond n.
@@ -598,6 +689,7 @@ cudaError_t tma_init(exx_plan* p) {
       st->d_img[ax][d] = nullptr;
       st->img_owned[ax][d] = false;
       st->d_img_im[ax][d] = nullptr;
+      st->d_img_c[ax][d] = nullptr;
     }
   p->tma_state = st;
   for (int ax = 0; ax < 3; ++ax) {
@@ -610,9 +702,37 @@ cudaError_t tma_init(exx_plan* p) {
       st->d_img[2][1] = st->d_img[1][1];
       st->d_img_im[2][0] = st->d_img_im[1][0];
       st->d_img_im[2][1] = st->d_img_im[1][1];
+      st->d_img_c[2][0] = st->d_img_c[1][0];
+      st->d_img_c[2][1] = st->d_img_c[1][1];
       continue;
     }
     const int n = p->n[ax], S = (n + 15) / 16, ldv = 8 * cc.mtot + 4;
+    // Bloch axis with n <= 64: the real embedding [[Mr, -Mi], [Mi, Mr]] for the single-launch complex product; rows:
+    // contraction index over the re plane (16 S rows) then the im plane, columns: output index, re rows then im rows
+    for (int d = 0; d < 2 && !p->h_Vi[ax].empty() && (p->n[ax] + 7) / 8 <= 8; ++d) {
+      const int need = (n + 7) / 8, mh = need <= 2 ? 2 : need <= 4 ? 4 : need <= 6 ? 6 : 8, ldc = 16 * mh + 4;
+      std::vector<double> img((size_t)32 * S * ldc, 0.0);
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int k = 16 * s + within_stage(xmode, n, s, kk, q);
+            if (k >= n) continue;
+            double* row_re = &img[(size_t)(16 * s + 4 * kk + q) * ldc];
+            double* row_im = &img[(size_t)(16 * S + 16 * s + 4 * kk + q) * ldc];
+            for (int m = 0; m < n; ++m) {
+              const double mr = d == 0 ? p->h_V[ax][(size_t)k * n + m] : p->h_V[ax][(size_t)m * n + k];
+              const double mi = d == 0 ? -p->h_Vi[ax][(size_t)k * n + m] : p->h_Vi[ax][(size_t)m * n + k];
+              row_re[m] = mr;            // out_re += Mr in_re
+              row_re[8 * mh + m] = mi;   // out_im += Mi in_re
+              row_im[m] = -mi;           // out_re -= Mi in_im
+              row_im[8 * mh + m] = mr;   // out_im += Mr in_im
+            }
+          }
+      cudaError_t e = cudaMalloc(&st->d_img_c[ax][d], sizeof(double) * img.size());
+      if (e != cudaSuccess) return e;
+      e = cudaMemcpy(st->d_img_c[ax][d], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+    }
     for (int d = 0; d < 2 && !p->h_Vi[ax].empty(); ++d) {  // Bloch axis: forward M = V^H, Im = -Vi^T; backward Im = Vi
       std::vector<double> img((size_t)16 * S * ldv, 0.0);
       for (int s = 0; s < S; ++s)
@@ -660,6 +780,7 @@ void tma_destroy(exx_plan* p) {
     {
       if (st->img_owned[ax][d] && st->d_img[ax][d]) cudaFree(st->d_img[ax][d]);
       if (st->d_img_im[ax][d] && !(ax == 2 && st->d_img_im[2][d] == st->d_img_im[1][d])) cudaFree(st->d_img_im[ax][d]);
+      if (st->d_img_c[ax][d] && !(ax == 2 && st->d_img_c[2][d] == st->d_img_c[1][d])) cudaFree(st->d_img_c[ax][d]);
     }
   delete st;
   p->tma_state = nullptr;

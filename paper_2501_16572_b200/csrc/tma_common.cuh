@@ -30,6 +30,8 @@ struct TmaState {
   double* d_img[3][2];  // [axis][0 = forward (V^T), 1 = backward (V)]
   bool img_owned[3][2];
   double* d_img_im[3][2];  // Bloch plans: images of the imaginary parts, forward = Im(V^H) = -Vi^T, backward = Vi
+  double* d_img_c[3][2];   // Bloch axes with n <= 64: real embedding [[Mr, -Mi], [Mi, Mr]] for the single-launch complex product
+  double* d_img_zz_c;      // the same for a complex z axis with n <= 64 (embedding E = [[Vr, -Vi], [Vi, Vr]])
   double* d_img_zz;  // fused z-forward/z-backward kernel: one image of Vz serving both products (kernels_fused.cu)
   std::vector<MapEntry> cache;
 };

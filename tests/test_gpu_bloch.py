@@ -45,6 +45,11 @@ SOLVE_CASES = [
     ((13, 8, 10), (0, 0, 1), (1.0, 2.0, 0.7), 0.0, 3, 2),
     ((48, 48, 48), (0, 0, 0), (np.pi / 2, 0.0, np.pi / 3), 0.106, 3, 2),
     ((60, 60, 120), (0, 0, 1), (0.8, -0.8, 0.0), 0.106, 2, 2),
+    # single-launch embedded complex products on every axis, ragged last stages (n % 16 = 10, 12, 12) and column chunks
+    ((26, 44, 60), (0, 0, 0), (0.7, -1.1, 0.4), 0.106, 3, 2),
+    # complex axes longer than 64 points: the two-launch read-modify-write path (y), the three-launch z path
+    ((16, 72, 10), (0, 0, 0), (0.3, 0.9, -0.5), 0.106, 3, 3),
+    ((8, 8, 100), (0, 0, 0), (0.3, 0.9, -0.5), 0.0, 2, 2),
 ]
 
 
@@ -65,6 +70,12 @@ def test_bloch_solve_matches_oracle(case, variant):
     torch.cuda.synchronize()
     assert torch.equal(d, keep)
     assert _rel(_cplx(out), ref) < TOL
+    if variant == exx.VARIANT_FUSED_DMMA:         # without the fused z pass (exx_plan_set_fusion bit 0)
+        plan.set_fusion(0)
+        out0 = plan.poisson_solve_bloch(d, n_c=n_c)
+        torch.cuda.synchronize()
+        assert _rel(_cplx(out0), ref) < TOL
+        plan.set_fusion(3)
     if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0:
         assert plan.tma_launch_count > 0          # the tensor-core kernels served it
     with pytest.raises(exx.ExxError):             # real entry points refuse a complex plan
