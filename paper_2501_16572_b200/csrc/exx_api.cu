@@ -11,6 +11,11 @@
 
 namespace {
 
+#ifndef EXX_ITEMS_PER_WARP
+#define EXX_ITEMS_PER_WARP 8
+#endif
+constexpr int kItemsPerWarp = EXX_ITEMS_PER_WARP;
+
 using exx::DeviceScope;
 
 thread_local cudaError_t g_last_cuda = cudaSuccess;
@@ -477,7 +482,9 @@ exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, i
     const int xacc_rows = plan->variant == EXX_VARIANT_FUSED_DMMA && (plan->fusion & 2) ? exx::fused_xacc_tile_rows(plan) : 0;
     if (xacc_rows > 0 && !(plan->n[0] & 1)) {
       const long long tiles_per_rhs = (N / plan->n[0] + xacc_rows - 1) / xacc_rows;
-      long long nk_want = (96LL * plan->sm_count + tiles_per_rhs - 1) / tiles_per_rhs;
+      // about kItemsPerWarp items for each of the 12 warps of an SM: the items of a launch are uniform, so the last round
+      // of an uneven split idles (items/warps)/ceil(items/warps) of the machine
+      long long nk_want = ((long long)kItemsPerWarp * 12 * plan->sm_count + tiles_per_rhs - 1) / tiles_per_rhs;
       if (nk_want > n_tgt) nk_want = n_tgt;
       if (nk_want > n_c) nk_want = n_c;
       int nj = (int)(n_c / nk_want);

@@ -29,18 +29,29 @@ inline int grid_for(long long work, int threads, int sm_count) {
   return (int)g;
 }
 
-// rho_b = conj(psi_j) .* tgt_k (Eq. 2), b = kk * nj + jj; planes [2][N].  grid.y = nb.
-__global__ void k_pair_density_c(const double* __restrict__ psi, const double* __restrict__ tgt, BatchDesc bd,
-                                 long long N, double* __restrict__ out) {
+// rho_b = conj(psi_j) .* tgt_k (Eq. 2), b = kk * nj + jj; planes [2][N].  grid.y = nb.  VEC = 2: 16-byte
+// accesses (N even, 16-byte aligned buffers).
+template <int VEC>
+__global__ void __launch_bounds__(256) k_pair_density_c(const double* __restrict__ psi, const double* __restrict__ tgt,
+                                                        BatchDesc bd, long long N, double* __restrict__ out) {
   const int b = blockIdx.y;
   const int j = bd.j0 + b % bd.nj, k = bd.k0 + b / bd.nj;
   const double* ar = psi + (size_t)j * 2 * N;
   const double* br = tgt + (size_t)k * 2 * N;
   double* o = out + (size_t)b * 2 * N;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-    const double a_re = ar[i], a_im = ar[N + i], b_re = br[i], b_im = br[N + i];
-    o[i] = a_re * b_re + a_im * b_im;
-    o[N + i] = a_re * b_im - a_im * b_re;
+  for (long long i = (blockIdx.x * (long long)blockDim.x + threadIdx.x) * VEC; i < N;
+       i += (long long)gridDim.x * blockDim.x * VEC) {
+    if (VEC == 2) {
+      const double2 a_re = *reinterpret_cast<const double2*>(ar + i), a_im = *reinterpret_cast<const double2*>(ar + N + i);
+      const double2 b_re = *reinterpret_cast<const double2*>(br + i), b_im = *reinterpret_cast<const double2*>(br + N + i);
+      *reinterpret_cast<double2*>(o + i) = make_double2(a_re.x * b_re.x + a_im.x * b_im.x, a_re.y * b_re.y + a_im.y * b_im.y);
+      *reinterpret_cast<double2*>(o + N + i) =
+          make_double2(a_re.x * b_im.x - a_im.x * b_re.x, a_re.y * b_im.y - a_im.y * b_re.y);
+    } else {
+      const double a_re = ar[i], a_im = ar[N + i], b_re = br[i], b_im = br[N + i];
+      o[i] = a_re * b_re + a_im * b_im;
+      o[N + i] = a_re * b_im - a_im * b_re;
+    }
   }
 }
 
@@ -55,23 +66,48 @@ __global__ void k_combine(double* __restrict__ P, const double* __restrict__ Q, 
 }
 
 // vx_k (-)= sum_j occ_j psi_j .* phi_jk (complex product, no conjugate; Eq. 1), j ascending.  grid.y = nk.
-__global__ void k_accumulate_c(const double* __restrict__ psi, const double* __restrict__ occ,
-                               const double* __restrict__ phi, BatchDesc bd, bool first, long long N,
-                               double* __restrict__ vx) {
+// VEC = 2: 16-byte accesses; the arithmetic per element is the same for both instantiations.
+template <int VEC>
+__global__ void __launch_bounds__(256) k_accumulate_c(const double* __restrict__ psi, const double* __restrict__ occ,
+                                                      const double* __restrict__ phi, BatchDesc bd, bool first,
+                                                      long long N, double* __restrict__ vx) {
   const int kk = blockIdx.y;
   double* v = vx + (size_t)(bd.k0 + kk) * 2 * N;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-    double v_re = first ? 0.0 : v[i], v_im = first ? 0.0 : v[N + i];
-    for (int jj = 0; jj < bd.nj; ++jj) {
-      const double* a = psi + (size_t)(bd.j0 + jj) * 2 * N;
-      const double* f = phi + ((size_t)kk * bd.nj + jj) * 2 * N;
-      const double o = occ[bd.j0 + jj];
-      const double a_re = a[i], a_im = a[N + i], f_re = f[i], f_im = f[N + i];
-      v_re -= o * (a_re * f_re - a_im * f_im);
-      v_im -= o * (a_re * f_im + a_im * f_re);
+  for (long long i = (blockIdx.x * (long long)blockDim.x + threadIdx.x) * VEC; i < N;
+       i += (long long)gridDim.x * blockDim.x * VEC) {
+    double v_re[VEC], v_im[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+      v_re[e] = first ? 0.0 : v[i + e];
+      v_im[e] = first ? 0.0 : v[N + i + e];
     }
-    v[i] = v_re;
-    v[N + i] = v_im;
+    const double* a = psi + (size_t)bd.j0 * 2 * N + i;
+    const double* f = phi + (size_t)kk * bd.nj * 2 * N + i;
+#pragma unroll 2
+    for (int jj = 0; jj < bd.nj; ++jj) {
+      const double o = occ[bd.j0 + jj];
+      double a_re[VEC], a_im[VEC], f_re[VEC], f_im[VEC];
+      if (VEC == 2) {
+        const double2 t0 = *reinterpret_cast<const double2*>(a), t1 = *reinterpret_cast<const double2*>(a + N);
+        const double2 t2 = *reinterpret_cast<const double2*>(f), t3 = *reinterpret_cast<const double2*>(f + N);
+        a_re[0] = t0.x; a_re[VEC - 1] = t0.y; a_im[0] = t1.x; a_im[VEC - 1] = t1.y;
+        f_re[0] = t2.x; f_re[VEC - 1] = t2.y; f_im[0] = t3.x; f_im[VEC - 1] = t3.y;
+      } else {
+        a_re[0] = a[0]; a_im[0] = a[N]; f_re[0] = f[0]; f_im[0] = f[N];
+      }
+#pragma unroll
+      for (int e = 0; e < VEC; ++e) {
+        v_re[e] -= o * (a_re[e] * f_re[e] - a_im[e] * f_im[e]);
+        v_im[e] -= o * (a_re[e] * f_im[e] + a_im[e] * f_re[e]);
+      }
+      a += 2 * N;
+      f += 2 * N;
+    }
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+      v[i + e] = v_re[e];
+      v[N + i + e] = v_im[e];
+    }
   }
 }
 
@@ -113,15 +149,27 @@ __global__ void k_mode_product_c(const double* __restrict__ in, double* __restri
 
 cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd, double* out,
                                cudaStream_t s) {
-  dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nj * bd.nk);
-  k_pair_density_c<<<grid, 256, 0, s>>>(psi, tgt, bd, p->N, out);
+  const bool vec2 = (p->N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)tgt | (uintptr_t)out) & 15) == 0);
+  if (vec2) {
+    dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nj * bd.nk);
+    k_pair_density_c<2><<<grid, 256, 0, s>>>(psi, tgt, bd, p->N, out);
+  } else {
+    dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nj * bd.nk);
+    k_pair_density_c<1><<<grid, 256, 0, s>>>(psi, tgt, bd, p->N, out);
+  }
   return cudaGetLastError();
 }
 
 cudaError_t bloch_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi, BatchDesc bd,
                              bool first, double* vx, cudaStream_t s) {
-  dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
-  k_accumulate_c<<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
+  const bool vec2 = (p->N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
+  if (vec2) {
+    dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nk);
+    k_accumulate_c<2><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
+  } else {
+    dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
+    k_accumulate_c<1><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
+  }
   return cudaGetLastError();
 }
 
