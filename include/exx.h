@@ -94,11 +94,13 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes);
 int exx_plan_get_lanes(const exx_plan* plan);
 
 /*
- * Pass fusion of the default variant (test and measurement hook; default 3 = both on).  Bit 0: the z-forward product,
+ * Pass fusion of the default variant (test and measurement hook; default 7 = all on).  Bit 0: the z-forward product,
  * the eigen-space multiply and the z-backward product of a batch (Eq. 11's third and fourth GEMM and Eq. 16,
  * PAPER.md:96-98, :134) run as ONE kernel, the intermediate staying in registers.  Bit 1: the x-backward product and
  * the accumulate of Eq. 1 run as one kernel; phi_jk is never written to memory and exx_apply shapes its
- * batches as nj occupied orbitals x nk targets with nk large enough to keep every SM busy.  With a bit off (or where
+ * batches as nj occupied orbitals x nk targets with nk large enough to keep every SM busy.  Bit 2: where nx is 8
+ * (mod 16) the y products tile their columns in half-chunks of 8 instead of chunks of 16, the last of which would be
+ * half empty in every row.  With a bit off (or where
  * TMA cannot address the buffers, or an axis has more than 128 points) the separate passes run.  The result does not
  * depend on the mask beyond rounding (the sum over j is taken in ascending order either way).
  */
@@ -150,7 +152,7 @@ exx_status exx_poisson_solve_nonbatch(exx_plan* plan, const double* d_rhs, doubl
  *   *d_ex    = 1/2 sum_k d_occ_tgt[k] d_ex_k[k]                                     optional (NULL); needs d_occ_tgt
  * d_psi [n_occ][N], d_occ [n_occ]; d_tgt [n_tgt][N] may alias a block of d_psi.  d_vx must not overlap
  * d_psi / d_tgt / the workspace (EXX_ERR_ALIAS).  n_c = right-hand sides per batch, 1..max_batch,
- * 0 = library default (about 1 GB of right-hand sides per
+ * 0 = library default (about 4 GB of right-hand sides per
  * batch, at least 32, at most max_batch).  Every (j,k) pair is solved (no symmetry shortcut, R12).  n_occ == 0 gives vx = 0.
  */
 exx_status exx_apply(exx_plan* plan, const double* d_psi, const double* d_occ, int n_occ,

@@ -12,7 +12,7 @@
 namespace {
 
 #ifndef EXX_ITEMS_PER_WARP
-#define EXX_ITEMS_PER_WARP 8
+#define EXX_ITEMS_PER_WARP 24
 #endif
 constexpr int kItemsPerWarp = EXX_ITEMS_PER_WARP;
 
@@ -64,7 +64,7 @@ inline bool is_complex_plan(const exx_plan* p) { return p->d_Vi[0] || p->d_Vi[1]
 // DESIGN.md section 9), at least kDefaultBatch, at most max_batch
 inline int resolve_nc(const exx_plan* p, int n_c) {
   if (n_c == 0) {
-    long long want = (1LL << 30) / (8 * p->N);
+    long long want = (4LL << 30) / (8 * p->N);  // about 4 GB of right-hand sides per batch
     if (want < kDefaultBatch) want = kDefaultBatch;
     n_c = want < p->max_batch ? (int)want : p->max_batch;
   }
@@ -129,7 +129,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false; p->accumulate = false;
-  p->fusion = 3;
+  p->fusion = 7;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
     p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
@@ -272,7 +272,7 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes) {
 int exx_plan_get_lanes(const exx_plan* plan) { return plan ? plan->lanes : 0; }
 
 exx_status exx_plan_set_fusion(exx_plan* plan, int mask) {
-  if (!plan || mask < 0 || mask > 3) return EXX_ERR_INVALID_ARG;
+  if (!plan || mask < 0 || mask > 7) return EXX_ERR_INVALID_ARG;
   plan->fusion = mask;
   return EXX_OK;
 }

@@ -66,7 +66,8 @@ struct exx_plan {
   // forked and joined with the two events
   int lanes;
   // bit 0: z-forward + multiplier + z-backward in one pass (k_mode_zz); bit 1: x-backward + accumulate in one pass
-  // (k_mode_xacc).  Default 3; exx_plan_set_fusion (test / measurement hook)
+  // (k_mode_xacc); bit 2: y passes on 8-column half-chunk tiles where nx == 8 (mod 16).  Default 7; exx_plan_set_fusion
+  // (test / measurement hook)
   int fusion;
   cudaStream_t lane_stream;
   cudaEvent_t ev_fork, ev_join;

@@ -65,22 +65,28 @@ struct TArgs {
   // the rest to the im plane.  plane_rows: rows (X-mode) / plane_outer: outer indices (L-mode) between the two planes.
   int plane_rows;
   int plane_outer;
+  int hc;  // L-mode plain pass on 8-column half-chunks (template flag HC): cpo / total_chunks count half-chunks
   int rmw;
   long long plane_stride;
   FastDiv div_plane;
 };
 
 // MTOT = ceil(n/8) rounded up to a supported class, NT = column tiles (of 8) per warp.
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false>
+// HC (L-mode, plain pass only): a tile is NT half-chunks of 8 columns (boxes of 8 x 16, 64-byte rows) instead of NT/2
+// chunks of 16, for an inner extent that is 8 (mod 16): the y pass at nx = 120 then runs 15 half-chunks per row
+// instead of 8 chunks, the last of them half empty (6.7 % of the pass).
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false, bool HC = false>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
     k_mode_t(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const TArgs a) {
   static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
   static_assert(!CPLX || (!TWO && !RMW && MTOT % 2 == 0), "the embedded complex product is a plain one-stream pass");
+  static_assert(!HC || (!XMODE && !TWO && !RMW && !CPLX), "half-chunk tiles: plain real L-mode pass only");
   constexpr int MH = CPLX ? MTOT / 2 : MTOT;  // row tiles per plane
   constexpr int LDV = 8 * MTOT + 4;  // == 4 (mod 8): the A-fragment reads are bank-conflict free
   constexpr int NS = TWO ? 2 : 1;    // two streams are staged separately and multiplied on consumption
   constexpr unsigned kStage = 1024u * NT;  // bytes per stage and stream: 16 x (8*NT) doubles
-  constexpr int CH = NT / 2;               // L-mode: 16-column chunks per tile
+  constexpr int CH = HC ? NT : NT / 2;     // L-mode: 16-column chunks (HC: 8-column half-chunks) per tile
+  constexpr int CW = HC ? 8 : 16;          // columns per chunk
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31;
   // warp index through a shuffle: the compiler then knows it is warp-uniform and keeps everything derived
@@ -160,7 +166,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           const unsigned o = fast_div(cc, a.div_cpo);
           // CPLX: o counts the outer indices of the re planes only; the re plane of function b starts 2 b planes in
           pc2[ch] = CPLX ? (int)(o + fast_div(o, a.div_plane) * (unsigned)a.plane_outer) : (int)o;
-          pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
+          pc0[ch] = CW * (int)(cc - o * (unsigned)a.cpo);
         } else {  // past the end: an all-out-of-bounds box (zeros), never stored
           pc2[ch] = a.outer;
           pc0[ch] = 0;
@@ -182,7 +188,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
       } else {
 #pragma unroll
         for (int ch = 0; ch < CH; ++ch) {
-          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * sl, pc2[ch] + (im ? a.plane_outer : 0), bar);
+          tma_load_3d(dst + (HC ? 1024u : 2048u) * ch, &tm0, pc0[ch], 16 * sl, pc2[ch] + (im ? a.plane_outer : 0), bar);
           if (TWO) tma_load_3d(dst + kStage + 2048u * ch, &tm1, pc0[ch], 16 * sl, 0, bar);
         }
       }
@@ -216,6 +222,12 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
   for (int i = 0; i < 4; ++i) {
     if (XMODE) {
       xo[i] = 128u * g + 16u * ((4u * (q >> 1) + i) ^ (unsigned)g) + 8u * (q & 1);
+    } else if (HC) {
+      // box of 8 columns x 16 rows, 64-byte rows, 64-byte swizzle (16-byte chunk index XOR (row >> 1) & 3): k-step i
+      // reads box row r = (q&1) + 4(q>>1) + 2(i&1) + 8(i>>1), column g (conflict-free: the 16-byte positions
+      // 4 (r&1) + ((g>>1) ^ ((r>>1)&3)) of a half-warp are all distinct for rows {0,1,4,5} + 2(i&1))
+      const unsigned r = (q & 1) + 4u * (q >> 1) + 2u * (i & 1) + 8u * (i >> 1);
+      xo[i] = 64u * r + 16u * ((g >> 1) ^ ((r >> 1) & 3u)) + 8u * (g & 1);
     } else {
       const unsigned row = 2u * q + (i & 1);
       xo[i] = 128u * row + 16u * ((4u * (i >> 1) + (g >> 1)) ^ row) + 8u * (g & 1);
@@ -246,8 +258,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
           double bf[NT];
 #pragma unroll
           for (int nt = 0; nt < NT; ++nt) {
-            const unsigned off = XMODE ? (sb + xo[kk] + 1024u * nt)
-                                       : (sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1));
+            const unsigned off = (XMODE || HC) ? (sb + xo[kk] + 1024u * nt)
+                                               : (sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1));
             bf[nt] = lds64(off);
             if (TWO) bf[nt] *= lds64(off + kStage);
           }
@@ -272,6 +284,9 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
               unsigned off;
               if (XMODE) {
                 off = sb + 1024u * nt + 128u * g + 16u * ((2u * kk + (q >> 1)) ^ (unsigned)g) + 8u * (q & 1);
+              } else if (HC) {
+                const unsigned r = 4u * kk + q;
+                off = sb + 1024u * nt + 64u * r + 16u * ((g >> 1) ^ ((r >> 1) & 3u)) + 8u * (g & 1);
               } else {
                 const unsigned row = 4u * kk + q;
                 off = sb + 2048u * (nt >> 1) + 128u * row + 16u * ((4u * (nt & 1) + (g >> 1)) ^ (row & 7u)) + 8u * (g & 1);
@@ -362,6 +377,23 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
                 if (8 * (mt >= MH ? mt - MH : mt) + g < n) dst[8 * mt + (mt >= MH ? xim : 0)] = acc[mt][nt][e];
             }
           }
+      }
+    } else if (HC) {
+      const long long mstep = 8LL * a.inner;
+#pragma unroll
+      for (int ch = 0; ch < NT; ++ch) {  // column tile nt = half-chunk ch
+        const unsigned cc = t * NT + ch;
+        if (cc < a.total_chunks) {
+          const unsigned o = fast_div(cc, a.div_cpo);
+          const int col0 = 8 * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
+          double* ptr = a.out + ((long long)o * n + g) * a.inner + col0;
+          const bool in0 = col0 < a.inner;  // inner is even: the pair (c, c+1) is inside or outside together
+#pragma unroll
+          for (int mt = 0; mt < MTOT; ++mt) {
+            if (in0 && 8 * mt + g < n) stg_v2(ptr, acc[mt][ch][0], acc[mt][ch][1]);
+            ptr += mstep;
+          }
+        }
       }
     } else {
       const long long mstep = 8LL * a.inner;  // doubles between consecutive row tiles
@@ -463,7 +495,7 @@ inline bool pick_class(int n, int lanes, ClassCfg* c) {
   return true;
 }
 
-template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false>
+template <int MTOT, int NT, bool XMODE, bool TWO, int WARPS, int MINB, bool RMW = false, bool CPLX = false, bool HC = false>
 cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs& a, int sm_count, int device,
                        cudaStream_t s) {
   constexpr int LDV = 8 * MTOT + 4;
@@ -474,7 +506,7 @@ cudaError_t launch_one(const CUtensorMap& m0, const CUtensorMap& m1, const TArgs
   const size_t floor_bytes = MINB == 1 ? 117 * 1024 : 77 * 1024;
   if (MINB == 2 && smem > 113 * 1024) return cudaErrorInvalidConfiguration;
   if (smem < floor_bytes) smem = floor_bytes;
-  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW, CPLX>;
+  auto kern = k_mode_t<MTOT, NT, XMODE, TWO, WARPS, MINB, RMW, CPLX, HC>;
   // always the largest shared-memory carveout: kernels of the two lanes must agree on the SM's L1/shared
   // split to be resident together (and a switch between launches drains the SM)
   static SmemOptIn opt;  // per instantiation and device
@@ -508,6 +540,7 @@ cudaError_t launch_class(bool xmode, bool two, const CUtensorMap& m0, const CUte
   }
   if (two) return launch_one<MTOT, NT2, false, true, WARPS2, MINB2>(m0, m1, a, sm_count, device, s);
   if (a.rmw) return launch_one<MTOT, NT, false, false, WARPS, MINB, true>(m0, m1, a, sm_count, device, s);
+  if (a.hc) return launch_one<MTOT, NT, false, false, WARPS, MINB, false, false, true>(m0, m1, a, sm_count, device, s);
   return launch_one<MTOT, NT, false, false, WARPS, MINB>(m0, m1, a, sm_count, device, s);
 }
 
@@ -567,18 +600,26 @@ cudaError_t tma_mode_product(exx_plan* p, int axis, bool forward, const double* 
   } else {
     const long long inner = axis == 1 ? p->n[0] : (long long)p->n[0] * p->n[1];
     const long long outer = p->N / (n * inner) * nb;
+    // half-chunk tiles where 16-column chunks would leave the last chunk of every row half empty
+    const double* img_hc = st->d_img_hc[forward ? 0 : 1];
+    const bool hc = axis == 1 && !two && !rmw && part == 0 && img_hc && inner % 16 == 8 && (p->fusion & 4);
+    if (hc) {
+      a.hc = 1;
+      a.V = img_hc;
+    }
+    const int cw = hc ? 8 : 16;
     a.kk_last = tail_ksteps(n);
     a.inner = (int)inner;
-    a.cpo = (int)((inner + 15) / 16);
+    a.cpo = (int)((inner + cw - 1) / cw);
     const long long chunks = (long long)a.cpo * outer;
     if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
     a.total_chunks = (unsigned)chunks;
     a.outer = (int)outer;
     a.div_cpo = make_fastdiv((unsigned)a.cpo);
     a.exact = (n == 8 * cc.mtot) && (inner % 16 == 0);
-    const int CH = NT / 2;
+    const int CH = hc ? NT : NT / 2;
     a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
-    if ((e = get_map(st, in, inner, n, outer, 16, &m0)) != cudaSuccess) return e;
+    if ((e = get_map(st, in, inner, n, outer, 16, &m0, cw)) != cudaSuccess) return e;
     if (apply_mult) {
       if ((e = get_map(st, p->d_mult, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
     } else {
@@ -691,6 +732,7 @@ cudaError_t tma_init(exx_plan* p) {
       st->d_img_im[ax][d] = nullptr;
       st->d_img_c[ax][d] = nullptr;
     }
+  st->d_img_hc[0] = st->d_img_hc[1] = nullptr;
   p->tma_state = st;
   for (int ax = 0; ax < 3; ++ax) {
     ClassCfg cc;
@@ -750,6 +792,23 @@ cudaError_t tma_init(exx_plan* p) {
       e = cudaMemcpy(st->d_img_im[ax][d], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
       if (e != cudaSuccess) return e;
     }
+    // y axis of a real plan with nx == 8 (mod 16): the same images in the row order of the half-chunk tiles
+    for (int d = 0; d < 2 && ax == 1 && p->h_Vi[ax].empty() && p->n[0] % 16 == 8; ++d) {
+      std::vector<double> img((size_t)16 * S * ldv, 0.0);
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int k = 16 * s + within_stage(false, n, s, kk, q, true);
+            if (k >= n) continue;
+            double* row = &img[(size_t)(16 * s + 4 * kk + q) * ldv];
+            for (int m = 0; m < n; ++m)
+              row[m] = d == 0 ? p->h_V[ax][(size_t)k * n + m] : p->h_V[ax][(size_t)m * n + k];
+          }
+      cudaError_t e = cudaMalloc(&st->d_img_hc[d], sizeof(double) * img.size());
+      if (e != cudaSuccess) return e;
+      e = cudaMemcpy(st->d_img_hc[d], img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+    }
     for (int d = 0; d < 2; ++d) {
       std::vector<double> img((size_t)16 * S * ldv, 0.0);
       for (int s = 0; s < S; ++s)
@@ -782,6 +841,8 @@ void tma_destroy(exx_plan* p) {
       if (st->d_img_im[ax][d] && !(ax == 2 && st->d_img_im[2][d] == st->d_img_im[1][d])) cudaFree(st->d_img_im[ax][d]);
       if (st->d_img_c[ax][d] && !(ax == 2 && st->d_img_c[2][d] == st->d_img_c[1][d])) cudaFree(st->d_img_c[ax][d]);
     }
+  for (int d = 0; d < 2; ++d)
+    if (st->d_img_hc[d]) cudaFree(st->d_img_hc[d]);
   delete st;
   p->tma_state = nullptr;
 }

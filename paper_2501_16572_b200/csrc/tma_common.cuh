@@ -16,9 +16,10 @@ namespace exx {
 struct MapKey {
   const void* base;
   unsigned long long d0, d1, d2;
-  unsigned b1;  // box rows (box is always 16 wide; third box dimension 1)
+  unsigned b1;  // box rows (third box dimension 1)
+  unsigned b0;  // box columns: 16, or 8 for the half-chunk tiles
   bool operator==(const MapKey& o) const {
-    return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b1 == o.b1;
+    return base == o.base && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b1 == o.b1 && b0 == o.b0;
   }
 };
 struct MapEntry {
@@ -31,6 +32,7 @@ struct TmaState {
   bool img_owned[3][2];
   double* d_img_im[3][2];  // Bloch plans: images of the imaginary parts, forward = Im(V^H) = -Vi^T, backward = Vi
   double* d_img_c[3][2];   // Bloch axes with n <= 64: real embedding [[Mr, -Mi], [Mi, Mr]] for the single-launch complex product
+  double* d_img_hc[2];     // y axis, nx == 8 (mod 16): L-mode images in the row order of the half-chunk tiles (HC)
   double* d_img_zz_c;      // the same for a complex z axis with n <= 64 (embedding E = [[Vr, -Vi], [Vi, Vr]])
   double* d_img_zz;  // fused z-forward/z-backward kernel: one image of Vz serving both products (kernels_fused.cu)
   std::vector<MapEntry> cache;
@@ -130,10 +132,11 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// 2-D ([d1][d0]) or 3-D ([d2][d1][d0]) FP64 tensor, box {16, box_rows(, 1)}, 128-byte swizzle, zero fill.
+// 2-D ([d1][d0]) or 3-D ([d2][d1][d0]) FP64 tensor, box {box_cols, box_rows(, 1)}, zero fill; the swizzle span equals the
+// box width: 128 bytes for 16 columns, 64 bytes for 8.
 cudaError_t get_map(TmaState* st, const void* base, unsigned long long d0, unsigned long long d1,
-                    unsigned long long d2, unsigned box_rows, CUtensorMap* out) {
-  const MapKey key{base, d0, d1, d2, box_rows};
+                    unsigned long long d2, unsigned box_rows, CUtensorMap* out, unsigned box_cols = 16) {
+  const MapKey key{base, d0, d1, d2, box_rows, box_cols};
   for (const auto& e : st->cache)
     if (e.key == key) {
       *out = e.map;
@@ -144,11 +147,12 @@ cudaError_t get_map(TmaState* st, const void* base, unsigned long long d0, unsig
   const cuuint32_t rank = d2 ? 3 : 2;
   cuuint64_t gdim[3] = {d0, d1, d2 ? d2 : 1};
   cuuint64_t gstr[2] = {d0 * 8ull, d0 * d1 * 8ull};
-  cuuint32_t box[3] = {16u, box_rows, 1u};
+  cuuint32_t box[3] = {box_cols, box_rows, 1u};
   cuuint32_t estr[3] = {1u, 1u, 1u};
   alignas(64) CUtensorMap m;
   const CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, const_cast<void*>(base), gdim, gstr, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, box_cols == 8 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   if (st->cache.size() >= 64) st->cache.clear();
@@ -164,8 +168,9 @@ inline int tail_ksteps(int n) { return (n % 16) ? (n % 16 + 3) / 4 : 0; }
 
 // Contraction index (within its block of 16) that the lane with this q reads in k-step kk of stage s: the order in
 // which the swizzled boxes deliver it in a standard stage, plain 4 kk + q in the ragged last stage.
-inline int within_stage(bool xmode, int n, int s, int kk, int q) {
+inline int within_stage(bool xmode, int n, int s, int kk, int q, bool hc = false) {
   if ((n % 16) && s == (n + 15) / 16 - 1) return 4 * kk + q;
+  if (hc) return (q & 1) + 4 * (q >> 1) + 2 * (kk & 1) + 8 * (kk >> 1);  // 8-column boxes, 64-byte rows
   return xmode ? ((q & 1) + 8 * (q >> 1) + 2 * kk) : (2 * q + (kk & 1) + 8 * (kk >> 1));
 }
 

@@ -63,9 +63,9 @@ P, D = PERIODIC, DIRICHLET
 WORKLOADS = {
     1: Workload("cfg1_tiny_16c_pbe0", 1, 16, 16, 16, 0.5, (P, P, P), 12, 0.0, 8, 0, 8, 0.0, 0.0, False, 64),
     2: Workload("cfg2_bulk_48c_hse", 2, 48, 48, 48, 0.25, (P, P, P), 12, 0.106, 64, 0, 64, 2.0, 0.0, False, 1024),
-    3: Workload("cfg3_slab_60x60x120_hse", 3, 60, 60, 120, 0.25, (P, P, D), 12, 0.106, 256, 0, 256, 2.0, 8.0, True, 512),
-    4: Workload("cfg4_metal_96c_hse", 4, 96, 96, 96, 0.2, (P, P, P), 12, 0.106, 1536, 896, 256, 2.0, 0.0, True, 256),
-    5: Workload("cfg5_metal_120c_hse", 5, 120, 120, 120, 0.2, (P, P, P), 12, 0.106, 3200, 2176, 128, 2.0, 0.0, True, 128),
+    3: Workload("cfg3_slab_60x60x120_hse", 3, 60, 60, 120, 0.25, (P, P, D), 12, 0.106, 256, 0, 256, 2.0, 8.0, True, 1024),
+    4: Workload("cfg4_metal_96c_hse", 4, 96, 96, 96, 0.2, (P, P, P), 12, 0.106, 1536, 896, 256, 2.0, 0.0, True, 512),
+    5: Workload("cfg5_metal_120c_hse", 5, 120, 120, 120, 0.2, (P, P, P), 12, 0.106, 3200, 2176, 128, 2.0, 0.0, True, 256),
 }
 
 

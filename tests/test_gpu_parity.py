@@ -172,6 +172,11 @@ FUSION_GRIDS = [
     (100, 4, 114, (1, 1, 1), 0.106),
     (126, 4, 128, (0, 0, 0), 0.0),
     (8, 132, 6, (0, 0, 0), 0.106),      # y axis on the plain kernel, x and z fused
+    # nx == 8 (mod 16): the y passes run on 8-column half-chunk tiles (k_mode_t HC), ragged and exact y extents
+    (24, 20, 10, (0, 0, 0), 0.106),
+    (40, 36, 6, (0, 1, 0), 0.0),
+    (56, 64, 4, (1, 0, 0), 0.106),
+    (120, 26, 8, (0, 0, 1), 0.106),
 ]
 
 
@@ -191,7 +196,7 @@ def test_fused_passes_match_oracle_and_unfused(grid):
     plan = exx.Plan(nx, ny, nz, 0.3, bc, 12, omega, max_batch=32, device=0)
     d_psi, d_occ, d_C = torch.from_numpy(psi).cuda(), torch.from_numpy(occ).cuda(), torch.from_numpy(C).cuda()
     results = {}
-    for mask in (0, 1, 2, 3):
+    for mask in (0, 1, 2, 3, 4, 7):
         plan.set_fusion(mask)
         assert plan.fusion == mask
         for n_c in (3, 32):
