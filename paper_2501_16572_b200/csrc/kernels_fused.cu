@@ -629,7 +629,9 @@ inline int mtot_class(int n) {
   return need <= 2 ? 2 : need <= 4 ? 4 : need <= 6 ? 6 : need <= 8 ? 8 : need <= 12 ? 12 : need <= 15 ? 15 : 16;
 }
 
-// rows per warp tile (in units of 8) of k_mode_xacc: two accumulator sets have to fit the register file
+// rows per warp tile (in units of 8) of k_mode_xacc: two accumulator sets have to fit the register file.  (Sharing a
+// 16-row tile between two warps above n = 64 -- one ring per pair, a named barrier per stage -- was built and measured
+// in round 2: 1 % SLOWER at 96^3 and 120^3 than 8-row tiles.)
 inline int xacc_nt(int mtot) { return mtot <= 8 ? 2 : 1; }
 
 }  // namespace
