@@ -94,13 +94,16 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes);
 int exx_plan_get_lanes(const exx_plan* plan);
 
 /*
- * Pass fusion of the default variant (test and measurement hook; default 7 = all on).  Bit 0: the z-forward product,
+ * Pass fusion of the default variant (test and measurement hook; default 15 = all on).  Bit 0: the z-forward product,
  * the eigen-space multiply and the z-backward product of a batch (Eq. 11's third and fourth GEMM and Eq. 16,
  * PAPER.md:96-98, :134) run as ONE kernel, the intermediate staying in registers.  Bit 1: the x-backward product and
  * the accumulate of Eq. 1 run as one kernel; phi_jk is never written to memory and exx_apply shapes its
  * batches as nj occupied orbitals x nk targets with nk large enough to keep every SM busy.  Bit 2: where nx is 8
  * (mod 16) the y products tile their columns in half-chunks of 8 instead of chunks of 16, the last of which would be
- * half empty in every row.  With a bit off (or where
+ * half empty in every row.  Bit 3 (needs bit 0): the fused z pass contracts with the reflection-adapted eigenbasis of
+ * the z axis -- every eigenvector even or odd under z -> mir(z), DESIGN.md 6.9 -- so both of its products run over half
+ * the range with two half-size blocks: about 55 % of the multiply-adds of the dense products, same result to rounding
+ * (f(L) does not depend on the basis chosen inside a degenerate eigenspace).  With a bit off (or where
  * TMA cannot address the buffers, or an axis has more than 128 points) the separate passes run.  The result does not
  * depend on the mask beyond rounding (the sum over j is taken in ascending order either way).
  */
@@ -122,6 +125,18 @@ size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c);
 /* Test hook: copy out one axis' eigenpairs. h_lambda: n doubles; h_V: n*n doubles, column-major
  * (h_V[i + n*m] = component i of eigenvector m).  Either may be NULL. axis: 0=x, 1=y, 2=z. */
 exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, double* h_V);
+
+/* Test hook: the reflection-adapted eigenbasis of a real axis that the fused z pass contracts with (even vectors under
+ * z -> mir(z) first, *n_even of them, then the odd ones; each block in ascending eigenvalue order; same layout as
+ * exx_plan_get_axis).  mir(z) = (n - z) mod n on a periodic axis, n - 1 - z on a Dirichlet axis.  Host only.
+ * INVALID_ARG for a Bloch axis, EIGENSOLVE if the basis cannot be built. */
+exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h_lambda, double* h_V, int* n_even);
+
+/* Instrumentation: FP64 operations the mode products of ONE pair solve execute with the plan's current settings
+ * (padding not counted).  4 N (nx + ny + nz) -- the algorithmic count of the dense products -- unless an axis runs on the
+ * reflection-adapted basis (exx_plan_set_fusion bit 3), whose two products cost about half of that.  bench.py reports
+ * the roofline fraction in these executed operations, so that it cannot exceed 1. */
+double exx_plan_executed_flops_per_solve(const exx_plan* plan);
 
 /* Test hook: copy out the multiplier table, N doubles, entry [a + nx*(b + ny*c)] = m(lam_x[a]+lam_y[b]+lam_z[c]). */
 exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult);

@@ -129,7 +129,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false; p->accumulate = false;
-  p->fusion = 7;
+  p->fusion = 15;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
     p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
@@ -164,7 +164,8 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
       }
     }
     const double w0 = std::fabs(exx::fd_weights(fd_order, h)[0]);
-    p->h_mult = exx::multiplier_table(p->h_lam[0], p->h_lam[1], p->h_lam[2], omega, 1e-8 * 3.0 * w0);
+    p->zero_tol = 1e-8 * 3.0 * w0;
+    p->h_mult = exx::multiplier_table(p->h_lam[0], p->h_lam[1], p->h_lam[2], omega, p->zero_tol);
   } catch (const std::bad_alloc&) {
     delete p;
     return EXX_ERR_ALLOC;
@@ -272,7 +273,7 @@ exx_status exx_plan_set_lanes(exx_plan* plan, int lanes) {
 int exx_plan_get_lanes(const exx_plan* plan) { return plan ? plan->lanes : 0; }
 
 exx_status exx_plan_set_fusion(exx_plan* plan, int mask) {
-  if (!plan || mask < 0 || mask > 7) return EXX_ERR_INVALID_ARG;
+  if (!plan || mask < 0 || mask > 15) return EXX_ERR_INVALID_ARG;
   plan->fusion = mask;
   return EXX_OK;
 }
@@ -302,10 +303,30 @@ exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, d
   return EXX_OK;
 }
 
+exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h_lambda, double* h_V, int* n_even) {
+  if (!plan || axis < 0 || axis > 2 || !plan->h_Vi[axis].empty()) return EXX_ERR_INVALID_ARG;
+  const int n = plan->n[axis];
+  std::vector<double> lam_s, Vs;
+  int nh = 0;
+  if (!exx::symmetrize_axis(n, plan->bc[axis], plan->h_lam[axis], plan->h_V[axis], lam_s, Vs, &nh)) return EXX_ERR_EIGENSOLVE;
+  if (h_lambda) std::memcpy(h_lambda, lam_s.data(), sizeof(double) * n);
+  if (h_V)
+    for (int i = 0; i < n; ++i)
+      for (int m = 0; m < n; ++m) h_V[i + (size_t)n * m] = Vs[(size_t)i * n + m];
+  if (n_even) *n_even = nh;
+  return EXX_OK;
+}
+
 exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult) {
   if (!plan || !h_mult) return EXX_ERR_INVALID_ARG;
   std::memcpy(h_mult, plan->h_mult.data(), sizeof(double) * plan->N);
   return EXX_OK;
+}
+
+double exx_plan_executed_flops_per_solve(const exx_plan* plan) {
+  if (!plan) return 0.0;
+  if (plan->device < 0 || is_complex_plan(plan)) return 4.0 * (double)plan->N * (plan->n[0] + plan->n[1] + plan->n[2]);
+  return exx::fused_executed_flops_per_solve(plan);
 }
 
 long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }

@@ -20,6 +20,9 @@ bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::v
 // Hermitian Bloch-periodic axis (R18): K(theta) = V diag(lam) V^H, V = Vr + i Vi row-major [i][m].
 bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& Vr,
                 std::vector<double>& Vi);
+// Reflection-adapted eigenbasis of a real axis: even vectors first, then odd (plan_host.cpp); false if it cannot be built.
+bool symmetrize_axis(int n, int bc, const std::vector<double>& lam, const std::vector<double>& V, std::vector<double>& lam_s,
+                     std::vector<double>& Vs, int* n_even);
 // f(Lambda~) table (PAPER.md:61 Eq. 5, :134 Eq. 16; R1-R3), entry [a + nx*(b + ny*c)].
 std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
                                      const std::vector<double>& lz, double omega, double zero_tol);
@@ -51,6 +54,7 @@ struct exx_plan {
   double theta[3];
   std::vector<double> h_Vi[3];
   std::vector<double> h_mult;
+  double zero_tol;  // R3 threshold on |lam_sum| the table was built with
   // device copies
   double* d_Vi[3];   // Bloch plans: imaginary parts, same layout; nullptr for a real axis
   double* d_V[3];    // row-major [i][m], n*n (axes with identical matrices share one allocation)
@@ -189,6 +193,7 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
 cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);
+double fused_executed_flops_per_solve(const exx_plan* p);
 // ---- non-batch Eq. 8 solver, the Fig. 2 comparison line (kernels_nonbatch.cu) ----
 cudaError_t nonbatch_solve_one(exx_plan* p, const double* rhs, double* phi, double* buf0, double* buf1, cudaStream_t s,
                                long long* launches);

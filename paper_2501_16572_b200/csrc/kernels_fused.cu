@@ -320,6 +320,312 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// k_mode_zz_sym: k_mode_zz on the reflection-adapted eigenbasis of a real z axis (plan_host.cpp symmetrize_axis).
+// Every eigenvector of the periodic or Dirichlet 1-D matrix can be taken even or odd under z -> mir(z), so
+//     forward:   T[m] = sum_{z <= mir z} V[z][m] (f[z] +- f[mir z])        (+ for an even mode, - for an odd one)
+//     backward:  a[z] = sum_{m even} V[z][m] t[m],  b[z] = sum_{m odd} V[z][m] t[m],  y[z] = a + b,  y[mir z] = a - b
+// i.e. both products contract over HALF the range with two blocks of the matrix: about 55 % of the DMMAs of the dense
+// kernel (n = 120: 2 x 512 against 2 x 900 per 16 columns).  A stage is two TMA boxes, rows [16 s, 16 s + 16) and the
+// mirrored rows (row 15 - r of the second box is mir(16 s + r)); the butterfly f +- f[mir] happens on the fragments,
+// the a +- b one on the accumulators.  Row tiles 0..MS-1 of the first accumulator set belong to the even modes, MS..2MS-1
+// to the odd ones; the multiplier table is the plan's table with its z index in the same (even | odd) order.
+// Everything else (operand swap, register chaining, image column permutation, multiplier tile through the ring) is
+// k_mode_zz's.
+// ---------------------------------------------------------------------------------------------------------------
+struct ZSArgs {
+  double* out;
+  const double* V;  // image [16*Sh][16*MS+4]: row = half-range z (k_mode_t's L-mode order), columns sigma(even m) | 8 MS + sigma(odd m)
+  int n;
+  int nh;       // half range: number of z with z <= mir(z) = number of even modes
+  int Sh;       // stages of 16 half-range indices
+  int kk_last;  // ragged last stage (nh % 16 != 0): its k-steps
+  int mir0;     // first row of the mirrored box of stage 0 (stage s: mir0 - 16 s)
+  int mirc;     // mir(z) = mirc - z (periodic: n, with mir(0) = n read as "none"; Dirichlet: n - 1)
+  int zfix;     // z == mir(z) inside the array (its mirrored read is replaced by zero), or -1
+  unsigned n_tiles;
+  int inner, cpo, outer;
+  unsigned total_chunks;
+  FastDiv div_cpo;
+};
+
+template <int MS, int NT, int WARPS, int IC>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_zz_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const ZSArgs a) {
+  static_assert(NT == 2 || NT == 4, "a tile is one or two 16-column chunks");
+  static_assert(MS % IC == 0, "output row tiles are processed IC at a time");
+  constexpr int MT = 2 * MS;
+  constexpr int LDV = 8 * MT + 4;
+  constexpr unsigned kS1 = 1024u * NT;  // one box set (all chunks of a tile)
+  constexpr unsigned kSlot = 2u * kS1;  // a data stage: the rows and the mirrored rows
+  constexpr int CH = NT / 2;
+  constexpr int TS = (MS + 1) / 2;      // multiplier stages per block
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, Sh = a.Sh;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * Sh) * LDV;
+
+  for (unsigned i = 2 * tid; i < 16u * Sh * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kSlot);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kSlot) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kSlot) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+
+  // ---- producer: Sh data stages (rows + mirrored rows), TS multiplier stages for the even modes, TS for the odd ----
+  const int stages_per_tile = Sh + 2 * TS;
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pc0[CH], pc2[CH];
+  auto tile_coords = [&](unsigned t) {
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        pc2[ch] = (int)o;
+        pc0[ch] = 16 * (int)(cc - o * (unsigned)a.cpo);
+      } else {
+        pc2[ch] = a.outer;
+        pc0[ch] = 0;
+      }
+    }
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kSlot;
+    if (elect_one()) {
+      if (s_p < Sh) {
+        mbar_expect_tx(bar, kSlot);
+#pragma unroll
+        for (int ch = 0; ch < CH; ++ch) {
+          tma_load_3d(dst + 2048u * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
+          tma_load_3d(dst + kS1 + 2048u * ch, &tm0, pc0[ch], a.mir0 - 16 * s_p, pc2[ch], bar);
+        }
+      } else {
+        const int ts = s_p - Sh;
+        const int row = ts < TS ? 16 * ts : a.nh + 16 * (ts - TS);  // even modes: table rows 0.., odd modes: rows nh..
+        mbar_expect_tx(bar, kS1);
+#pragma unroll
+        for (int ch = 0; ch < CH; ++ch) tma_load_3d(dst + 2048u * ch, &tm1, pc0[ch], row, 0, bar);
+      }
+    }
+    if (++s_p == stages_per_tile) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  // ---- per-lane fragment addresses --------------------------------------------------------------------------
+  const unsigned b1 = (unsigned)(q >> 1);
+  unsigned v1_lane = smem0 + 8u * (q * LDV + (g ^ ((g >> 2) & 1)));
+  // data fragment of k-step kk, column tile nt: box row 2q + (kk&1) + 8(kk>>1); its mirror image is row 15 - that of
+  // the second box
+  unsigned xo[4], xm[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const unsigned row = 2u * q + (i & 1), rowm = 7u - row;
+    xo[i] = 128u * row + 16u * ((4u * (i >> 1) + (g >> 1)) ^ row) + 8u * (g & 1);
+    xm[i] = kS1 + 128u * rowm + 16u * ((4u * (i >> 1) + (g >> 1)) ^ rowm) + 8u * (g & 1);
+  }
+  unsigned tq[2][2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e)
+#pragma unroll
+    for (int np = 0; np < 2; ++np) {
+      const unsigned row = 2u * q + e;
+      tq[e][np] = 128u * row + 16u * ((4u * np + (g >> 1)) ^ row) + 8u * (g & 1);
+    }
+  unsigned v2_lane[2];
+  v2_lane[0] = smem0 + 8u * (g * LDV + 2u * q + b1);
+  v2_lane[1] = smem0 + 8u * (g * LDV + 2u * q + (1u ^ b1));
+  const int zo_std[2] = {4 * (q & 1) + (q >> 1), 4 * (q & 1) + 2 + (q >> 1)};
+  const int zo_lin[2] = {2 * q, 2 * q + 1};
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+
+    // ---- forward: acc[mt][nt][e] = T[mode 8(mt % MS) + 2q + e of block mt / MS][column 8nt + g] -----------------
+    for (int s = 0; s < Sh; ++s) {
+      asm volatile("" : "+r"(v1_lane), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kSlot;
+      const unsigned aa = v1_lane + (unsigned)s * (16u * LDV * 8u);
+      const int zf = a.zfix - 16 * s;  // local row whose mirror image is itself (its second read counts as zero)
+      const bool ragged = a.kk_last && s == Sh - 1;
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (!ragged || kk < a.kk_last) {
+          double be[NT], bo[NT];
+          const int rowl = ragged ? 4 * kk + q : 2 * q + (kk & 1) + 8 * (kk >> 1);
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            unsigned oa, ob;
+            if (!ragged) {
+              oa = sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1);
+              ob = sb + xm[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (1 - (kk >> 1));
+            } else {
+              const unsigned row = 4u * kk + q, rowm = 15u - row;
+              oa = sb + 2048u * (nt >> 1) + 128u * row + 16u * ((4u * (nt & 1) + (g >> 1)) ^ (row & 7u)) + 8u * (g & 1);
+              ob = sb + kS1 + 2048u * (nt >> 1) + 128u * rowm + 16u * ((4u * (nt & 1) + (g >> 1)) ^ (rowm & 7u)) + 8u * (g & 1);
+            }
+            const double va = lds64(oa);
+            double vb = lds64(ob);
+            if (rowl == zf) vb = 0.0;
+            be[nt] = va + vb;
+            bo[nt] = va - vb;
+          }
+          double af[MT];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], mt < MS ? be[nt] : bo[nt], af[mt]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+
+    // ---- eigen-space multiply: TS stages for the even block, TS for the odd block ---------------------------------
+#pragma unroll
+    for (int sp = 0; sp < 2 * TS; ++sp) {
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kSlot;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        constexpr int kZ = 0;
+        const int blk = sp < TS ? 0 : 1, mtl = 2 * (sp < TS ? sp : sp - TS) + h;  // compile-time after unrolling
+        if (mtl < MS) {
+          const int mt = blk * MS + mtl;
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+              acc[mt < MT ? mt : kZ][nt][e] *= lds64(sb + 2048u * (nt >> 1) + 1024u * h + tq[e][nt & 1]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+
+    // ---- backward: a = E t_even, b = O t_odd over the half range, IC row tiles at a time; y = a + b, y[mir] = a - b ---
+    int o_ch[CH], col_ch[CH];
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        o_ch[ch] = (int)o;
+        col_ch[ch] = 16 * (int)(cc - o * (unsigned)a.cpo) + g;
+      } else {
+        o_ch[ch] = 0;
+        col_ch[ch] = a.inner;
+      }
+    }
+#pragma unroll 1
+    for (int it0 = 0; it0 < MS; it0 += IC) {
+      double pa[IC][NT][2], pb[IC][NT][2];
+#pragma unroll
+      for (int ic = 0; ic < IC; ++ic)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) pa[ic][nt][0] = pa[ic][nt][1] = pb[ic][nt][0] = pb[ic][nt][1] = 0.0;
+      const unsigned wrow = (unsigned)it0 * (8u * LDV * 8u);
+#pragma unroll
+      for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          double w[IC];
+#pragma unroll
+          for (int ic = 0; ic < IC; ++ic) w[ic] = lds64(v2_lane[e] + wrow + (8u * ic * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int ic = 0; ic < IC; ++ic)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(mt < MS ? pa[ic][nt] : pb[ic][nt], acc[mt][nt][e], w[ic]);
+        }
+#pragma unroll
+      for (int ic = 0; ic < IC; ++ic) {
+        const int it = it0 + ic;
+        const bool lin = a.kk_last && (it >> 1) == Sh - 1;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int z = 8 * it + (lin ? zo_lin[e] : zo_std[e]);
+          if (z < a.nh) {
+            const int zb = a.mirc - z;
+            const bool two = zb != z && zb < n;
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              const int col = col_ch[nt >> 1] + 8 * (nt & 1);
+              if (col < a.inner) {
+                double* base = a.out + ((long long)o_ch[nt >> 1] * n) * a.inner + col;
+                base[(long long)z * a.inner] = pa[ic][nt][e] + pb[ic][nt][e];
+                if (two) base[(long long)zb * a.inner] = pa[ic][nt][e] - pb[ic][nt][e];
+              }
+            }
+          }
+        }
+      }
+    }
+
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // k_mode_xacc
 // ---------------------------------------------------------------------------------------------------------------
 struct XArgs {
@@ -615,6 +921,14 @@ cudaError_t launch_zz_c(const exx_plan* p, const CUtensorMap& m0, const CUtensor
                            p, m0, m1, a, s);
 }
 
+template <int MS, int NT, int WARPS, int IC>
+cudaError_t launch_zz_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const ZSArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  const size_t img = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4);
+  const size_t smem = img + 1024 + (size_t)WARPS * kDepth * 2 * 1024 * NT + (size_t)WARPS * kDepth * 8 + 16;
+  return launch_persistent(k_mode_zz_sym<MS, NT, WARPS, IC>, opt, smem, WARPS, a.n_tiles, p, m0, m1, a, s);
+}
+
 template <int MTOT, int NT, int WARPS>
 cudaError_t launch_xacc(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
@@ -651,9 +965,39 @@ cudaError_t fused_init(exx_plan* p) {
   if (!st) return cudaSuccess;
   st->d_img_zz = nullptr;
   st->d_img_zz_c = nullptr;
+  st->d_img_zzs = nullptr;
+  st->d_mult_zs = nullptr;
+  st->zs_nh = 0;
   const int n = p->n[2], mtot = mtot_class(n);
   if (!mtot) return cudaSuccess;
   const int S = (n + 15) / 16, ldv = 8 * mtot + 4;
+  if (p->h_Vi[2].empty() && p->h_Vi[0].empty() && p->h_Vi[1].empty()) {
+    // reflection-adapted basis of the z axis: image over the half range and the table in (even | odd) order
+    std::vector<double> lam_s, Vs;
+    int nh = 0;
+    if (symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh) && (nh + 7) / 8 <= 8) {
+      const int ms = (nh + 7) / 8, Sh = (nh + 15) / 16, lds = 16 * ms + 4;
+      std::vector<double> img((size_t)16 * Sh * lds, 0.0);
+      for (int s = 0; s < Sh; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int z = 16 * s + within_stage(false, nh, s, kk, q);
+            if (z >= nh) continue;
+            double* row = &img[(size_t)(16 * s + 4 * kk + q) * lds];
+            for (int m = 0; m < n; ++m) {
+              const int mm = m < nh ? m : m - nh;
+              row[(m < nh ? 0 : 8 * ms) + (mm ^ ((mm >> 2) & 1))] = Vs[(size_t)z * n + m];
+            }
+          }
+      const std::vector<double> tab = multiplier_table(p->h_lam[0], p->h_lam[1], lam_s, p->omega, p->zero_tol);
+      cudaError_t e = cudaMalloc(&st->d_img_zzs, sizeof(double) * img.size());
+      if (e == cudaSuccess) e = cudaMemcpy(st->d_img_zzs, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+      if (e == cudaSuccess) e = cudaMalloc(&st->d_mult_zs, sizeof(double) * tab.size());
+      if (e == cudaSuccess) e = cudaMemcpy(st->d_mult_zs, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+      st->zs_nh = nh;
+    }
+  }
   if (!p->h_Vi[2].empty()) {
     // complex z axis: E = [[Vr, -Vi], [Vi, Vr]], rows (plane, z) and columns (plane, m), same permutations per block
     if (mtot > 8) return cudaSuccess;
@@ -698,6 +1042,9 @@ void fused_destroy(exx_plan* p) {
   if (!st) return;
   if (st->d_img_zz) cudaFree(st->d_img_zz);
   if (st->d_img_zz_c) cudaFree(st->d_img_zz_c);
+  if (st->d_img_zzs) cudaFree(st->d_img_zzs);
+  if (st->d_mult_zs) cudaFree(st->d_mult_zs);
+  st->d_img_zzs = st->d_mult_zs = nullptr;
   st->d_img_zz = nullptr;
   st->d_img_zz_c = nullptr;
 }
@@ -711,6 +1058,46 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
   if (!mtot) return cudaErrorNotSupported;
   if ((p->n[0] & 1) || !aligned16(out) || !aligned16(in) || !aligned16(p->d_mult)) return cudaErrorNotSupported;
   const long long inner = (long long)p->n[0] * p->n[1];
+  // reflection-adapted basis: half the contraction range, two blocks.  Only where it pays: below nz = 66 (five row tiles
+  // per block) the two-box stages and the padding of the blocks to whole row tiles cost more than the saved DMMAs
+  // (48^3: -2 %)
+  if (st->d_img_zzs && (p->fusion & 8) && (st->zs_nh + 7) / 8 >= 5) {
+    const int nh = st->zs_nh, ms = (nh + 7) / 8;
+    const bool per = p->bc[2] == EXX_BC_PERIODIC;
+    ZSArgs z{};
+    z.out = out;
+    z.V = st->d_img_zzs;
+    z.n = n;
+    z.nh = nh;
+    z.Sh = (nh + 15) / 16;
+    z.kk_last = tail_ksteps(nh);
+    z.mir0 = per ? n - 15 : n - 16;
+    z.mirc = per ? n : n - 1;
+    z.zfix = per ? ((n % 2 == 0 && n >= 2) ? n / 2 : -1) : ((n % 2) ? (n - 1) / 2 : -1);
+    z.inner = (int)inner;
+    z.cpo = (int)((inner + 15) / 16);
+    const long long chunks = (long long)z.cpo * nb;
+    if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    z.total_chunks = (unsigned)chunks;
+    z.outer = nb;
+    z.div_cpo = make_fastdiv((unsigned)z.cpo);
+    CUtensorMap m0, m1;
+    cudaError_t e;
+    if ((e = get_map(st, in, inner, n, nb, 16, &m0)) != cudaSuccess) return e;
+    if ((e = get_map(st, st->d_mult_zs, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+    const int NT = ms <= 4 ? 4 : 2;
+    const int CH = NT / 2;
+    z.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+    if (z.n_tiles == 0) return cudaSuccess;
+    switch (ms) {
+      case 5: e = launch_zz_sym<5, 2, 12, 1>(p, m0, m1, z, s); break;
+      case 6: e = launch_zz_sym<6, 2, 12, 1>(p, m0, m1, z, s); break;
+      case 7: e = launch_zz_sym<7, 2, 12, 1>(p, m0, m1, z, s); break;
+      default: e = launch_zz_sym<8, 2, 12, 1>(p, m0, m1, z, s); break;
+    }
+    if (e == cudaSuccess) ++p->tma_launches;
+    if (e != cudaErrorNotSupported) return e;  // else: the dense fused kernel below
+  }
   ZArgs a{};
   a.out = out;
   a.V = st->d_img_zz;
@@ -742,6 +1129,27 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
     case 15: return launch_zz<15, 2, 12, 1>(p, m0, m1, a, s);
     default: return launch_zz<16, 2, 12, 1>(p, m0, m1, a, s);
   }
+}
+
+// FP64 operations one pair solve executes in the mode products when every buffer is TMA-addressable: 4 N n per dense
+// axis (two products, a multiply-add = 2, padding not counted); a z axis on the reflection-adapted basis contracts
+// nh even modes over nh points and n - nh odd modes over n - nh points per column and product, plus n butterfly
+// additions per column and product.
+double fused_executed_flops_per_solve(const exx_plan* p) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  double f = 0.0;
+  for (int ax = 0; ax < 3; ++ax) {
+    const double n = p->n[ax];
+    const bool sym = ax == 2 && st && st->d_img_zzs && (p->fusion & 8) && (p->fusion & 1) && (st->zs_nh + 7) / 8 >= 5 &&
+                     p->variant == EXX_VARIANT_FUSED_DMMA;
+    if (sym) {
+      const double nh = st->zs_nh, no = n - nh;
+      f += 4.0 * (nh * nh + no * no) * (double)p->N / n + 2.0 * (double)p->N;
+    } else {
+      f += 4.0 * (double)p->N * n;
+    }
+  }
+  return f;
 }
 
 // The same for nb complex functions ([nb][2][N] planes) of a Bloch plan whose z axis is complex with n <= 64, in place.

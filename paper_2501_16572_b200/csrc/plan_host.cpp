@@ -187,6 +187,88 @@ bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& l
   return kept == n;
 }
 
+// Reflection-adapted eigenbasis of a REAL axis (R13: f(L) does not depend on the basis chosen inside a
+// degenerate eigenspace).  The periodic matrix is circulant and symmetric, the Dirichlet one symmetric Toeplitz: both
+// commute with the reflection z -> mir(z) (periodic: (n - z) mod n, Dirichlet: n - 1 - z), so every eigenspace splits
+// into vectors that are even (v[mir z] = v[z]) or odd (v[mir z] = -v[z]) under it.  Output: the same eigenpairs
+// re-expressed in such a basis, EVEN vectors first (n_even of them = number of z with z <= mir z), each block in
+// ascending eigenvalue order; Vs row-major [z][m'].  A contraction with an even (odd) vector only needs the half range
+// z <= mir(z) of the symmetrised (antisymmetrised) data: half the multiply-adds of the dense product.
+bool symmetrize_axis(int n, int bc, const std::vector<double>& lam, const std::vector<double>& V, std::vector<double>& lam_s,
+                     std::vector<double>& Vs, int* n_even) {
+  auto mir = [&](int z) { return bc == EXX_BC_PERIODIC ? (n - z) % n : n - 1 - z; };
+  int nh = 0;
+  for (int z = 0; z < n; ++z) nh += z <= mir(z) ? 1 : 0;
+  double scale = 0.0;
+  for (int m = 0; m < n; ++m) scale = std::fmax(scale, std::fabs(lam[m]));
+  const double tol = 1e-9 * (scale > 0.0 ? scale : 1.0);
+  std::vector<std::vector<double>> ev, od;  // kept vectors
+  std::vector<double> ev_l, od_l;
+  int m0 = 0;
+  while (m0 < n) {  // clusters of (numerically) equal eigenvalues, lam ascending
+    int m1 = m0 + 1;
+    while (m1 < n && std::fabs(lam[m1] - lam[m0]) < tol) ++m1;
+    size_t ne0 = ev.size(), no0 = od.size();
+    for (int parity = 0; parity < 2; ++parity) {
+      auto& keep = parity ? od : ev;
+      auto& keep_l = parity ? od_l : ev_l;
+      const size_t first = parity ? no0 : ne0;
+      // parity parts of the cluster's vectors; keep them by decreasing norm (pivoted Gram-Schmidt): the parts of a
+      // vector that is nearly of the other parity are rounding noise and must not be normalised
+      std::vector<std::vector<double>> cand;
+      for (int m = m0; m < m1; ++m) {
+        std::vector<double> v(n);
+        for (int z = 0; z < n; ++z) {
+          const double a = V[(size_t)z * n + m], b = V[(size_t)mir(z) * n + m];
+          v[z] = 0.5 * (parity ? a - b : a + b);
+        }
+        cand.push_back(v);
+      }
+      while (!cand.empty()) {
+        size_t best = 0;
+        double best_n = -1.0;
+        for (size_t c = 0; c < cand.size(); ++c) {
+          std::vector<double>& v = cand[c];
+          for (int pass = 0; pass < 2; ++pass)
+            for (size_t k = first; k < keep.size(); ++k) {
+              double d = 0.0;
+              for (int z = 0; z < n; ++z) d += v[z] * keep[k][z];
+              for (int z = 0; z < n; ++z) v[z] -= d * keep[k][z];
+            }
+          double nrm = 0.0;
+          for (int z = 0; z < n; ++z) nrm += v[z] * v[z];
+          if (nrm > best_n) { best_n = nrm; best = c; }
+        }
+        if (best_n < 1e-3) break;  // what is left has no component of this parity (the squared norms sum to the dimension)
+        std::vector<double> v = cand[best];
+        cand.erase(cand.begin() + (long)best);
+        const double nrm = std::sqrt(best_n);
+        for (int z = 0; z < n; ++z) v[z] /= nrm;
+        for (int z = 0; z < n; ++z) {  // make the parity exact
+          const int zb = mir(z);
+          if (zb == z) { if (parity) v[z] = 0.0; }
+          else if (z < zb) { const double a = 0.5 * (v[z] + (parity ? -v[zb] : v[zb])); v[z] = a; v[zb] = parity ? -a : a; }
+        }
+        keep.push_back(v);
+        keep_l.push_back(lam[m0]);
+      }
+    }
+    if ((int)(ev.size() - ne0 + od.size() - no0) != m1 - m0) return false;  // the cluster did not split cleanly
+    m0 = m1;
+  }
+  if ((int)ev.size() != nh || (int)(ev.size() + od.size()) != n) return false;
+  lam_s.assign(n, 0.0);
+  Vs.assign((size_t)n * n, 0.0);
+  for (int m = 0; m < n; ++m) {
+    const bool is_ev = m < nh;
+    const std::vector<double>& v = is_ev ? ev[m] : od[m - nh];
+    lam_s[m] = is_ev ? ev_l[m] : od_l[m - nh];
+    for (int z = 0; z < n; ++z) Vs[(size_t)z * n + m] = v[z];
+  }
+  *n_even = nh;
+  return true;
+}
+
 std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
                                      const std::vector<double>& lz, double omega, double zero_tol) {
   const size_t nx = lx.size(), ny = ly.size(), nz = lz.size();

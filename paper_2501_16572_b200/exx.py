@@ -56,6 +56,10 @@ def load_library():
     lib.exx_plan_get_axis.argtypes = [vp, C.c_int, dp, dp]
     lib.exx_plan_get_multiplier.restype = C.c_int
     lib.exx_plan_get_multiplier.argtypes = [vp, dp]
+    lib.exx_plan_get_axis_symmetric.restype = C.c_int
+    lib.exx_plan_get_axis_symmetric.argtypes = [vp, C.c_int, dp, dp, C.POINTER(C.c_int)]
+    lib.exx_plan_executed_flops_per_solve.restype = C.c_double
+    lib.exx_plan_executed_flops_per_solve.argtypes = [vp]
     lib.exx_poisson_solve.restype = C.c_int
     lib.exx_poisson_solve.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
     lib.exx_poisson_solve_nonbatch.restype = C.c_int
@@ -219,6 +223,20 @@ class Plan:
         _check(self._lib.exx_plan_get_axis(self._h, axis, C.c_void_p(lam.ctypes.data), C.c_void_p(V.ctypes.data)),
                "exx_plan_get_axis")
         return lam, V
+
+    def get_axis_symmetric(self, axis: int):
+        """exx_plan_get_axis_symmetric: (lam, V, n_even) of the reflection-adapted eigenbasis (even vectors first)."""
+        n = (self.nx, self.ny, self.nz)[axis]
+        lam = np.empty(n)
+        V = np.empty((n, n), order="F")
+        ne = C.c_int(0)
+        _check(self._lib.exx_plan_get_axis_symmetric(self._h, axis, C.c_void_p(lam.ctypes.data), C.c_void_p(V.ctypes.data),
+                                                     C.byref(ne)), "exx_plan_get_axis_symmetric")
+        return lam, V, int(ne.value)
+
+    @property
+    def executed_flops_per_solve(self) -> float:
+        return float(self._lib.exx_plan_executed_flops_per_solve(self._h))
 
     def get_multiplier(self) -> np.ndarray:
         m = np.empty((self.nz, self.ny, self.nx))

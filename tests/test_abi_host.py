@@ -91,6 +91,32 @@ def test_library_planner_agrees_with_oracle_planner(lib, dims, bc, omega, h):
     p.close()
 
 
+@pytest.mark.parametrize("dims,bc,h", [((16, 12, 9), (0, 0, 1), 0.3), ((48, 60, 120), (0, 0, 1), 0.25), ((120, 96, 7), (0, 0, 0), 0.2),
+                                       ((5, 13, 126), (1, 1, 0), 0.4), ((1, 2, 3), (0, 0, 0), 0.5), ((2, 4, 128), (1, 1, 1), 0.5)])
+def test_reflection_adapted_eigenbasis(lib, dims, bc, h):
+    """exx_plan_get_axis_symmetric (the basis the fused z pass contracts with): the same eigenpairs as the
+    oracle's matrix, every vector EXACTLY even or odd under z -> mir(z), even block first with one vector per z <= mir(z),
+    and the spectral projector of every eigenvalue cluster equal to the one of the plain basis (so f(L) is unchanged)."""
+    nx, ny, nz = dims
+    p = exx.Plan(nx, ny, nz, h, bc, 12, 0.106, max_batch=4, device=-1)
+    scale = abs(orc.fd_weights(12, h)[0])
+    for ax, n in enumerate(dims):
+        lam0, V0 = p.get_axis(ax)
+        lam, V, ne = p.get_axis_symmetric(ax)
+        mir = np.array([(n - z) % n if bc[ax] == 0 else n - 1 - z for z in range(n)])
+        assert ne == int(np.sum(np.arange(n) <= mir))
+        assert np.all(V[mir, :ne] == V[:, :ne]) and np.all(V[mir, ne:] == -V[:, ne:])      # exact parity
+        assert np.all(np.diff(lam[:ne]) >= -1e-12 * scale) and np.all(np.diff(lam[ne:]) >= -1e-12 * scale)
+        assert np.allclose(np.sort(lam), lam0, rtol=0, atol=1e-12 * scale)
+        assert np.allclose(V.T @ V, np.eye(n), atol=1e-12)      # parity parts are renormalised: a decade above Jacobi's own
+        K = orc.second_derivative_matrix(n, h, bc[ax], 12)
+        assert np.allclose(K @ V, V * lam[None, :], rtol=0, atol=1e-12 * scale)
+        # any function of K is the same in both bases
+        f = lambda l: np.exp(l / scale)
+        assert np.allclose((V * f(lam)[None, :]) @ V.T, (V0 * f(lam0)[None, :]) @ V0.T, rtol=0, atol=1e-12)
+    p.close()
+
+
 @pytest.mark.parametrize("dims,bc,theta", [((16, 12, 9), (0, 0, 1), (0.7, -2.1, 0.5)), ((48, 48, 48), (0, 0, 0), (np.pi, 0.0, 1.0)),
                                            ((7, 60, 5), (1, 0, 0), (0.3, np.pi / 2, -np.pi))])
 def test_bloch_planner_agrees_with_bloch_oracle(lib, dims, bc, theta):

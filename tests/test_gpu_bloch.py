@@ -75,7 +75,7 @@ def test_bloch_solve_matches_oracle(case, variant):
         out0 = plan.poisson_solve_bloch(d, n_c=n_c)
         torch.cuda.synchronize()
         assert _rel(_cplx(out0), ref) < TOL
-        plan.set_fusion(7)
+        plan.set_fusion(15)
     if variant == exx.VARIANT_FUSED_DMMA and nx % 2 == 0:
         assert plan.tma_launch_count > 0          # the tensor-core kernels served it
     with pytest.raises(exx.ExxError):             # real entry points refuse a complex plan

@@ -177,6 +177,10 @@ FUSION_GRIDS = [
     (40, 36, 6, (0, 1, 0), 0.0),
     (56, 64, 4, (1, 0, 0), 0.106),
     (120, 26, 8, (0, 0, 1), 0.106),
+    # z axis on the reflection-adapted basis (k_mode_zz_sym), five row tiles per block: periodic even n (z = n/2 is its
+    # own mirror image), Dirichlet odd n (the middle point is)
+    (16, 4, 70, (0, 0, 0), 0.106),
+    (16, 4, 77, (0, 0, 1), 0.0),
 ]
 
 
@@ -196,7 +200,7 @@ def test_fused_passes_match_oracle_and_unfused(grid):
     plan = exx.Plan(nx, ny, nz, 0.3, bc, 12, omega, max_batch=32, device=0)
     d_psi, d_occ, d_C = torch.from_numpy(psi).cuda(), torch.from_numpy(occ).cuda(), torch.from_numpy(C).cuda()
     results = {}
-    for mask in (0, 1, 2, 3, 6, 7):
+    for mask in (0, 1, 2, 3, 6, 7, 9, 15):
         plan.set_fusion(mask)
         assert plan.fusion == mask
         for n_c in (3, 32):
