@@ -197,6 +197,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
       e = cudaMalloc(&p->ex.d_energy_scratch, sizeof(double) * kEnergyChunk * kEnergyBlocks);
     if (e == cudaSuccess) e = exx::fast_init(p);
     if (e == cudaSuccess) e = exx::tma_init(p);
+    if (e == cudaSuccess) e = exx::sym_init(p);
     if (e == cudaSuccess) e = exx::fused_init(p);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->lane_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
@@ -230,6 +231,7 @@ exx_status exx_plan_destroy(exx_plan* plan) {
     DeviceScope dev_scope(p->device);
     exx::fast_destroy(p);
     exx::fused_destroy(p);
+    exx::sym_destroy(p);
     exx::tma_destroy(p);
     if (p->lane_stream) cudaStreamDestroy(p->lane_stream);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);

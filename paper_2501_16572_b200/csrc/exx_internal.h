@@ -189,7 +189,12 @@ cudaError_t tma_mode_product_c(exx_plan* p, int axis, bool forward, double* buf,
 // ---- fused passes (kernels_fused.cu); cudaErrorNotSupported -> the unfused passes above ----
 cudaError_t fused_init(exx_plan* p);   // after tma_init
 void fused_destroy(exx_plan* p);       // before tma_destroy
-cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s);
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, bool sym = false);
+bool fused_sym_mode(const exx_plan* p);
+// y products on the reflection-adapted basis (kernels_sym.cu); sym_init after tma_init and before fused_init
+cudaError_t sym_init(exx_plan* p);
+void sym_destroy(exx_plan* p);
+cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s);
 cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);

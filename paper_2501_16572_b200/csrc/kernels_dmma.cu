@@ -508,6 +508,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   cudaError_t e;
   double *cur = work, *other = scratch;
   bool first_done = false, mult_pending = true;
+  const long long tma_before = p->tma_launches;
   if (fa) {
     // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
@@ -527,18 +528,32 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
     if (e != cudaSuccess) return e;
   }
   if (!first_done && (e = one_product(p, 0, true, src, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
-  if ((e = one_product(p, 1, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  // Symmetric mode: the y and z products on the reflection-adapted eigenbases, eigen-space data and
+  // table in (even | odd) mode order.  Decided once per batch: it needs every remaining pass on the TMA kernels, which
+  // the x-forward pass having run there (same buffer, same alignment rules) establishes.
+  const bool sym = fused_sym_mode(p) && p->tma_launches > tma_before && (((uintptr_t)cur) & 15) == 0;
+  auto y_product = [&](bool fwd) -> cudaError_t {
+    if (sym) {
+      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      const cudaError_t ey = sym_mode_product_y(p, fwd, cur, nb, s);
+      if (ey == cudaSuccess) return ey;
+      ps.cancel();
+      if (ey != cudaErrorNotSupported) return ey;  // NotSupported: the plan has no symmetric y axis, dense product below
+    }
+    return one_product(p, 1, fwd, cur, cur, other, nb, mult_pending, s);
+  };
+  if ((e = y_product(true)) != cudaSuccess) return e;
   // z-forward + multiplier + z-backward: one fused pass where k_mode_zz can run, else two passes
   e = cudaErrorNotSupported;
   if (p->variant == EXX_VARIANT_FUSED_DMMA) {
     ProfScope ps(p, KC_MODE_PRODUCT, s);
-    e = fused_zz(p, cur, cur, nb, s);
+    e = fused_zz(p, cur, cur, nb, s, sym);
     if (e != cudaSuccess) ps.cancel();
   }
   if (e == cudaSuccess) {
     mult_pending = false;
     *launches += 1;
-  } else if (e == cudaErrorNotSupported) {
+  } else if (e == cudaErrorNotSupported && !sym) {
     if ((e = one_product(p, 2, true, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
     if ((e = one_product(p, 2, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
     *launches += 2;
@@ -546,7 +561,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
     return e;
   }
   if (mult_pending) return cudaErrorUnknown;  // cannot happen: same axis, same support decision
-  if ((e = one_product(p, 1, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
+  if ((e = y_product(false)) != cudaSuccess) return e;
   *launches += 3;
   // x-backward + accumulate: one fused pass where k_mode_xacc can run
   if (fa && p->variant == EXX_VARIANT_FUSED_DMMA) {

@@ -966,16 +966,18 @@ cudaError_t fused_init(exx_plan* p) {
   st->d_img_zz = nullptr;
   st->d_img_zz_c = nullptr;
   st->d_img_zzs = nullptr;
-  st->d_mult_zs = nullptr;
+  st->d_mult_sym = nullptr;
   st->zs_nh = 0;
   const int n = p->n[2], mtot = mtot_class(n);
-  if (!mtot) return cudaSuccess;
-  const int S = (n + 15) / 16, ldv = 8 * mtot + 4;
   if (p->h_Vi[2].empty() && p->h_Vi[0].empty() && p->h_Vi[1].empty()) {
-    // reflection-adapted basis of the z axis: image over the half range and the table in (even | odd) order
+    // reflection-adapted basis of the z axis: image over the half range.  Only where it pays: below five row tiles per
+    // block (nz < 66) the two-box stages and the padding of the blocks to whole row tiles cost more than the saved
+    // DMMAs (measured at 48^3: -2 %).
     std::vector<double> lam_s, Vs;
     int nh = 0;
-    if (symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh) && (nh + 7) / 8 <= 8) {
+    const bool zcap = mtot && symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh) && (nh + 7) / 8 >= 5 &&
+                      (nh + 7) / 8 <= 8;
+    if (zcap) {
       const int ms = (nh + 7) / 8, Sh = (nh + 15) / 16, lds = 16 * ms + 4;
       std::vector<double> img((size_t)16 * Sh * lds, 0.0);
       for (int s = 0; s < Sh; ++s)
@@ -989,15 +991,21 @@ cudaError_t fused_init(exx_plan* p) {
               row[(m < nh ? 0 : 8 * ms) + (mm ^ ((mm >> 2) & 1))] = Vs[(size_t)z * n + m];
             }
           }
-      const std::vector<double> tab = multiplier_table(p->h_lam[0], p->h_lam[1], lam_s, p->omega, p->zero_tol);
       cudaError_t e = cudaMalloc(&st->d_img_zzs, sizeof(double) * img.size());
       if (e == cudaSuccess) e = cudaMemcpy(st->d_img_zzs, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
-      if (e == cudaSuccess) e = cudaMalloc(&st->d_mult_zs, sizeof(double) * tab.size());
-      if (e == cudaSuccess) e = cudaMemcpy(st->d_mult_zs, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
       if (e != cudaSuccess) return e;
       st->zs_nh = nh;
     }
+    if (zcap || st->ys_nh) {  // the table in the mode order of the symmetric pipeline
+      const std::vector<double> tab = multiplier_table(p->h_lam[0], st->ys_nh ? st->lam_ys : p->h_lam[1],
+                                                       zcap ? lam_s : p->h_lam[2], p->omega, p->zero_tol);
+      cudaError_t e = cudaMalloc(&st->d_mult_sym, sizeof(double) * tab.size());
+      if (e == cudaSuccess) e = cudaMemcpy(st->d_mult_sym, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return e;
+    }
   }
+  if (!mtot) return cudaSuccess;
+  const int S = (n + 15) / 16, ldv = 8 * mtot + 4;
   if (!p->h_Vi[2].empty()) {
     // complex z axis: E = [[Vr, -Vi], [Vi, Vr]], rows (plane, z) and columns (plane, m), same permutations per block
     if (mtot > 8) return cudaSuccess;
@@ -1043,25 +1051,26 @@ void fused_destroy(exx_plan* p) {
   if (st->d_img_zz) cudaFree(st->d_img_zz);
   if (st->d_img_zz_c) cudaFree(st->d_img_zz_c);
   if (st->d_img_zzs) cudaFree(st->d_img_zzs);
-  if (st->d_mult_zs) cudaFree(st->d_mult_zs);
-  st->d_img_zzs = st->d_mult_zs = nullptr;
+  if (st->d_mult_sym) cudaFree(st->d_mult_sym);
+  st->d_img_zzs = st->d_mult_sym = nullptr;
   st->d_img_zz = nullptr;
   st->d_img_zz_c = nullptr;
 }
 
 // z-forward product, multiplier and z-backward product of nb right-hand sides in one pass, in place or out of place.
 // cudaErrorNotSupported: the caller runs the two k_mode_t passes instead.
-cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s) {
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, bool sym) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st || !st->d_img_zz || !(p->fusion & 1)) return cudaErrorNotSupported;
   const int n = p->n[2], mtot = mtot_class(n);
   if (!mtot) return cudaErrorNotSupported;
   if ((p->n[0] & 1) || !aligned16(out) || !aligned16(in) || !aligned16(p->d_mult)) return cudaErrorNotSupported;
   const long long inner = (long long)p->n[0] * p->n[1];
-  // reflection-adapted basis: half the contraction range, two blocks.  Only where it pays: below nz = 66 (five row tiles
-  // per block) the two-box stages and the padding of the blocks to whole row tiles cost more than the saved DMMAs
-  // (48^3: -2 %)
-  if (st->d_img_zzs && (p->fusion & 8) && (st->zs_nh + 7) / 8 >= 5) {
+  // symmetric mode (the caller decides it for the whole batch): the z axis on its reflection-adapted basis where the plan
+  // has one, and in any case the table in the symmetric pipeline's mode order
+  const double* table = sym ? st->d_mult_sym : p->d_mult;
+  if (sym && !table) return cudaErrorInvalidValue;
+  if (sym && st->d_img_zzs) {
     const int nh = st->zs_nh, ms = (nh + 7) / 8;
     const bool per = p->bc[2] == EXX_BC_PERIODIC;
     ZSArgs z{};
@@ -1084,7 +1093,7 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
     CUtensorMap m0, m1;
     cudaError_t e;
     if ((e = get_map(st, in, inner, n, nb, 16, &m0)) != cudaSuccess) return e;
-    if ((e = get_map(st, st->d_mult_zs, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+    if ((e = get_map(st, table, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
     const int NT = ms <= 4 ? 4 : 2;
     const int CH = NT / 2;
     z.n_tiles = (unsigned)((chunks + CH - 1) / CH);
@@ -1114,7 +1123,7 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
   CUtensorMap m0, m1;
   cudaError_t e;
   if ((e = get_map(st, in, inner, n, nb, 16, &m0)) != cudaSuccess) return e;
-  if ((e = get_map(st, p->d_mult, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
+  if ((e = get_map(st, table, inner, n, 1, 16, &m1)) != cudaSuccess) return e;
   const int NT = mtot <= 8 ? 4 : 2;
   const int CH = NT / 2;
   a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
@@ -1137,19 +1146,28 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
 // additions per column and product.
 double fused_executed_flops_per_solve(const exx_plan* p) {
   const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  const bool sym = fused_sym_mode(p);
   double f = 0.0;
   for (int ax = 0; ax < 3; ++ax) {
     const double n = p->n[ax];
-    const bool sym = ax == 2 && st && st->d_img_zzs && (p->fusion & 8) && (p->fusion & 1) && (st->zs_nh + 7) / 8 >= 5 &&
-                     p->variant == EXX_VARIANT_FUSED_DMMA;
-    if (sym) {
-      const double nh = st->zs_nh, no = n - nh;
+    const int nh_ax = !sym ? 0 : ax == 2 ? st->zs_nh : ax == 1 ? st->ys_nh : 0;
+    if (nh_ax) {
+      const double nh = nh_ax, no = n - nh;
       f += 4.0 * (nh * nh + no * no) * (double)p->N / n + 2.0 * (double)p->N;
     } else {
       f += 4.0 * (double)p->N * n;
     }
   }
   return f;
+}
+
+// Whether a batch whose buffers TMA can address runs in symmetric mode: the fused z pass on, bit 3 on, a capable axis,
+// and (where the y images are in half-chunk row order) the half-chunk tiles on.
+bool fused_sym_mode(const exx_plan* p) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  if (!st || p->variant != EXX_VARIANT_FUSED_DMMA || (p->fusion & 9) != 9 || !st->d_mult_sym || !st->d_img_zz) return false;
+  if (st->ys_nh && st->ys_hc && !(p->fusion & 4)) return false;
+  return st->zs_nh || st->ys_nh;
 }
 
 // The same for nb complex functions ([nb][2][N] planes) of a Bloch plan whose z axis is complex with n <= 64, in place.

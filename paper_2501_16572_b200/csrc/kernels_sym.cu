@@ -1,0 +1,583 @@
+// Mode products of the y axis on the reflection-adapted eigenbasis (plan_host.cpp symmetrize_axis).
+// Every eigenvector of a real periodic or Dirichlet axis is even or odd under y -> mir(y), so
+//     forward  (k_mode_lf_sym):  T[m] = sum_{y <= mir y} V[y][m] (f[y] +- f[mir y])     (+: even mode, -: odd mode)
+//     backward (k_mode_lb_sym):  a[y] = sum_{m even} V[y][m] t[m],  b[y] = sum_{m odd} V[y][m] t[m],
+//                                out[y] = a + b,  out[mir y] = a - b
+// contract over half the range with two blocks of the matrix: about 55 % of the DMMAs of k_mode_t.  In eigen-space
+// the modes are stored even block first (nh modes), then the odd block; the plan's "symmetric" multiplier table uses the
+// same order.  Machinery as k_mode_t's L-mode (kernels_tma.cu): per-warp TMA rings, one persistent CTA per SM,
+// programmatic dependent launch, 16-column chunks or (HC) 8-column half-chunks.  The forward kernel's stage is two boxes,
+// rows [16 s, 16 s + 16) and the mirrored rows (row 15 - r of the second box is mir(16 s + r)).
+#include "tma_common.cuh"
+
+namespace exx {
+namespace {
+
+struct SArgs {
+  double* out;
+  const double* V;
+  int n;
+  int nh;               // even modes = half-range points
+  int Sh;               // forward: stages over the half range; backward: stages over the even modes
+  int So;               // backward: stages over the odd modes
+  int kk_last, kk_last_o;  // k-steps of the ragged last stage of the (even | half-range) block and of the odd block; 0: none
+  int mir0, mirc, zfix;    // as k_mode_zz_sym
+  unsigned n_tiles;
+  int inner, cpo, outer;
+  unsigned total_chunks;
+  FastDiv div_cpo;
+};
+
+// box-row offset of (k-step kk, lane) inside a stage, and of its mirror image 15 - r, for 16-column boxes (128-byte rows,
+// 128-byte swizzle; np = which 8-column half) and for 8-column boxes (64-byte rows, 64-byte swizzle)
+__device__ __forceinline__ unsigned off16(unsigned r, unsigned np, unsigned g) {
+  return 128u * r + 16u * ((4u * np + (g >> 1)) ^ (r & 7u)) + 8u * (g & 1);
+}
+__device__ __forceinline__ unsigned off8(unsigned r, unsigned g) {
+  return 64u * r + 16u * ((g >> 1) ^ ((r >> 1) & 3u)) + 8u * (g & 1);
+}
+template <bool HC>
+__device__ __forceinline__ unsigned row_of(int kk, int q, bool ragged) {
+  if (ragged) return 4u * kk + q;
+  return HC ? (unsigned)((q & 1) + 4 * (q >> 1) + 2 * (kk & 1) + 8 * (kk >> 1)) : (unsigned)(2 * q + (kk & 1) + 8 * (kk >> 1));
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// forward
+// ---------------------------------------------------------------------------------------------------------------
+template <int MS, int NT, int WARPS, bool HC>
+__global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lf_sym(const __grid_constant__ CUtensorMap tm0, const SArgs a) {
+  constexpr int MT = 2 * MS;
+  constexpr int LDV = 8 * MT + 4;
+  constexpr unsigned kS1 = 1024u * NT;
+  constexpr unsigned kSlot = 2u * kS1;
+  constexpr int CH = HC ? NT : NT / 2;
+  constexpr int CW = HC ? 8 : 16;
+  constexpr unsigned kBox = HC ? 1024u : 2048u;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, Sh = a.Sh;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * Sh) * LDV;
+  for (unsigned i = 2 * tid; i < 16u * Sh * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kSlot);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kSlot) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kSlot) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pc0[CH], pc2[CH];
+  auto tile_coords = [&](unsigned t) {
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        pc2[ch] = (int)o;
+        pc0[ch] = CW * (int)(cc - o * (unsigned)a.cpo);
+      } else {
+        pc2[ch] = a.outer;
+        pc0[ch] = 0;
+      }
+    }
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kSlot;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kSlot);
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) {
+        tma_load_3d(dst + kBox * ch, &tm0, pc0[ch], 16 * s_p, pc2[ch], bar);
+        tma_load_3d(dst + kS1 + kBox * ch, &tm0, pc0[ch], a.mir0 - 16 * s_p, pc2[ch], bar);
+      }
+    }
+    if (++s_p == Sh) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  // standard stages: offsets of this lane's row and of its mirror image; HC: index kk; else index 2 (nt&1) + (kk&1)
+  unsigned xo[4], xm[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (HC) {
+      const unsigned r = row_of<true>(i, q, false);
+      xo[i] = off8(r, g);
+      xm[i] = kS1 + off8(15u - r, g);
+    } else {
+      const unsigned r = 2u * q + (i & 1);  // rows 0..7; k-steps 2, 3 add 8 rows
+      xo[i] = off16(r, i >> 1, g);
+      xm[i] = kS1 + off16(7u - r, i >> 1, g);
+    }
+  }
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+    for (int s = 0; s < Sh; ++s) {
+      asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kSlot;
+      const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+      const int zf = a.zfix - 16 * s;
+      const bool ragged = a.kk_last && s == Sh - 1;
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (!ragged || kk < a.kk_last) {
+          double be[NT], bo[NT];
+          const int rowl = (int)row_of<HC>(kk, q, ragged);
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            unsigned oa, ob;
+            if (HC) {
+              if (!ragged) {
+                oa = sb + 1024u * nt + xo[kk];
+                ob = sb + 1024u * nt + xm[kk];
+              } else {
+                oa = sb + 1024u * nt + off8((unsigned)rowl, g);
+                ob = sb + kS1 + 1024u * nt + off8(15u - (unsigned)rowl, g);
+              }
+            } else {
+              if (!ragged) {
+                oa = sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1);
+                ob = sb + xm[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (1 - (kk >> 1));
+              } else {
+                oa = sb + 2048u * (nt >> 1) + off16((unsigned)rowl, nt & 1, g);
+                ob = sb + kS1 + 2048u * (nt >> 1) + off16(15u - (unsigned)rowl, nt & 1, g);
+              }
+            }
+            const double va = lds64(oa);
+            double vb = lds64(ob);
+            if (rowl == zf) vb = 0.0;
+            be[nt] = va + vb;
+            bo[nt] = va - vb;
+          }
+          double af[MT];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], mt < MS ? be[nt] : bo[nt]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+    // epilogue: C[mode 8 (mt % MS) + g of block mt / MS][column 8nt + 2q + e]; even modes -> rows 0.., odd modes -> rows nh..
+    const long long rstep = a.inner;
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        const int col0 = CW * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
+        double* base = a.out + (long long)o * n * a.inner + col0;
+        const bool in0 = col0 < a.inner, in1 = !HC && col0 + 8 < a.inner;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+          const int blk = mt >= MS ? 1 : 0;
+          const int ml = 8 * (mt - blk * MS) + g;
+          if (ml < (blk ? n - a.nh : a.nh)) {
+            double* ptr = base + (long long)(blk * a.nh + ml) * rstep;
+            if (HC) {
+              if (in0) stg_v2(ptr, acc[mt][ch][0], acc[mt][ch][1]);
+            } else {
+              if (in0) stg_v2(ptr, acc[mt][2 * ch < NT ? 2 * ch : 0][0], acc[mt][2 * ch < NT ? 2 * ch : 0][1]);
+              if (in1) stg_v2(ptr + 8, acc[mt][2 * ch + 1 < NT ? 2 * ch + 1 : 0][0], acc[mt][2 * ch + 1 < NT ? 2 * ch + 1 : 0][1]);
+            }
+          }
+        }
+      }
+    }
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// backward
+// ---------------------------------------------------------------------------------------------------------------
+template <int MS, int NT, int WARPS, bool HC>
+__global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lb_sym(const __grid_constant__ CUtensorMap tm0, const SArgs a) {
+  constexpr int LDV = 8 * MS + 4;
+  constexpr unsigned kS1 = 1024u * NT;
+  constexpr int CH = HC ? NT : NT / 2;
+  constexpr int CW = HC ? 8 : 16;
+  constexpr unsigned kBox = HC ? 1024u : 2048u;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, SE = a.Sh, ST = a.Sh + a.So;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * ST) * LDV;
+  for (unsigned i = 2 * tid; i < 16u * ST * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kS1);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kS1) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kS1) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pc0[CH], pc2[CH];
+  auto tile_coords = [&](unsigned t) {
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        pc2[ch] = (int)o;
+        pc0[ch] = CW * (int)(cc - o * (unsigned)a.cpo);
+      } else {
+        pc2[ch] = a.outer;
+        pc0[ch] = 0;
+      }
+    }
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kS1;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kS1);
+      const int row = s_p < SE ? 16 * s_p : a.nh + 16 * (s_p - SE);  // even modes: rows 0.., odd modes: rows nh..
+#pragma unroll
+      for (int ch = 0; ch < CH; ++ch) tma_load_3d(dst + kBox * ch, &tm0, pc0[ch], row, pc2[ch], bar);
+    }
+    if (++s_p == ST) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (HC) xo[i] = off8(row_of<true>(i, q, false), g);
+    else xo[i] = off16(2u * q + (i & 1), i >> 1, g);
+  }
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    double pa[MS][NT][2], pb[MS][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
+    auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+      asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kS1;
+      const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (!ragged || kk < kk_last) {
+          double bf[NT];
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            unsigned off;
+            if (HC) off = sb + 1024u * nt + (ragged ? off8(4u * kk + q, g) : xo[kk]);
+            else off = ragged ? sb + 2048u * (nt >> 1) + off16(4u * kk + q, nt & 1, g)
+                              : sb + xo[2 * (nt & 1) + (kk & 1)] + 2048u * (nt >> 1) + 1024u * (kk >> 1);
+            bf[nt] = lds64(off);
+          }
+          double af[MS];
+#pragma unroll
+          for (int mt = 0; mt < MS; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    };
+    for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
+    for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+
+    // epilogue: out[y] = a + b, out[mir y] = a - b for the half-range rows y = 8mt + g
+#pragma unroll
+    for (int ch = 0; ch < CH; ++ch) {
+      const unsigned cc = t * CH + ch;
+      if (cc < a.total_chunks) {
+        const unsigned o = fast_div(cc, a.div_cpo);
+        const int col0 = CW * (int)(cc - o * (unsigned)a.cpo) + 2 * q;
+        double* base = a.out + (long long)o * n * a.inner + col0;
+        const bool in0 = col0 < a.inner, in1 = !HC && col0 + 8 < a.inner;
+#pragma unroll
+        for (int mt = 0; mt < MS; ++mt) {
+          const int y = 8 * mt + g;
+          if (y < a.nh) {
+            const int yb = a.mirc - y;
+            const bool two = yb != y && yb < n;
+            double* p0 = base + (long long)y * a.inner;
+            double* p1 = base + (long long)yb * a.inner;
+            constexpr int kZ = 0;
+            const int n0 = HC ? ch : (2 * ch < NT ? 2 * ch : kZ), n1 = HC ? kZ : (2 * ch + 1 < NT ? 2 * ch + 1 : kZ);
+            if (in0) {
+              stg_v2(p0, pa[mt][n0][0] + pb[mt][n0][0], pa[mt][n0][1] + pb[mt][n0][1]);
+              if (two) stg_v2(p1, pa[mt][n0][0] - pb[mt][n0][0], pa[mt][n0][1] - pb[mt][n0][1]);
+            }
+            if (in1) {
+              stg_v2(p0 + 8, pa[mt][n1][0] + pb[mt][n1][0], pa[mt][n1][1] + pb[mt][n1][1]);
+              if (two) stg_v2(p1 + 8, pa[mt][n1][0] - pb[mt][n1][0], pa[mt][n1][1] - pb[mt][n1][1]);
+            }
+          }
+        }
+      }
+    }
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+
+template <typename Kern>
+cudaError_t launch_sym(Kern kern, SmemOptIn& opt, size_t smem, int warps, const exx_plan* p, const CUtensorMap& m0,
+                       const SArgs& a, cudaStream_t s) {
+  const size_t floor_bytes = 117 * 1024;  // exactly one CTA per SM
+  if (smem < floor_bytes) smem = floor_bytes;
+  if (smem > (size_t)p->smem_optin) return cudaErrorNotSupported;
+  cudaError_t e = opt.ensure(kern, p->device, smem, true);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  const unsigned grid = a.n_tiles < (unsigned)p->sm_count ? a.n_tiles : (unsigned)p->sm_count;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * warps);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, m0, a);
+}
+
+template <int MS, bool HC>
+cudaError_t launch_lf(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 12, NT = 2;
+  const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym(k_mode_lf_sym<MS, NT, W, HC>, opt, smem, W, p, m0, a, s);
+}
+template <int MS, bool HC>
+cudaError_t launch_lb(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 12, NT = 2;
+  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 1024 * NT +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym(k_mode_lb_sym<MS, NT, W, HC>, opt, smem, W, p, m0, a, s);
+}
+
+}  // namespace
+
+// Images of the y axis on the reflection-adapted basis; `hc`: row order of the half-chunk tiles.  Forward: rows = half
+// range (k_mode_t's L-mode stage order), columns = even modes | 8 MS + odd modes.  Backward: rows = even modes in stages
+// of 16, then odd modes in stages of 16, columns = half-range points.
+cudaError_t sym_init(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return cudaSuccess;
+  st->d_img_yf = st->d_img_yb = nullptr;
+  st->ys_nh = 0;
+  if (!p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty()) return cudaSuccess;
+  const int n = p->n[1];
+  if (n > 128 || (p->n[0] & 1)) return cudaSuccess;
+  int nh = 0;
+  if (!symmetrize_axis(n, p->bc[1], p->h_lam[1], p->h_V[1], st->lam_ys, st->V_ys, &nh)) return cudaSuccess;
+  const int ms = (nh + 7) / 8;
+  if (ms < 5 || ms > 8) return cudaSuccess;
+  const bool hc = p->n[0] % 16 == 8;
+  const int no = n - nh, Sh = (nh + 15) / 16, So = (no + 15) / 16;
+  const std::vector<double>& Vs = st->V_ys;
+  {
+    const int ld = 16 * ms + 4;
+    std::vector<double> img((size_t)16 * Sh * ld, 0.0);
+    for (int s = 0; s < Sh; ++s)
+      for (int kk = 0; kk < 4; ++kk)
+        for (int q = 0; q < 4; ++q) {
+          const int y = 16 * s + within_stage(false, nh, s, kk, q, hc);
+          if (y >= nh) continue;
+          double* row = &img[(size_t)(16 * s + 4 * kk + q) * ld];
+          for (int m = 0; m < n; ++m) row[m < nh ? m : 8 * ms + (m - nh)] = Vs[(size_t)y * n + m];
+        }
+    cudaError_t e = cudaMalloc(&st->d_img_yf, sizeof(double) * img.size());
+    if (e == cudaSuccess) e = cudaMemcpy(st->d_img_yf, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
+  {
+    const int ld = 8 * ms + 4;
+    std::vector<double> img((size_t)16 * (Sh + So) * ld, 0.0);
+    for (int blk = 0; blk < 2; ++blk) {
+      const int cnt = blk ? no : nh, S = blk ? So : Sh, row0 = blk ? 16 * Sh : 0;
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int m = 16 * s + within_stage(false, cnt, s, kk, q, hc);
+            if (m >= cnt) continue;
+            double* row = &img[(size_t)(row0 + 16 * s + 4 * kk + q) * ld];
+            for (int y = 0; y < nh; ++y) row[y] = Vs[(size_t)y * n + (blk ? nh + m : m)];
+          }
+    }
+    cudaError_t e = cudaMalloc(&st->d_img_yb, sizeof(double) * img.size());
+    if (e == cudaSuccess) e = cudaMemcpy(st->d_img_yb, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
+  st->ys_nh = nh;
+  st->ys_hc = hc;
+  return cudaSuccess;
+}
+
+void sym_destroy(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st) return;
+  if (st->d_img_yf) cudaFree(st->d_img_yf);
+  if (st->d_img_yb) cudaFree(st->d_img_yb);
+  st->d_img_yf = st->d_img_yb = nullptr;
+}
+
+// y product of nb right-hand sides on the reflection-adapted basis, in place.  The caller has established that the whole
+// batch runs in "symmetric" mode (sym_axis_capable(p, 1) and TMA-addressable buffers).
+cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!st || !st->ys_nh || !aligned16(buf)) return cudaErrorNotSupported;
+  const int n = p->n[1], nh = st->ys_nh, no = n - nh, ms = (nh + 7) / 8;
+  const bool per = p->bc[1] == EXX_BC_PERIODIC, hc = st->ys_hc;
+  const long long inner = p->n[0], outer = (long long)p->n[2] * nb;
+  SArgs a{};
+  a.out = buf;
+  a.V = forward ? st->d_img_yf : st->d_img_yb;
+  a.n = n;
+  a.nh = nh;
+  a.Sh = (nh + 15) / 16;
+  a.So = (no + 15) / 16;
+  a.kk_last = tail_ksteps(nh);
+  a.kk_last_o = tail_ksteps(no);
+  a.mir0 = per ? n - 15 : n - 16;
+  a.mirc = per ? n : n - 1;
+  a.zfix = per ? ((n % 2 == 0 && n >= 2) ? n / 2 : -1) : ((n % 2) ? (n - 1) / 2 : -1);
+  const int cw = hc ? 8 : 16;
+  a.inner = (int)inner;
+  a.cpo = (int)((inner + cw - 1) / cw);
+  const long long chunks = (long long)a.cpo * outer;
+  if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.total_chunks = (unsigned)chunks;
+  a.outer = (int)outer;
+  a.div_cpo = make_fastdiv((unsigned)a.cpo);
+  const int CH = hc ? 2 : 1;
+  a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0;
+  cudaError_t e;
+  if ((e = get_map(st, buf, inner, n, outer, 16, &m0, cw)) != cudaSuccess) return e;
+  ++p->tma_launches;
+#define EXX_SYM_CASE(MSV)                                                                       \
+  case MSV:                                                                                     \
+    if (forward) return hc ? launch_lf<MSV, true>(p, m0, a, s) : launch_lf<MSV, false>(p, m0, a, s); \
+    return hc ? launch_lb<MSV, true>(p, m0, a, s) : launch_lb<MSV, false>(p, m0, a, s);
+  switch (ms) {
+    EXX_SYM_CASE(5)
+    EXX_SYM_CASE(6)
+    EXX_SYM_CASE(7)
+    default:
+      if (forward) return hc ? launch_lf<8, true>(p, m0, a, s) : launch_lf<8, false>(p, m0, a, s);
+      return hc ? launch_lb<8, true>(p, m0, a, s) : launch_lb<8, false>(p, m0, a, s);
+  }
+#undef EXX_SYM_CASE
+}
+
+}  // namespace exx

@@ -33,11 +33,17 @@ struct TmaState {
   double* d_img_im[3][2];  // Bloch plans: images of the imaginary parts, forward = Im(V^H) = -Vi^T, backward = Vi
   double* d_img_c[3][2];   // Bloch axes with n <= 64: real embedding [[Mr, -Mi], [Mi, Mr]] for the single-launch complex product
   double* d_img_hc[2];     // y axis, nx == 8 (mod 16): L-mode images in the row order of the half-chunk tiles (HC)
-  // reflection-adapted z axis (k_mode_zz_sym): image over the half range, multiplier table with its z index in
-  // (even | odd) order, number of even modes
+  // reflection-adapted eigenbases ("symmetric mode").  z axis (k_mode_zz_sym): image over the half range,
+  // number of even modes (0: not capable).  y axis (kernels_sym.cu): forward and backward images, their row order (hc),
+  // the basis itself.  d_mult_sym: the multiplier table with the eigen index of every capable axis in (even | odd) order.
   double* d_img_zzs;
-  double* d_mult_zs;
   int zs_nh;
+  double* d_img_yf;
+  double* d_img_yb;
+  int ys_nh;
+  bool ys_hc;
+  std::vector<double> lam_ys, V_ys;
+  double* d_mult_sym;
   double* d_img_zz_c;      // the same for a complex z axis with n <= 64 (embedding E = [[Vr, -Vi], [Vi, Vr]])
   double* d_img_zz;  // fused z-forward/z-backward kernel: one image of Vz serving both products (kernels_fused.cu)
   std::vector<MapEntry> cache;

@@ -181,6 +181,12 @@ FUSION_GRIDS = [
     # own mirror image), Dirichlet odd n (the middle point is)
     (16, 4, 70, (0, 0, 0), 0.106),
     (16, 4, 77, (0, 0, 1), 0.0),
+    # y axis on the reflection-adapted basis (k_mode_lf_sym / k_mode_lb_sym): 16-column chunks and half-chunks, periodic
+    # and Dirichlet, with and without a symmetric z axis
+    (16, 70, 4, (0, 0, 0), 0.106),
+    (24, 77, 4, (0, 1, 0), 0.0),
+    (40, 126, 5, (1, 0, 0), 0.106),
+    (16, 120, 70, (0, 0, 1), 0.106),
 ]
 
 
