@@ -128,7 +128,8 @@ exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, d
 
 /* Test hook: the reflection-adapted eigenbasis of a real axis that the fused z pass contracts with (even vectors under
  * z -> mir(z) first, *n_even of them, then the odd ones; each block in ascending eigenvalue order; same layout as
- * exx_plan_get_axis).  mir(z) = (n - z) mod n on a periodic axis, n - 1 - z on a Dirichlet axis.  Host only.
+ * exx_plan_get_axis).  mir(z) = n - 1 - z on either kind of axis (a symmetric circulant matrix commutes with every
+ * reflection, a symmetric Toeplitz one with this one).  Host only.
  * INVALID_ARG for a Bloch axis, EIGENSOLVE if the basis cannot be built. */
 exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h_lambda, double* h_V, int* n_even);
 

@@ -310,7 +310,7 @@ exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h
   const int n = plan->n[axis];
   std::vector<double> lam_s, Vs;
   int nh = 0;
-  if (!exx::symmetrize_axis(n, plan->bc[axis], plan->h_lam[axis], plan->h_V[axis], lam_s, Vs, &nh)) return EXX_ERR_EIGENSOLVE;
+  if (!exx::symmetrize_axis(n, plan->bc[axis], plan->h_lam[axis], plan->h_V[axis], lam_s, Vs, &nh, true)) return EXX_ERR_EIGENSOLVE;
   if (h_lambda) std::memcpy(h_lambda, lam_s.data(), sizeof(double) * n);
   if (h_V)
     for (int i = 0; i < n; ++i)

@@ -22,7 +22,7 @@ bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& l
                 std::vector<double>& Vi);
 // Reflection-adapted eigenbasis of a real axis: even vectors first, then odd (plan_host.cpp); false if it cannot be built.
 bool symmetrize_axis(int n, int bc, const std::vector<double>& lam, const std::vector<double>& V, std::vector<double>& lam_s,
-                     std::vector<double>& Vs, int* n_even);
+                     std::vector<double>& Vs, int* n_even, bool centered = false);
 // f(Lambda~) table (PAPER.md:61 Eq. 5, :134 Eq. 16; R1-R3), entry [a + nx*(b + ny*c)].
 std::vector<double> multiplier_table(const std::vector<double>& lx, const std::vector<double>& ly,
                                      const std::vector<double>& lz, double omega, double zero_tol);
@@ -189,12 +189,16 @@ cudaError_t tma_mode_product_c(exx_plan* p, int axis, bool forward, double* buf,
 // ---- fused passes (kernels_fused.cu); cudaErrorNotSupported -> the unfused passes above ----
 cudaError_t fused_init(exx_plan* p);   // after tma_init
 void fused_destroy(exx_plan* p);       // before tma_destroy
-cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, bool sym = false);
+// sym: 0 = plain mode order and table, 1 = symmetric mode (y, z), 2 = symmetric mode with the x axis too
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, int sym = 0);
 bool fused_sym_mode(const exx_plan* p);
 // y products on the reflection-adapted basis (kernels_sym.cu); sym_init after tma_init and before fused_init
 cudaError_t sym_init(exx_plan* p);
 void sym_destroy(exx_plan* p);
 cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s);
+bool sym_x_usable(const exx_plan* p, const double* work, const FastArgs* fa);
+cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStream_t s);
+cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);

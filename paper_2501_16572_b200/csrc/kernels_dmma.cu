@@ -509,12 +509,19 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   double *cur = work, *other = scratch;
   bool first_done = false, mult_pending = true;
   const long long tma_before = p->tma_launches;
+  // symmetric mode with the x axis: both x passes of the exchange apply on the reflection-adapted basis (decided here,
+  // before the first pass writes the batch in that mode order)
+  bool xsym = fa && fused_sym_mode(p) && sym_x_usable(p, cur, fa);
   if (fa) {
     // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
       ProfScope ps(p, KC_MODE_PRODUCT, s);
       e = cudaErrorNotSupported;
-      if (p->variant == EXX_VARIANT_FUSED_DMMA) e = tma_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
+      if (xsym) {
+        e = sym_xf(p, cur, nb, fa, s);
+        if (e == cudaErrorNotSupported) xsym = false;
+      }
+      if (!xsym && p->variant == EXX_VARIANT_FUSED_DMMA) e = tma_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
       if (e == cudaErrorNotSupported) e = fast_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
     }
     if (e == cudaSuccess) {
@@ -547,7 +554,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   e = cudaErrorNotSupported;
   if (p->variant == EXX_VARIANT_FUSED_DMMA) {
     ProfScope ps(p, KC_MODE_PRODUCT, s);
-    e = fused_zz(p, cur, cur, nb, s, sym);
+    e = fused_zz(p, cur, cur, nb, s, xsym ? 2 : sym ? 1 : 0);
     if (e != cudaSuccess) ps.cancel();
   }
   if (e == cudaSuccess) {
@@ -567,7 +574,8 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   if (fa && p->variant == EXX_VARIANT_FUSED_DMMA) {
     {
       ProfScope ps(p, KC_MODE_PRODUCT, s);
-      e = fused_xacc(p, cur, nb, fa, s);
+      e = xsym ? sym_xacc(p, cur, nb, fa, s) : fused_xacc(p, cur, nb, fa, s);
+      if (xsym && e == cudaErrorNotSupported) e = cudaErrorUnknown;  // the batch is in x-symmetric order: no fallback
       if (e != cudaSuccess) ps.cancel();
     }
     if (e == cudaSuccess) {

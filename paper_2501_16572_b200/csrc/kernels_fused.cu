@@ -975,7 +975,7 @@ cudaError_t fused_init(exx_plan* p) {
     // DMMAs (measured at 48^3: -2 %).
     std::vector<double> lam_s, Vs;
     int nh = 0;
-    const bool zcap = mtot && symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh) && (nh + 7) / 8 >= 5 &&
+    const bool zcap = mtot && symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh, true) && (nh + 7) / 8 >= 5 &&
                       (nh + 7) / 8 <= 8;
     if (zcap) {
       const int ms = (nh + 7) / 8, Sh = (nh + 15) / 16, lds = 16 * ms + 4;
@@ -996,12 +996,15 @@ cudaError_t fused_init(exx_plan* p) {
       if (e != cudaSuccess) return e;
       st->zs_nh = nh;
     }
-    if (zcap || st->ys_nh) {  // the table in the mode order of the symmetric pipeline
-      const std::vector<double> tab = multiplier_table(p->h_lam[0], st->ys_nh ? st->lam_ys : p->h_lam[1],
-                                                       zcap ? lam_s : p->h_lam[2], p->omega, p->zero_tol);
-      cudaError_t e = cudaMalloc(&st->d_mult_sym, sizeof(double) * tab.size());
-      if (e == cudaSuccess) e = cudaMemcpy(st->d_mult_sym, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
-      if (e != cudaSuccess) return e;
+    if (zcap || st->ys_nh || st->xs_nh) {  // the tables in the mode order of the symmetric pipeline, without and with x
+      for (int withx = 0; withx < (st->xs_nh ? 2 : 1); ++withx) {
+        const std::vector<double> tab = multiplier_table(withx ? st->lam_xs : p->h_lam[0], st->ys_nh ? st->lam_ys : p->h_lam[1],
+                                                         zcap ? lam_s : p->h_lam[2], p->omega, p->zero_tol);
+        double** dst = withx ? &st->d_mult_symx : &st->d_mult_sym;
+        cudaError_t e = cudaMalloc(dst, sizeof(double) * tab.size());
+        if (e == cudaSuccess) e = cudaMemcpy(*dst, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return e;
+      }
     }
   }
   if (!mtot) return cudaSuccess;
@@ -1059,7 +1062,7 @@ void fused_destroy(exx_plan* p) {
 
 // z-forward product, multiplier and z-backward product of nb right-hand sides in one pass, in place or out of place.
 // cudaErrorNotSupported: the caller runs the two k_mode_t passes instead.
-cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, bool sym) {
+cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s, int sym) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st || !st->d_img_zz || !(p->fusion & 1)) return cudaErrorNotSupported;
   const int n = p->n[2], mtot = mtot_class(n);
@@ -1068,11 +1071,11 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
   const long long inner = (long long)p->n[0] * p->n[1];
   // symmetric mode (the caller decides it for the whole batch): the z axis on its reflection-adapted basis where the plan
   // has one, and in any case the table in the symmetric pipeline's mode order
-  const double* table = sym ? st->d_mult_sym : p->d_mult;
+  const double* table = sym == 2 ? st->d_mult_symx : sym ? st->d_mult_sym : p->d_mult;
   if (sym && !table) return cudaErrorInvalidValue;
   if (sym && st->d_img_zzs) {
     const int nh = st->zs_nh, ms = (nh + 7) / 8;
-    const bool per = p->bc[2] == EXX_BC_PERIODIC;
+    const bool per = false;  // centred reflection z -> n - 1 - z on either kind of axis (fused_init)
     ZSArgs z{};
     z.out = out;
     z.V = st->d_img_zzs;
@@ -1150,7 +1153,7 @@ double fused_executed_flops_per_solve(const exx_plan* p) {
   double f = 0.0;
   for (int ax = 0; ax < 3; ++ax) {
     const double n = p->n[ax];
-    const int nh_ax = !sym ? 0 : ax == 2 ? st->zs_nh : ax == 1 ? st->ys_nh : 0;
+    const int nh_ax = !sym ? 0 : ax == 2 ? st->zs_nh : ax == 1 ? st->ys_nh : ((p->fusion & 2) && st->d_mult_symx ? st->xs_nh : 0);
     if (nh_ax) {
       const double nh = nh_ax, no = n - nh;
       f += 4.0 * (nh * nh + no * no) * (double)p->N / n + 2.0 * (double)p->N;
@@ -1167,7 +1170,7 @@ bool fused_sym_mode(const exx_plan* p) {
   const TmaState* st = static_cast<const TmaState*>(p->tma_state);
   if (!st || p->variant != EXX_VARIANT_FUSED_DMMA || (p->fusion & 9) != 9 || !st->d_mult_sym || !st->d_img_zz) return false;
   if (st->ys_nh && st->ys_hc && !(p->fusion & 4)) return false;
-  return st->zs_nh || st->ys_nh;
+  return st->zs_nh || st->ys_nh || st->xs_nh;
 }
 
 // The same for nb complex functions ([nb][2][N] planes) of a Bloch plan whose z axis is complex with n <= 64, in place.

@@ -423,6 +423,406 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lb_sym(const __grid_cons
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// x axis.  k_mode_xf_sym: the x-forward product of the exchange apply -- pair density psi_j * tgt_k formed on the fly
+// from two TMA streams (a1), each staged as rows x in [16 s, 16 s + 16) and the mirrored block, butterflied on the
+// fragments -- on the reflection-adapted basis of the x axis.  Output rows hold the modes even block first.
+// k_mode_xacc_sym: the x-backward product fused with the accumulate (k_mode_xacc, kernels_fused.cu) on the same basis:
+// a = E t_even, b = O t_odd over the half range, phi[x] = a + b, phi[mir x] = a - b, and vx_k's tile kept in two
+// accumulator sets (x and mir x); the psi_j tile arrives as a pair of boxes (x block and mirrored block).
+// ---------------------------------------------------------------------------------------------------------------
+struct XSArgs {
+  double* out;         // xf: the batch buffer
+  const double* V;
+  const double* occ;   // xacc: occ + j0
+  double* vx;          // xacc: vx + k0 * N
+  int n, nh;
+  int Sh, So;          // xf: Sh stages over the half range; xacc: Sh stages over the even modes, So over the odd modes
+  int Sp;              // xacc: stages of the psi tile (half range)
+  int kk_last, kk_last_o, kk_last_p;
+  int mir0, mirc, zfix;
+  unsigned n_tiles;
+  int rows_per_rhs, tiles_per_rhs;
+  int nj, nk, j0;
+  int first;
+  FastDiv div_tiles, div_nj, div_nk;
+  BatchDesc bd;
+};
+
+// X-mode box ({16 x, rows}, 128-byte rows and swizzle): offset of (row 8nt + g, x) without the 1024 nt term
+__device__ __forceinline__ unsigned offx(unsigned x, unsigned g) { return 128u * g + 16u * ((x >> 1) ^ g) + 8u * (x & 1); }
+
+template <int MS, int NT, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_xf_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
+  constexpr int MT = 2 * MS;
+  constexpr int LDV = 8 * MT + 4;
+  constexpr unsigned kBox = 1024u * NT;   // one {16 x, 8 NT rows} box
+  constexpr unsigned kSlot = 4u * kBox;   // psi block, psi mirrored block, tgt block, tgt mirrored block
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, Sh = a.Sh;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * Sh) * LDV;
+  for (unsigned i = 2 * tid; i < 16u * Sh * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kSlot);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kSlot) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kSlot) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int pr0 = 0, pr1 = 0;
+  auto tile_coords = [&](unsigned t) {
+    const int rhs = (int)fast_div(t, a.div_tiles);
+    const int rb = (int)t - rhs * a.tiles_per_rhs;
+    const int kq = (int)fast_div((unsigned)rhs, a.div_nj);
+    const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
+    pr0 = j * a.rows_per_rhs + rb * (8 * NT);
+    pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kSlot;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kSlot);
+      tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
+      tma_load_2d(dst + kBox, &tm0, a.mir0 - 16 * s_p, pr0, bar);
+      tma_load_2d(dst + 2 * kBox, &tm1, 16 * s_p, pr1, bar);
+      tma_load_2d(dst + 3 * kBox, &tm1, a.mir0 - 16 * s_p, pr1, bar);
+    }
+    if (++s_p == Sh) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  // k-step kk reads x = (q&1) + 8(q>>1) + 2kk of the block and 15 - x of the mirrored block
+  unsigned xo[4], xm[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const unsigned x = (q & 1) + 8u * (q >> 1) + 2u * i;
+    xo[i] = offx(x, g);
+    xm[i] = kBox + offx(15u - x, g);
+  }
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+    for (int s = 0; s < Sh; ++s) {
+      asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kSlot;
+      const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+      const int zf = a.zfix - 16 * s;
+      const bool ragged = a.kk_last && s == Sh - 1;
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (!ragged || kk < a.kk_last) {
+          double be[NT], bo[NT];
+          const int xl = ragged ? 4 * kk + q : (q & 1) + 8 * (q >> 1) + 2 * kk;
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            const unsigned oa = sb + 1024u * nt + (ragged ? offx((unsigned)xl, g) : xo[kk]);
+            const unsigned ob = sb + 1024u * nt + (ragged ? kBox + offx(15u - (unsigned)xl, g) : xm[kk]);
+            const double va = lds64(oa) * lds64(oa + 2 * kBox);
+            double vb = lds64(ob) * lds64(ob + 2 * kBox);
+            if (xl == zf) vb = 0.0;
+            be[nt] = va + vb;
+            bo[nt] = va - vb;
+          }
+          double af[MT];
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], mt < MS ? be[nt] : bo[nt]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    }
+    // epilogue: C[mode 8 (mt % MS) + g of block mt / MS][row 8nt + 2q + e]; positions: even modes 0.., odd modes nh..
+    {
+      const int rhs = (int)fast_div(t, a.div_tiles);
+      const int rb = (int)t - rhs * a.tiles_per_rhs;
+      const int row0 = rhs * a.rows_per_rhs + rb * (8 * NT);
+      const int limit = (rhs + 1) * a.rows_per_rhs;
+      double* base = a.out + (long long)(row0 + 2 * q) * n;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          if (row0 + 8 * nt + 2 * q + e < limit) {
+            double* dst = base + (long long)(8 * nt + e) * n;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+              const int blk = mt >= MS ? 1 : 0;
+              const int ml = 8 * (mt - blk * MS) + g;
+              if (ml < (blk ? n - a.nh : a.nh)) dst[blk * a.nh + ml] = acc[mt][nt][e];
+            }
+          }
+        }
+    }
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
+template <int MS, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1)
+    k_mode_xacc_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
+  constexpr int NT = 1;
+  constexpr int LDV = 8 * MS + 4;
+  constexpr unsigned kBox = 1024u * NT;
+  constexpr unsigned kSlot = 2u * kBox;  // a psi stage is a pair of boxes; a data stage uses the first half
+  constexpr int SPMAX = (MS + 1) / 2;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, SE = a.Sh, ST = a.Sh + a.So, SP = a.Sp;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * ST) * LDV;
+  for (unsigned i = 2 * tid; i < 16u * ST * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kSlot);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kSlot) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kSlot) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+
+  // producer: item (row tile, target) = nj steps of ST data stages (even modes, then odd modes) + SP psi stage pairs
+  const int stages_per_step = ST + SP;
+  unsigned t_p = tfirst;
+  int s_p = 0, jj_p = 0;
+  int prow_d = 0, prow_p = 0;
+  auto tile_coords = [&](unsigned t) {
+    const int rb = (int)fast_div(t, a.div_nk);
+    const int kq = (int)t - rb * a.nk;
+    prow_d = (a.nj * kq) * a.rows_per_rhs + rb * (8 * NT);
+    prow_p = a.j0 * a.rows_per_rhs + rb * (8 * NT);
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kSlot;
+    if (elect_one()) {
+      if (s_p < ST) {
+        mbar_expect_tx(bar, kBox);
+        tma_load_2d(dst, &tm0, s_p < SE ? 16 * s_p : a.nh + 16 * (s_p - SE), prow_d, bar);
+      } else {
+        const int sp = s_p - ST;
+        mbar_expect_tx(bar, kSlot);
+        tma_load_2d(dst, &tm1, 16 * sp, prow_p, bar);
+        tma_load_2d(dst + kBox, &tm1, a.mir0 - 16 * sp, prow_p, bar);
+      }
+    }
+    if (++s_p == stages_per_step) {
+      s_p = 0;
+      if (++jj_p == a.nj) {
+        jj_p = 0;
+        t_p = claim_tile();
+#pragma unroll
+        for (int i = 0; i < kDepth + 1; ++i)
+          if (i == fifo_n) fifo[i] = t_p;
+        ++fifo_n;
+        if (t_p < a.n_tiles) tile_coords(t_p);
+      } else {
+        prow_d += a.rows_per_rhs;
+        prow_p += a.rows_per_rhs;
+      }
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) xo[i] = offx((q & 1) + 8u * (q >> 1) + 2u * i, g);
+  // psi fragments in accumulator layout: box row 2q + e, x = 8h + g of the block / 15 - (8h + g) of the mirrored block
+  unsigned pq[2][2], pm[2][2];
+#pragma unroll
+  for (int e = 0; e < 2; ++e)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const unsigned row = 2u * q + e, x = 8u * h + g, xb = 15u - x;
+      pq[e][h] = 128u * row + 16u * ((x >> 1) ^ row) + 8u * (x & 1);
+      pm[e][h] = kBox + 128u * row + 16u * ((xb >> 1) ^ row) + 8u * (xb & 1);
+    }
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    const int rb = (int)fast_div(t, a.div_nk);
+    const int kq = (int)t - rb * a.nk;
+    const int row0 = rb * (8 * NT);
+    double* vbase = a.vx + ((long long)kq * a.rows_per_rhs + row0 + 2 * q) * n;
+    // vx_k's tile: lo[mt][e] at x = 8mt + g, hi[mt][e] at mir(x)
+    double lo[MS][2], hi[MS][2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const bool rok = !a.first && row0 + 2 * q + e < a.rows_per_rhs;
+      const double* src = vbase + (long long)e * n;
+#pragma unroll
+      for (int mt = 0; mt < MS; ++mt) {
+        const int x = 8 * mt + g, xb = a.mirc - x;
+        lo[mt][e] = (rok && x < a.nh) ? src[x] : 0.0;
+        hi[mt][e] = (rok && x < a.nh && xb != x && xb < n) ? src[xb] : 0.0;
+      }
+    }
+    for (int jj = 0; jj < a.nj; ++jj) {
+      const double oc = __ldg(a.occ + jj);
+      double pa[MS][2], pb[MS][2];
+#pragma unroll
+      for (int mt = 0; mt < MS; ++mt) pa[mt][0] = pa[mt][1] = pb[mt][0] = pb[mt][1] = 0.0;
+      auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+        asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+        mbar_wait(my_bar + 8u * slot, parity);
+        const unsigned sb = my_ring + slot * kSlot;
+        const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          if (!ragged || kk < kk_last) {
+            const double bf = lds64(sb + (ragged ? offx(4u * kk + q, g) : xo[kk]));
+            double af[MS];
+#pragma unroll
+            for (int mt = 0; mt < MS; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+            for (int mt = 0; mt < MS; ++mt) dmma884(acc[mt], af[mt], bf);
+          }
+        }
+        __syncwarp();
+        produce(slot);
+        if (++slot == kDepth) {
+          slot = 0;
+          parity ^= 1u;
+        }
+      };
+      for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
+      for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+      // a5: vx_k[x] -= occ_j psi_j[x] (a + b), vx_k[mir x] -= occ_j psi_j[mir x] (a - b)
+#pragma unroll
+      for (int sp = 0; sp < SPMAX; ++sp) {
+        if (sp < SP) {
+          mbar_wait(my_bar + 8u * slot, parity);
+          const unsigned sb = my_ring + slot * kSlot;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            constexpr int kZ = 0;
+            const int mt = 2 * sp + h < MS ? 2 * sp + h : kZ;
+            if (2 * sp + h < MS) {
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const double p0 = lds64(sb + pq[e][h]), p1 = lds64(sb + pm[e][h]);
+                lo[mt][e] -= oc * p0 * (pa[mt][e] + pb[mt][e]);
+                hi[mt][e] -= oc * p1 * (pa[mt][e] - pb[mt][e]);
+              }
+            }
+          }
+          __syncwarp();
+          produce(slot);
+          if (++slot == kDepth) {
+            slot = 0;
+            parity ^= 1u;
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      if (row0 + 2 * q + e < a.rows_per_rhs) {
+        double* dst = vbase + (long long)e * n;
+#pragma unroll
+        for (int mt = 0; mt < MS; ++mt) {
+          const int x = 8 * mt + g, xb = a.mirc - x;
+          if (x < a.nh) {
+            dst[x] = lo[mt][e];
+            if (xb != x && xb < n) dst[xb] = hi[mt][e];
+          }
+        }
+      }
+    }
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
 // ---- host side ------------------------------------------------------------------------------------------------
 
 template <typename Kern>
@@ -464,21 +864,122 @@ cudaError_t launch_lb(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, 
   return launch_sym(k_mode_lb_sym<MS, NT, W, HC>, opt, smem, W, p, m0, a, s);
 }
 
+template <typename Kern>
+cudaError_t launch_sym2(Kern kern, SmemOptIn& opt, size_t smem, int warps, const exx_plan* p, const CUtensorMap& m0,
+                        const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
+  const size_t floor_bytes = 117 * 1024;
+  if (smem < floor_bytes) smem = floor_bytes;
+  if (smem > (size_t)p->smem_optin) return cudaErrorNotSupported;
+  cudaError_t e = opt.ensure(kern, p->device, smem, true);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  const unsigned grid = a.n_tiles < (unsigned)p->sm_count ? a.n_tiles : (unsigned)p->sm_count;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * warps);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, m0, m1, a);
+}
+
+template <int MS>
+cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 8, NT = 2;
+  const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 4 * 1024 * NT +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym2(k_mode_xf_sym<MS, NT, W>, opt, smem, W, p, m0, m1, a, s);
+}
+template <int MS>
+cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 12;
+  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym2(k_mode_xacc_sym<MS, W>, opt, smem, W, p, m0, m1, a, s);
+}
+
 }  // namespace
 
 // Images of the y axis on the reflection-adapted basis; `hc`: row order of the half-chunk tiles.  Forward: rows = half
 // range (k_mode_t's L-mode stage order), columns = even modes | 8 MS + odd modes.  Backward: rows = even modes in stages
 // of 16, then odd modes in stages of 16, columns = half-range points.
+static cudaError_t sym_init_y(exx_plan* p);
+static cudaError_t sym_init_x(exx_plan* p);
+
 cudaError_t sym_init(exx_plan* p) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st) return cudaSuccess;
-  st->d_img_yf = st->d_img_yb = nullptr;
-  st->ys_nh = 0;
+  st->d_img_yf = st->d_img_yb = st->d_img_xf = st->d_img_xb = st->d_mult_symx = nullptr;
+  st->ys_nh = st->xs_nh = 0;
   if (!p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty()) return cudaSuccess;
+  cudaError_t e = sym_init_y(p);
+  if (e == cudaSuccess) e = sym_init_x(p);
+  return e;
+}
+
+// x axis: forward image = rows over the half range in X-mode stage order, columns even modes | 8 MS + odd modes;
+// backward image = rows over the even modes in stages of 16 then the odd modes, columns over the half range.
+static cudaError_t sym_init_x(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  const int n = p->n[0];
+  // x is the contiguous index: the boxes of the mirrored block and of the odd modes must start at an even element (TMA
+  // wants 16-byte aligned starts along the innermost dimension), hence the reflection x -> n - 1 - x on either kind of
+  // axis (mirrored block of stage s starts at n - 16 - 16 s) and nx a multiple of 4 (odd modes start at n / 2)
+  if (n > 128 || (n & 3)) return cudaSuccess;
+  int nh = 0;
+  if (!symmetrize_axis(n, p->bc[0], p->h_lam[0], p->h_V[0], st->lam_xs, st->V_xs, &nh, true)) return cudaSuccess;
+  const int ms = (nh + 7) / 8;
+  if (ms < 5 || ms > 8) return cudaSuccess;
+  const int no = n - nh, Sh = (nh + 15) / 16, So = (no + 15) / 16;
+  const std::vector<double>& Vs = st->V_xs;
+  {
+    const int ld = 16 * ms + 4;
+    std::vector<double> img((size_t)16 * Sh * ld, 0.0);
+    for (int s = 0; s < Sh; ++s)
+      for (int kk = 0; kk < 4; ++kk)
+        for (int q = 0; q < 4; ++q) {
+          const int x = 16 * s + within_stage(true, nh, s, kk, q);
+          if (x >= nh) continue;
+          double* row = &img[(size_t)(16 * s + 4 * kk + q) * ld];
+          for (int m = 0; m < n; ++m) row[m < nh ? m : 8 * ms + (m - nh)] = Vs[(size_t)x * n + m];
+        }
+    cudaError_t e = cudaMalloc(&st->d_img_xf, sizeof(double) * img.size());
+    if (e == cudaSuccess) e = cudaMemcpy(st->d_img_xf, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
+  {
+    const int ld = 8 * ms + 4;
+    std::vector<double> img((size_t)16 * (Sh + So) * ld, 0.0);
+    for (int blk = 0; blk < 2; ++blk) {
+      const int cnt = blk ? no : nh, S = blk ? So : Sh, row0 = blk ? 16 * Sh : 0;
+      for (int s = 0; s < S; ++s)
+        for (int kk = 0; kk < 4; ++kk)
+          for (int q = 0; q < 4; ++q) {
+            const int m = 16 * s + within_stage(true, cnt, s, kk, q);
+            if (m >= cnt) continue;
+            double* row = &img[(size_t)(row0 + 16 * s + 4 * kk + q) * ld];
+            for (int x = 0; x < nh; ++x) row[x] = Vs[(size_t)x * n + (blk ? nh + m : m)];
+          }
+    }
+    cudaError_t e = cudaMalloc(&st->d_img_xb, sizeof(double) * img.size());
+    if (e == cudaSuccess) e = cudaMemcpy(st->d_img_xb, img.data(), sizeof(double) * img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
+  st->xs_nh = nh;
+  return cudaSuccess;
+}
+
+static cudaError_t sym_init_y(exx_plan* p) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
   const int n = p->n[1];
   if (n > 128 || (p->n[0] & 1)) return cudaSuccess;
   int nh = 0;
-  if (!symmetrize_axis(n, p->bc[1], p->h_lam[1], p->h_V[1], st->lam_ys, st->V_ys, &nh)) return cudaSuccess;
+  if (!symmetrize_axis(n, p->bc[1], p->h_lam[1], p->h_V[1], st->lam_ys, st->V_ys, &nh, true)) return cudaSuccess;
   const int ms = (nh + 7) / 8;
   if (ms < 5 || ms > 8) return cudaSuccess;
   const bool hc = p->n[0] % 16 == 8;
@@ -527,7 +1028,10 @@ void sym_destroy(exx_plan* p) {
   if (!st) return;
   if (st->d_img_yf) cudaFree(st->d_img_yf);
   if (st->d_img_yb) cudaFree(st->d_img_yb);
-  st->d_img_yf = st->d_img_yb = nullptr;
+  if (st->d_img_xf) cudaFree(st->d_img_xf);
+  if (st->d_img_xb) cudaFree(st->d_img_xb);
+  if (st->d_mult_symx) cudaFree(st->d_mult_symx);
+  st->d_img_yf = st->d_img_yb = st->d_img_xf = st->d_img_xb = st->d_mult_symx = nullptr;
 }
 
 // y product of nb right-hand sides on the reflection-adapted basis, in place.  The caller has established that the whole
@@ -536,7 +1040,7 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!st || !st->ys_nh || !aligned16(buf)) return cudaErrorNotSupported;
   const int n = p->n[1], nh = st->ys_nh, no = n - nh, ms = (nh + 7) / 8;
-  const bool per = p->bc[1] == EXX_BC_PERIODIC, hc = st->ys_hc;
+  const bool per = false, hc = st->ys_hc;  // centred reflection y -> n - 1 - y on either kind of axis (sym_init_y)
   const long long inner = p->n[0], outer = (long long)p->n[2] * nb;
   SArgs a{};
   a.out = buf;
@@ -578,6 +1082,96 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
       return hc ? launch_lb<8, true>(p, m0, a, s) : launch_lb<8, false>(p, m0, a, s);
   }
 #undef EXX_SYM_CASE
+}
+
+// Whether the exchange-apply batch `fa` can run its x passes on the reflection-adapted basis: the plan has the images and
+// the symmetric table with x, the fused accumulate is on, and every buffer the two kernels touch is TMA-addressable.
+bool sym_x_usable(const exx_plan* p, const double* work, const FastArgs* fa) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  if (!st || !st->xs_nh || !st->d_mult_symx || !fa || fa->sym || !(p->fusion & 2)) return false;
+  if (!aligned16(work) || !aligned16(fa->psi) || !aligned16(fa->tgt) || !aligned16(fa->vx)) return false;
+  const long long rpr = p->N / p->n[0];
+  return rpr * fa->n_occ < (1LL << 31) - 64 && rpr * fa->n_tgt < (1LL << 31) - 64;
+}
+
+static void fill_x(const exx_plan* p, const TmaState* st, XSArgs& a) {
+  const int n = p->n[0], nh = st->xs_nh, no = n - nh;
+  const bool per = false;  // the x axis always uses the centred reflection x -> n - 1 - x (sym_init_x)
+  a.n = n;
+  a.nh = nh;
+  a.Sh = (nh + 15) / 16;
+  a.So = (no + 15) / 16;
+  a.Sp = (nh + 15) / 16;
+  a.kk_last = tail_ksteps(nh);
+  a.kk_last_o = tail_ksteps(no);
+  a.kk_last_p = tail_ksteps(nh);
+  a.mir0 = per ? n - 15 : n - 16;
+  a.mirc = per ? n : n - 1;
+  a.zfix = per ? ((n % 2 == 0 && n >= 2) ? n / 2 : -1) : ((n % 2) ? (n - 1) / 2 : -1);
+  a.rows_per_rhs = (int)(p->N / n);
+}
+
+// x-forward product with the pair density formed on the fly, modes stored even block first.
+cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!sym_x_usable(p, out, fa)) return cudaErrorNotSupported;
+  constexpr int NT = 2;
+  XSArgs a{};
+  fill_x(p, st, a);
+  a.out = out;
+  a.V = st->d_img_xf;
+  a.bd = fa->bd;
+  a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+  a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+  a.div_nj = make_fastdiv((unsigned)fa->bd.nj);
+  if ((long long)a.rows_per_rhs * nb >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if ((e = get_map(st, fa->psi, a.n, (long long)a.rows_per_rhs * fa->n_occ, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, fa->tgt, a.n, (long long)a.rows_per_rhs * fa->n_tgt, 0, 8 * NT, &m1)) != cudaSuccess) return e;
+  ++p->tma_launches;
+  switch ((a.nh + 7) / 8) {
+    case 5: return launch_xf<5>(p, m0, m1, a, s);
+    case 6: return launch_xf<6>(p, m0, m1, a, s);
+    case 7: return launch_xf<7>(p, m0, m1, a, s);
+    default: return launch_xf<8>(p, m0, m1, a, s);
+  }
+}
+
+// x-backward product fused with the accumulate; `in` holds the batch with the x modes even block first.
+cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!sym_x_usable(p, in, fa)) return cudaErrorNotSupported;
+  if (nb != fa->bd.nj * fa->bd.nk) return cudaErrorInvalidValue;
+  XSArgs a{};
+  fill_x(p, st, a);
+  a.V = st->d_img_xb;
+  a.occ = fa->occ + fa->bd.j0;
+  a.vx = fa->vx + (size_t)fa->bd.k0 * (size_t)p->N;
+  a.nj = fa->bd.nj;
+  a.nk = fa->bd.nk;
+  a.j0 = fa->bd.j0;
+  a.first = fa->first ? 1 : 0;
+  a.div_nk = make_fastdiv((unsigned)a.nk);
+  const long long rows_total = (long long)a.rows_per_rhs * nb, rows_psi = (long long)a.rows_per_rhs * fa->n_occ;
+  if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  const long long tiles_per_rhs = (a.rows_per_rhs + 7) / 8;
+  if (tiles_per_rhs * a.nk >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.n_tiles = (unsigned)(tiles_per_rhs * a.nk);
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0, m1;
+  cudaError_t e;
+  if ((e = get_map(st, in, a.n, rows_total, 0, 8, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, fa->psi, a.n, rows_psi, 0, 8, &m1)) != cudaSuccess) return e;
+  ++p->tma_launches;
+  switch ((a.nh + 7) / 8) {
+    case 5: return launch_xacc_sym<5>(p, m0, m1, a, s);
+    case 6: return launch_xacc_sym<6>(p, m0, m1, a, s);
+    case 7: return launch_xacc_sym<7>(p, m0, m1, a, s);
+    default: return launch_xacc_sym<8>(p, m0, m1, a, s);
+  }
 }
 
 }  // namespace exx

@@ -194,9 +194,11 @@ bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& l
 // re-expressed in such a basis, EVEN vectors first (n_even of them = number of z with z <= mir z), each block in
 // ascending eigenvalue order; Vs row-major [z][m'].  A contraction with an even (odd) vector only needs the half range
 // z <= mir(z) of the symmetrised (antisymmetrised) data: half the multiply-adds of the dense product.
+// `centered`: use z -> n - 1 - z on a periodic axis too (a symmetric circulant matrix commutes with every reflection);
+// the x-axis kernels want it because their mirrored TMA boxes then start at an even, i.e. 16-byte aligned, element.
 bool symmetrize_axis(int n, int bc, const std::vector<double>& lam, const std::vector<double>& V, std::vector<double>& lam_s,
-                     std::vector<double>& Vs, int* n_even) {
-  auto mir = [&](int z) { return bc == EXX_BC_PERIODIC ? (n - z) % n : n - 1 - z; };
+                     std::vector<double>& Vs, int* n_even, bool centered) {
+  auto mir = [&](int z) { return (bc == EXX_BC_PERIODIC && !centered) ? (n - z) % n : n - 1 - z; };
   int nh = 0;
   for (int z = 0; z < n; ++z) nh += z <= mir(z) ? 1 : 0;
   double scale = 0.0;

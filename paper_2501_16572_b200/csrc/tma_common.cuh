@@ -44,6 +44,12 @@ struct TmaState {
   bool ys_hc;
   std::vector<double> lam_ys, V_ys;
   double* d_mult_sym;
+  // x axis (k_mode_xf_sym / k_mode_xacc_sym, exchange apply only): images, basis, and the table with x in that order too
+  double* d_img_xf;
+  double* d_img_xb;
+  int xs_nh;
+  std::vector<double> lam_xs, V_xs;
+  double* d_mult_symx;
   double* d_img_zz_c;      // the same for a complex z axis with n <= 64 (embedding E = [[Vr, -Vi], [Vi, Vr]])
   double* d_img_zz;  // fused z-forward/z-backward kernel: one image of Vz serving both products (kernels_fused.cu)
   std::vector<MapEntry> cache;

@@ -103,7 +103,7 @@ def test_reflection_adapted_eigenbasis(lib, dims, bc, h):
     for ax, n in enumerate(dims):
         lam0, V0 = p.get_axis(ax)
         lam, V, ne = p.get_axis_symmetric(ax)
-        mir = np.array([(n - z) % n if bc[ax] == 0 else n - 1 - z for z in range(n)])
+        mir = n - 1 - np.arange(n)
         assert ne == int(np.sum(np.arange(n) <= mir))
         assert np.all(V[mir, :ne] == V[:, :ne]) and np.all(V[mir, ne:] == -V[:, ne:])      # exact parity
         assert np.all(np.diff(lam[:ne]) >= -1e-12 * scale) and np.all(np.diff(lam[ne:]) >= -1e-12 * scale)

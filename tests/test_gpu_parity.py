@@ -187,6 +187,10 @@ FUSION_GRIDS = [
     (24, 77, 4, (0, 1, 0), 0.0),
     (40, 126, 5, (1, 0, 0), 0.106),
     (16, 120, 70, (0, 0, 1), 0.106),
+    # x axis too (k_mode_xf_sym / k_mode_xacc_sym; nx a multiple of 4): exchange apply only
+    (72, 4, 4, (0, 0, 0), 0.106),
+    (124, 4, 4, (1, 0, 0), 0.0),
+    (72, 70, 70, (0, 0, 0), 0.106),
 ]
 
 
@@ -225,10 +229,13 @@ def test_fused_passes_match_oracle_and_unfused(grid):
         plan.set_accumulate(False)
         torch.cuda.synchronize()
         assert _rel(vx2.cpu().numpy(), vx_o) < TOL
-    # the sum over j is ascending whatever the batch shape and the mask: rounding-level agreement between all of them
-    ref = results[(0, 32)]
-    for key, v in results.items():
-        assert float((v - ref).abs().max() / ref.abs().max()) < 1e-12, key
+    # the sum over j is ascending whatever the batch shape and the mask: rounding-level agreement between all runs that
+    # contract with the same eigenbasis (bit 3 changes the basis: those agree with the others through the oracle bound)
+    for bit3 in (0, 8):
+        ref = results[(bit3 + 1, 32)]
+        for key, v in results.items():
+            if (key[0] & 8) == bit3:
+                assert float((v - ref).abs().max() / ref.abs().max()) < 1e-12, key
     plan.close()
 
 
