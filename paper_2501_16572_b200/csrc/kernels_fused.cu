@@ -970,12 +970,11 @@ cudaError_t fused_init(exx_plan* p) {
   st->zs_nh = 0;
   const int n = p->n[2], mtot = mtot_class(n);
   if (p->h_Vi[2].empty() && p->h_Vi[0].empty() && p->h_Vi[1].empty()) {
-    // reflection-adapted basis of the z axis: image over the half range.  Only where it pays: below five row tiles per
-    // block (nz < 66) the two-box stages and the padding of the blocks to whole row tiles cost more than the saved
-    // DMMAs (measured at 48^3: -2 %).
+    // reflection-adapted basis of the z axis: image over the half range; three to eight row tiles per block (nz = 34
+    // .. 128; below, the padding of the two blocks to whole row tiles eats the saving)
     std::vector<double> lam_s, Vs;
     int nh = 0;
-    const bool zcap = mtot && symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh, true) && (nh + 7) / 8 >= 5 &&
+    const bool zcap = mtot && symmetrize_axis(n, p->bc[2], p->h_lam[2], p->h_V[2], lam_s, Vs, &nh, true) && (nh + 7) / 8 >= 3 &&
                       (nh + 7) / 8 <= 8;
     if (zcap) {
       const int ms = (nh + 7) / 8, Sh = (nh + 15) / 16, lds = 16 * ms + 4;
@@ -1102,6 +1101,8 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
     z.n_tiles = (unsigned)((chunks + CH - 1) / CH);
     if (z.n_tiles == 0) return cudaSuccess;
     switch (ms) {
+      case 3: e = launch_zz_sym<3, 4, 8, 1>(p, m0, m1, z, s); break;
+      case 4: e = launch_zz_sym<4, 4, 8, 1>(p, m0, m1, z, s); break;
       case 5: e = launch_zz_sym<5, 2, 12, 1>(p, m0, m1, z, s); break;
       case 6: e = launch_zz_sym<6, 2, 12, 1>(p, m0, m1, z, s); break;
       case 7: e = launch_zz_sym<7, 2, 12, 1>(p, m0, m1, z, s); break;

@@ -617,10 +617,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   }
 }
 
-template <int MS, int WARPS>
+template <int MS, int NT, int WARPS>
 __global__ void __launch_bounds__(32 * WARPS, 1)
     k_mode_xacc_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
-  constexpr int NT = 1;
   constexpr int LDV = 8 * MS + 4;
   constexpr unsigned kBox = 1024u * NT;
   constexpr unsigned kSlot = 2u * kBox;  // a psi stage is a pair of boxes; a data stage uses the first half
@@ -731,24 +730,28 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     const int kq = (int)t - rb * a.nk;
     const int row0 = rb * (8 * NT);
     double* vbase = a.vx + ((long long)kq * a.rows_per_rhs + row0 + 2 * q) * n;
-    // vx_k's tile: lo[mt][e] at x = 8mt + g, hi[mt][e] at mir(x)
-    double lo[MS][2], hi[MS][2];
+    // vx_k's tile: lo[mt][nt][e] at row 8nt + 2q + e, x = 8mt + g; hi[mt][nt][e] at mir(x)
+    double lo[MS][NT][2], hi[MS][NT][2];
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      const bool rok = !a.first && row0 + 2 * q + e < a.rows_per_rhs;
-      const double* src = vbase + (long long)e * n;
+    for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-      for (int mt = 0; mt < MS; ++mt) {
-        const int x = 8 * mt + g, xb = a.mirc - x;
-        lo[mt][e] = (rok && x < a.nh) ? src[x] : 0.0;
-        hi[mt][e] = (rok && x < a.nh && xb != x && xb < n) ? src[xb] : 0.0;
+      for (int e = 0; e < 2; ++e) {
+        const bool rok = !a.first && row0 + 8 * nt + 2 * q + e < a.rows_per_rhs;
+        const double* src = vbase + (long long)(8 * nt + e) * n;
+#pragma unroll
+        for (int mt = 0; mt < MS; ++mt) {
+          const int x = 8 * mt + g, xb = a.mirc - x;
+          lo[mt][nt][e] = (rok && x < a.nh) ? src[x] : 0.0;
+          hi[mt][nt][e] = (rok && x < a.nh && xb != x && xb < n) ? src[xb] : 0.0;
+        }
       }
-    }
     for (int jj = 0; jj < a.nj; ++jj) {
       const double oc = __ldg(a.occ + jj);
-      double pa[MS][2], pb[MS][2];
+      double pa[MS][NT][2], pb[MS][NT][2];
 #pragma unroll
-      for (int mt = 0; mt < MS; ++mt) pa[mt][0] = pa[mt][1] = pb[mt][0] = pb[mt][1] = 0.0;
+      for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
       auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
         asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
         mbar_wait(my_bar + 8u * slot, parity);
@@ -757,12 +760,16 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
           if (!ragged || kk < kk_last) {
-            const double bf = lds64(sb + (ragged ? offx(4u * kk + q, g) : xo[kk]));
+            double bf[NT];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) bf[nt] = lds64(sb + 1024u * nt + (ragged ? offx(4u * kk + q, g) : xo[kk]));
             double af[MS];
 #pragma unroll
             for (int mt = 0; mt < MS; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
 #pragma unroll
-            for (int mt = 0; mt < MS; ++mt) dmma884(acc[mt], af[mt], bf);
+            for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
           }
         }
         __syncwarp();
@@ -786,11 +793,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
             const int mt = 2 * sp + h < MS ? 2 * sp + h : kZ;
             if (2 * sp + h < MS) {
 #pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const double p0 = lds64(sb + pq[e][h]), p1 = lds64(sb + pm[e][h]);
-                lo[mt][e] -= oc * p0 * (pa[mt][e] + pb[mt][e]);
-                hi[mt][e] -= oc * p1 * (pa[mt][e] - pb[mt][e]);
-              }
+              for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const double p0 = lds64(sb + 1024u * nt + pq[e][h]), p1 = lds64(sb + 1024u * nt + pm[e][h]);
+                  lo[mt][nt][e] -= oc * p0 * (pa[mt][nt][e] + pb[mt][nt][e]);
+                  hi[mt][nt][e] -= oc * p1 * (pa[mt][nt][e] - pb[mt][nt][e]);
+                }
             }
           }
           __syncwarp();
@@ -803,19 +812,21 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       }
     }
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      if (row0 + 2 * q + e < a.rows_per_rhs) {
-        double* dst = vbase + (long long)e * n;
+    for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-        for (int mt = 0; mt < MS; ++mt) {
-          const int x = 8 * mt + g, xb = a.mirc - x;
-          if (x < a.nh) {
-            dst[x] = lo[mt][e];
-            if (xb != x && xb < n) dst[xb] = hi[mt][e];
+      for (int e = 0; e < 2; ++e) {
+        if (row0 + 8 * nt + 2 * q + e < a.rows_per_rhs) {
+          double* dst = vbase + (long long)(8 * nt + e) * n;
+#pragma unroll
+          for (int mt = 0; mt < MS; ++mt) {
+            const int x = 8 * mt + g, xb = a.mirc - x;
+            if (x < a.nh) {
+              dst[x] = lo[mt][nt][e];
+              if (xb != x && xb < n) dst[xb] = hi[mt][nt][e];
+            }
           }
         }
       }
-    }
     t = fifo[0];
 #pragma unroll
     for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
@@ -850,7 +861,7 @@ cudaError_t launch_sym(Kern kern, SmemOptIn& opt, size_t smem, int warps, const 
 template <int MS, bool HC>
 cudaError_t launch_lf(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 12, NT = 2;
+  constexpr int W = 12, NT = MS <= 4 ? 4 : 2;
   const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym(k_mode_lf_sym<MS, NT, W, HC>, opt, smem, W, p, m0, a, s);
@@ -858,7 +869,7 @@ cudaError_t launch_lf(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, 
 template <int MS, bool HC>
 cudaError_t launch_lb(const exx_plan* p, const CUtensorMap& m0, const SArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 12, NT = 2;
+  constexpr int W = 12, NT = MS <= 4 ? 4 : 2;
   const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym(k_mode_lb_sym<MS, NT, W, HC>, opt, smem, W, p, m0, a, s);
@@ -897,10 +908,10 @@ cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMa
 template <int MS>
 cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 12;
-  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 +
+  constexpr int W = 12, NT = MS <= 4 ? 2 : 1;
+  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
-  return launch_sym2(k_mode_xacc_sym<MS, W>, opt, smem, W, p, m0, m1, a, s);
+  return launch_sym2(k_mode_xacc_sym<MS, NT, W>, opt, smem, W, p, m0, m1, a, s);
 }
 
 }  // namespace
@@ -934,7 +945,7 @@ static cudaError_t sym_init_x(exx_plan* p) {
   int nh = 0;
   if (!symmetrize_axis(n, p->bc[0], p->h_lam[0], p->h_V[0], st->lam_xs, st->V_xs, &nh, true)) return cudaSuccess;
   const int ms = (nh + 7) / 8;
-  if (ms < 5 || ms > 8) return cudaSuccess;
+  if (ms < 3 || ms > 8) return cudaSuccess;
   const int no = n - nh, Sh = (nh + 15) / 16, So = (no + 15) / 16;
   const std::vector<double>& Vs = st->V_xs;
   {
@@ -981,7 +992,7 @@ static cudaError_t sym_init_y(exx_plan* p) {
   int nh = 0;
   if (!symmetrize_axis(n, p->bc[1], p->h_lam[1], p->h_V[1], st->lam_ys, st->V_ys, &nh, true)) return cudaSuccess;
   const int ms = (nh + 7) / 8;
-  if (ms < 5 || ms > 8) return cudaSuccess;
+  if (ms < 3 || ms > 8) return cudaSuccess;
   const bool hc = p->n[0] % 16 == 8;
   const int no = n - nh, Sh = (nh + 15) / 16, So = (no + 15) / 16;
   const std::vector<double>& Vs = st->V_ys;
@@ -1062,7 +1073,7 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
   a.total_chunks = (unsigned)chunks;
   a.outer = (int)outer;
   a.div_cpo = make_fastdiv((unsigned)a.cpo);
-  const int CH = hc ? 2 : 1;
+  const int NT = ms <= 4 ? 4 : 2, CH = hc ? NT : NT / 2;
   a.n_tiles = (unsigned)((chunks + CH - 1) / CH);
   if (a.n_tiles == 0) return cudaSuccess;
   CUtensorMap m0;
@@ -1074,6 +1085,8 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
     if (forward) return hc ? launch_lf<MSV, true>(p, m0, a, s) : launch_lf<MSV, false>(p, m0, a, s); \
     return hc ? launch_lb<MSV, true>(p, m0, a, s) : launch_lb<MSV, false>(p, m0, a, s);
   switch (ms) {
+    EXX_SYM_CASE(3)
+    EXX_SYM_CASE(4)
     EXX_SYM_CASE(5)
     EXX_SYM_CASE(6)
     EXX_SYM_CASE(7)
@@ -1133,6 +1146,8 @@ cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStr
   if ((e = get_map(st, fa->tgt, a.n, (long long)a.rows_per_rhs * fa->n_tgt, 0, 8 * NT, &m1)) != cudaSuccess) return e;
   ++p->tma_launches;
   switch ((a.nh + 7) / 8) {
+    case 3: return launch_xf<3>(p, m0, m1, a, s);
+    case 4: return launch_xf<4>(p, m0, m1, a, s);
     case 5: return launch_xf<5>(p, m0, m1, a, s);
     case 6: return launch_xf<6>(p, m0, m1, a, s);
     case 7: return launch_xf<7>(p, m0, m1, a, s);
@@ -1157,16 +1172,19 @@ cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, 
   a.div_nk = make_fastdiv((unsigned)a.nk);
   const long long rows_total = (long long)a.rows_per_rhs * nb, rows_psi = (long long)a.rows_per_rhs * fa->n_occ;
   if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
-  const long long tiles_per_rhs = (a.rows_per_rhs + 7) / 8;
+  const int ms = (a.nh + 7) / 8, NT = ms <= 4 ? 2 : 1;
+  const long long tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
   if (tiles_per_rhs * a.nk >= (1LL << 31) - 64) return cudaErrorNotSupported;
   a.n_tiles = (unsigned)(tiles_per_rhs * a.nk);
   if (a.n_tiles == 0) return cudaSuccess;
   CUtensorMap m0, m1;
   cudaError_t e;
-  if ((e = get_map(st, in, a.n, rows_total, 0, 8, &m0)) != cudaSuccess) return e;
-  if ((e = get_map(st, fa->psi, a.n, rows_psi, 0, 8, &m1)) != cudaSuccess) return e;
+  if ((e = get_map(st, in, a.n, rows_total, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  if ((e = get_map(st, fa->psi, a.n, rows_psi, 0, 8 * NT, &m1)) != cudaSuccess) return e;
   ++p->tma_launches;
-  switch ((a.nh + 7) / 8) {
+  switch (ms) {
+    case 3: return launch_xacc_sym<3>(p, m0, m1, a, s);
+    case 4: return launch_xacc_sym<4>(p, m0, m1, a, s);
     case 5: return launch_xacc_sym<5>(p, m0, m1, a, s);
     case 6: return launch_xacc_sym<6>(p, m0, m1, a, s);
     case 7: return launch_xacc_sym<7>(p, m0, m1, a, s);

@@ -191,6 +191,9 @@ FUSION_GRIDS = [
     (72, 4, 4, (0, 0, 0), 0.106),
     (124, 4, 4, (1, 0, 0), 0.0),
     (72, 70, 70, (0, 0, 0), 0.106),
+    # three and four row tiles per block (axes of 34 .. 64 points), all three axes symmetric
+    (40, 36, 34, (0, 1, 0), 0.106),
+    (64, 50, 44, (1, 0, 0), 0.0),
 ]
 
 
