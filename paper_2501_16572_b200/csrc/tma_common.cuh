@@ -72,11 +72,15 @@ __device__ __forceinline__ double lds64(unsigned addr) {
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
 }
+// Called by the elected lane right before it re-arms a ring slot and issues the TMA copies into it, after the
+// __syncwarp that follows the warp's last reads of that slot: the proxy fence orders those generic-proxy reads before
+// the async-proxy writes of the copies (the release half of the per-warp ring; the acquire half is the mbarrier wait).
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Blocks until the phase with the given parity has completed.  A bounded spin turns a lost transaction (a
-// bug) into a trap instead of a hung GPU.
+// Blocks until the phase with the given parity has completed.  A (very generously) bounded spin turns a lost
+// transaction (a bug) into a trap instead of a hung GPU.
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
   unsigned done = 0;
   for (unsigned spin = 0; !done; ++spin) {
@@ -85,7 +89,7 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         : "=r"(done)
         : "r"(bar), "r"(parity)
         : "memory");
-    if (spin > (1u << 24)) __trap();
+    if (spin > (1u << 30)) __trap();  // tens of seconds: far beyond any profiler replay or time-slicing delay
   }
 }
 __device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {

@@ -216,6 +216,10 @@ def test_fused_passes_match_oracle_and_unfused(grid):
     for mask in (0, 1, 2, 3, 6, 7, 9, 15):
         plan.set_fusion(mask)
         assert plan.fusion == mask
+        dense = 4.0 * nx * ny * nz * (nx + ny + nz)
+        assert plan.executed_flops_per_solve <= dense * (1 + 1e-12)
+        if not (mask & 8) or not (mask & 1):
+            assert plan.executed_flops_per_solve == dense        # symmetric mode needs bits 0 and 3
         for n_c in (3, 32):
             phi = plan.poisson_solve(d_C, n_c=n_c)
             assert _rel(phi.cpu().numpy(), phi_o) < TOL
