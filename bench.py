@@ -359,12 +359,9 @@ def measure_ace_and_symmetric(plan, w, d_psi, d_occ, vx, ms_per_step, n_c, nc_sy
         ts.append(a.elapsed_time(b))
     ms_s = statistics.median(ts)
     executed = plan.last_solve_count
-    # the pair-symmetric apply keeps dense x passes (its two-sided accumulate is not fused): with bit 1 off
-    # the plan counts the x axis as dense
-    saved_fusion = plan.fusion
-    plan.set_fusion(saved_fusion & ~2)
-    flops_exec_sym = plan.executed_flops_per_solve
-    plan.set_fusion(saved_fusion)
+    # executed FP64 operations of one executed solve of the pair-symmetric apply: the x-backward product runs once per
+    # side of the two-sided accumulate
+    flops_exec_sym = plan.executed_flops_per_symmetric_solve
     symmetric = {"ms_per_step": ms_s, "n_c": n_c_sym, "executed_solves_per_step": int(executed),
                  "executed_solves_per_s": executed / (ms_s * 1e-3),
                  "pair_equivalent_solves_per_s": w.pair_solves / (ms_s * 1e-3),

@@ -138,6 +138,9 @@ exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h
  * reflection-adapted basis (exx_plan_set_fusion bit 3), whose two products cost about half of that.  bench.py reports
  * the roofline fraction in these executed operations, so that it cannot exceed 1. */
 double exx_plan_executed_flops_per_solve(const exx_plan* plan);
+/* The same for one EXECUTED solve of exx_apply_symmetric: with the x axis on the reflection-adapted basis its x-backward
+ * product runs twice (once for vx_k, once for vx_j: the two-sided accumulate never materialises phi_jk). */
+double exx_plan_executed_flops_per_symmetric_solve(const exx_plan* plan);
 
 /* Test hook: copy out the multiplier table, N doubles, entry [a + nx*(b + ny*c)] = m(lam_x[a]+lam_y[b]+lam_z[c]). */
 exx_status exx_plan_get_multiplier(const exx_plan* plan, double* h_mult);
@@ -257,6 +260,24 @@ exx_status exx_apply_bloch(exx_plan* plan, const double* d_psi, const double* d_
                            size_t workspace_bytes, void* cuda_stream);
 /* Test hook: eigenpairs of one axis of a Bloch plan; h_V_re / h_V_im column-major like exx_plan_get_axis. */
 exx_status exx_plan_get_axis_bloch(const exx_plan* plan, int axis, double* h_lambda, double* h_V_re, double* h_V_im);
+
+/*
+ * ACE tail and application for COMPLEX (k-point) orbitals ("cublasDgemm/cublasZgemm",
+ * "cusolver_dpotrf/cusolver_zpotrf", "cublasDtrsm/cublasZtrsm ... in the case of real/complex-valued computations";
+ * Eqs. 17-20, 26-29 with the transposes read as conjugate transposes, R21):
+ *   M  = h^3 Psi^H W   [n_orb][n_orb] complex,   R R^H = -(M + M^H)/2 (R lower triangular, real positive diagonal),
+ *   xi = W R^-H,       chi = h^3 xi^H Phi,       d_out = -xi chi.
+ * Every function set is [n][2][N] (real plane, then imaginary plane, as in exx_apply_bloch); d_M (optional) receives
+ * M row-major with interleaved (re, im) pairs, 2 n_orb^2 doubles, 16-byte aligned.  The operator does not depend on
+ * the plan's phase (only on N and h), so any plan of the grid serves.  d_xi may equal d_w; d_info, aliasing rules,
+ * workspace alignment and errors as for exx_ace_build / exx_ace_apply; n_orb, n_trial <= 16384.
+ * Workspace: exx_ace_workspace_bytes_bloch(plan, n_orb, n_trial).
+ */
+size_t exx_ace_workspace_bytes_bloch(const exx_plan* plan, int n_orb, int n_trial);
+exx_status exx_ace_build_bloch(exx_plan* plan, const double* d_psi, const double* d_w, int n_orb, double* d_xi,
+                               double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+exx_status exx_ace_apply_bloch(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
+                               double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);

@@ -331,6 +331,12 @@ double exx_plan_executed_flops_per_solve(const exx_plan* plan) {
   return exx::fused_executed_flops_per_solve(plan);
 }
 
+double exx_plan_executed_flops_per_symmetric_solve(const exx_plan* plan) {
+  if (!plan) return 0.0;
+  if (plan->device < 0 || is_complex_plan(plan)) return 4.0 * (double)plan->N * (plan->n[0] + plan->n[1] + plan->n[2]);
+  return exx::fused_executed_flops_per_solve(plan, true);
+}
+
 long long exx_plan_last_launch_count(const exx_plan* plan) { return plan ? plan->last_launches : 0; }
 
 long long exx_plan_last_solve_count(const exx_plan* plan) { return plan ? plan->last_solves : 0; }
@@ -621,19 +627,29 @@ exx_status exx_apply_symmetric(exx_plan* plan, const double* d_psi, const double
   };
   // Batches are rectangles of the (j,k) plane that cover the triangle j <= k: a block of nk consecutive targets
   // against the orbitals 0 .. k0+nk-1 (the nk(nk-1)/2 pairs with j > k inside the diagonal block are solved and
-  // ignored), nk as large as n_c allows; a target with more than n_c partners is cut into j-chunks.
+  // ignored), nk as large as n_c allows; a block with more than n_c pairs is cut into j-chunks.  Where both sides of
+  // the accumulate run fused with the x-backward product (k_mode_xacc_sym, twice), a block has enough targets (at most
+  // 8) to give every warp of the target-side pass a work item.
+  int nk_min = 1;
+  if (plan->variant == EXX_VARIANT_FUSED_DMMA && n_orb > 0) {
+    const exx::FastArgs probe{d_psi, d_psi, d_occ, d_vx, exx::BatchDesc{0, 1, 0, 1}, n_orb, n_orb, false, true};
+    const int rows = exx::sym_xacc_tile_rows(plan);
+    if (rows > 0 && exx::fused_sym_mode(plan) && exx::sym_x_usable(plan, buf0, &probe)) {
+      const long long tiles = ((long long)(N / plan->n[0]) + rows - 1) / rows;
+      const long long want = (12LL * plan->sm_count + tiles - 1) / tiles;
+      nk_min = (int)(want < 1 ? 1 : want > 8 ? 8 : want);
+    }
+  }
   for (int k0 = 0; k0 < n_orb;) {
     int nk = 1;
     while (k0 + nk + 1 <= n_orb && (long long)(nk + 1) * (k0 + nk + 1) <= n_c) ++nk;
-    if (k0 + nk > n_c) {
-      nk = 1;
-      for (int j0 = 0; j0 <= k0; j0 += n_c) {
-        const int nj = k0 + 1 - j0 < n_c ? k0 + 1 - j0 : n_c;
-        exx_status st = run_batch(j0, nj, k0, 1);
-        if (st != EXX_OK) return st;
-      }
-    } else {
-      exx_status st = run_batch(0, k0 + nk, k0, nk);
+    if (nk < nk_min) nk = nk_min;
+    if (nk > n_orb - k0) nk = n_orb - k0;
+    if (nk > n_c) nk = n_c;
+    const int nj_max = n_c / nk;
+    for (int j0 = 0; j0 < k0 + nk; j0 += nj_max) {
+      const int nj = k0 + nk - j0 < nj_max ? k0 + nk - j0 : nj_max;
+      exx_status st = run_batch(j0, nj, k0, nk);
       if (st != EXX_OK) return st;
     }
     k0 += nk;
@@ -849,6 +865,59 @@ exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const do
   long long launches = 0;
   EXX_CUDA(exx::ace_apply(plan, d_xi, n_orb, d_phi, n_trial, d_out, (double*)d_workspace,
                           (cudaStream_t)cuda_stream, &launches));
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+size_t exx_ace_workspace_bytes_bloch(const exx_plan* plan, int n_orb, int n_trial) {
+  if (!plan || n_orb < 1 || n_trial < 0) return 0;
+  const size_t b = exx::ace_build_c_workspace_doubles(plan, n_orb);
+  const size_t a = n_trial > 0 ? exx::ace_apply_c_workspace_doubles(plan, n_orb, n_trial) : 0;
+  return sizeof(double) * (a > b ? a : b);
+}
+
+exx_status exx_ace_build_bloch(exx_plan* plan, const double* d_psi, const double* d_w, int n_orb, double* d_xi,
+                               double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_orb < 1 || n_orb > 16384 || !d_psi || !d_w || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
+  const size_t need = sizeof(double) * exx::ace_build_c_workspace_doubles(plan, n_orb);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if ((((uintptr_t)d_workspace) & 15) || (((uintptr_t)d_M) & 15)) return EXX_ERR_INVALID_ARG;
+  const size_t fn = 2 * sizeof(double) * (size_t)plan->N * (size_t)n_orb;
+  const size_t mm = 2 * sizeof(double) * (size_t)n_orb * n_orb;
+  if ((d_xi != d_w && overlaps(d_xi, fn, d_w, fn)) || overlaps(d_xi, fn, d_psi, fn) ||
+      overlaps(d_xi, fn, d_workspace, need) || overlaps(d_workspace, need, d_psi, fn) ||
+      overlaps(d_workspace, need, d_w, fn) || overlaps(d_M, mm, d_workspace, need) || overlaps(d_M, mm, d_xi, fn) ||
+      overlaps(d_info, sizeof(int), d_workspace, need) || overlaps(d_info, sizeof(int), d_xi, fn))
+    return EXX_ERR_ALIAS;
+  long long launches = 0;
+  EXX_CUDA(exx::ace_build_c(plan, d_psi, d_w, n_orb, d_xi, d_M, d_info, (double*)d_workspace,
+                            (cudaStream_t)cuda_stream, &launches));
+  plan->last_launches = launches;
+  return EXX_OK;
+}
+
+exx_status exx_ace_apply_bloch(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
+                               double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || n_orb < 1 || n_orb > 16384 || n_trial < 0 || n_trial > 16384 || !d_xi) return EXX_ERR_INVALID_ARG;
+  if (n_trial > 0 && (!d_phi || !d_out)) return EXX_ERR_INVALID_ARG;
+  if (plan->device < 0) return cuda_fail(cudaErrorNoDevice);
+  DeviceScope dev_scope(plan->device);
+  if (!dev_scope.ok()) return cuda_fail(dev_scope.err);
+  if (n_trial == 0) { plan->last_launches = 0; return EXX_OK; }
+  const size_t need = sizeof(double) * exx::ace_apply_c_workspace_doubles(plan, n_orb, n_trial);
+  if (!d_workspace || workspace_bytes < need) return EXX_ERR_WORKSPACE;
+  if (((uintptr_t)d_workspace) & 15) return EXX_ERR_INVALID_ARG;
+  const size_t fx = 2 * sizeof(double) * (size_t)plan->N * (size_t)n_orb;
+  const size_t fp = 2 * sizeof(double) * (size_t)plan->N * (size_t)n_trial;
+  if (overlaps(d_out, fp, d_xi, fx) || overlaps(d_out, fp, d_phi, fp) || overlaps(d_out, fp, d_workspace, need) ||
+      overlaps(d_workspace, need, d_xi, fx) || overlaps(d_workspace, need, d_phi, fp))
+    return EXX_ERR_ALIAS;
+  long long launches = 0;
+  EXX_CUDA(exx::ace_apply_c(plan, d_xi, n_orb, d_phi, n_trial, d_out, (double*)d_workspace,
+                            (cudaStream_t)cuda_stream, &launches));
   plan->last_launches = launches;
   return EXX_OK;
 }

@@ -197,12 +197,13 @@ cudaError_t sym_init(exx_plan* p);
 void sym_destroy(exx_plan* p);
 cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s);
 bool sym_x_usable(const exx_plan* p, const double* work, const FastArgs* fa);
+int sym_xacc_tile_rows(const exx_plan* p);
 cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStream_t s);
-cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
+cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s, int side = 0);
 cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);
-double fused_executed_flops_per_solve(const exx_plan* p);
+double fused_executed_flops_per_solve(const exx_plan* p, bool pair_symmetric = false);
 // ---- non-batch Eq. 8 solver, the Fig. 2 comparison line (kernels_nonbatch.cu) ----
 cudaError_t nonbatch_solve_one(exx_plan* p, const double* rhs, double* phi, double* buf0, double* buf1, cudaStream_t s,
                                long long* launches);
@@ -213,6 +214,13 @@ cudaError_t ace_build(exx_plan* p, const double* psi, const double* w, int n, do
                       double* ws, cudaStream_t s, long long* launches);
 cudaError_t ace_apply(exx_plan* p, const double* xi, int n, const double* phi, int m, double* out, double* ws,
                       cudaStream_t s, long long* launches);
+// complex (k-point) orbitals, [n][2][N] planes
+size_t ace_build_c_workspace_doubles(const exx_plan* p, int n);
+size_t ace_apply_c_workspace_doubles(const exx_plan* p, int n, int m);
+cudaError_t ace_build_c(exx_plan* p, const double* psi, const double* w, int n, double* xi, double* M_out, int* info,
+                        double* ws, cudaStream_t s, long long* launches);
+cudaError_t ace_apply_c(exx_plan* p, const double* xi, int n, const double* phi, int m, double* out, double* ws,
+                        cudaStream_t s, long long* launches);
 // ---- Bloch-periodic complex variant (kernels_bloch.cu) ----
 cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd, double* out,
                                cudaStream_t s);

@@ -364,6 +364,190 @@ __global__ void k_subst_op(const double* __restrict__ R, int n, int kb, int nb, 
   G[(long long)i * ldg + k] = v;
 }
 
+// ---- complex (k-point) ACE: the small n x n work in complex arithmetic (cublasZgemm, zpotrf, Ztrsm) ---
+// A set of n complex functions [n][2][N] is also a set of 2n real rows [2n][N] (row 2j = Re psi_j, row 2j+1 = Im psi_j),
+// so the two big products run on the real kernels above with "embedded" shapes: the real Gram matrix G'[2n][2n] of the
+// planes holds all four plane products of Psi^H W, and a complex combination out_i = sum_k T[i][k] in_k is the real
+// k_expand with T'[(i,re)][(k,re)] = T'[(i,im)][(k,im)] = Re T, T'[(i,im)][(k,re)] = -T'[(i,re)][(k,im)] = Im T.
+// Complex n x n matrices are row-major double2 (re, im).
+constexpr int kNBc = 32;  // complex Cholesky / substitution block: 64 real rows, what k_expand's in-place rule allows
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) {  // a * conj(b)
+  return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+
+// M[j][k] = (G[2j][2k] + G[2j+1][2k+1]) + i (G[2j][2k+1] - G[2j+1][2k])  (= h^3 sum conj(psi_j) w_k; G carries the h^3),
+// A = -(M + M^H)/2.  Mout optional.
+__global__ void k_ace_prepare_c(const double* __restrict__ G, int n, double2* __restrict__ A, double2* __restrict__ Mout,
+                                int* info) {
+  const long long ld = 2LL * n;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < (long long)n * n;
+       e += (long long)gridDim.x * blockDim.x) {
+    const long long j = e / n, k = e - j * n;
+    const double mr = G[(2 * j) * ld + 2 * k] + G[(2 * j + 1) * ld + 2 * k + 1];
+    const double mi = G[(2 * j) * ld + 2 * k + 1] - G[(2 * j + 1) * ld + 2 * k];
+    const double tr = G[(2 * k) * ld + 2 * j] + G[(2 * k + 1) * ld + 2 * j + 1];   // M[k][j]
+    const double ti = G[(2 * k) * ld + 2 * j + 1] - G[(2 * k + 1) * ld + 2 * j];
+    if (Mout) Mout[e] = make_double2(mr, mi);
+    A[e] = make_double2(-0.5 * (mr + tr), -0.5 * (mi - ti));
+  }
+  if (info && blockIdx.x == 0 && threadIdx.x == 0) *info = 0;
+}
+
+// One CTA: complex Cholesky of the diagonal block (nb <= 32), R11 written back (real positive diagonal), Tinv = R11^-1.
+__global__ void __launch_bounds__(256) k_potrf_diag_c(double2* A, int n, int kb, int nb, double2* Tinv, int* info) {
+  __shared__ double2 s[kNBc][kNBc + 1];
+  const int tid = threadIdx.x;
+  for (int e = tid; e < kNBc * kNBc; e += 256) {
+    const int i = e / kNBc, j = e % kNBc;
+    s[i][j] = (i < nb && j <= i) ? A[(long long)(kb + i) * n + kb + j] : make_double2(0.0, 0.0);
+    Tinv[e] = make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int c = 0; c < nb; ++c) {
+    if (tid == 0) {
+      const double piv = s[c][c].x;
+      if (!(piv > 0.0) && info && *info == 0) *info = kb + c + 1;
+      s[c][c] = make_double2(sqrt(piv), 0.0);
+    }
+    __syncthreads();
+    const double d = s[c][c].x;
+    for (int i = c + 1 + tid; i < nb; i += 256) s[i][c] = make_double2(s[i][c].x / d, s[i][c].y / d);
+    __syncthreads();
+    const int m = nb - c - 1;
+    for (int e = tid; e < m * m; e += 256) {
+      const int i = c + 1 + e / m, j = c + 1 + e % m;
+      if (j <= i) {
+        const double2 t = cmulc(s[i][c], s[j][c]);
+        s[i][j] = make_double2(s[i][j].x - t.x, s[i][j].y - t.y);
+      }
+    }
+    __syncthreads();
+  }
+  for (int e = tid; e < kNBc * kNBc; e += 256) {
+    const int i = e / kNBc, j = e % kNBc;
+    if (i < nb && j <= i) A[(long long)(kb + i) * n + kb + j] = s[i][j];
+  }
+  if (tid < nb) {  // inverse by forward substitution, one column per thread
+    const int col = tid;
+    double2 x[kNBc];
+    x[col] = make_double2(1.0 / s[col][col].x, 0.0);
+    Tinv[col * kNBc + col] = x[col];
+    for (int i = col + 1; i < nb; ++i) {
+      double2 acc = make_double2(0.0, 0.0);
+      for (int k = col; k < i; ++k) {
+        const double2 t = cmul(s[i][k], x[k]);
+        acc.x += t.x;
+        acc.y += t.y;
+      }
+      x[i] = make_double2(-acc.x / s[i][i].x, -acc.y / s[i][i].x);
+      Tinv[i * kNBc + col] = x[i];
+    }
+  }
+}
+
+// R21 = A21 R11^-H: R21[i][c] = sum_{t <= c} A21[i][t] conj(Tinv[c][t]).  16 rows per CTA.
+__global__ void __launch_bounds__(256) k_potrf_panel_c(double2* A, int n, int kb, int nb, const double2* __restrict__ Tinv) {
+  __shared__ double2 ti[kNBc][kNBc + 1];
+  __shared__ double2 a[16][kNBc + 1];
+  const int tid = threadIdx.x;
+  const int row0 = kb + nb + 16 * blockIdx.x;
+  for (int e = tid; e < kNBc * kNBc; e += 256) ti[e / kNBc][e % kNBc] = Tinv[e];
+  for (int e = tid; e < 16 * kNBc; e += 256) {
+    const int r = e / kNBc, c = e % kNBc;
+    a[r][c] = (row0 + r < n && c < nb) ? A[(long long)(row0 + r) * n + kb + c] : make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int e = tid; e < 16 * kNBc; e += 256) {
+    const int r = e / kNBc, c = e % kNBc;
+    if (row0 + r < n && c < nb) {
+      double2 acc = make_double2(0.0, 0.0);
+      for (int k = 0; k <= c; ++k) {
+        const double2 t = cmulc(a[r][k], ti[c][k]);
+        acc.x += t.x;
+        acc.y += t.y;
+      }
+      A[(long long)(row0 + r) * n + kb + c] = acc;
+    }
+  }
+}
+
+// Trailing update, lower triangle: A[i][j] -= sum_c R[i][kb+c] conj(R[j][kb+c]).  32 x 32 outputs per CTA.
+__global__ void __launch_bounds__(256) k_potrf_update_c(double2* A, int n, int kb, int nb) {
+  if (blockIdx.y > blockIdx.x) return;
+  __shared__ double2 li[32][kNBc + 1];
+  __shared__ double2 lj[32][kNBc + 1];
+  const int tid = threadIdx.x;
+  const int i0 = kb + nb + 32 * blockIdx.x, j0 = kb + nb + 32 * blockIdx.y;
+  for (int e = tid; e < 32 * kNBc; e += 256) {
+    const int r = e / kNBc, c = e % kNBc;
+    li[r][c] = (i0 + r < n && c < nb) ? A[(long long)(i0 + r) * n + kb + c] : make_double2(0.0, 0.0);
+    lj[r][c] = (j0 + r < n && c < nb) ? A[(long long)(j0 + r) * n + kb + c] : make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int e = tid; e < 32 * 32; e += 256) {
+    const int r = e / 32, c = e % 32;
+    const int i = i0 + r, j = j0 + c;
+    if (i < n && j <= i) {
+      double2 acc = make_double2(0.0, 0.0);
+      for (int k = 0; k < nb; ++k) {
+        const double2 t = cmulc(li[r][k], lj[c][k]);
+        acc.x += t.x;
+        acc.y += t.y;
+      }
+      double2 v = A[(long long)i * n + j];
+      A[(long long)i * n + j] = make_double2(v.x - acc.x, v.y - acc.y);
+    }
+  }
+}
+
+// Substitution operator of block row B = [kb, kb+nb): conj(R) xi = W (functions as rows) gives
+//   xi_B = conj(Tinv) (W_B - conj(R[B, <kb]) xi_<kb) = Gc [xi_<kb ; W_B],
+//   Gc[i][k] = conj(-sum_{t <= i} Tinv[i][t] R[kb+t][k])  (k < kb),   Gc[i][kb+t] = conj(Tinv[i][t]),
+// written as its real embedding G'[2 nb][ldg] (ldg >= 2 (kb + nb)).  One thread per complex entry.
+__global__ void k_subst_op_c(const double2* __restrict__ R, int n, int kb, int nb, const double2* __restrict__ Tinv,
+                             double* __restrict__ G, int ldg) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = blockIdx.y;
+  if (k >= kb + nb || i >= nb) return;
+  double2 v;
+  if (k >= kb) {
+    v = Tinv[i * kNBc + (k - kb)];
+  } else {
+    double2 acc = make_double2(0.0, 0.0);
+    for (int t = 0; t <= i; ++t) {
+      const double2 x = cmul(Tinv[i * kNBc + t], R[(long long)(kb + t) * n + k]);
+      acc.x += x.x;
+      acc.y += x.y;
+    }
+    v = make_double2(-acc.x, -acc.y);
+  }
+  const double gr = v.x, gi = -v.y;  // conj
+  double* r0 = G + (long long)(2 * i) * ldg + 2 * k;
+  double* r1 = r0 + ldg;
+  r0[0] = gr;
+  r0[1] = -gi;
+  r1[0] = gi;
+  r1[1] = gr;
+}
+
+// chi[j][a] = h^3 sum conj(xi_j) phi_a from the plane Gram matrix G[2m][2n] (rows: planes of phi, columns: planes of xi),
+// written as the real embedding T'[2m][2n] of T[a][j] = chi[j][a].
+__global__ void k_chi_embed(const double* __restrict__ G, int m, int n, double* __restrict__ T) {
+  const long long ld = 2LL * n;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < (long long)m * n;
+       e += (long long)gridDim.x * blockDim.x) {
+    const long long a = e / n, j = e - a * n;
+    const double tr = G[(2 * a) * ld + 2 * j] + G[(2 * a + 1) * ld + 2 * j + 1];
+    const double ti = G[(2 * a + 1) * ld + 2 * j] - G[(2 * a) * ld + 2 * j + 1];
+    T[(2 * a) * ld + 2 * j] = tr;
+    T[(2 * a) * ld + 2 * j + 1] = -ti;
+    T[(2 * a + 1) * ld + 2 * j] = ti;
+    T[(2 * a + 1) * ld + 2 * j + 1] = tr;
+  }
+}
+
 struct GramSplit {
   int ksplit;
   long long slice;
@@ -514,6 +698,93 @@ cudaError_t ace_apply(exx_plan* p, const double* xi, int n, const double* phi, i
   cudaError_t e;
   if ((e = gram(p, phi, m, xi, n, dV, part, chiT, s, launches)) != cudaSuccess) return e;
   return expand(p, chiT, n, m, n, xi, xi, 0, -1.0, out, s, launches);
+}
+
+// ---- complex (k-point) ACE --------------------------------------------------------------------
+// build: plane Gram partials | G' [2n][2n] | A (complex n x n) | inverses of the diagonal blocks | substitution operator
+// (real embedding, [2 kNBc][2n]) | M (complex n x n)
+size_t ace_build_c_workspace_doubles(const exx_plan* p, int n) {
+  const GramSplit gs = gram_split(2 * n, 2 * n, p->N, p->sm_count);
+  const size_t nblk = (size_t)(n + kNBc - 1) / kNBc;
+  return (size_t)gs.ksplit * 4 * n * n + (size_t)4 * n * n + (size_t)2 * n * n + nblk * 2 * kNBc * kNBc +
+         (size_t)2 * kNBc * 2 * n + (size_t)2 * n * n + 8;
+}
+// apply: plane Gram partials | G' [2m][2n] | T' [2m][2n]
+size_t ace_apply_c_workspace_doubles(const exx_plan* p, int n, int m) {
+  const GramSplit gs = gram_split(2 * m, 2 * n, p->N, p->sm_count);
+  return (size_t)gs.ksplit * 4 * m * n + (size_t)8 * m * n + 8;
+}
+
+// xi = W R^-H with R R^H = -(M + M^H)/2, M = h^3 Psi^H W; psi, w, xi are [n][2][N].  xi may be w (in place).
+cudaError_t ace_build_c(exx_plan* p, const double* psi, const double* w, int n, double* xi, double* M_out, int* info,
+                        double* ws, cudaStream_t s, long long* launches) {
+  const GramSplit gs = gram_split(2 * n, 2 * n, p->N, p->sm_count);
+  double* part = ws;
+  double* Gp = part + (size_t)gs.ksplit * 4 * n * n;
+  double2* A = reinterpret_cast<double2*>(Gp + (size_t)4 * n * n);
+  double2* Tinv = A + (size_t)n * n;
+  const size_t nblk = (size_t)(n + kNBc - 1) / kNBc;
+  double* G = reinterpret_cast<double*>(Tinv + nblk * kNBc * kNBc);
+  double2* M = M_out ? reinterpret_cast<double2*>(M_out) : reinterpret_cast<double2*>(G + (size_t)2 * kNBc * 2 * n);
+  const double dV = p->h * p->h * p->h;
+  cudaError_t e;
+  if ((e = gram(p, psi, 2 * n, w, 2 * n, dV, part, Gp, s, launches)) != cudaSuccess) return e;
+  {
+    int blocks = (int)(((long long)n * n + 255) / 256);
+    if (blocks > 4 * p->sm_count) blocks = 4 * p->sm_count;
+    k_ace_prepare_c<<<blocks, 256, 0, s>>>(Gp, n, A, M_out ? M : nullptr, info);
+    ++*launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  {
+    ProfScope ps(p, KC_OTHER, s);
+    for (int kb = 0, b = 0; kb < n; kb += kNBc, ++b) {
+      const int nb = n - kb < kNBc ? n - kb : kNBc;
+      double2* Tb = Tinv + (size_t)b * kNBc * kNBc;
+      k_potrf_diag_c<<<1, 256, 0, s>>>(A, n, kb, nb, Tb, info);
+      ++*launches;
+      const int below = n - kb - nb;
+      if (below > 0) {
+        k_potrf_panel_c<<<(below + 15) / 16, 256, 0, s>>>(A, n, kb, nb, Tb);
+        const int t = (below + 31) / 32;
+        k_potrf_update_c<<<dim3(t, t), 256, 0, s>>>(A, n, kb, nb);
+        *launches += 2;
+      }
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+  }
+  for (int kb = 0, b = 0; kb < n; kb += kNBc, ++b) {
+    const int nb = n - kb < kNBc ? n - kb : kNBc;
+    const double2* Tb = Tinv + (size_t)b * kNBc * kNBc;
+    k_subst_op_c<<<dim3((kb + nb + 127) / 128, nb), 128, 0, s>>>(A, n, kb, nb, Tb, G, 2 * n);
+    ++*launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    // real rows < 2 kb come from xi (already final), the rows of the block itself from W
+    if ((e = expand(p, G, 2 * n, 2 * nb, 2 * (kb + nb), xi, w, 2 * kb, 1.0, xi + (size_t)2 * kb * p->N, s, launches)) !=
+        cudaSuccess)
+      return e;
+  }
+  return cudaSuccess;
+}
+
+// out = -xi (h^3 xi^H Phi) for complex functions [.][2][N].
+cudaError_t ace_apply_c(exx_plan* p, const double* xi, int n, const double* phi, int m, double* out, double* ws,
+                        cudaStream_t s, long long* launches) {
+  const GramSplit gs = gram_split(2 * m, 2 * n, p->N, p->sm_count);
+  double* part = ws;
+  double* Gp = part + (size_t)gs.ksplit * 4 * m * n;
+  double* T = Gp + (size_t)4 * m * n;
+  const double dV = p->h * p->h * p->h;
+  cudaError_t e;
+  if ((e = gram(p, phi, 2 * m, xi, 2 * n, dV, part, Gp, s, launches)) != cudaSuccess) return e;
+  {
+    int blocks = (int)(((long long)m * n + 255) / 256);
+    if (blocks > 4 * p->sm_count) blocks = 4 * p->sm_count;
+    k_chi_embed<<<blocks, 256, 0, s>>>(Gp, m, n, T);
+    ++*launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  return expand(p, T, 2 * n, 2 * m, 2 * n, xi, xi, 0, -1.0, out, s, launches);
 }
 
 }  // namespace exx

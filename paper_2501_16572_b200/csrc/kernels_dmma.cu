@@ -578,6 +578,13 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
       if (xsym && e == cudaErrorNotSupported) e = cudaErrorUnknown;  // the batch is in x-symmetric order: no fallback
       if (e != cudaSuccess) ps.cancel();
     }
+    if (e == cudaSuccess && xsym && fa->sym) {
+      // pair-symmetric apply: the same pass again with the orbitals as work items (vx_j -= sum_{k > j} occ_k psi_k phi_jk)
+      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      e = sym_xacc(p, cur, nb, fa, s, 1);
+      if (e != cudaSuccess) return e;
+      *launches += 1;
+    }
     if (e == cudaSuccess) {
       *launches += 1;
       return e;

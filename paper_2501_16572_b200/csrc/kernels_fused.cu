@@ -1148,7 +1148,9 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
 // axis (two products, a multiply-add = 2, padding not counted); a z axis on the reflection-adapted basis contracts
 // nh even modes over nh points and n - nh odd modes over n - nh points per column and product, plus n butterfly
 // additions per column and product.
-double fused_executed_flops_per_solve(const exx_plan* p) {
+// pair_symmetric: one executed solve of exx_apply_symmetric, whose x-backward product runs twice (once per side of the
+// two-sided accumulate) when the x axis is on the reflection-adapted basis.
+double fused_executed_flops_per_solve(const exx_plan* p, bool pair_symmetric) {
   const TmaState* st = static_cast<const TmaState*>(p->tma_state);
   const bool sym = fused_sym_mode(p);
   double f = 0.0;
@@ -1157,7 +1159,8 @@ double fused_executed_flops_per_solve(const exx_plan* p) {
     const int nh_ax = !sym ? 0 : ax == 2 ? st->zs_nh : ax == 1 ? st->ys_nh : ((p->fusion & 2) && st->d_mult_symx ? st->xs_nh : 0);
     if (nh_ax) {
       const double nh = nh_ax, no = n - nh;
-      f += 4.0 * (nh * nh + no * no) * (double)p->N / n + 2.0 * (double)p->N;
+      const double one = 2.0 * (nh * nh + no * no) * (double)p->N / n + (double)p->N;
+      f += (ax == 0 && pair_symmetric ? 3.0 : 2.0) * one;
     } else {
       f += 4.0 * (double)p->N * n;
     }

@@ -443,9 +443,13 @@ struct XSArgs {
   int mir0, mirc, zfix;
   unsigned n_tiles;
   int rows_per_rhs, tiles_per_rhs;
-  int nj, nk, j0;
+  // xacc: a work item is (row tile, item i < n_items) and loops over l in [max(0, i + c_lo), min(L, i + c_hi)): right-hand
+  // side i stride_i + l stride_l of the batch, psi / occ of orbital p0 + l, result tile of vx function i.  Full apply and
+  // the target side of the pair-symmetric apply: i = target, l = occupied orbital (j <= k: c_hi = k0 - j0 + 1); its
+  // orbital side: i = orbital j, l = target k > j (c_lo = j0 - k0 + 1).
+  int n_items, L, stride_i, stride_l, c_lo, c_hi, p0;
   int first;
-  FastDiv div_tiles, div_nj, div_nk;
+  FastDiv div_tiles, div_nj, div_items;
   BatchDesc bd;
 };
 
@@ -617,7 +621,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   }
 }
 
-template <int MS, int NT, int WARPS>
+// GEN: items with individual loop ranges and general strides (the pair-symmetric apply); without it every item loops over
+// all L = nj orbitals of the batch with i = target (the full apply).
+template <int MS, int NT, int WARPS, bool GEN>
 __global__ void __launch_bounds__(32 * WARPS, 1)
     k_mode_xacc_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
   constexpr int LDV = 8 * MS + 4;
@@ -648,7 +654,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
   asm volatile("griddepcontrol.wait;\n" ::: "memory");
 
-  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  unsigned tfirst = blockIdx.x + gridDim.x * warp;
   auto claim_tile = [&]() -> unsigned {
     unsigned i = 0;
     if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
@@ -659,16 +665,43 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned fifo[kDepth + 1];
   int fifo_n = 0;
 
-  // producer: item (row tile, target) = nj steps of ST data stages (even modes, then odd modes) + SP psi stage pairs
+  // producer: item (row tile, i) = hi - lo steps of ST data stages (even modes, then odd modes) + SP psi stage pairs
   const int stages_per_step = ST + SP;
+  auto item_range = [&](unsigned t, int& rb, int& i, int& lo, int& hi) {
+    rb = (int)fast_div(t, a.div_items);
+    i = (int)t - rb * a.n_items;
+    lo = 0;
+    hi = a.L;
+    if (GEN) {
+      lo = i + a.c_lo;
+      if (lo < 0) lo = 0;
+      hi = i + a.c_hi;
+      if (hi > a.L) hi = a.L;
+    }
+  };
+  auto next_tile = [&]() -> unsigned {  // the next claimed item whose loop is not empty
+    for (;;) {
+      const unsigned tn = claim_tile();
+      if (!GEN || tn >= a.n_tiles) return tn;
+      int rb, i, lo, hi;
+      item_range(tn, rb, i, lo, hi);
+      if (lo < hi) return tn;
+    }
+  };
+  if (GEN) {
+    int rb, i, lo = 0, hi = 0;
+    if (tfirst < a.n_tiles) item_range(tfirst, rb, i, lo, hi);
+    if (lo >= hi) tfirst = next_tile();
+  }
   unsigned t_p = tfirst;
-  int s_p = 0, jj_p = 0;
+  int s_p = 0, rem_p = 0;  // rem_p: steps of the current item still to be produced
   int prow_d = 0, prow_p = 0;
   auto tile_coords = [&](unsigned t) {
-    const int rb = (int)fast_div(t, a.div_nk);
-    const int kq = (int)t - rb * a.nk;
-    prow_d = (a.nj * kq) * a.rows_per_rhs + rb * (8 * NT);
-    prow_p = a.j0 * a.rows_per_rhs + rb * (8 * NT);
+    int rb, i, lo, hi;
+    item_range(t, rb, i, lo, hi);
+    rem_p = hi - lo;
+    prow_d = (GEN ? i * a.stride_i + lo * a.stride_l : a.L * i) * a.rows_per_rhs + rb * (8 * NT);
+    prow_p = (a.p0 + lo) * a.rows_per_rhs + rb * (8 * NT);
   };
   auto produce = [&](int slot) {
     if (t_p >= a.n_tiles) return;
@@ -687,16 +720,15 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     }
     if (++s_p == stages_per_step) {
       s_p = 0;
-      if (++jj_p == a.nj) {
-        jj_p = 0;
-        t_p = claim_tile();
+      if (--rem_p == 0) {
+        t_p = next_tile();
 #pragma unroll
         for (int i = 0; i < kDepth + 1; ++i)
           if (i == fifo_n) fifo[i] = t_p;
         ++fifo_n;
         if (t_p < a.n_tiles) tile_coords(t_p);
       } else {
-        prow_d += a.rows_per_rhs;
+        prow_d += GEN ? a.stride_l * a.rows_per_rhs : a.rows_per_rhs;
         prow_p += a.rows_per_rhs;
       }
     }
@@ -726,10 +758,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned parity = 0;
   unsigned t = tfirst;
   while (t < a.n_tiles) {
-    const int rb = (int)fast_div(t, a.div_nk);
-    const int kq = (int)t - rb * a.nk;
+    int rb, it, l_lo, l_hi;
+    item_range(t, rb, it, l_lo, l_hi);
     const int row0 = rb * (8 * NT);
-    double* vbase = a.vx + ((long long)kq * a.rows_per_rhs + row0 + 2 * q) * n;
+    double* vbase = a.vx + ((long long)it * a.rows_per_rhs + row0 + 2 * q) * n;
     // vx_k's tile: lo[mt][nt][e] at row 8nt + 2q + e, x = 8mt + g; hi[mt][nt][e] at mir(x)
     double lo[MS][NT][2], hi[MS][NT][2];
 #pragma unroll
@@ -745,7 +777,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
           hi[mt][nt][e] = (rok && x < a.nh && xb != x && xb < n) ? src[xb] : 0.0;
         }
       }
-    for (int jj = 0; jj < a.nj; ++jj) {
+    for (int jj = l_lo; jj < l_hi; ++jj) {
       const double oc = __ldg(a.occ + jj);
       double pa[MS][NT][2], pb[MS][NT][2];
 #pragma unroll
@@ -905,13 +937,13 @@ cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMa
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym2(k_mode_xf_sym<MS, NT, W>, opt, smem, W, p, m0, m1, a, s);
 }
-template <int MS>
+template <int MS, bool GEN>
 cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
   constexpr int W = 12, NT = MS <= 4 ? 2 : 1;
   const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
-  return launch_sym2(k_mode_xacc_sym<MS, NT, W>, opt, smem, W, p, m0, m1, a, s);
+  return launch_sym2(k_mode_xacc_sym<MS, NT, W, GEN>, opt, smem, W, p, m0, m1, a, s);
 }
 
 }  // namespace
@@ -1101,10 +1133,17 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
 // the symmetric table with x, the fused accumulate is on, and every buffer the two kernels touch is TMA-addressable.
 bool sym_x_usable(const exx_plan* p, const double* work, const FastArgs* fa) {
   const TmaState* st = static_cast<const TmaState*>(p->tma_state);
-  if (!st || !st->xs_nh || !st->d_mult_symx || !fa || fa->sym || !(p->fusion & 2)) return false;
+  if (!st || !st->xs_nh || !st->d_mult_symx || !fa || !(p->fusion & 2)) return false;
   if (!aligned16(work) || !aligned16(fa->psi) || !aligned16(fa->tgt) || !aligned16(fa->vx)) return false;
   const long long rpr = p->N / p->n[0];
   return rpr * fa->n_occ < (1LL << 31) - 64 && rpr * fa->n_tgt < (1LL << 31) - 64;
+}
+
+// rows of a work item of k_mode_xacc_sym (0: the plan has no symmetric x axis)
+int sym_xacc_tile_rows(const exx_plan* p) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  if (!st || !st->xs_nh) return 0;
+  return (st->xs_nh + 7) / 8 <= 4 ? 16 : 8;
 }
 
 static void fill_x(const exx_plan* p, const TmaState* st, XSArgs& a) {
@@ -1155,41 +1194,64 @@ cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStr
   }
 }
 
-// x-backward product fused with the accumulate; `in` holds the batch with the x modes even block first.
-cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s) {
+// x-backward product fused with the accumulate; `in` holds the batch with the x modes even block first.  side 0: the
+// work items are the batch's targets (vx_k -= sum_j occ_j psi_j phi_jk; pair-symmetric apply: only j <= k).  side 1
+// (pair-symmetric apply only): the items are the batch's orbitals, vx_j -= sum_{k > j} occ_k psi_k phi_jk -- the same
+// product over the same batch with the roles of the two indices exchanged, so phi never exists in memory either way.
+cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s, int side) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
   if (!sym_x_usable(p, in, fa)) return cudaErrorNotSupported;
-  if (nb != fa->bd.nj * fa->bd.nk) return cudaErrorInvalidValue;
+  if (nb != fa->bd.nj * fa->bd.nk || (side && !fa->sym)) return cudaErrorInvalidValue;
+  constexpr int kBig = 1 << 28;
   XSArgs a{};
   fill_x(p, st, a);
   a.V = st->d_img_xb;
-  a.occ = fa->occ + fa->bd.j0;
-  a.vx = fa->vx + (size_t)fa->bd.k0 * (size_t)p->N;
-  a.nj = fa->bd.nj;
-  a.nk = fa->bd.nk;
-  a.j0 = fa->bd.j0;
+  if (!side) {
+    a.n_items = fa->bd.nk;
+    a.L = fa->bd.nj;
+    a.stride_i = fa->bd.nj;
+    a.stride_l = 1;
+    a.p0 = fa->bd.j0;
+    a.c_lo = -kBig;
+    a.c_hi = fa->sym ? fa->bd.k0 - fa->bd.j0 + 1 : kBig;
+    a.vx = fa->vx + (size_t)fa->bd.k0 * (size_t)p->N;
+  } else {
+    a.n_items = fa->bd.nj;
+    a.L = fa->bd.nk;
+    a.stride_i = 1;
+    a.stride_l = fa->bd.nj;
+    a.p0 = fa->bd.k0;
+    a.c_lo = fa->bd.j0 - fa->bd.k0 + 1;
+    a.c_hi = kBig;
+    a.vx = fa->vx + (size_t)fa->bd.j0 * (size_t)p->N;
+  }
+  a.occ = fa->occ + a.p0;
   a.first = fa->first ? 1 : 0;
-  a.div_nk = make_fastdiv((unsigned)a.nk);
+  a.div_items = make_fastdiv((unsigned)a.n_items);
   const long long rows_total = (long long)a.rows_per_rhs * nb, rows_psi = (long long)a.rows_per_rhs * fa->n_occ;
   if (rows_total >= (1LL << 31) - 64) return cudaErrorNotSupported;
   const int ms = (a.nh + 7) / 8, NT = ms <= 4 ? 2 : 1;
   const long long tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
-  if (tiles_per_rhs * a.nk >= (1LL << 31) - 64) return cudaErrorNotSupported;
-  a.n_tiles = (unsigned)(tiles_per_rhs * a.nk);
+  if (tiles_per_rhs * a.n_items >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  a.n_tiles = (unsigned)(tiles_per_rhs * a.n_items);
   if (a.n_tiles == 0) return cudaSuccess;
   CUtensorMap m0, m1;
   cudaError_t e;
   if ((e = get_map(st, in, a.n, rows_total, 0, 8 * NT, &m0)) != cudaSuccess) return e;
   if ((e = get_map(st, fa->psi, a.n, rows_psi, 0, 8 * NT, &m1)) != cudaSuccess) return e;
   ++p->tma_launches;
+  const bool gen = fa->sym;
+#define EXX_XACC_CASE(MSV) \
+  case MSV: return gen ? launch_xacc_sym<MSV, true>(p, m0, m1, a, s) : launch_xacc_sym<MSV, false>(p, m0, m1, a, s);
   switch (ms) {
-    case 3: return launch_xacc_sym<3>(p, m0, m1, a, s);
-    case 4: return launch_xacc_sym<4>(p, m0, m1, a, s);
-    case 5: return launch_xacc_sym<5>(p, m0, m1, a, s);
-    case 6: return launch_xacc_sym<6>(p, m0, m1, a, s);
-    case 7: return launch_xacc_sym<7>(p, m0, m1, a, s);
-    default: return launch_xacc_sym<8>(p, m0, m1, a, s);
+    EXX_XACC_CASE(3)
+    EXX_XACC_CASE(4)
+    EXX_XACC_CASE(5)
+    EXX_XACC_CASE(6)
+    EXX_XACC_CASE(7)
+    default: return gen ? launch_xacc_sym<8, true>(p, m0, m1, a, s) : launch_xacc_sym<8, false>(p, m0, m1, a, s);
   }
+#undef EXX_XACC_CASE
 }
 
 }  // namespace exx

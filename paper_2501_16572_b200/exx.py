@@ -60,6 +60,8 @@ def load_library():
     lib.exx_plan_get_axis_symmetric.argtypes = [vp, C.c_int, dp, dp, C.POINTER(C.c_int)]
     lib.exx_plan_executed_flops_per_solve.restype = C.c_double
     lib.exx_plan_executed_flops_per_solve.argtypes = [vp]
+    lib.exx_plan_executed_flops_per_symmetric_solve.restype = C.c_double
+    lib.exx_plan_executed_flops_per_symmetric_solve.argtypes = [vp]
     lib.exx_poisson_solve.restype = C.c_int
     lib.exx_poisson_solve.argtypes = [vp, dp, dp, C.c_int, C.c_int, vp, C.c_size_t, vp]
     lib.exx_poisson_solve_nonbatch.restype = C.c_int
@@ -92,6 +94,12 @@ def load_library():
     lib.exx_ace_build.argtypes = [vp, dp, dp, C.c_int, dp, dp, vp, vp, C.c_size_t, vp]
     lib.exx_ace_apply.restype = C.c_int
     lib.exx_ace_apply.argtypes = [vp, dp, C.c_int, dp, C.c_int, dp, vp, C.c_size_t, vp]
+    lib.exx_ace_workspace_bytes_bloch.restype = C.c_size_t
+    lib.exx_ace_workspace_bytes_bloch.argtypes = [vp, C.c_int, C.c_int]
+    lib.exx_ace_build_bloch.restype = C.c_int
+    lib.exx_ace_build_bloch.argtypes = [vp, dp, dp, C.c_int, dp, dp, vp, vp, C.c_size_t, vp]
+    lib.exx_ace_apply_bloch.restype = C.c_int
+    lib.exx_ace_apply_bloch.argtypes = [vp, dp, C.c_int, dp, C.c_int, dp, vp, C.c_size_t, vp]
     lib.exx_plan_create_bloch.restype = C.c_int
     lib.exx_plan_create_bloch.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, ip, C.c_int,
                                           C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int]
@@ -237,6 +245,10 @@ class Plan:
     @property
     def executed_flops_per_solve(self) -> float:
         return float(self._lib.exx_plan_executed_flops_per_solve(self._h))
+
+    @property
+    def executed_flops_per_symmetric_solve(self) -> float:
+        return float(self._lib.exx_plan_executed_flops_per_symmetric_solve(self._h))
 
     def get_multiplier(self) -> np.ndarray:
         m = np.empty((self.nz, self.ny, self.nx))
@@ -471,6 +483,53 @@ class Plan:
                                      _dev_ptr(out, self.device, "out"), C.c_void_p(ws.data_ptr()), ws.numel(),
                                      C.c_void_p(s.cuda_stream))
         _check(st, "exx_ace_apply")
+        return out
+
+    def _ace_ws_c(self, n_orb: int, n_trial: int) -> torch.Tensor:
+        need = int(self._lib.exx_ace_workspace_bytes_bloch(self._h, n_orb, n_trial))
+        if getattr(self, "_aws", None) is None or self._aws.numel() < need:
+            if getattr(self, "_aws", None) is not None:
+                torch.cuda.synchronize(self.device)
+            self._aws = None
+            self._aws = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._aws
+
+    def ace_build_bloch(self, psi: torch.Tensor, w: torch.Tensor, xi: torch.Tensor | None = None, want_M: bool = True,
+                        stream: torch.cuda.Stream | None = None):
+        """exx_ace_build_bloch: complex orbitals [n, 2, nz, ny, nx] (real plane, imaginary plane).
+        Returns (xi, M [n, n, 2] interleaved (re, im) or None, info)."""
+        n = psi.shape[0]
+        if psi.numel() != 2 * n * self.N or w.numel() != 2 * n * self.N:
+            raise ValueError("psi/w must be [n, 2, nz, ny, nx]")
+        if xi is None:
+            xi = torch.empty_like(w)
+        self._expect(xi, 2 * n * self.N, "xi")
+        M = torch.empty((n, n, 2), dtype=torch.float64, device=self.device) if want_M else None
+        info = torch.zeros((), dtype=torch.int32, device=self.device)
+        ws = self._ace_ws_c(n, 0)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_ace_build_bloch(self._h, _dev_ptr(psi, self.device, "psi"), _dev_ptr(w, self.device, "w"), n,
+                                           _dev_ptr(xi, self.device, "xi"), _dev_ptr(M, self.device, "M"),
+                                           C.c_void_p(info.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(),
+                                           C.c_void_p(s.cuda_stream))
+        _check(st, "exx_ace_build_bloch")
+        return xi, M, info
+
+    def ace_apply_bloch(self, xi: torch.Tensor, phi: torch.Tensor, out: torch.Tensor | None = None,
+                        stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+        """exx_ace_apply_bloch: out = -xi (h^3 xi^H phi) for complex functions [m, 2, nz, ny, nx]."""
+        n, m = xi.shape[0], phi.shape[0]
+        if xi.numel() != 2 * n * self.N or phi.numel() != 2 * m * self.N:
+            raise ValueError("xi/phi must be [n, 2, nz, ny, nx]")
+        if out is None:
+            out = torch.empty_like(phi)
+        self._expect(out, 2 * m * self.N, "out")
+        ws = self._ace_ws_c(n, m)
+        s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        st = self._lib.exx_ace_apply_bloch(self._h, _dev_ptr(xi, self.device, "xi"), n, _dev_ptr(phi, self.device, "phi"),
+                                           m, _dev_ptr(out, self.device, "out"), C.c_void_p(ws.data_ptr()), ws.numel(),
+                                           C.c_void_p(s.cuda_stream))
+        _check(st, "exx_ace_apply_bloch")
         return out
 
     def apply_host(self, psi, occ, tgt=None, tgt_start: int = -1, n_tgt: int | None = None, occ_tgt=None,

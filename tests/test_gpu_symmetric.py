@@ -23,20 +23,28 @@ def _rel(a, b):
     return float(np.abs(a - b).max() / np.abs(b).max())
 
 
-def _expected_solves(n, n_c):
-    """The batching rule of exx_apply_symmetric, restated: rectangles covering the triangle j <= k."""
+def _expected_solves(n, n_c, nk_min=1):
+    """The batching rule of exx_apply_symmetric, restated: blocks of nk consecutive targets against the orbitals
+    0 .. k0+nk-1 (cut into j-chunks when that exceeds n_c), nk as large as n_c allows but at least nk_min."""
     k0, total = 0, 0
     while k0 < n:
         nk = 1
         while k0 + nk + 1 <= n and (nk + 1) * (k0 + nk + 1) <= n_c:
             nk += 1
-        if k0 + nk > n_c:
-            nk = 1
-            total += k0 + 1
-        else:
-            total += nk * (k0 + nk)
+        nk = min(max(nk, nk_min), n - k0, n_c)
+        total += nk * (k0 + nk)
         k0 += nk
     return total
+
+
+def _nk_min(nx, ny, nz):
+    """Targets per block the two-sided fused accumulate asks for (exx_api.cu): enough (at most 8) to give each of the 12
+    warps of every SM a work item of 16 (up to 64 half-range x points) or 8 rows."""
+    nh = (nx + 1) // 2
+    rows = 16 if (nh + 7) // 8 <= 4 else 8
+    tiles = (ny * nz + rows - 1) // rows
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    return max(1, min(8, (12 * sms + tiles - 1) // tiles))
 
 
 # (dims, bc, omega, h, n_orb, n_c)
@@ -46,6 +54,11 @@ CASES = [
     ((20, 12, 9), (0, 1, 0), 0.106, 0.3, 7, 5),         # targets with more partners than n_c: j-chunks
     ((13, 17, 11), (1, 1, 1), 0.0, 0.4, 9, 64),         # odd N, whole triangle in few rectangles
     ((24, 20, 16), (0, 0, 1), 0.106, 0.3, 37, 16),
+    # every axis on the reflection-adapted basis: both sides of the accumulate fused with the x-backward product
+    ((40, 36, 34), (0, 0, 1), 0.106, 0.3, 21, 16),      # j-chunks that straddle the diagonal
+    ((36, 40, 44), (1, 0, 0), 0.0, 0.3, 19, 64),
+    ((48, 34, 38), (0, 1, 0), 0.106, 0.25, 9, 1),       # single-pair batches
+    ((72, 36, 34), (0, 0, 0), 0.106, 0.3, 12, 40),      # 8-row work items (more than 32 half-range x points)
 ]
 
 
@@ -62,9 +75,13 @@ def test_symmetric_apply_matches_full_oracle(case, variant):
     plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=64, device=0)
     plan.set_variant(variant)
     d_psi, d_occ = torch.from_numpy(psi).cuda(), torch.from_numpy(occ).cuda()
+    tma0 = plan.tma_launch_count
     vx, e_k, ex = plan.apply_symmetric(d_psi, d_occ, n_c=n_c)
     torch.cuda.synchronize()
-    assert plan.last_solve_count == _expected_solves(n, n_c)
+    two_sided = variant == exx.VARIANT_FUSED_DMMA and min(dims) >= 34
+    assert plan.last_solve_count == _expected_solves(n, n_c, _nk_min(*dims) if two_sided else 1)
+    if two_sided:       # six TMA-staged launches per batch (no streaming accumulate kernel) + zero fills and the energy
+        assert plan.tma_launch_count - tma0 == plan.last_launch_count - 4 and (plan.last_launch_count - 4) % 6 == 0
     assert n * (n + 1) // 2 <= plan.last_solve_count < n * n or n == 1
     assert _rel(vx.cpu().numpy(), vx_o) < TOL
     assert np.abs(e_k.cpu().numpy() - e_o).max() < TOL * np.abs(e_o).max()
@@ -85,7 +102,7 @@ def test_symmetric_on_config2_full_size():
     plan = exx.Plan.for_workload(w, device=0)
     vx, e_k, ex = plan.apply_symmetric(psi.cuda(), occ.cuda(), n_c=128)
     torch.cuda.synchronize()
-    assert plan.last_solve_count == _expected_solves(w.n_orb, 128) < 0.55 * w.n_orb ** 2
+    assert plan.last_solve_count == _expected_solves(w.n_orb, 128, _nk_min(w.nx, w.ny, w.nz)) < 0.6 * w.n_orb ** 2
     assert _rel(vx.cpu().numpy(), vx_o) < TOL
     assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
     plan.close()
