@@ -216,21 +216,49 @@ class ClockSampler:
 
 
 def load_ncu_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` captures: the newest profiles/r*_ncu_traffic.csv (columns cfg,n_c,kernel,dram_read_bytes,
-    dram_write_bytes,...).  {(cfg, n_c): (bytes, file)}; shapes that were not captured report null."""
-    out = {}
+    """Per-kernel dram bytes per launch from the committed `ncu --set full` captures: the newest
+    profiles/r*_ncu_traffic.csv (columns cfg,n_c,kernel,dram_read_bytes,dram_write_bytes,...).
+    {(cfg, n_c): {kernel base name: bytes}}; shapes that were not captured report null."""
+    out, name = {}, None
     files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_ncu_traffic.csv")))
     if not files:
-        return out
+        return out, name
+    name = os.path.basename(files[-1])
     with open(files[-1], newline="") as fh:
         for row in csv.DictReader(r for r in fh if not r.startswith("#")):
             try:
                 key = (int(row["cfg"]), int(row["n_c"]))
-                out[key] = (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), os.path.basename(files[-1]))
+                base = row["kernel"].split("<")[0]
+                out.setdefault(key, {})[base] = float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
             except (KeyError, ValueError):
                 continue
-    return out
+    return out, name
+
+
+def hbm_peak():
+    """Measured copy bandwidth (GB/s) from the driver-written MEASURED_PEAKS.json, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "of measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# Algorithmic HBM bytes per grid point and pair solve of the five-pass structure (DESIGN.md 6): pass 1 writes the batch
+# (8; psi_j and tgt_k tiles are shared by the nk / nj pairs of a batch: 8/nk + 8/nj), passes 2-4 read and write it (48),
+# pass 5 reads it (8) plus the psi tiles (8/nk) and vx_k (16/nj): 64 + 16/nk + 24/nj.  The bound below uses 64.
+ALG_BYTES_PER_POINT = 64.0
+
+
+def step_roofline(flops_exec_per_solve: float, N: int, peak_tflops: float, us_per_solve: float) -> dict:
+    """Whole-step roofline: the slower of (executed FP64 operations / DMMA peak) and (algorithmic bytes / copy bandwidth)."""
+    hbm, src = hbm_peak()
+    t_tensor = flops_exec_per_solve / (peak_tflops * 1e12) * 1e6
+    t_hbm = ALG_BYTES_PER_POINT * N / (hbm * 1e9) * 1e6
+    bound = "tensor" if t_tensor >= t_hbm else "hbm"
+    return {"bound": bound, "us_per_solve_tensor": t_tensor, "us_per_solve_hbm": t_hbm, "us_per_solve_measured": us_per_solve,
+            "frac": max(t_tensor, t_hbm) / us_per_solve, "hbm_peak_gbs": hbm, "hbm_peak_source": src,
+            "algorithmic_bytes_per_solve": ALG_BYTES_PER_POINT * N}
 
 
 def timed_apply(step, steps: int, warmup: int, flush, stream, barrier=None):
@@ -255,22 +283,39 @@ def timed_apply(step, steps: int, warmup: int, flush, stream, barrier=None):
     return sum(e0.elapsed_time(e1) for e0, e1 in ev), res
 
 
-def instrumented(plan, step, flush, prof_steps: int, flops_step: float, peak: float):
-    """Per-kernel-class durations from separate instrumented steps (a CUDA-event pair around every launch on the
-    caller's stream; this defeats the overlap of consecutive launches, so these steps are slightly slower than the
-    timed ones).  Returns the mode-product class's achieved TFLOP/s and the per-class table."""
+KERNEL_OF_PASS = {"x_forward": ("k_mode_xf_sym", "k_mode_t<X, TWO>"), "y_forward": ("k_mode_lf_sym", "k_mode_t<L>"),
+                  "z": ("k_mode_zz_sym", "k_mode_zz"), "z_backward": ("k_mode_t<L, TWO>", "k_mode_t<L, TWO>"),
+                  "y_backward": ("k_mode_lb_sym", "k_mode_t<L>"), "x_backward": ("k_mode_xacc_sym", "k_mode_xacc"),
+                  "x_backward_orbital_side": ("k_mode_xacc_sym", "k_mode_xacc_sym")}
+
+
+def instrumented(plan, step, flush, prof_steps: int, flops_step: float, peak: float, solves_step: int, dense_axis_flops):
+    """Per-kernel durations from separate instrumented steps (a CUDA-event pair around every launch on the caller's
+    stream; this defeats the overlap of consecutive launches, so these steps are slightly slower than the timed ones).
+    Returns the mode-product class's achieved TFLOP/s, the per-class table and the per-kernel table (one kernel per pass
+    of a batch, each with its executed FP64 operations / its summed launch time against the DMMA peak)."""
     plan.set_profiling(True)
     for _ in range(prof_steps):
         flush.fill_(1)
         step()
     prof = plan.get_profile()
+    passes = plan.get_profile_passes()
     plan.set_profiling(False)
     mp_ms, mp_cnt = prof["mode_product"]
     all_ms = sum(v[0] for v in prof.values())
     achieved = flops_step * prof_steps / (mp_ms * 1e-3) / 1e12 if mp_ms > 0 else 0.0
+    kernels = {}
+    for name, (ms, cnt, fl) in passes.items():
+        dense = dense_axis_flops[name[0]] * (2 if name == "z" and "z_backward" not in passes else 1)
+        sym = fl < dense * (1 - 1e-9)
+        tf = fl * solves_step * prof_steps / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        kernels[name] = {"kernel": KERNEL_OF_PASS[name][0 if sym else 1], "launches_per_step": cnt // prof_steps,
+                         "avg_launch_ms": ms / max(cnt, 1), "ms_per_step": ms / prof_steps,
+                         "share_of_step": ms / all_ms if all_ms > 0 else None, "executed_flops_per_solve": fl,
+                         "achieved_tflops": tf, "frac_of_dmma_peak": tf / peak}
     return {"achieved": achieved, "frac": achieved / peak, "avg_launch_ms": mp_ms / max(mp_cnt, 1),
             "launches": mp_cnt // prof_steps, "share_of_step": mp_ms / all_ms if all_ms > 0 else None,
-            "class_ms_per_step": {k: v[0] / prof_steps for k, v in prof.items()}}
+            "class_ms_per_step": {k: v[0] / prof_steps for k, v in prof.items()}, "kernels": kernels}
 
 
 def measure_extra(exx, cfg: int, dev, local: int, peak: float, flush, stream, n_tgt: int = 0, n_c: int = 0,
@@ -300,6 +345,7 @@ def measure_extra(exx, cfg: int, dev, local: int, peak: float, flush, stream, n_
            "n_c": n_c, "pair_solves_per_step": w.pair_solves, "steps": steps, "ms_per_step": ms,
            "value": w.pair_solves / (ms * 1e-3), "unit": UNIT, "applies_per_s": w.n_tgt / (ms * 1e-3),
            "step_frac": flops / (ms * 1e-3) / 1e12 / peak,
+           "step_roofline": step_roofline(plan.executed_flops_per_solve, w.N, peak, ms * 1e3 / w.pair_solves),
            "executed_over_algorithmic_flops": plan.executed_flops_per_solve / w.flops_per_solve, "E_x": float(ex.item()),
            "launches_per_step": plan.last_launch_count}
     if want_ace and w.n_tgt == w.n_orb and w.tgt_start == 0:
@@ -463,30 +509,56 @@ def run_b200(args):
     flops_exec = plan.executed_flops_per_solve
     flops_step = w.n_orb * n_tgt_local * flops_exec
     prof_steps = 1 if ms_per_step > 2000 else min(2, args.steps)
-    inst = instrumented(plan, step, flush, prof_steps, flops_step, peak_dmma)
-    traffic = load_ncu_traffic().get((w.cfg, n_c))
+    dense_axis = {"x": 2.0 * w.N * w.nx, "y": 2.0 * w.N * w.ny, "z": 2.0 * w.N * w.nz}
+    inst = instrumented(plan, step, flush, prof_steps, flops_step, peak_dmma, w.n_orb * n_tgt_local, dense_axis)
+    # the dominant kernel: the pass with the largest share of the step
+    dom_pass, dom = max(inst["kernels"].items(), key=lambda kv: kv[1]["ms_per_step"]) if inst["kernels"] else (None, None)
+    traffic_tab, traffic_file = load_ncu_traffic()
+    traffic = None
+    if dom is not None:
+        traffic = traffic_tab.get((w.cfg, n_c), {}).get(dom["kernel"].split("<")[0])
     n_batch = min(n_c, w.n_orb * n_tgt_local)
+    us_per_solve = ms_per_step * 1e3 / (w.n_orb * n_tgt_local)
     roofline = {"bound": "tensor",
-                "kernel": "k_mode_t (the mode products of a batch, FP64 mma.sync -> DMMA.8x8x4, operands by TMA)",
-                "achieved": inst["achieved"], "peak": peak_dmma, "unit": "TFLOP/s", "frac": inst["frac"],
-                "traffic": traffic[0] if traffic else None,
-                "traffic_note": (f"dram bytes per launch from the committed ncu --set full capture profiles/{traffic[1]}"
-                                 if traffic else "no committed ncu capture for this (config, n_c)")
+                "kernel": (f"{dom['kernel']} ({dom_pass} pass of a batch; FP64 mma.sync -> DMMA.8x8x4, operands by TMA)"
+                           if dom is not None else "mode products"),
+                "achieved": dom["achieved_tflops"] if dom is not None else inst["achieved"], "peak": peak_dmma,
+                "unit": "TFLOP/s", "frac": dom["frac_of_dmma_peak"] if dom is not None else inst["frac"],
+                "traffic": traffic,
+                "traffic_note": (f"dram read + write bytes per launch of this kernel from the committed ncu --set full capture "
+                                 f"profiles/{traffic_file}" if traffic else "no committed ncu capture for this (config, n_c)")
                                 + f"; algorithmic bytes of an in-place pass over one batch = {2 * 8 * w.N * n_batch:.4g}",
+                "achieved_note": "FP64 operations this kernel EXECUTES per launch (exx_plan_get_profile_passes; the dense "
+                                 "algorithmic count of its products would be higher where it runs on the reflection-adapted "
+                                 "basis, DESIGN.md 6.9) / its average launch duration (CUDA events, live)",
                 "peak_source": "measured live by this repo's own probe (exx_probe_fp64_peak, a register-resident DMMA issue "
                                "loop, 1.5 s): MEASURED_PEAKS.json has no FP64 entry and the profiling guide states no FP64 "
                                f"fallback; 148 SMs x 128 flop/clk x 1.965 GHz = 37.2; DFMA loop {peak_dfma:.2f} TF",
-                "avg_launch_ms": inst["avg_launch_ms"], "launches": inst["launches"],
-                "share_of_step": inst["share_of_step"],
+                "avg_launch_ms": dom["avg_launch_ms"] if dom is not None else inst["avg_launch_ms"],
+                "launches": dom["launches_per_step"] if dom is not None else inst["launches"],
+                "share_of_step": dom["share_of_step"] if dom is not None else inst["share_of_step"],
+                "kernels": inst["kernels"],
+                "all_mode_products": {"achieved": inst["achieved"], "frac": inst["frac"], "launches": inst["launches"],
+                                      "avg_launch_ms": inst["avg_launch_ms"], "share_of_step": inst["share_of_step"]},
                 "step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
+                "step": step_roofline(flops_exec, w.N, peak_dmma, us_per_solve),
                 "flops_per_solve_executed": flops_exec, "flops_per_solve_algorithmic": w.flops_per_solve,
                 "executed_over_algorithmic_flops": flops_exec / w.flops_per_solve,
                 "algorithmic_tflops_whole_step": w.n_orb * n_tgt_local * w.flops_per_solve / (ms_per_step * 1e-3) / 1e12,
                 "flops_note": "achieved / frac / step_frac count the FP64 operations the kernels execute (padding excluded); "
-                              "the reflection-adapted z basis halves the operations of the z products, so the dense "
+                              "the reflection-adapted bases halve the operations of the products, so the dense "
                               "algorithmic count would give fractions above 1",
                 "class_ms_per_step": inst["class_ms_per_step"],
                 "measured": f"{prof_steps} separate instrumented step(s) (CUDA-event pair around every launch, caller's stream)"}
+    if roofline["step"]["bound"] == "hbm" and dom is not None:
+        # small grids (48^3): the five passes move more time through HBM than through the tensor pipe -- report the dominant
+        # kernel against the copy bandwidth (algorithmic bytes of one in-place pass over a full batch), tensor numbers in "kernels"
+        gbs = 2 * 8 * w.N * n_batch / (dom["avg_launch_ms"] * 1e-3) / 1e9
+        roofline.update({"bound": "hbm", "achieved": gbs, "peak": roofline["step"]["hbm_peak_gbs"], "unit": "GB/s",
+                         "frac": gbs / roofline["step"]["hbm_peak_gbs"],
+                         "peak_source": roofline["step"]["hbm_peak_source"],
+                         "achieved_note": "algorithmic bytes of one in-place pass over a full batch (2 x 8 x N x n_c) / this "
+                                          "kernel's average launch duration (CUDA events, live)"})
 
     # ---- launch-bound steps (config 1: 64 solves in 7 launches): the same step replayed from a CUDA graph ----
     graph = None
@@ -673,9 +745,6 @@ def run_solver_sweep(args):
     rhs = wl.make_rhs(w, n_rhs, dev)
     out = torch.empty_like(rhs)
     plan = exx.Plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, max_batch=512, device=0)
-    # the bare solver has no symmetric x passes: with bit 1 off the plan counts the x axis as dense, which
-    # is what exx_poisson_solve executes (bit 1 only concerns the accumulate of exx_apply)
-    plan.set_fusion(plan.fusion & ~2)
     flops_exec = plan.executed_flops_per_solve
     peak = exx.probe_fp64_peak(1, 0, 1.0)
     stream = torch.cuda.current_stream(dev)

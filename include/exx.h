@@ -297,6 +297,13 @@ long long exx_plan_tma_launch_count(const exx_plan* plan);
  */
 exx_status exx_plan_set_profiling(exx_plan* plan, int on);
 exx_status exx_plan_get_profile(exx_plan* plan, double* h_ms, long long* h_count);
+/* The mode-product launches of the records the last exx_plan_get_profile call consumed, per pass of a batch, h_ms[8] /
+ * h_count[8]: 0 = x-forward (with a1), 1 = y-forward, 2 = z (the fused z-forward / a3 / z-backward pass, or the z-forward
+ * product where it is not fused), 3 = z-backward (unfused only), 4 = y-backward, 5 = x-backward (with a5 where fused),
+ * 6 = the second x-backward pass of exx_apply_symmetric (orbital side), 7 = unused.  h_flops_per_solve[8] (optional, NULL):
+ * the FP64 operations one pair solve executes in that pass with the plan's current settings (as
+ * exx_plan_executed_flops_per_solve counts them).  Host only, no synchronisation. */
+exx_status exx_plan_get_profile_passes(const exx_plan* plan, double* h_ms, long long* h_count, double* h_flops_per_solve);
 
 /*
  * Diagnostic: sustained FP64 throughput of this GPU in TFLOP/s over about `seconds` (0 < seconds <= 30) of

@@ -129,6 +129,7 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->N = (long long)nx * ny * nz;
   p->d_mult = nullptr; p->tma_state = nullptr; p->sm_count = 148; p->smem_optin = 0; p->last_launches = 0; p->last_solves = 0; p->tma_launches = 0;
   p->prof_on = false; p->accumulate = false;
+  for (int c = 0; c < exx::PASS_COUNT; ++c) { p->prof_pass_ms[c] = 0.0; p->prof_pass_count[c] = 0; }
   p->fusion = 15;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
@@ -352,18 +353,43 @@ exx_status exx_plan_set_profiling(exx_plan* plan, int on) {
 exx_status exx_plan_get_profile(exx_plan* plan, double* h_ms, long long* h_count) {
   if (!plan || !h_ms || !h_count) return EXX_ERR_INVALID_ARG;
   for (int c = 0; c < exx::KC_COUNT; ++c) { h_ms[c] = 0.0; h_count[c] = 0; }
+  for (int c = 0; c < exx::PASS_COUNT; ++c) { plan->prof_pass_ms[c] = 0.0; plan->prof_pass_count[c] = 0; }
   cudaError_t err = cudaSuccess;
   for (auto& r : plan->prof) {
     float ms = 0.f;
     cudaError_t e = cudaEventSynchronize(r.e1);
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.e0, r.e1);
     if (e != cudaSuccess) err = e;
-    else { h_ms[r.cls] += ms; h_count[r.cls] += 1; }
+    else {
+      h_ms[r.cls] += ms;
+      h_count[r.cls] += 1;
+      if (r.pass >= 0 && r.pass < exx::PASS_COUNT) { plan->prof_pass_ms[r.pass] += ms; plan->prof_pass_count[r.pass] += 1; }
+    }
     cudaEventDestroy(r.e0);
     cudaEventDestroy(r.e1);
   }
   plan->prof.clear();
   return err == cudaSuccess ? EXX_OK : cuda_fail(err);
+}
+
+exx_status exx_plan_get_profile_passes(const exx_plan* plan, double* h_ms, long long* h_count, double* h_flops_per_solve) {
+  if (!plan || !h_ms || !h_count) return EXX_ERR_INVALID_ARG;
+  for (int c = 0; c < exx::PASS_COUNT; ++c) {
+    h_ms[c] = plan->prof_pass_ms[c];
+    h_count[c] = plan->prof_pass_count[c];
+    if (h_flops_per_solve) h_flops_per_solve[c] = 0.0;
+  }
+  if (h_flops_per_solve && plan->device >= 0 && !is_complex_plan(plan)) {
+    // executed operations of one product per axis (exx_plan_executed_flops_per_solve counts two per axis)
+    const int ax_of[exx::PASS_COUNT] = {0, 1, 2, 2, 1, 0, 0, -1};
+    for (int c = 0; c < exx::PASS_COUNT; ++c)
+      if (ax_of[c] >= 0) h_flops_per_solve[c] = exx::fused_executed_flops_axis(plan, ax_of[c]);
+    if (plan->prof_pass_count[exx::PASS_ZB] == 0) {  // fused z pass: both z products in PASS_Z
+      h_flops_per_solve[exx::PASS_Z] *= 2.0;
+      h_flops_per_solve[exx::PASS_ZB] = 0.0;
+    }
+  }
+  return EXX_OK;
 }
 
 }  // extern "C"

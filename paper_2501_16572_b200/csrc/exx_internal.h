@@ -31,9 +31,14 @@ std::vector<double> multiplier_table(const std::vector<double>& lx, const std::v
 
 namespace exx {
 enum KernelClass { KC_MODE_PRODUCT = 0, KC_PAIR_DENSITY = 1, KC_ACCUMULATE = 2, KC_OTHER = 3, KC_COUNT = 4 };
+// Passes of a batch (exx_plan_get_profile_passes): x-forward (+ a1), y-forward, z (fused z-forward / a3 / z-backward, or
+// the z-forward product alone), z-backward (unfused only), y-backward, x-backward (+ a5), x-backward of the orbital side
+// of the pair-symmetric apply.
+enum PassId { PASS_XF = 0, PASS_YF = 1, PASS_Z = 2, PASS_ZB = 3, PASS_YB = 4, PASS_XB = 5, PASS_XB2 = 6, PASS_COUNT = 8 };
 struct ProfRec {
   cudaEvent_t e0, e1;
   int cls;
+  int pass;  // PassId, or -1
 };
 }  // namespace exx
 
@@ -79,6 +84,8 @@ struct exx_plan {
   bool accumulate;  // exx_plan_set_accumulate: exx_apply adds into d_vx instead of overwriting it
   bool prof_on;
   std::vector<exx::ProfRec> prof;
+  double prof_pass_ms[exx::PASS_COUNT];        // filled by exx_plan_get_profile, read by exx_plan_get_profile_passes
+  long long prof_pass_count[exx::PASS_COUNT];
 };
 
 namespace exx {
@@ -144,13 +151,13 @@ struct ProfScope {
   exx_plan* p;
   cudaStream_t s;
   cudaEvent_t e1;
-  ProfScope(exx_plan* plan, int cls, cudaStream_t stream) : p(plan), s(stream), e1(nullptr) {
+  ProfScope(exx_plan* plan, int cls, cudaStream_t stream, int pass = -1) : p(plan), s(stream), e1(nullptr) {
     if (!p->prof_on) return;
     cudaEvent_t e0;
     if (cudaEventCreate(&e0) != cudaSuccess) return;
     if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); e1 = nullptr; return; }
     cudaEventRecord(e0, s);
-    p->prof.push_back(ProfRec{e0, e1, cls});
+    p->prof.push_back(ProfRec{e0, e1, cls, pass});
   }
   ~ProfScope() {
     if (e1) cudaEventRecord(e1, s);
@@ -198,12 +205,16 @@ void sym_destroy(exx_plan* p);
 cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s);
 bool sym_x_usable(const exx_plan* p, const double* work, const FastArgs* fa);
 int sym_xacc_tile_rows(const exx_plan* p);
+bool sym_x_usable_plain(const exx_plan* p, const double* src, const double* work, int nb);
+cudaError_t sym_xf_plain(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s);
+cudaError_t sym_xb_plain(exx_plan* p, double* buf, int nb, cudaStream_t s);
 cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStream_t s);
 cudaError_t sym_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s, int side = 0);
 cudaError_t fused_zz_c(exx_plan* p, double* buf, int nb, cudaStream_t s);  // Bloch plans, complex z axis, n <= 64
 cudaError_t fused_xacc(exx_plan* p, const double* in, int nb, const FastArgs* fa, cudaStream_t s);
 int fused_xacc_tile_rows(const exx_plan* p);
 double fused_executed_flops_per_solve(const exx_plan* p, bool pair_symmetric = false);
+double fused_executed_flops_axis(const exx_plan* p, int ax);
 // ---- non-batch Eq. 8 solver, the Fig. 2 comparison line (kernels_nonbatch.cu) ----
 cudaError_t nonbatch_solve_one(exx_plan* p, const double* rhs, double* phi, double* buf0, double* buf1, cudaStream_t s,
                                long long* launches);

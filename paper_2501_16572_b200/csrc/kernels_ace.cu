@@ -130,14 +130,18 @@ __global__ void __launch_bounds__(128)
   }
 }
 
-// C[i][j] = alpha * sum_ks part[ks][i][j], ks ascending (fixed order)
-__global__ void k_gram_reduce(const double* __restrict__ part, int ksplit, long long nn, double alpha,
-                              double* __restrict__ C) {
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < nn;
-       e += (long long)gridDim.x * blockDim.x) {
+// C[i][j] = alpha * sum_ks part[ks][i][j] in a fixed order (bitwise reproducible): a block of 256 threads handles 8
+// entries; lane l of an entry's 32 lanes adds the slices l, l + 32, ... in ascending order, then the 32 lane sums are
+// combined by a fixed shuffle tree.
+__global__ void __launch_bounds__(256) k_gram_reduce(const double* __restrict__ part, int ksplit, long long nn, double alpha,
+                                                     double* __restrict__ C) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (long long e = blockIdx.x * 8LL + w; e < nn; e += 8LL * gridDim.x) {
     double s = 0.0;
-    for (int k = 0; k < ksplit; ++k) s += part[(long long)k * nn + e];
-    C[e] = alpha * s;
+    for (int k = lane; k < ksplit; k += 32) s += part[(long long)k * nn + e];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    if (lane == 0) C[e] = alpha * s;
   }
 }
 
@@ -282,18 +286,32 @@ __global__ void __launch_bounds__(256) k_potrf_diag(double* A, int n, int kb, in
     const int i = e / kNB, j = e % kNB;
     if (i < nb && j <= i) A[(long long)(kb + i) * n + kb + j] = s[i][j];
   }
-  // inverse by forward substitution, one column per thread: R11 x = e_col (x lives in local memory)
-  if (tid < nb) {
-    const int col = tid;
-    double x[kNB];
-    x[col] = 1.0 / s[col][col];
-    Tinv[col * kNB + col] = x[col];
-    for (int i = col + 1; i < nb; ++i) {
-      double acc = 0.0;
-      for (int k = col; k < i; ++k) acc += s[i][k] * x[k];
-      x[i] = -acc / s[i][i];
-      Tinv[i * kNB + col] = x[i];
+  // Tinv = R11^-1 by forward substitution on all nb unit right-hand sides at once: X starts as the identity; step k
+  // scales row k by 1 / R[k][k] and subtracts R[i][k] X[k][:] from every row i > k.  X is lower triangular like R, so it
+  // lives in the unused strict upper triangle of s (X[i][j] at s[j][i], i > j) plus its diagonal in xd.  Thread t owns
+  // column t % 64 of the rows i == t / 64 (mod 4).
+  __shared__ double xd[kNB];
+  __syncthreads();
+  if (tid < kNB) xd[tid] = 1.0;
+  __syncthreads();
+  {
+    const int col = tid & (kNB - 1), r0 = tid >> 6;
+    for (int k = 0; k < nb; ++k) {
+      if (r0 == 0 && col <= k) {
+        if (col == k) xd[k] /= s[k][k];
+        else s[col][k] /= s[k][k];
+      }
+      __syncthreads();
+      if (col <= k) {
+        const double xk = col == k ? xd[k] : s[col][k];
+        for (int i = k + 1 + r0; i < nb; i += 4) s[col][i] -= s[i][k] * xk;
+      }
+      __syncthreads();
     }
+  }
+  for (int e = tid; e < kNB * kNB; e += 256) {
+    const int i = e / kNB, j = e % kNB;
+    if (i < nb && j <= i) Tinv[e] = i == j ? xd[i] : s[j][i];
   }
 }
 
@@ -596,8 +614,8 @@ cudaError_t gram(exx_plan* p, const double* A, int ni, const double* B, int nj, 
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
   const long long nn = (long long)ni * nj;
-  int blocks = (int)((nn + 255) / 256);
-  if (blocks > 4 * p->sm_count) blocks = 4 * p->sm_count;
+  int blocks = (int)((nn + 7) / 8);
+  if (blocks > 8 * p->sm_count) blocks = 8 * p->sm_count;
   k_gram_reduce<<<blocks, 256, 0, s>>>(part, gs.ksplit, nn, alpha, C);
   *launches += 2;
   return cudaGetLastError();

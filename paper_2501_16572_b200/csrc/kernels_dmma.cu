@@ -475,7 +475,8 @@ void fast_destroy(exx_plan* p) {
 // in the DMMA kernel; `mult_pending` carries it from one to the other.
 static cudaError_t one_product(exx_plan* p, int axis, bool fwd, const double* src, double*& cur, double*& other,
                                int nb, bool& mult_pending, cudaStream_t s) {
-  ProfScope ps(p, KC_MODE_PRODUCT, s);
+  static const int kPass[3][2] = {{PASS_XB, PASS_XF}, {PASS_YB, PASS_YF}, {PASS_ZB, PASS_Z}};
+  ProfScope ps(p, KC_MODE_PRODUCT, s, kPass[axis][fwd ? 1 : 0]);
   const bool z_bwd = axis == 2 && !fwd;
   cudaError_t e = cudaErrorNotSupported;
   if (p->variant == EXX_VARIANT_FUSED_DMMA)
@@ -515,7 +516,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   if (fa) {
     // a1 fused into the first product: rho = psi_j .* tgt_k is formed in the load path
     {
-      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_XF);
       e = cudaErrorNotSupported;
       if (xsym) {
         e = sym_xf(p, cur, nb, fa, s);
@@ -534,6 +535,20 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
     }
     if (e != cudaSuccess) return e;
   }
+  // bare solver: both x passes on the reflection-adapted basis where the plan and the buffers allow it
+  bool xsym_plain = !fa && p->variant == EXX_VARIANT_FUSED_DMMA && fused_sym_mode(p) && sym_x_usable_plain(p, src, cur, nb);
+  if (xsym_plain) {
+    ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_XF);
+    e = sym_xf_plain(p, src, cur, nb, s);
+    if (e == cudaErrorNotSupported) {
+      ps.cancel();
+      xsym_plain = false;
+    } else if (e != cudaSuccess) {
+      return e;
+    } else {
+      first_done = true;
+    }
+  }
   if (!first_done && (e = one_product(p, 0, true, src, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
   // Symmetric mode: the y and z products on the reflection-adapted eigenbases, eigen-space data and
   // table in (even | odd) mode order.  Decided once per batch: it needs every remaining pass on the TMA kernels, which
@@ -541,7 +556,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   const bool sym = fused_sym_mode(p) && p->tma_launches > tma_before && (((uintptr_t)cur) & 15) == 0;
   auto y_product = [&](bool fwd) -> cudaError_t {
     if (sym) {
-      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      ProfScope ps(p, KC_MODE_PRODUCT, s, fwd ? PASS_YF : PASS_YB);
       const cudaError_t ey = sym_mode_product_y(p, fwd, cur, nb, s);
       if (ey == cudaSuccess) return ey;
       ps.cancel();
@@ -553,8 +568,8 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   // z-forward + multiplier + z-backward: one fused pass where k_mode_zz can run, else two passes
   e = cudaErrorNotSupported;
   if (p->variant == EXX_VARIANT_FUSED_DMMA) {
-    ProfScope ps(p, KC_MODE_PRODUCT, s);
-    e = fused_zz(p, cur, cur, nb, s, xsym ? 2 : sym ? 1 : 0);
+    ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_Z);
+    e = fused_zz(p, cur, cur, nb, s, (xsym || xsym_plain) ? 2 : sym ? 1 : 0);
     if (e != cudaSuccess) ps.cancel();
   }
   if (e == cudaSuccess) {
@@ -573,14 +588,14 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
   // x-backward + accumulate: one fused pass where k_mode_xacc can run
   if (fa && p->variant == EXX_VARIANT_FUSED_DMMA) {
     {
-      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_XB);
       e = xsym ? sym_xacc(p, cur, nb, fa, s) : fused_xacc(p, cur, nb, fa, s);
       if (xsym && e == cudaErrorNotSupported) e = cudaErrorUnknown;  // the batch is in x-symmetric order: no fallback
       if (e != cudaSuccess) ps.cancel();
     }
     if (e == cudaSuccess && xsym && fa->sym) {
       // pair-symmetric apply: the same pass again with the orbitals as work items (vx_j -= sum_{k > j} occ_k psi_k phi_jk)
-      ProfScope ps(p, KC_MODE_PRODUCT, s);
+      ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_XB2);
       e = sym_xacc(p, cur, nb, fa, s, 1);
       if (e != cudaSuccess) return e;
       *launches += 1;
@@ -590,6 +605,12 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
       return e;
     }
     if (e != cudaErrorNotSupported) return e;
+  }
+  if (xsym_plain) {  // the batch is in x-symmetric mode order: no fallback
+    ProfScope ps(p, KC_MODE_PRODUCT, s, PASS_XB);
+    e = sym_xb_plain(p, cur, nb, s);
+    *launches += 1;
+    return e == cudaErrorNotSupported ? cudaErrorUnknown : e;
   }
   if ((e = one_product(p, 0, false, cur, cur, other, nb, mult_pending, s)) != cudaSuccess) return e;
   *launches += 1;

@@ -1148,6 +1148,17 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
 // axis (two products, a multiply-add = 2, padding not counted); a z axis on the reflection-adapted basis contracts
 // nh even modes over nh points and n - nh odd modes over n - nh points per column and product, plus n butterfly
 // additions per column and product.
+// FP64 operations of ONE product along axis ax per pair solve with the plan's current settings.
+double fused_executed_flops_axis(const exx_plan* p, int ax) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  const bool sym = fused_sym_mode(p);
+  const double n = p->n[ax];
+  const int nh_ax = !sym ? 0 : ax == 2 ? st->zs_nh : ax == 1 ? st->ys_nh : ((p->fusion & 2) && st->d_mult_symx ? st->xs_nh : 0);
+  if (!nh_ax) return 2.0 * (double)p->N * n;
+  const double nh = nh_ax, no = n - nh;
+  return 2.0 * (nh * nh + no * no) * (double)p->N / n + (double)p->N;
+}
+
 // pair_symmetric: one executed solve of exx_apply_symmetric, whose x-backward product runs twice (once per side of the
 // two-sided accumulate) when the x axis is on the reflection-adapted basis.
 double fused_executed_flops_per_solve(const exx_plan* p, bool pair_symmetric) {

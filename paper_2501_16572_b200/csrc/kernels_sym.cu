@@ -456,13 +456,15 @@ struct XSArgs {
 // X-mode box ({16 x, rows}, 128-byte rows and swizzle): offset of (row 8nt + g, x) without the 1024 nt term
 __device__ __forceinline__ unsigned offx(unsigned x, unsigned g) { return 128u * g + 16u * ((x >> 1) ^ g) + 8u * (x & 1); }
 
-template <int MS, int NT, int WARPS>
+// PD: the right-hand side is the pair density psi_j * tgt_k formed from two TMA streams (exchange apply); without it the
+// kernel reads nb right-hand sides from tm0 (the bare solver) and a stage is two boxes.
+template <int MS, int NT, int WARPS, bool PD>
 __global__ void __launch_bounds__(32 * WARPS, 1)
     k_mode_xf_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
   constexpr int MT = 2 * MS;
   constexpr int LDV = 8 * MT + 4;
   constexpr unsigned kBox = 1024u * NT;   // one {16 x, 8 NT rows} box
-  constexpr unsigned kSlot = 4u * kBox;   // psi block, psi mirrored block, tgt block, tgt mirrored block
+  constexpr unsigned kSlot = (PD ? 4u : 2u) * kBox;   // psi block, psi mirrored block(, tgt block, tgt mirrored block)
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
@@ -503,10 +505,14 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   auto tile_coords = [&](unsigned t) {
     const int rhs = (int)fast_div(t, a.div_tiles);
     const int rb = (int)t - rhs * a.tiles_per_rhs;
-    const int kq = (int)fast_div((unsigned)rhs, a.div_nj);
-    const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
-    pr0 = j * a.rows_per_rhs + rb * (8 * NT);
-    pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+    if (PD) {
+      const int kq = (int)fast_div((unsigned)rhs, a.div_nj);
+      const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
+      pr0 = j * a.rows_per_rhs + rb * (8 * NT);
+      pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+    } else {
+      pr0 = rhs * a.rows_per_rhs + rb * (8 * NT);
+    }
   };
   auto produce = [&](int slot) {
     if (t_p >= a.n_tiles) return;
@@ -516,8 +522,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       mbar_expect_tx(bar, kSlot);
       tma_load_2d(dst, &tm0, 16 * s_p, pr0, bar);
       tma_load_2d(dst + kBox, &tm0, a.mir0 - 16 * s_p, pr0, bar);
-      tma_load_2d(dst + 2 * kBox, &tm1, 16 * s_p, pr1, bar);
-      tma_load_2d(dst + 3 * kBox, &tm1, a.mir0 - 16 * s_p, pr1, bar);
+      if (PD) {
+        tma_load_2d(dst + 2 * kBox, &tm1, 16 * s_p, pr1, bar);
+        tma_load_2d(dst + 3 * kBox, &tm1, a.mir0 - 16 * s_p, pr1, bar);
+      }
     }
     if (++s_p == Sh) {
       s_p = 0;
@@ -570,8 +578,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
           for (int nt = 0; nt < NT; ++nt) {
             const unsigned oa = sb + 1024u * nt + (ragged ? offx((unsigned)xl, g) : xo[kk]);
             const unsigned ob = sb + 1024u * nt + (ragged ? kBox + offx(15u - (unsigned)xl, g) : xm[kk]);
-            const double va = lds64(oa) * lds64(oa + 2 * kBox);
-            double vb = lds64(ob) * lds64(ob + 2 * kBox);
+            const double va = PD ? lds64(oa) * lds64(oa + 2 * kBox) : lds64(oa);
+            double vb = PD ? lds64(ob) * lds64(ob + 2 * kBox) : lds64(ob);
             if (xl == zf) vb = 0.0;
             be[nt] = va + vb;
             bo[nt] = va - vb;
@@ -866,6 +874,152 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   }
 }
 
+// k_mode_xb_sym: the x-backward product alone (the bare solver): a = E t_even, b = O t_odd over the half range,
+// out[x] = a + b, out[mir x] = a - b, in place over the rows of a tile.  Data stages as in k_mode_xacc_sym.
+template <int MS, int NT, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS, 1) k_mode_xb_sym(const __grid_constant__ CUtensorMap tm0, const XSArgs a) {
+  constexpr int LDV = 8 * MS + 4;
+  constexpr unsigned kBox = 1024u * NT;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int g = lane >> 2, q = lane & 3;
+  const int n = a.n, SE = a.Sh, ST = a.Sh + a.So;
+  const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
+  const unsigned img_bytes = 8u * (16u * ST) * LDV;
+  for (unsigned i = 2 * tid; i < 16u * ST * LDV; i += 2 * 32 * WARPS)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
+  asm volatile("cp.async.commit_group;\n" ::: "memory");
+  const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
+  const unsigned my_ring = ring0 + warp * (kDepth * kBox);
+  const unsigned my_bar = ring0 + WARPS * (kDepth * kBox) + warp * (kDepth * 8u);
+  const unsigned ctr_addr = ring0 + WARPS * (kDepth * kBox) + WARPS * (kDepth * 8u);
+  if (tid == 0) asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(ctr_addr), "r"((unsigned)WARPS) : "memory");
+  if (lane == 0) {
+#pragma unroll
+    for (int d = 0; d < kDepth; ++d) mbar_init(my_bar + 8u * d, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+
+  const unsigned tfirst = blockIdx.x + gridDim.x * warp;
+  auto claim_tile = [&]() -> unsigned {
+    unsigned i = 0;
+    if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;\n" : "=r"(i) : "r"(ctr_addr) : "memory");
+    i = __shfl_sync(0xffffffffu, i, 0);
+    const unsigned long long t = (unsigned long long)blockIdx.x + (unsigned long long)gridDim.x * i;
+    return t < a.n_tiles ? (unsigned)t : 0xffffffffu;
+  };
+  unsigned fifo[kDepth + 1];
+  int fifo_n = 0;
+  unsigned t_p = tfirst;
+  int s_p = 0;
+  int prow = 0;
+  auto tile_coords = [&](unsigned t) {
+    const int rhs = (int)fast_div(t, a.div_tiles);
+    const int rb = (int)t - rhs * a.tiles_per_rhs;
+    prow = rhs * a.rows_per_rhs + rb * (8 * NT);
+  };
+  auto produce = [&](int slot) {
+    if (t_p >= a.n_tiles) return;
+    const unsigned bar = my_bar + 8u * slot;
+    const unsigned dst = my_ring + slot * kBox;
+    if (elect_one()) {
+      mbar_expect_tx(bar, kBox);
+      tma_load_2d(dst, &tm0, s_p < SE ? 16 * s_p : a.nh + 16 * (s_p - SE), prow, bar);
+    }
+    if (++s_p == ST) {
+      s_p = 0;
+      t_p = claim_tile();
+#pragma unroll
+      for (int i = 0; i < kDepth + 1; ++i)
+        if (i == fifo_n) fifo[i] = t_p;
+      ++fifo_n;
+      if (t_p < a.n_tiles) tile_coords(t_p);
+    }
+  };
+  if (t_p < a.n_tiles) tile_coords(t_p);
+#pragma unroll
+  for (int d = 0; d < kDepth; ++d) produce(d);
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  __syncthreads();
+
+  unsigned a_lane_v = smem0 + 8u * (q * LDV + g);
+  unsigned xo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) xo[i] = offx((q & 1) + 8u * (q >> 1) + 2u * i, g);
+
+  int slot = 0;
+  unsigned parity = 0;
+  unsigned t = tfirst;
+  while (t < a.n_tiles) {
+    double pa[MS][NT][2], pb[MS][NT][2];
+#pragma unroll
+    for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
+    auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+      asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
+      mbar_wait(my_bar + 8u * slot, parity);
+      const unsigned sb = my_ring + slot * kBox;
+      const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
+#pragma unroll
+      for (int kk = 0; kk < 4; ++kk) {
+        if (!ragged || kk < kk_last) {
+          double bf[NT];
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) bf[nt] = lds64(sb + 1024u * nt + (ragged ? offx(4u * kk + q, g) : xo[kk]));
+          double af[MS];
+#pragma unroll
+          for (int mt = 0; mt < MS; ++mt) af[mt] = lds64(aa + (4u * kk * LDV + 8u * mt) * 8u);
+#pragma unroll
+          for (int mt = 0; mt < MS; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
+        }
+      }
+      __syncwarp();
+      produce(slot);
+      if (++slot == kDepth) {
+        slot = 0;
+        parity ^= 1u;
+      }
+    };
+    for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
+    for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+    // epilogue: C[x = 8mt + g][row 8nt + 2q + e]: out[x] = a + b, out[mir x] = a - b
+    {
+      const int rhs = (int)fast_div(t, a.div_tiles);
+      const int rb = (int)t - rhs * a.tiles_per_rhs;
+      const int row0 = rhs * a.rows_per_rhs + rb * (8 * NT);
+      const int limit = (rhs + 1) * a.rows_per_rhs;
+      double* base = a.out + (long long)(row0 + 2 * q) * n;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          if (row0 + 8 * nt + 2 * q + e < limit) {
+            double* dst = base + (long long)(8 * nt + e) * n;
+#pragma unroll
+            for (int mt = 0; mt < MS; ++mt) {
+              const int x = 8 * mt + g, xb = a.mirc - x;
+              if (x < a.nh) {
+                dst[x] = pa[mt][nt][e] + pb[mt][nt][e];
+                if (xb != x && xb < n) dst[xb] = pa[mt][nt][e] - pb[mt][nt][e];
+              }
+            }
+          }
+        }
+    }
+    t = fifo[0];
+#pragma unroll
+    for (int i = 0; i < kDepth; ++i) fifo[i] = fifo[i + 1];
+    --fifo_n;
+  }
+}
+
 // ---- host side ------------------------------------------------------------------------------------------------
 
 template <typename Kern>
@@ -935,7 +1089,45 @@ cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMa
   constexpr int W = 8, NT = 2;
   const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 4 * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
-  return launch_sym2(k_mode_xf_sym<MS, NT, W>, opt, smem, W, p, m0, m1, a, s);
+  return launch_sym2(k_mode_xf_sym<MS, NT, W, true>, opt, smem, W, p, m0, m1, a, s);
+}
+// bare solver: one stream, two boxes per stage, twelve warps
+template <int MS>
+cudaError_t launch_xf_plain(const exx_plan* p, const CUtensorMap& m0, const XSArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 12, NT = 2;
+  const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym2(k_mode_xf_sym<MS, NT, W, false>, opt, smem, W, p, m0, m0, a, s);
+}
+template <typename Kern>
+cudaError_t launch_sym1x(Kern kern, SmemOptIn& opt, size_t smem, int warps, const exx_plan* p, const CUtensorMap& m0,
+                         const XSArgs& a, cudaStream_t s) {
+  const size_t floor_bytes = 117 * 1024;
+  if (smem < floor_bytes) smem = floor_bytes;
+  if (smem > (size_t)p->smem_optin) return cudaErrorNotSupported;
+  cudaError_t e = opt.ensure(kern, p->device, smem, true);
+  if (e != cudaSuccess) return e;
+  cudaLaunchConfig_t cfg = {};
+  const unsigned grid = a.n_tiles < (unsigned)p->sm_count ? a.n_tiles : (unsigned)p->sm_count;
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * warps);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, m0, a);
+}
+template <int MS>
+cudaError_t launch_xb(const exx_plan* p, const CUtensorMap& m0, const XSArgs& a, cudaStream_t s) {
+  static SmemOptIn opt;
+  constexpr int W = 12, NT = 2;
+  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 1024 * NT +
+                      (size_t)W * kDepth * 8 + 16;
+  return launch_sym1x(k_mode_xb_sym<MS, NT, W>, opt, smem, W, p, m0, a, s);
 }
 template <int MS, bool GEN>
 cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
@@ -1191,6 +1383,69 @@ cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStr
     case 6: return launch_xf<6>(p, m0, m1, a, s);
     case 7: return launch_xf<7>(p, m0, m1, a, s);
     default: return launch_xf<8>(p, m0, m1, a, s);
+  }
+}
+
+// Bare solver (exx_poisson_solve): whether its x passes can run on the reflection-adapted basis.
+bool sym_x_usable_plain(const exx_plan* p, const double* src, const double* work, int nb) {
+  const TmaState* st = static_cast<const TmaState*>(p->tma_state);
+  if (!st || !st->xs_nh || !st->d_mult_symx || !(p->fusion & 2)) return false;
+  if (!aligned16(src) || !aligned16(work)) return false;
+  return (p->N / p->n[0]) * (long long)nb < (1LL << 31) - 64;
+}
+
+// x-forward product of nb right-hand sides in `in` (modes stored even block first in `out`; in == out allowed) and the
+// x-backward product in place over `buf`, both on the reflection-adapted basis.
+cudaError_t sym_xf_plain(exx_plan* p, const double* in, double* out, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!sym_x_usable_plain(p, in, out, nb)) return cudaErrorNotSupported;
+  constexpr int NT = 2;
+  XSArgs a{};
+  fill_x(p, st, a);
+  a.out = out;
+  a.V = st->d_img_xf;
+  a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+  a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+  a.div_nj = make_fastdiv(1u);
+  a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0;
+  cudaError_t e;
+  if ((e = get_map(st, in, a.n, (long long)a.rows_per_rhs * nb, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  ++p->tma_launches;
+  switch ((a.nh + 7) / 8) {
+    case 3: return launch_xf_plain<3>(p, m0, a, s);
+    case 4: return launch_xf_plain<4>(p, m0, a, s);
+    case 5: return launch_xf_plain<5>(p, m0, a, s);
+    case 6: return launch_xf_plain<6>(p, m0, a, s);
+    case 7: return launch_xf_plain<7>(p, m0, a, s);
+    default: return launch_xf_plain<8>(p, m0, a, s);
+  }
+}
+
+cudaError_t sym_xb_plain(exx_plan* p, double* buf, int nb, cudaStream_t s) {
+  TmaState* st = static_cast<TmaState*>(p->tma_state);
+  if (!sym_x_usable_plain(p, buf, buf, nb)) return cudaErrorNotSupported;
+  constexpr int NT = 2;
+  XSArgs a{};
+  fill_x(p, st, a);
+  a.out = buf;
+  a.V = st->d_img_xb;
+  a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
+  a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
+  a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
+  if (a.n_tiles == 0) return cudaSuccess;
+  CUtensorMap m0;
+  cudaError_t e;
+  if ((e = get_map(st, buf, a.n, (long long)a.rows_per_rhs * nb, 0, 8 * NT, &m0)) != cudaSuccess) return e;
+  ++p->tma_launches;
+  switch ((a.nh + 7) / 8) {
+    case 3: return launch_xb<3>(p, m0, a, s);
+    case 4: return launch_xb<4>(p, m0, a, s);
+    case 5: return launch_xb<5>(p, m0, a, s);
+    case 6: return launch_xb<6>(p, m0, a, s);
+    case 7: return launch_xb<7>(p, m0, a, s);
+    default: return launch_xb<8>(p, m0, a, s);
   }
 }
 

@@ -117,6 +117,8 @@ def load_library():
     lib.exx_plan_set_profiling.argtypes = [vp, C.c_int]
     lib.exx_plan_get_profile.restype = C.c_int
     lib.exx_plan_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    lib.exx_plan_get_profile_passes.restype = C.c_int
+    lib.exx_plan_get_profile_passes.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     lib.exx_probe_fp64_peak.restype = C.c_int
     lib.exx_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double)]
     lib.exx_version.restype = C.c_char_p
@@ -266,6 +268,17 @@ class Plan:
         _check(self._lib.exx_plan_get_profile(self._h, ms, cnt), "exx_plan_get_profile")
         names = ("mode_product", "pair_density", "accumulate", "other")
         return {n: (ms[i], int(cnt[i])) for i, n in enumerate(names)}
+
+    PASS_NAMES = ("x_forward", "y_forward", "z", "z_backward", "y_backward", "x_backward", "x_backward_orbital_side")
+
+    def get_profile_passes(self):
+        """exx_plan_get_profile_passes: {pass: (ms, launches, executed flops per pair solve)} of the records the last
+        get_profile() call consumed."""
+        ms = (C.c_double * 8)()
+        cnt = (C.c_longlong * 8)()
+        fl = (C.c_double * 8)()
+        _check(self._lib.exx_plan_get_profile_passes(self._h, ms, cnt, fl), "exx_plan_get_profile_passes")
+        return {n: (ms[i], int(cnt[i]), fl[i]) for i, n in enumerate(self.PASS_NAMES) if cnt[i]}
 
     @property
     def last_launch_count(self) -> int:
