@@ -15,6 +15,8 @@
 //     reads the psi_j tile, which follows the data tile through the TMA ring, in accumulator layout:
 //     vx_k -= occ_j psi_j phi_jk with j ascending, exactly the order of k_accumulate (bitwise run-to-run
 //     reproducible, independent of the batch shape).  phi is never written to memory.
+#include <type_traits>
+
 #include "tma_common.cuh"
 
 namespace exx {
@@ -488,13 +490,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 
     // ---- forward: acc[mt][nt][e] = T[mode 8(mt % MS) + 2q + e of block mt / MS][column 8nt + g] -----------------
-    for (int s = 0; s < Sh; ++s) {
+    auto do_stage = [&](int s, auto rag_c) {  // `ragged` at compile time: standard stages carry none of its address math
+      constexpr bool ragged = decltype(rag_c)::value;
       asm volatile("" : "+r"(v1_lane), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kSlot;
       const unsigned aa = v1_lane + (unsigned)s * (16u * LDV * 8u);
       const int zf = a.zfix - 16 * s;  // local row whose mirror image is itself (its second read counts as zero)
-      const bool ragged = a.kk_last && s == Sh - 1;
 #pragma unroll
       for (int kk = 0; kk < 4; ++kk) {
         if (!ragged || kk < a.kk_last) {
@@ -532,6 +534,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
         slot = 0;
         parity ^= 1u;
       }
+    };
+    {
+      const int s_full = a.kk_last ? Sh - 1 : Sh;
+      for (int s = 0; s < s_full; ++s) do_stage(s, std::false_type{});
+      if (a.kk_last) do_stage(Sh - 1, std::true_type{});
     }
 
     // ---- eigen-space multiply: TS stages for the even block, TS for the odd block ---------------------------------

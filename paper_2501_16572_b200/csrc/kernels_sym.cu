@@ -8,6 +8,8 @@
 // same order.  Machinery as k_mode_t's L-mode (kernels_tma.cu): per-warp TMA rings, one persistent CTA per SM,
 // programmatic dependent launch, 16-column chunks or (HC) 8-column half-chunks.  The forward kernel's stage is two boxes,
 // rows [16 s, 16 s + 16) and the mirrored rows (row 15 - r of the second box is mir(16 s + r)).
+#include <type_traits>
+
 #include "tma_common.cuh"
 
 namespace exx {
@@ -158,13 +160,15 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lf_sym(const __grid_cons
     for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-    for (int s = 0; s < Sh; ++s) {
+    // one stage of 16 half-range rows; `ragged` (the last stage when nh % 16 != 0: plain row order, kk_last k-steps) is a
+    // compile-time flag so that the standard stages carry none of its address arithmetic
+    auto do_stage = [&](int s, auto rag_c) {
+      constexpr bool ragged = decltype(rag_c)::value;
       asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kSlot;
       const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
       const int zf = a.zfix - 16 * s;
-      const bool ragged = a.kk_last && s == Sh - 1;
 #pragma unroll
       for (int kk = 0; kk < 4; ++kk) {
         if (!ragged || kk < a.kk_last) {
@@ -211,6 +215,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lf_sym(const __grid_cons
         slot = 0;
         parity ^= 1u;
       }
+    };
+    {
+      const int s_full = a.kk_last ? Sh - 1 : Sh;
+      for (int s = 0; s < s_full; ++s) do_stage(s, std::false_type{});
+      if (a.kk_last) do_stage(Sh - 1, std::true_type{});
     }
     // epilogue: C[mode 8 (mt % MS) + g of block mt / MS][column 8nt + 2q + e]; even modes -> rows 0.., odd modes -> rows nh..
     const long long rstep = a.inner;
@@ -349,7 +358,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lb_sym(const __grid_cons
     for (int mt = 0; mt < MS; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
-    auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+    auto stage = [&](auto& acc, int s, auto rag_c, int kk_last) {
+      constexpr bool ragged = decltype(rag_c)::value;
       asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kS1;
@@ -382,8 +392,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_lb_sym(const __grid_cons
         parity ^= 1u;
       }
     };
-    for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
-    for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+    {
+      const int se_full = a.kk_last ? SE - 1 : SE, st_full = a.kk_last_o ? ST - 1 : ST;
+      for (int s = 0; s < se_full; ++s) stage(pa, s, std::false_type{}, 0);
+      if (a.kk_last) stage(pa, SE - 1, std::true_type{}, a.kk_last);
+      for (int s = SE; s < st_full; ++s) stage(pb, s, std::false_type{}, 0);
+      if (a.kk_last_o) stage(pb, ST - 1, std::true_type{}, a.kk_last_o);
+    }
 
     // epilogue: out[y] = a + b, out[mir y] = a - b for the half-range rows y = 8mt + g
 #pragma unroll
@@ -562,13 +577,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-    for (int s = 0; s < Sh; ++s) {
+    auto do_stage = [&](int s, auto rag_c) {  // `ragged` at compile time, as in k_mode_lf_sym
+      constexpr bool ragged = decltype(rag_c)::value;
       asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kSlot;
       const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
       const int zf = a.zfix - 16 * s;
-      const bool ragged = a.kk_last && s == Sh - 1;
 #pragma unroll
       for (int kk = 0; kk < 4; ++kk) {
         if (!ragged || kk < a.kk_last) {
@@ -599,6 +614,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
         slot = 0;
         parity ^= 1u;
       }
+    };
+    {
+      const int s_full = a.kk_last ? Sh - 1 : Sh;
+      for (int s = 0; s < s_full; ++s) do_stage(s, std::false_type{});
+      if (a.kk_last) do_stage(Sh - 1, std::true_type{});
     }
     // epilogue: C[mode 8 (mt % MS) + g of block mt / MS][row 8nt + 2q + e]; positions: even modes 0.., odd modes nh..
     {
@@ -792,7 +812,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       for (int mt = 0; mt < MS; ++mt)
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
-      auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+      auto stage = [&](auto& acc, int s, auto rag_c, int kk_last) {
+      constexpr bool ragged = decltype(rag_c)::value;
         asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
         mbar_wait(my_bar + 8u * slot, parity);
         const unsigned sb = my_ring + slot * kSlot;
@@ -819,8 +840,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
           parity ^= 1u;
         }
       };
-      for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
-      for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+      {
+        const int se_full = a.kk_last ? SE - 1 : SE, st_full = a.kk_last_o ? ST - 1 : ST;
+        for (int s = 0; s < se_full; ++s) stage(pa, s, std::false_type{}, 0);
+        if (a.kk_last) stage(pa, SE - 1, std::true_type{}, a.kk_last);
+        for (int s = SE; s < st_full; ++s) stage(pb, s, std::false_type{}, 0);
+        if (a.kk_last_o) stage(pb, ST - 1, std::true_type{}, a.kk_last_o);
+      }
       // a5: vx_k[x] -= occ_j psi_j[x] (a + b), vx_k[mir x] -= occ_j psi_j[mir x] (a - b)
 #pragma unroll
       for (int sp = 0; sp < SPMAX; ++sp) {
@@ -960,7 +986,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_xb_sym(const __grid_cons
     for (int mt = 0; mt < MS; ++mt)
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
-    auto stage = [&](auto& acc, int s, bool ragged, int kk_last) {
+    auto stage = [&](auto& acc, int s, auto rag_c, int kk_last) {
+      constexpr bool ragged = decltype(rag_c)::value;
       asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kBox;
@@ -987,8 +1014,13 @@ __global__ void __launch_bounds__(32 * WARPS, 1) k_mode_xb_sym(const __grid_cons
         parity ^= 1u;
       }
     };
-    for (int s = 0; s < SE; ++s) stage(pa, s, a.kk_last && s == SE - 1, a.kk_last);
-    for (int s = SE; s < ST; ++s) stage(pb, s, a.kk_last_o && s == ST - 1, a.kk_last_o);
+    {
+      const int se_full = a.kk_last ? SE - 1 : SE, st_full = a.kk_last_o ? ST - 1 : ST;
+      for (int s = 0; s < se_full; ++s) stage(pa, s, std::false_type{}, 0);
+      if (a.kk_last) stage(pa, SE - 1, std::true_type{}, a.kk_last);
+      for (int s = SE; s < st_full; ++s) stage(pb, s, std::false_type{}, 0);
+      if (a.kk_last_o) stage(pb, ST - 1, std::true_type{}, a.kk_last_o);
+    }
     // epilogue: C[x = 8mt + g][row 8nt + 2q + e]: out[x] = a + b, out[mir x] = a - b
     {
       const int rhs = (int)fast_div(t, a.div_tiles);
