@@ -465,6 +465,10 @@ struct XSArgs {
   int n_items, L, stride_i, stride_l, c_lo, c_hi, p0;
   int first;
   FastDiv div_tiles, div_nj, div_items;
+  // xf with the pair density: tile t = (row tile, orbital, target) with the target index fastest, so that the tiles that
+  // share a psi_j tile run back to back and find it in L2 (nb_rhs = nj nk right-hand sides, nkq = nk)
+  FastDiv div_nb, div_nkq;
+  int nb_rhs, nkq;
   BatchDesc bd;
 };
 
@@ -517,14 +521,25 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned t_p = tfirst;
   int s_p = 0;
   int pr0 = 0, pr1 = 0;
-  auto tile_coords = [&](unsigned t) {
-    const int rhs = (int)fast_div(t, a.div_tiles);
-    const int rb = (int)t - rhs * a.tiles_per_rhs;
+  auto split_tile = [&](unsigned t, int& rhs, int& rb, int& jj, int& kq) {
     if (PD) {
-      const int kq = (int)fast_div((unsigned)rhs, a.div_nj);
-      const int j = a.bd.j0 + (rhs - kq * a.bd.nj), k = a.bd.k0 + kq;
-      pr0 = j * a.rows_per_rhs + rb * (8 * NT);
-      pr1 = k * a.rows_per_rhs + rb * (8 * NT);
+      rb = (int)fast_div(t, a.div_nb);
+      const int r = (int)t - rb * a.nb_rhs;
+      jj = (int)fast_div((unsigned)r, a.div_nkq);
+      kq = r - jj * a.nkq;
+      rhs = kq * a.bd.nj + jj;
+    } else {
+      rhs = (int)fast_div(t, a.div_tiles);
+      rb = (int)t - rhs * a.tiles_per_rhs;
+      jj = kq = 0;
+    }
+  };
+  auto tile_coords = [&](unsigned t) {
+    int rhs, rb, jj, kq;
+    split_tile(t, rhs, rb, jj, kq);
+    if (PD) {
+      pr0 = (a.bd.j0 + jj) * a.rows_per_rhs + rb * (8 * NT);
+      pr1 = (a.bd.k0 + kq) * a.rows_per_rhs + rb * (8 * NT);
     } else {
       pr0 = rhs * a.rows_per_rhs + rb * (8 * NT);
     }
@@ -622,8 +637,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     }
     // epilogue: C[mode 8 (mt % MS) + g of block mt / MS][row 8nt + 2q + e]; positions: even modes 0.., odd modes nh..
     {
-      const int rhs = (int)fast_div(t, a.div_tiles);
-      const int rb = (int)t - rhs * a.tiles_per_rhs;
+      int rhs, rb, jj_, kq_;
+      split_tile(t, rhs, rb, jj_, kq_);
       const int row0 = rhs * a.rows_per_rhs + rb * (8 * NT);
       const int limit = (rhs + 1) * a.rows_per_rhs;
       double* base = a.out + (long long)(row0 + 2 * q) * n;
@@ -1400,6 +1415,10 @@ cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStr
   a.tiles_per_rhs = (a.rows_per_rhs + 8 * NT - 1) / (8 * NT);
   a.div_tiles = make_fastdiv((unsigned)a.tiles_per_rhs);
   a.div_nj = make_fastdiv((unsigned)fa->bd.nj);
+  a.nb_rhs = nb;
+  a.nkq = fa->bd.nk;
+  a.div_nb = make_fastdiv((unsigned)nb);
+  a.div_nkq = make_fastdiv((unsigned)fa->bd.nk);
   if ((long long)a.rows_per_rhs * nb >= (1LL << 31) - 64) return cudaErrorNotSupported;
   a.n_tiles = (unsigned)a.tiles_per_rhs * (unsigned)nb;
   if (a.n_tiles == 0) return cudaSuccess;
