@@ -488,3 +488,31 @@ def test_accumulate_mode_splits_the_orbital_sum():
     torch.cuda.synchronize()
     assert torch.equal(vx2, vx_full)
     plan.close()
+
+
+@pytest.mark.parametrize("dims,sym", [((48, 48, 48), True), ((16, 16, 16), False)], ids=["symmetric_mode", "dense"])
+def test_per_pass_profile_accounts_for_every_mode_product_launch(dims, sym):
+    """exx_plan_get_profile_passes (bench.py's per-kernel roofline): the passes add up to the mode-product class in
+    launches and time, and their executed operations to exx_plan_executed_flops_per_solve."""
+    nx, ny, nz = dims
+    plan = exx.Plan(nx, ny, nz, 0.25, (0, 0, 0), 12, 0.106, max_batch=64, device=0)
+    rng = np.random.default_rng(3)
+    psi = torch.from_numpy(rng.standard_normal((6, nz, ny, nx))).cuda()
+    occ = torch.full((6,), 2.0, dtype=torch.float64, device="cuda")
+    plan.apply(psi, occ, psi, occ, n_c=12)
+    plan.set_profiling(True)
+    plan.apply(psi, occ, psi, occ, n_c=12)
+    prof = plan.get_profile()
+    passes = plan.get_profile_passes()
+    plan.set_profiling(False)
+    assert set(passes) == {"x_forward", "y_forward", "z", "y_backward", "x_backward"}      # fused z pass, fused accumulate
+    assert sum(c for _, c, _ in passes.values()) == prof["mode_product"][1] == 5 * 3        # 36 pairs in batches of 12
+    assert abs(sum(ms for ms, _, _ in passes.values()) - prof["mode_product"][0]) < 1e-6 * prof["mode_product"][0] + 1e-9
+    flops = sum(f for _, _, f in passes.values())
+    assert abs(flops - plan.executed_flops_per_solve) < 1e-9 * flops
+    dense = 4.0 * nx * ny * nz * (nx + ny + nz)
+    assert (flops < 0.6 * dense) if sym else (flops == dense)
+    # one executed solve of the pair-symmetric apply runs the x-backward product once more (two-sided accumulate)
+    extra = plan.executed_flops_per_symmetric_solve - plan.executed_flops_per_solve
+    assert abs(extra - passes["x_backward"][2]) < 1e-9 * flops if sym else extra == 0.0
+    plan.close()
