@@ -671,8 +671,15 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     k_mode_xacc_sym(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, const XSArgs a) {
   constexpr int LDV = 8 * MS + 4;
   constexpr unsigned kBox = 1024u * NT;
-  constexpr unsigned kSlot = 2u * kBox;  // a psi stage is a pair of boxes; a data stage uses the first half
+  // A ring slot holds BPS boxes: a data stage is ALL boxes of one parity block of the modes (at most 4 for NT = 1, at most
+  // 2 for NT = 2), a psi stage PP = BPS / 2 pairs (block, mirrored block) of 16 half-range points.  Per step (one j) that
+  // is 2 data stages + ceil(SP / PP) psi stages = 4 barrier waits instead of one per box (12 at n = 120).
+  constexpr int BPS = NT == 1 ? 4 : 2;
+  constexpr int PP = BPS / 2;
+  constexpr unsigned kSlot = BPS * kBox;
   constexpr int SPMAX = (MS + 1) / 2;
+  constexpr int PSMAX = (SPMAX + PP - 1) / PP;
+  static_assert((MS + 1) / 2 <= BPS, "a parity block of the modes must fit one ring slot");
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
@@ -708,8 +715,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned fifo[kDepth + 1];
   int fifo_n = 0;
 
-  // producer: item (row tile, i) = hi - lo steps of ST data stages (even modes, then odd modes) + SP psi stage pairs
-  const int stages_per_step = ST + SP;
+  // producer: item (row tile, i) = hi - lo steps of 2 data stages (even modes, odd modes) + PS psi stages
+  const int PS = (SP + PP - 1) / PP;
+  const int stages_per_step = 2 + PS;
   auto item_range = [&](unsigned t, int& rb, int& i, int& lo, int& hi) {
     rb = (int)fast_div(t, a.div_items);
     i = (int)t - rb * a.n_items;
@@ -751,14 +759,22 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
     const unsigned bar = my_bar + 8u * slot;
     const unsigned dst = my_ring + slot * kSlot;
     if (elect_one()) {
-      if (s_p < ST) {
-        mbar_expect_tx(bar, kBox);
-        tma_load_2d(dst, &tm0, s_p < SE ? 16 * s_p : a.nh + 16 * (s_p - SE), prow_d, bar);
+      if (s_p < 2) {
+        const int cnt = s_p ? ST - SE : SE, col0 = s_p ? a.nh : 0;
+        mbar_expect_tx(bar, kBox * (unsigned)cnt);
+#pragma unroll
+        for (int b = 0; b < BPS; ++b)
+          if (b < cnt) tma_load_2d(dst + kBox * b, &tm0, col0 + 16 * b, prow_d, bar);
       } else {
-        const int sp = s_p - ST;
-        mbar_expect_tx(bar, kSlot);
-        tma_load_2d(dst, &tm1, 16 * sp, prow_p, bar);
-        tma_load_2d(dst + kBox, &tm1, a.mir0 - 16 * sp, prow_p, bar);
+        const int sp0 = (s_p - 2) * PP;
+        const int np = SP - sp0 < PP ? SP - sp0 : PP;
+        mbar_expect_tx(bar, 2u * kBox * (unsigned)np);
+#pragma unroll
+        for (int pp = 0; pp < PP; ++pp)
+          if (pp < np) {
+            tma_load_2d(dst + 2u * kBox * pp, &tm1, 16 * (sp0 + pp), prow_p, bar);
+            tma_load_2d(dst + 2u * kBox * pp + kBox, &tm1, a.mir0 - 16 * (sp0 + pp), prow_p, bar);
+          }
       }
     }
     if (++s_p == stages_per_step) {
@@ -827,11 +843,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       for (int mt = 0; mt < MS; ++mt)
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) pa[mt][nt][0] = pa[mt][nt][1] = pb[mt][nt][0] = pb[mt][nt][1] = 0.0;
-      auto stage = [&](auto& acc, int s, auto rag_c, int kk_last) {
-      constexpr bool ragged = decltype(rag_c)::value;
+      // one box of 16 modes (`ragged`, a compile-time flag: the last box of a block when its size is not a multiple of 16)
+      auto box = [&](auto& acc, unsigned sb, int s, auto rag_c, int kk_last) {
+        constexpr bool ragged = decltype(rag_c)::value;
         asm volatile("" : "+r"(a_lane_v), "+r"(xo[0]), "+r"(xo[1]), "+r"(xo[2]), "+r"(xo[3]));
-        mbar_wait(my_bar + 8u * slot, parity);
-        const unsigned sb = my_ring + slot * kSlot;
         const unsigned aa = a_lane_v + (unsigned)s * (16u * LDV * 8u);
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
@@ -848,6 +863,14 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
               for (int nt = 0; nt < NT; ++nt) dmma884(acc[mt][nt], af[mt], bf[nt]);
           }
         }
+      };
+      // a data stage: every box of one parity block (image stages s0 .. s0 + cnt - 1) behind a single barrier wait
+      auto data_stage = [&](auto& acc, int s0, int cnt, int kk_last) {
+        mbar_wait(my_bar + 8u * slot, parity);
+        const unsigned sb = my_ring + slot * kSlot;
+        for (int b = 0; b < cnt - 1; ++b) box(acc, sb + kBox * b, s0 + b, std::false_type{}, 0);
+        if (kk_last) box(acc, sb + kBox * (cnt - 1), s0 + cnt - 1, std::true_type{}, kk_last);
+        else box(acc, sb + kBox * (cnt - 1), s0 + cnt - 1, std::false_type{}, 0);
         __syncwarp();
         produce(slot);
         if (++slot == kDepth) {
@@ -855,32 +878,34 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
           parity ^= 1u;
         }
       };
-      {
-        const int se_full = a.kk_last ? SE - 1 : SE, st_full = a.kk_last_o ? ST - 1 : ST;
-        for (int s = 0; s < se_full; ++s) stage(pa, s, std::false_type{}, 0);
-        if (a.kk_last) stage(pa, SE - 1, std::true_type{}, a.kk_last);
-        for (int s = SE; s < st_full; ++s) stage(pb, s, std::false_type{}, 0);
-        if (a.kk_last_o) stage(pb, ST - 1, std::true_type{}, a.kk_last_o);
-      }
+      data_stage(pa, 0, SE, a.kk_last);
+      data_stage(pb, SE, ST - SE, a.kk_last_o);
       // a5: vx_k[x] -= occ_j psi_j[x] (a + b), vx_k[mir x] -= occ_j psi_j[mir x] (a - b)
 #pragma unroll
-      for (int sp = 0; sp < SPMAX; ++sp) {
-        if (sp < SP) {
+      for (int ps = 0; ps < PSMAX; ++ps) {
+        if (ps < PS) {
           mbar_wait(my_bar + 8u * slot, parity);
-          const unsigned sb = my_ring + slot * kSlot;
+          const unsigned sb0 = my_ring + slot * kSlot;
 #pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            constexpr int kZ = 0;
-            const int mt = 2 * sp + h < MS ? 2 * sp + h : kZ;
-            if (2 * sp + h < MS) {
+          for (int pp = 0; pp < PP; ++pp) {
+            const int sp = ps * PP + pp;  // compile-time after unrolling
+            if (sp < SPMAX && sp < SP) {
+              const unsigned sb = sb0 + 2u * kBox * pp;
 #pragma unroll
-              for (int nt = 0; nt < NT; ++nt)
+              for (int h = 0; h < 2; ++h) {
+                constexpr int kZ = 0;
+                const int mt = 2 * sp + h < MS ? 2 * sp + h : kZ;
+                if (2 * sp + h < MS) {
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const double p0 = lds64(sb + 1024u * nt + pq[e][h]), p1 = lds64(sb + 1024u * nt + pm[e][h]);
-                  lo[mt][nt][e] -= oc * p0 * (pa[mt][nt][e] + pb[mt][nt][e]);
-                  hi[mt][nt][e] -= oc * p1 * (pa[mt][nt][e] - pb[mt][nt][e]);
+                  for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                      const double p0 = lds64(sb + 1024u * nt + pq[e][h]), p1 = lds64(sb + 1024u * nt + pm[e][h]);
+                      lo[mt][nt][e] -= oc * p0 * (pa[mt][nt][e] + pb[mt][nt][e]);
+                      hi[mt][nt][e] -= oc * p1 * (pa[mt][nt][e] - pb[mt][nt][e]);
+                    }
                 }
+              }
             }
           }
           __syncwarp();
@@ -1179,8 +1204,8 @@ cudaError_t launch_xb(const exx_plan* p, const CUtensorMap& m0, const XSArgs& a,
 template <int MS, bool GEN>
 cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 12, NT = MS <= 4 ? 2 : 1;
-  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * 2 * 1024 * NT +
+  constexpr int W = 12, NT = MS <= 4 ? 2 : 1, BPS = NT == 1 ? 4 : 2;  // boxes per ring slot, as in the kernel
+  const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * BPS * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym2(k_mode_xacc_sym<MS, NT, W, GEN>, opt, smem, W, p, m0, m1, a, s);
 }
