@@ -152,9 +152,11 @@ def run_reference(args):
     if rank != 0:
         return
     w = workload_from_args(args)
-    steps = max(1, min(args.steps, 3))
-    warmup = min(args.warmup, 1)
-    budget = min(args.cpu_seconds, 120.0 / (steps + warmup + 1))
+    # exactly the K timed and W warm-up steps asked for; each step is a bounded sample of the workload sized so that the
+    # whole run ends within a few minutes (about 150 s of oracle time in total)
+    steps = max(1, args.steps)
+    warmup = max(0, args.warmup)
+    budget = min(args.cpu_seconds, 150.0 / (steps + warmup + 1))
     cb, dt, solves = time_oracle(w, budget, steps=steps, warmup=warmup)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": steps, "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,

@@ -10,12 +10,13 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_reference_arm_prints_one_json_line():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
-                          "--steps", "1", "--warmup", "0", "--cpu-seconds", "2"], capture_output=True, text=True,
+                          "--steps", "4", "--warmup", "2", "--cpu-seconds", "1"], capture_output=True, text=True,
                          cwd=ROOT, timeout=600)
     assert out.returncode == 0, out.stderr[-2000:]
     lines = [l for l in out.stdout.splitlines() if l.strip()]
     assert len(lines) == 1
     d = json.loads(lines[0])
+    assert d["steps"] == 4 and d["warmup"] == 2          # the K and W asked for, not a clamped count
     assert d["impl"] == "reference" and d["metric"] == "poisson_pair_solves_per_s" and d["unit"] == "solves/s"
     assert d["higher_is_better"] is True and d["dtype"] == "f64" and d["data"] == "synthetic"
     assert d["value"] > 0 and d["gpu_launches"] == 0
