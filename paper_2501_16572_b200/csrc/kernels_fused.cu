@@ -360,7 +360,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   constexpr unsigned kS1 = 1024u * NT;  // one box set (all chunks of a tile)
   constexpr unsigned kSlot = 2u * kS1;  // a data stage: the rows and the mirrored rows
   constexpr int CH = NT / 2;
-  constexpr int TS = (MS + 1) / 2;      // multiplier stages per block
+  constexpr int TS = (MS + 1) / 2;      // multiplier boxes (16 modes = two row tiles) per block
+  constexpr int TS2 = (TS + 1) / 2;     // multiplier stages per block: a slot (rows + mirrored rows of a data stage) holds two boxes
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
@@ -398,8 +399,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   unsigned fifo[kDepth + 1];
   int fifo_n = 0;
 
-  // ---- producer: Sh data stages (rows + mirrored rows), TS multiplier stages for the even modes, TS for the odd ----
-  const int stages_per_tile = Sh + 2 * TS;
+  // ---- producer: Sh data stages (rows + mirrored rows), TS2 multiplier stages for the even modes, TS2 for the odd ----
+  const int stages_per_tile = Sh + 2 * TS2;
   unsigned t_p = tfirst;
   int s_p = 0;
   int pc0[CH], pc2[CH];
@@ -430,11 +431,17 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
           tma_load_3d(dst + kS1 + 2048u * ch, &tm0, pc0[ch], a.mir0 - 16 * s_p, pc2[ch], bar);
         }
       } else {
-        const int ts = s_p - Sh;
-        const int row = ts < TS ? 16 * ts : a.nh + 16 * (ts - TS);  // even modes: table rows 0.., odd modes: rows nh..
-        mbar_expect_tx(bar, kS1);
+        const int ts2 = s_p - Sh;
+        const int blk = ts2 < TS2 ? 0 : 1, t0 = 2 * (ts2 - blk * TS2);  // first box of this stage within its block
+        const int nbx = TS - t0 < 2 ? TS - t0 : 2;
+        mbar_expect_tx(bar, kS1 * (unsigned)nbx);
 #pragma unroll
-        for (int ch = 0; ch < CH; ++ch) tma_load_3d(dst + 2048u * ch, &tm1, pc0[ch], row, 0, bar);
+        for (int hh = 0; hh < 2; ++hh)
+          if (hh < nbx) {
+            const int row = (blk ? a.nh : 0) + 16 * (t0 + hh);  // even modes: table rows 0.., odd modes: rows nh..
+#pragma unroll
+            for (int ch = 0; ch < CH; ++ch) tma_load_3d(dst + kS1 * hh + 2048u * ch, &tm1, pc0[ch], row, 0, bar);
+          }
       }
     }
     if (++s_p == stages_per_tile) {
@@ -541,24 +548,26 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
       if (a.kk_last) do_stage(Sh - 1, std::true_type{});
     }
 
-    // ---- eigen-space multiply: TS stages for the even block, TS for the odd block ---------------------------------
+    // ---- eigen-space multiply: TS2 stages for the even block, TS2 for the odd block, two boxes of 16 modes per stage ------
 #pragma unroll
-    for (int sp = 0; sp < 2 * TS; ++sp) {
+    for (int sp = 0; sp < 2 * TS2; ++sp) {
       mbar_wait(my_bar + 8u * slot, parity);
       const unsigned sb = my_ring + slot * kSlot;
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        constexpr int kZ = 0;
-        const int blk = sp < TS ? 0 : 1, mtl = 2 * (sp < TS ? sp : sp - TS) + h;  // compile-time after unrolling
-        if (mtl < MS) {
-          const int mt = blk * MS + mtl;
+      for (int hh = 0; hh < 2; ++hh)
 #pragma unroll
-          for (int nt = 0; nt < NT; ++nt)
+        for (int h = 0; h < 2; ++h) {
+          constexpr int kZ = 0;
+          const int blk = sp < TS2 ? 0 : 1, ts = 2 * (sp < TS2 ? sp : sp - TS2) + hh, mtl = 2 * ts + h;  // compile-time
+          if (ts < TS && mtl < MS) {
+            const int mt = blk * MS + mtl;
 #pragma unroll
-            for (int e = 0; e < 2; ++e)
-              acc[mt < MT ? mt : kZ][nt][e] *= lds64(sb + 2048u * (nt >> 1) + 1024u * h + tq[e][nt & 1]);
+            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+              for (int e = 0; e < 2; ++e)
+                acc[mt < MT ? mt : kZ][nt][e] *= lds64(sb + kS1 * hh + 2048u * (nt >> 1) + 1024u * h + tq[e][nt & 1]);
+          }
         }
-      }
       __syncwarp();
       produce(slot);
       if (++slot == kDepth) {
