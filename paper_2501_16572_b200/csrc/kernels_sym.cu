@@ -689,9 +689,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   constexpr int LDV = 8 * MS + 4;
   constexpr unsigned kBox = 1024u * NT;
   // A ring slot holds BPS boxes: a data stage is ALL boxes of one parity block of the modes (at most 4 for NT = 1, at most
-  // 2 for NT = 2), a psi stage PP = BPS / 2 pairs (block, mirrored block) of 16 half-range points.  Per step (one j) that
+  // 2 for NT = 2, where the image is small enough for the larger ring), a psi stage PP = BPS / 2 pairs (block, mirrored block) of 16 half-range points.  Per step (one j) that
   // is 2 data stages + ceil(SP / PP) psi stages = 4 barrier waits instead of one per box (12 at n = 120).
-  constexpr int BPS = NT == 1 ? 4 : 2;
+  constexpr int BPS = 4;
   constexpr int PP = BPS / 2;
   constexpr unsigned kSlot = BPS * kBox;
   constexpr int SPMAX = (MS + 1) / 2;
@@ -1233,7 +1233,7 @@ cudaError_t launch_xb(const exx_plan* p, const CUtensorMap& m0, const XSArgs& a,
 template <int MS, bool GEN>
 cudaError_t launch_xacc_sym(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 12, NT = MS <= 4 ? 2 : 1, BPS = NT == 1 ? 4 : 2;  // boxes per ring slot, as in the kernel
+  constexpr int W = 12, NT = MS <= 4 ? 2 : 1, BPS = 4;  // boxes per ring slot, as in the kernel
   const size_t smem = sizeof(double) * 16 * (size_t)(a.Sh + a.So) * (8 * MS + 4) + 1024 + (size_t)W * kDepth * BPS * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym2(k_mode_xacc_sym<MS, NT, W, GEN>, opt, smem, W, p, m0, m1, a, s);
