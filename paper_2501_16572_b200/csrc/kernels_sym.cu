@@ -1187,7 +1187,8 @@ cudaError_t launch_sym2(Kern kern, SmemOptIn& opt, size_t smem, int warps, const
 template <int MS>
 cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
-  constexpr int W = 8, NT = 2;
+  // twelve warps where the image leaves room for twelve four-box rings (up to 80 points per axis), ten up to 112, else eight
+  constexpr int W = MS <= 5 ? 12 : MS <= 7 ? 10 : 8, NT = 2;
   const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 4 * 1024 * NT +
                       (size_t)W * kDepth * 8 + 16;
   return launch_sym2(k_mode_xf_sym<MS, NT, W, true>, opt, smem, W, p, m0, m1, a, s);
