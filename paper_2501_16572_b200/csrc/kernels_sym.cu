@@ -507,8 +507,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1)
   const int g = lane >> 2, q = lane & 3;
   const int n = a.n, Sh = a.Sh;
   const unsigned smem0 = (unsigned)__cvta_generic_to_shared(smem_raw);
-  const unsigned img_bytes = 8u * (16u * Sh) * LDV;
-  for (unsigned i = 2 * tid; i < 16u * Sh * LDV; i += 2 * 32 * WARPS)
+  // image rows actually read: the ragged last stage only uses its first 4 kk_last rows (that trims 4 KB at n = 120, which
+  // is what lets a tenth warp's ring fit)
+  const unsigned img_rows = a.kk_last ? 16u * (Sh - 1) + 4u * a.kk_last : 16u * Sh;
+  const unsigned img_bytes = 8u * img_rows * LDV;
+  for (unsigned i = 2 * tid; i < img_rows * LDV; i += 2 * 32 * WARPS)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem0 + 8u * i), "l"(a.V + i) : "memory");
   asm volatile("cp.async.commit_group;\n" ::: "memory");
   const unsigned ring0 = (smem0 + img_bytes + 1023u) & ~1023u;
@@ -1188,9 +1191,19 @@ template <int MS>
 cudaError_t launch_xf(const exx_plan* p, const CUtensorMap& m0, const CUtensorMap& m1, const XSArgs& a, cudaStream_t s) {
   static SmemOptIn opt;
   // twelve warps where the image leaves room for twelve four-box rings (up to 80 points per axis), ten up to 112, else eight
-  constexpr int W = MS <= 5 ? 12 : MS <= 7 ? 10 : 8, NT = 2;
-  const size_t smem = sizeof(double) * 16 * (size_t)a.Sh * (16 * MS + 4) + 1024 + (size_t)W * kDepth * 4 * 1024 * NT +
-                      (size_t)W * kDepth * 8 + 16;
+  constexpr int NT = 2;
+  const size_t rows = a.kk_last ? 16 * (size_t)(a.Sh - 1) + 4 * a.kk_last : 16 * (size_t)a.Sh;  // image rows the kernel stages
+  const size_t img = (sizeof(double) * rows * (16 * MS + 4) + 1023) / 1024 * 1024;
+  auto need = [&](int w) { return img + 1024 + (size_t)w * kDepth * 4 * 1024 * NT + (size_t)w * kDepth * 8 + 16; };
+  if (MS >= 8) {  // 120-128 points: ten warps if the (trimmed) image leaves room, else eight
+    if (need(10) <= (size_t)p->smem_optin) {
+      static SmemOptIn opt10;
+      return launch_sym2(k_mode_xf_sym<MS, NT, 10, true>, opt10, need(10), 10, p, m0, m1, a, s);
+    }
+    return launch_sym2(k_mode_xf_sym<MS, NT, 8, true>, opt, need(8), 8, p, m0, m1, a, s);
+  }
+  constexpr int W = MS <= 5 ? 12 : 10;
+  const size_t smem = need(W);
   return launch_sym2(k_mode_xf_sym<MS, NT, W, true>, opt, smem, W, p, m0, m1, a, s);
 }
 // bare solver: one stream, two boxes per stage, twelve warps
