@@ -190,6 +190,8 @@ FUSION_GRIDS = [
     # x axis too (k_mode_xf_sym / k_mode_xacc_sym; nx a multiple of 4): exchange apply only
     (72, 4, 4, (0, 0, 0), 0.106),
     (124, 4, 4, (1, 0, 0), 0.0),
+    (104, 6, 4, (0, 0, 0), 0.106),       # seven row tiles per block: the ten-warp x-forward kernel
+    (128, 4, 4, (0, 0, 0), 0.0),         # eight full row tiles, no ragged stage: untrimmed image, eight warps
     (72, 70, 70, (0, 0, 0), 0.106),
     # three and four row tiles per block (axes of 34 .. 64 points), all three axes symmetric
     (40, 36, 34, (0, 1, 0), 0.106),
