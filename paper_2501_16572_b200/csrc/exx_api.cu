@@ -57,7 +57,7 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
 inline bool all_axes_fast(const exx_plan* p) { return p->d_Vpad[0] && p->d_Vpad[1] && p->d_Vpad[2]; }
 
 // a plan with a nonzero Bloch phase has complex eigenvectors: only the *_bloch entry points may use it
-inline bool is_complex_plan(const exx_plan* p) { return p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
+inline bool is_complex_plan(const exx_plan* p) { return p->bloch || p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
                                                          !p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty(); }
 
 // n_c == 0: about 1 GB of right-hand sides per batch (measured: larger batches only amortise launch ramps and tails,
@@ -131,9 +131,10 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
   p->prof_on = false; p->accumulate = false;
   for (int c = 0; c < exx::PASS_COUNT; ++c) { p->prof_pass_ms[c] = 0.0; p->prof_pass_count[c] = 0; }
   p->fusion = 15;
+  p->bloch = false;
   p->lanes = 1; p->lane_stream = nullptr; p->ev_fork = nullptr; p->ev_join = nullptr;
   for (int a = 0; a < 3; ++a) {
-    p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr;
+    p->bc[a] = bc[a]; p->d_V[a] = nullptr; p->d_Vpad[a] = nullptr; p->d_Vi[a] = nullptr; p->bfly[a] = false;
     // a Bloch phase only exists on a periodic axis; theta == 0 there is the real periodic matrix
     p->theta[a] = (theta && bc[a] == EXX_BC_PERIODIC) ? theta[a] : 0.0;
     if (theta && !std::isfinite(theta[a])) { delete p; return EXX_ERR_INVALID_ARG; }
@@ -149,13 +150,20 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
         p->h_lam[a] = p->h_lam[same];
         p->h_V[a] = p->h_V[same];
         p->h_Vi[a] = p->h_Vi[same];
+        p->h_Vc_re[a] = p->h_Vc_re[same];
+        p->h_Vc_im[a] = p->h_Vc_im[same];
+        p->bfly[a] = p->bfly[same];
         continue;
       }
       if (p->theta[a] != 0.0) {
-        if (!exx::bloch_eigh(p->n[a], h, fd_order, p->theta[a], p->h_lam[a], p->h_V[a], p->h_Vi[a])) {
+        // the axis in its real form: h_V = W (real orthogonal), the kernels apply the butterfly U around the real products
+        if (!exx::bloch_eigh_real_form(p->n[a], h, fd_order, p->theta[a], p->h_lam[a], p->h_V[a], p->h_Vc_re[a],
+                                       p->h_Vc_im[a])) {
           delete p;
           return EXX_ERR_EIGENSOLVE;
         }
+        p->bfly[a] = true;
+        p->bloch = true;
         continue;
       }
       std::vector<double> K = exx::second_derivative_matrix(p->n[a], h, bc[a], fd_order);
@@ -961,8 +969,11 @@ exx_status exx_plan_get_axis_bloch(const exx_plan* plan, int axis, double* h_lam
   if (h_lambda) std::memcpy(h_lambda, plan->h_lam[axis].data(), sizeof(double) * n);
   for (int i = 0; i < n; ++i)
     for (int m = 0; m < n; ++m) {
-      if (h_V_re) h_V_re[i + (size_t)n * m] = plan->h_V[axis][(size_t)i * n + m];
-      if (h_V_im) h_V_im[i + (size_t)n * m] = plan->h_Vi[axis].empty() ? 0.0 : plan->h_Vi[axis][(size_t)i * n + m];
+      const bool cplx = plan->bfly[axis] && !plan->h_Vc_re[axis].empty();  // V = U W of an axis held in its real form
+      if (h_V_re) h_V_re[i + (size_t)n * m] = cplx ? plan->h_Vc_re[axis][(size_t)i * n + m] : plan->h_V[axis][(size_t)i * n + m];
+      if (h_V_im)
+        h_V_im[i + (size_t)n * m] = cplx ? plan->h_Vc_im[axis][(size_t)i * n + m]
+                                         : plan->h_Vi[axis].empty() ? 0.0 : plan->h_Vi[axis][(size_t)i * n + m];
     }
   return EXX_OK;
 }
@@ -991,7 +1002,9 @@ exx_status exx_poisson_solve_bloch(exx_plan* plan, const double* d_rhs, double* 
     const int nb = n_rhs - r0 < n_c ? n_rhs - r0 : n_c;
     EXX_CUDA(cudaMemcpyAsync(buf[0], d_rhs + 2 * N * (size_t)r0, fn * nb, cudaMemcpyDeviceToDevice, s));
     double* res = nullptr;
+    EXX_CUDA(exx::bloch_butterfly(plan, buf[0], nb, false, s, &launches));  // axes held in their real form: g = U^H f
     EXX_CUDA(exx::bloch_solve_batch(plan, buf, nb, s, &launches, &res));
+    EXX_CUDA(exx::bloch_butterfly(plan, res, nb, true, s, &launches));      // phi = U (W ...)
     EXX_CUDA(cudaMemcpyAsync(d_phi + 2 * N * (size_t)r0, res, fn * nb, cudaMemcpyDeviceToDevice, s));
   }
   plan->last_launches = launches;

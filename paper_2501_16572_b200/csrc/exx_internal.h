@@ -20,6 +20,9 @@ bool jacobi_eigh(int n, std::vector<double>& A, std::vector<double>& lam, std::v
 // Hermitian Bloch-periodic axis (R18): K(theta) = V diag(lam) V^H, V = Vr + i Vi row-major [i][m].
 bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& Vr,
                 std::vector<double>& Vi);
+// The same axis through its real form K' = U^H K U = W diag(lam) W^T (U: the fixed butterfly of plan_host.cpp); V = U W.
+bool bloch_eigh_real_form(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& W,
+                          std::vector<double>& Vr, std::vector<double>& Vi);
 // Reflection-adapted eigenbasis of a real axis: even vectors first, then odd (plan_host.cpp); false if it cannot be built.
 bool symmetrize_axis(int n, int bc, const std::vector<double>& lam, const std::vector<double>& V, std::vector<double>& lam_s,
                      std::vector<double>& Vs, int* n_even, bool centered = false);
@@ -58,6 +61,11 @@ struct exx_plan {
   // matrix is real (Dirichlet, or theta == 0)
   double theta[3];
   std::vector<double> h_Vi[3];
+  // Bloch plans, round 2: an axis with a phase is held in its REAL form (h_V = W, h_Vi empty) and the kernels apply the
+  // butterfly U^H / U around the real products (bfly[a]); the complex eigenvectors V = U W are kept for the test hook
+  bool bloch;
+  bool bfly[3];
+  std::vector<double> h_Vc_re[3], h_Vc_im[3];
   std::vector<double> h_mult;
   double zero_tol;  // R3 threshold on |lam_sum| the table was built with
   // device copies
@@ -237,6 +245,7 @@ cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const doubl
                                cudaStream_t s);
 cudaError_t bloch_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi, BatchDesc bd,
                              bool first, double* vx, cudaStream_t s);
+cudaError_t bloch_butterfly(const exx_plan* p, double* buf, int nb, bool inverse, cudaStream_t s, long long* launches);
 cudaError_t bloch_solve_batch(exx_plan* p, double* const buf[3], int nb, cudaStream_t s, long long* launches,
                               double** result);
 cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, double* scratch, int nb,

@@ -111,6 +111,198 @@ __global__ void __launch_bounds__(256) k_accumulate_c(const double* __restrict__
   }
 }
 
+// ---- axes held in their real form (plan_host.cpp bloch_eigh_real_form): the butterfly U^H / U -----------------------------
+// For an axis with a Bloch phase the plan holds the REAL orthogonal W of K' = U^H K U; a complex mode product V^H f is
+// g = U^H f followed by the real product W^T on both planes, and V t = U (W t).  U only couples a point x with its mirror
+// image Rx = n - 1 - x:
+//     forward  g[x] = (f[x] + f[Rx])/sqrt 2,        g[Rx] = -i (f[x] - f[Rx])/sqrt 2      (x < Rx; a self-paired point is kept)
+//     inverse  f[x] = (g[x] + i g[Rx])/sqrt 2,      f[Rx] = (g[x] - i g[Rx])/sqrt 2
+// and the butterflies of different axes commute with the products of the other axes, so all of them are applied at once,
+// on the orbit of a point under the reflections of the butterfly axes (up to 8 points), in the kernels that stream the
+// data anyway: the pair density (forward) and the accumulate (inverse); k_bfly_c serves the bare solver.
+struct BflyDims {
+  int n[3];     // nx, ny, nz
+  int half[3];  // points per axis a thread block enumerates: ceil(n/2) on a butterfly axis, n otherwise
+  int on[3];
+};
+
+struct Orbit {
+  long long idx[8];
+  int px, py, pz;  // 1: the axis pairs two distinct points
+};
+
+__device__ __forceinline__ Orbit orbit_of(const BflyDims& d, long long t) {
+  const int hx = (int)(t % d.half[0]);
+  const long long u = t / d.half[0];
+  const int hy = (int)(u % d.half[1]), hz = (int)(u / d.half[1]);
+  const int x1 = d.on[0] ? d.n[0] - 1 - hx : hx, y1 = d.on[1] ? d.n[1] - 1 - hy : hy, z1 = d.on[2] ? d.n[2] - 1 - hz : hz;
+  Orbit o;
+  o.px = x1 != hx;
+  o.py = y1 != hy;
+  o.pz = z1 != hz;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    const int x = (c & 1) ? x1 : hx, y = (c & 2) ? y1 : hy, z = (c & 4) ? z1 : hz;
+    o.idx[c] = x + (long long)d.n[0] * (y + (long long)d.n[1] * z);
+  }
+  return o;
+}
+// point c of the orbit is distinct from the points before it
+__device__ __forceinline__ bool orbit_has(const Orbit& o, int c) {
+  return (!(c & 1) || o.px) && (!(c & 2) || o.py) && (!(c & 4) || o.pz);
+}
+
+template <bool INVERSE>
+__device__ __forceinline__ void bfly_pair(double& ar, double& ai, double& br, double& bi) {
+  const double r = 0.70710678118654752440;
+  if (!INVERSE) {  // a' = (a + b) r, b' = -i (a - b) r
+    const double sr = (ar + br) * r, si = (ai + bi) * r, dr = (ar - br) * r, di = (ai - bi) * r;
+    ar = sr; ai = si; br = di; bi = -dr;
+  } else {         // a' = (a + i b) r, b' = (a - i b) r
+    const double pr = (ar - bi) * r, pi = (ai + br) * r, mr = (ar + bi) * r, mi = (ai - br) * r;
+    ar = pr; ai = pi; br = mr; bi = mi;
+  }
+}
+// all butterfly axes of one orbit, values v[c] = (vr[c], vi[c]) at orbit point c (bit 0: x, bit 1: y, bit 2: z)
+template <bool INVERSE>
+__device__ __forceinline__ void bfly_orbit(const Orbit& o, double (&vr)[8], double (&vi)[8]) {
+  if (o.px) {
+#pragma unroll
+    for (int c = 0; c < 8; c += 2) bfly_pair<INVERSE>(vr[c], vi[c], vr[c + 1], vi[c + 1]);
+  }
+  if (o.py) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      if (!(c & 2)) bfly_pair<INVERSE>(vr[c], vi[c], vr[c + 2], vi[c + 2]);
+  }
+  if (o.pz) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) bfly_pair<INVERSE>(vr[c], vi[c], vr[c + 4], vi[c + 4]);
+  }
+}
+
+// rho_b = conj(psi_j) .* tgt_k followed by the forward butterflies; grid.y = nb, a thread per orbit
+__global__ void __launch_bounds__(256) k_pair_density_c_bfly(const double* __restrict__ psi, const double* __restrict__ tgt,
+                                                             BatchDesc bd, long long N, BflyDims d, long long orbits,
+                                                             double* __restrict__ out) {
+  const int b = blockIdx.y;
+  const int j = bd.j0 + b % bd.nj, k = bd.k0 + b / bd.nj;
+  const double* ar = psi + (size_t)j * 2 * N;
+  const double* br = tgt + (size_t)k * 2 * N;
+  double* o = out + (size_t)b * 2 * N;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
+    const Orbit ob = orbit_of(d, t);
+    double vr[8], vi[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      vr[c] = vi[c] = 0.0;
+      if (orbit_has(ob, c)) {
+        const long long i = ob.idx[c];
+        const double a_re = ar[i], a_im = ar[N + i], b_re = br[i], b_im = br[N + i];
+        vr[c] = a_re * b_re + a_im * b_im;
+        vi[c] = a_re * b_im - a_im * b_re;
+      }
+    }
+    bfly_orbit<false>(ob, vr, vi);
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      if (orbit_has(ob, c)) {
+        o[ob.idx[c]] = vr[c];
+        o[N + ob.idx[c]] = vi[c];
+      }
+  }
+}
+
+// in-place butterflies of nb complex functions (the bare solver): forward before the products, inverse after them
+template <bool INVERSE>
+__global__ void __launch_bounds__(256) k_bfly_c(double* __restrict__ buf, long long N, BflyDims d, long long orbits) {
+  double* o = buf + (size_t)blockIdx.y * 2 * N;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
+    const Orbit ob = orbit_of(d, t);
+    double vr[8], vi[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      vr[c] = vi[c] = 0.0;
+      if (orbit_has(ob, c)) {
+        vr[c] = o[ob.idx[c]];
+        vi[c] = o[N + ob.idx[c]];
+      }
+    }
+    bfly_orbit<INVERSE>(ob, vr, vi);
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      if (orbit_has(ob, c)) {
+        o[ob.idx[c]] = vr[c];
+        o[N + ob.idx[c]] = vi[c];
+      }
+  }
+}
+
+// vx_k (-)= sum_j occ_j psi_j .* (U phi~_jk): inverse butterflies of the solver's output, then the complex product, j
+// ascending; grid.y = nk, a thread per orbit
+__global__ void __launch_bounds__(256) k_accumulate_c_bfly(const double* __restrict__ psi, const double* __restrict__ occ,
+                                                           const double* __restrict__ phi, BatchDesc bd, bool first,
+                                                           long long N, BflyDims d, long long orbits,
+                                                           double* __restrict__ vx) {
+  const int kk = blockIdx.y;
+  double* v = vx + (size_t)(bd.k0 + kk) * 2 * N;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
+    const Orbit ob = orbit_of(d, t);
+    double ar[8], ai[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      ar[c] = ai[c] = 0.0;
+      if (!first && orbit_has(ob, c)) {
+        ar[c] = v[ob.idx[c]];
+        ai[c] = v[N + ob.idx[c]];
+      }
+    }
+    const double* a = psi + (size_t)bd.j0 * 2 * N;
+    const double* f = phi + (size_t)kk * bd.nj * 2 * N;
+    for (int jj = 0; jj < bd.nj; ++jj) {
+      const double oc = occ[bd.j0 + jj];
+      double fr[8], fi[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        fr[c] = fi[c] = 0.0;
+        if (orbit_has(ob, c)) {
+          fr[c] = f[ob.idx[c]];
+          fi[c] = f[N + ob.idx[c]];
+        }
+      }
+      bfly_orbit<true>(ob, fr, fi);
+#pragma unroll
+      for (int c = 0; c < 8; ++c)
+        if (orbit_has(ob, c)) {
+          const double p_re = a[ob.idx[c]], p_im = a[N + ob.idx[c]];
+          ar[c] -= oc * (p_re * fr[c] - p_im * fi[c]);
+          ai[c] -= oc * (p_re * fi[c] + p_im * fr[c]);
+        }
+      a += 2 * N;
+      f += 2 * N;
+    }
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      if (orbit_has(ob, c)) {
+        v[ob.idx[c]] = ar[c];
+        v[N + ob.idx[c]] = ai[c];
+      }
+  }
+}
+
+inline bool any_bfly(const exx_plan* p) { return p->bfly[0] || p->bfly[1] || p->bfly[2]; }
+inline BflyDims bfly_dims(const exx_plan* p, long long* orbits) {
+  BflyDims d;
+  *orbits = 1;
+  for (int a = 0; a < 3; ++a) {
+    d.n[a] = p->n[a];
+    d.on[a] = p->bfly[a] ? 1 : 0;
+    d.half[a] = p->bfly[a] ? (p->n[a] + 1) / 2 : p->n[a];
+    *orbits *= d.half[a];
+  }
+  return d;
+}
+
 // Plain complex mode product, one thread per output point: out[m] = sum_i M[m][i] in[i] along `axis`,
 // forward M = V^H (M[m][i] = conj(V[i][m])), backward M = V.  Vi == nullptr: real matrix.  mult (optional) is applied
 // to the output.  total = nb * N complex points.
@@ -149,6 +341,13 @@ __global__ void k_mode_product_c(const double* __restrict__ in, double* __restri
 
 cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const double* tgt, BatchDesc bd, double* out,
                                cudaStream_t s) {
+  if (any_bfly(p)) {  // axes held in their real form: the forward butterflies ride on the pair density
+    long long orbits;
+    const BflyDims d = bfly_dims(p, &orbits);
+    dim3 grid(grid_for(orbits, 256, p->sm_count), bd.nj * bd.nk);
+    k_pair_density_c_bfly<<<grid, 256, 0, s>>>(psi, tgt, bd, p->N, d, orbits, out);
+    return cudaGetLastError();
+  }
   const bool vec2 = (p->N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)tgt | (uintptr_t)out) & 15) == 0);
   if (vec2) {
     dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nj * bd.nk);
@@ -162,6 +361,13 @@ cudaError_t bloch_pair_density(const exx_plan* p, const double* psi, const doubl
 
 cudaError_t bloch_accumulate(const exx_plan* p, const double* psi, const double* occ, const double* phi, BatchDesc bd,
                              bool first, double* vx, cudaStream_t s) {
+  if (any_bfly(p)) {  // the inverse butterflies ride on the accumulate
+    long long orbits;
+    const BflyDims d = bfly_dims(p, &orbits);
+    dim3 grid(grid_for(orbits, 256, p->sm_count), bd.nk);
+    k_accumulate_c_bfly<<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, d, orbits, vx);
+    return cudaGetLastError();
+  }
   const bool vec2 = (p->N % 2 == 0) && ((((uintptr_t)psi | (uintptr_t)phi | (uintptr_t)vx) & 15) == 0);
   if (vec2) {
     dim3 grid(grid_for(p->N / 2, 256, p->sm_count), bd.nk);
@@ -170,6 +376,18 @@ cudaError_t bloch_accumulate(const exx_plan* p, const double* psi, const double*
     dim3 grid(grid_for(p->N, 256, p->sm_count), bd.nk);
     k_accumulate_c<1><<<grid, 256, 0, s>>>(psi, occ, phi, bd, first, p->N, vx);
   }
+  return cudaGetLastError();
+}
+
+// In-place butterflies of nb complex functions for the bare solver (no-op for a plan without real-form axes).
+cudaError_t bloch_butterfly(const exx_plan* p, double* buf, int nb, bool inverse, cudaStream_t s, long long* launches) {
+  if (!any_bfly(p) || nb <= 0) return cudaSuccess;
+  long long orbits;
+  const BflyDims d = bfly_dims(p, &orbits);
+  dim3 grid(grid_for(orbits, 256, p->sm_count), nb);
+  if (inverse) k_bfly_c<true><<<grid, 256, 0, s>>>(buf, p->N, d, orbits);
+  else k_bfly_c<false><<<grid, 256, 0, s>>>(buf, p->N, d, orbits);
+  ++*launches;
   return cudaGetLastError();
 }
 

@@ -985,7 +985,7 @@ cudaError_t fused_init(exx_plan* p) {
   st->d_mult_sym = nullptr;
   st->zs_nh = 0;
   const int n = p->n[2], mtot = mtot_class(n);
-  if (p->h_Vi[2].empty() && p->h_Vi[0].empty() && p->h_Vi[1].empty()) {
+  if (!p->bloch && p->h_Vi[2].empty() && p->h_Vi[0].empty() && p->h_Vi[1].empty()) {
     // reflection-adapted basis of the z axis: image over the half range; three to eight row tiles per block (nz = 34
     // .. 128; below, the padding of the two blocks to whole row tiles eats the saving)
     std::vector<double> lam_s, Vs;

@@ -1266,7 +1266,7 @@ cudaError_t sym_init(exx_plan* p) {
   if (!st) return cudaSuccess;
   st->d_img_yf = st->d_img_yb = st->d_img_xf = st->d_img_xb = st->d_mult_symx = nullptr;
   st->ys_nh = st->xs_nh = 0;
-  if (!p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty()) return cudaSuccess;
+  if (p->bloch || !p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty()) return cudaSuccess;
   cudaError_t e = sym_init_y(p);
   if (e == cudaSuccess) e = sym_init_x(p);
   return e;

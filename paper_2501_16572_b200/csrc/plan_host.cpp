@@ -187,6 +187,87 @@ bool bloch_eigh(int n, double h, int order, double theta, std::vector<double>& l
   return kept == n;
 }
 
+// Bloch axis through its REAL form (round 2).  K(theta) is Hermitian and, with the phase carried by the
+// wrapped stencil entries, satisfies R K R = conj(K) for the centred reflection R: x -> n - 1 - x, i.e. it commutes with
+// the antiunitary T = R o conj (T^2 = 1).  In a basis of T-invariant vectors a T-symmetric Hermitian matrix is REAL
+// symmetric.  Such a basis is the fixed, sparse unitary U whose columns are, for every pair x < Rx,
+//     (e_x + e_Rx)/sqrt 2   (stored at index x)    and    i (e_x - e_Rx)/sqrt 2   (stored at index Rx),
+// and e_x for a self-paired point.  K' = U^H K U is real symmetric, K' = W diag(lam) W^T with W real orthogonal (Jacobi),
+// and K = (U W) diag(lam) (U W)^H.  A complex mode product V^H f then is the butterfly g = U^H f (a +- b on pairs of
+// points, mixing the real and imaginary planes) followed by the REAL product W^T on the two planes: half the real
+// operations of a complex matrix product.  Outputs: lam ascending, W row-major [i][m], and V = U W as (Vr, Vi) for the
+// test hook.
+bool bloch_eigh_real_form(int n, double h, int order, double theta, std::vector<double>& lam, std::vector<double>& W,
+                          std::vector<double>& Vr, std::vector<double>& Vi) {
+  const std::vector<double> w = fd_weights(order, h);
+  const int n0 = order / 2;
+  std::vector<double> Kr((size_t)n * n, 0.0), Ki((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int q = -n0; q <= n0; ++q) {
+      int j = i + q, wraps = 0;
+      while (j < 0) { j += n; --wraps; }
+      while (j >= n) { j -= n; ++wraps; }
+      Kr[(size_t)i * n + j] += w[std::abs(q)] * std::cos(theta * wraps);
+      Ki[(size_t)i * n + j] += w[std::abs(q)] * std::sin(theta * wraps);
+    }
+  // U as dense complex columns (n <= a few hundred: the n^3 products below are trivial)
+  const double r = 1.0 / std::sqrt(2.0);
+  std::vector<double> Ur((size_t)n * n, 0.0), Ui((size_t)n * n, 0.0);
+  for (int x = 0; x < n; ++x) {
+    const int xb = n - 1 - x;
+    if (x < xb) {
+      Ur[(size_t)x * n + x] = r;  Ur[(size_t)xb * n + x] = r;      // column x: (e_x + e_Rx)/sqrt 2
+      Ui[(size_t)x * n + xb] = r; Ui[(size_t)xb * n + xb] = -r;    // column Rx: i (e_x - e_Rx)/sqrt 2
+    } else if (x == xb) {
+      Ur[(size_t)x * n + x] = 1.0;
+    }
+  }
+  // T = K U (complex), K' = U^H T; keep the real part, symmetrise (the imaginary part is rounding)
+  std::vector<double> Tr((size_t)n * n, 0.0), Ti((size_t)n * n, 0.0), Kp((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      const double kr = Kr[(size_t)i * n + k], ki = Ki[(size_t)i * n + k];
+      if (kr == 0.0 && ki == 0.0) continue;
+      for (int b = 0; b < n; ++b) {
+        const double ur = Ur[(size_t)k * n + b], ui = Ui[(size_t)k * n + b];
+        Tr[(size_t)i * n + b] += kr * ur - ki * ui;
+        Ti[(size_t)i * n + b] += kr * ui + ki * ur;
+      }
+    }
+  double im_max = 0.0, re_max = 0.0;
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b) {
+      double sr = 0.0, si = 0.0;  // sum_i conj(U[i][a]) T[i][b]
+      for (int i = 0; i < n; ++i) {
+        const double ur = Ur[(size_t)i * n + a], ui = Ui[(size_t)i * n + a];
+        sr += ur * Tr[(size_t)i * n + b] + ui * Ti[(size_t)i * n + b];
+        si += ur * Ti[(size_t)i * n + b] - ui * Tr[(size_t)i * n + b];
+      }
+      Kp[(size_t)a * n + b] = sr;
+      im_max = std::fmax(im_max, std::fabs(si));
+      re_max = std::fmax(re_max, std::fabs(sr));
+    }
+  if (im_max > 1e-10 * (re_max > 0.0 ? re_max : 1.0)) return false;  // not T-symmetric: cannot happen for this stencil
+  for (int a = 0; a < n; ++a)
+    for (int b = a + 1; b < n; ++b) {
+      const double v = 0.5 * (Kp[(size_t)a * n + b] + Kp[(size_t)b * n + a]);
+      Kp[(size_t)a * n + b] = Kp[(size_t)b * n + a] = v;
+    }
+  if (!jacobi_eigh(n, Kp, lam, W)) return false;
+  Vr.assign((size_t)n * n, 0.0);
+  Vi.assign((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      const double ur = Ur[(size_t)i * n + k], ui = Ui[(size_t)i * n + k];
+      if (ur == 0.0 && ui == 0.0) continue;
+      for (int m = 0; m < n; ++m) {
+        Vr[(size_t)i * n + m] += ur * W[(size_t)k * n + m];
+        Vi[(size_t)i * n + m] += ui * W[(size_t)k * n + m];
+      }
+    }
+  return true;
+}
+
 // Reflection-adapted eigenbasis of a REAL axis (R13: f(L) does not depend on the basis chosen inside a
 // degenerate eigenspace).  The periodic matrix is circulant and symmetric, the Dirichlet one symmetric Toeplitz: both
 // commute with the reflection z -> mir(z) (periodic: (n - z) mod n, Dirichlet: n - 1 - z), so every eigenspace splits
