@@ -245,9 +245,11 @@ exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const do
  *       d_vx[k] (+)= - sum_j d_occ[j] * d_psi[j] .* f(L_theta)( conj(d_psi[j]) .* d_tgt[k] )
  *       d_ex_k[k] = h^3 Re <d_tgt[k], d_vx[k]>            (optional, NULL; computed after the update)
  * exx_plan_create_bloch validates like exx_plan_create (theta must be finite).  Workspace:
- * exx_plan_workspace_bytes_bloch(plan, n_c) (three buffers of n_c complex functions).  A complex mode product runs
- * as two launches of the real tensor-core kernel (real and imaginary part of V) plus a combine; axes whose matrix is
- * real (Dirichlet, theta = 0) take one.  exx_apply / exx_poisson_solve / exx_ace_* on a plan with a nonzero phase
+ * exx_plan_workspace_bytes_bloch(plan, n_c) (three buffers of n_c complex functions).  An axis with a phase is held
+ * in its real form: K(theta) commutes with (reflection x -> n-1-x) o (complex conjugation), so in the fixed butterfly basis
+ * U it is real symmetric, K = (U W) diag(lam) (U W)^H with W real; a complex mode product is the butterfly U^H / U (fused
+ * into the pair-density and accumulate kernels) and one real tensor-core launch over both planes, like a real axis
+ * (Dirichlet, theta = 0).  exx_apply / exx_poisson_solve / exx_ace_* on a plan with a nonzero phase
  * return EXX_ERR_INVALID_ARG.  Errors and aliasing rules as for exx_apply.
  */
 exx_status exx_plan_create_bloch(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,

@@ -126,25 +126,26 @@ struct BflyDims {
   int on[3];
 };
 
+// Orbit of a half-domain point under the reflections of the butterfly axes: point c (bit 0: x, bit 1: y, bit 2: z mirrored)
+// sits at base + (c & 1 ? dx : 0) + (c & 2 ? dy : 0) + (c & 4 ? dz : 0); a zero offset means the axis does not pair here
+// (no butterfly on it, or a self-paired point).  N < 2^31 (exx_plan_create), so 32-bit offsets suffice.
 struct Orbit {
-  long long idx[8];
+  int base, dx, dy, dz;
   int px, py, pz;  // 1: the axis pairs two distinct points
+  __device__ __forceinline__ int idx(int c) const { return base + ((c & 1) ? dx : 0) + ((c & 2) ? dy : 0) + ((c & 4) ? dz : 0); }
 };
 
-__device__ __forceinline__ Orbit orbit_of(const BflyDims& d, long long t) {
-  const int hx = (int)(t % d.half[0]);
-  const long long u = t / d.half[0];
-  const int hy = (int)(u % d.half[1]), hz = (int)(u / d.half[1]);
-  const int x1 = d.on[0] ? d.n[0] - 1 - hx : hx, y1 = d.on[1] ? d.n[1] - 1 - hy : hy, z1 = d.on[2] ? d.n[2] - 1 - hz : hz;
+__device__ __forceinline__ Orbit orbit_of(const BflyDims& d, unsigned t) {
+  const unsigned hx = t % (unsigned)d.half[0], u = t / (unsigned)d.half[0];
+  const unsigned hy = u % (unsigned)d.half[1], hz = u / (unsigned)d.half[1];
   Orbit o;
-  o.px = x1 != hx;
-  o.py = y1 != hy;
-  o.pz = z1 != hz;
-#pragma unroll
-  for (int c = 0; c < 8; ++c) {
-    const int x = (c & 1) ? x1 : hx, y = (c & 2) ? y1 : hy, z = (c & 4) ? z1 : hz;
-    o.idx[c] = x + (long long)d.n[0] * (y + (long long)d.n[1] * z);
-  }
+  o.base = (int)(hx + (unsigned)d.n[0] * (hy + (unsigned)d.n[1] * hz));
+  o.dx = d.on[0] ? d.n[0] - 1 - 2 * (int)hx : 0;
+  o.dy = d.on[1] ? (d.n[1] - 1 - 2 * (int)hy) * d.n[0] : 0;
+  o.dz = d.on[2] ? (d.n[2] - 1 - 2 * (int)hz) * d.n[0] * d.n[1] : 0;
+  o.px = o.dx != 0;
+  o.py = o.dy != 0;
+  o.pz = o.dz != 0;
   return o;
 }
 // point c of the orbit is distinct from the points before it
@@ -182,22 +183,26 @@ __device__ __forceinline__ void bfly_orbit(const Orbit& o, double (&vr)[8], doub
 }
 
 // rho_b = conj(psi_j) .* tgt_k followed by the forward butterflies; grid.y = nb, a thread per orbit
-__global__ void __launch_bounds__(256) k_pair_density_c_bfly(const double* __restrict__ psi, const double* __restrict__ tgt,
+__global__ void __launch_bounds__(256, 3) k_pair_density_c_bfly(const double* __restrict__ psi, const double* __restrict__ tgt,
                                                              BatchDesc bd, long long N, BflyDims d, long long orbits,
                                                              double* __restrict__ out) {
-  const int b = blockIdx.y;
-  const int j = bd.j0 + b % bd.nj, k = bd.k0 + b / bd.nj;
+  // blocks in (orbital, target) order with the target fastest: the nk right-hand sides that share psi_j are formed back to
+  // back and find it in L2 (with the right-hand-side order b = kk nj + jj a batch of 64 orbitals cycles through more
+  // than the L2 holds between two uses of the same psi_j)
+  const int jj = blockIdx.y / bd.nk, kk = blockIdx.y - jj * bd.nk;
+  const int b = kk * bd.nj + jj;
+  const int j = bd.j0 + jj, k = bd.k0 + kk;
   const double* ar = psi + (size_t)j * 2 * N;
   const double* br = tgt + (size_t)k * 2 * N;
   double* o = out + (size_t)b * 2 * N;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
-    const Orbit ob = orbit_of(d, t);
+    const Orbit ob = orbit_of(d, (unsigned)t);
     double vr[8], vi[8];
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
       vr[c] = vi[c] = 0.0;
       if (orbit_has(ob, c)) {
-        const long long i = ob.idx[c];
+        const int i = ob.idx(c);
         const double a_re = ar[i], a_im = ar[N + i], b_re = br[i], b_im = br[N + i];
         vr[c] = a_re * b_re + a_im * b_im;
         vi[c] = a_re * b_im - a_im * b_re;
@@ -207,54 +212,54 @@ __global__ void __launch_bounds__(256) k_pair_density_c_bfly(const double* __res
 #pragma unroll
     for (int c = 0; c < 8; ++c)
       if (orbit_has(ob, c)) {
-        o[ob.idx[c]] = vr[c];
-        o[N + ob.idx[c]] = vi[c];
+        o[ob.idx(c)] = vr[c];
+        o[N + ob.idx(c)] = vi[c];
       }
   }
 }
 
 // in-place butterflies of nb complex functions (the bare solver): forward before the products, inverse after them
 template <bool INVERSE>
-__global__ void __launch_bounds__(256) k_bfly_c(double* __restrict__ buf, long long N, BflyDims d, long long orbits) {
+__global__ void __launch_bounds__(256, 3) k_bfly_c(double* __restrict__ buf, long long N, BflyDims d, long long orbits) {
   double* o = buf + (size_t)blockIdx.y * 2 * N;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
-    const Orbit ob = orbit_of(d, t);
+    const Orbit ob = orbit_of(d, (unsigned)t);
     double vr[8], vi[8];
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
       vr[c] = vi[c] = 0.0;
       if (orbit_has(ob, c)) {
-        vr[c] = o[ob.idx[c]];
-        vi[c] = o[N + ob.idx[c]];
+        vr[c] = o[ob.idx(c)];
+        vi[c] = o[N + ob.idx(c)];
       }
     }
     bfly_orbit<INVERSE>(ob, vr, vi);
 #pragma unroll
     for (int c = 0; c < 8; ++c)
       if (orbit_has(ob, c)) {
-        o[ob.idx[c]] = vr[c];
-        o[N + ob.idx[c]] = vi[c];
+        o[ob.idx(c)] = vr[c];
+        o[N + ob.idx(c)] = vi[c];
       }
   }
 }
 
 // vx_k (-)= sum_j occ_j psi_j .* (U phi~_jk): inverse butterflies of the solver's output, then the complex product, j
 // ascending; grid.y = nk, a thread per orbit
-__global__ void __launch_bounds__(256) k_accumulate_c_bfly(const double* __restrict__ psi, const double* __restrict__ occ,
+__global__ void __launch_bounds__(256, 2) k_accumulate_c_bfly(const double* __restrict__ psi, const double* __restrict__ occ,
                                                            const double* __restrict__ phi, BatchDesc bd, bool first,
                                                            long long N, BflyDims d, long long orbits,
                                                            double* __restrict__ vx) {
   const int kk = blockIdx.y;
   double* v = vx + (size_t)(bd.k0 + kk) * 2 * N;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
-    const Orbit ob = orbit_of(d, t);
+    const Orbit ob = orbit_of(d, (unsigned)t);
     double ar[8], ai[8];
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
       ar[c] = ai[c] = 0.0;
       if (!first && orbit_has(ob, c)) {
-        ar[c] = v[ob.idx[c]];
-        ai[c] = v[N + ob.idx[c]];
+        ar[c] = v[ob.idx(c)];
+        ai[c] = v[N + ob.idx(c)];
       }
     }
     const double* a = psi + (size_t)bd.j0 * 2 * N;
@@ -266,15 +271,15 @@ __global__ void __launch_bounds__(256) k_accumulate_c_bfly(const double* __restr
       for (int c = 0; c < 8; ++c) {
         fr[c] = fi[c] = 0.0;
         if (orbit_has(ob, c)) {
-          fr[c] = f[ob.idx[c]];
-          fi[c] = f[N + ob.idx[c]];
+          fr[c] = f[ob.idx(c)];
+          fi[c] = f[N + ob.idx(c)];
         }
       }
       bfly_orbit<true>(ob, fr, fi);
 #pragma unroll
       for (int c = 0; c < 8; ++c)
         if (orbit_has(ob, c)) {
-          const double p_re = a[ob.idx[c]], p_im = a[N + ob.idx[c]];
+          const double p_re = a[ob.idx(c)], p_im = a[N + ob.idx(c)];
           ar[c] -= oc * (p_re * fr[c] - p_im * fi[c]);
           ai[c] -= oc * (p_re * fi[c] + p_im * fr[c]);
         }
@@ -284,8 +289,8 @@ __global__ void __launch_bounds__(256) k_accumulate_c_bfly(const double* __restr
 #pragma unroll
     for (int c = 0; c < 8; ++c)
       if (orbit_has(ob, c)) {
-        v[ob.idx[c]] = ar[c];
-        v[N + ob.idx[c]] = ai[c];
+        v[ob.idx(c)] = ar[c];
+        v[N + ob.idx(c)] = ai[c];
       }
   }
 }
