@@ -254,6 +254,14 @@ exx_status exx_ace_apply(exx_plan* plan, const double* d_xi, int n_orb, const do
  */
 exx_status exx_plan_create_bloch(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
                                  double omega, const double theta[3], int max_batch, int device);
+/* Test / measurement hook: the same plan with the form of its phase axes chosen.  EXX_BLOCH_FORM_REAL (what
+ * exx_plan_create_bloch builds) is the real form described above; EXX_BLOCH_FORM_EMBEDDED keeps complex eigenvectors
+ * V = Vr + i Vi and runs every complex mode product on the real embedding [[Mr, -Mi], [Mi, Mr]] (one launch for axes of up
+ * to 64 points, two read-modify-write launches above; twice the real operations) -- the cross-check the GPU tests
+ * compare with the oracle as well. */
+enum { EXX_BLOCH_FORM_REAL = 0, EXX_BLOCH_FORM_EMBEDDED = 1 };
+exx_status exx_plan_create_bloch_form(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
+                                      double omega, const double theta[3], int max_batch, int device, int form);
 size_t exx_plan_workspace_bytes_bloch(const exx_plan* plan, int n_c);
 exx_status exx_poisson_solve_bloch(exx_plan* plan, const double* d_rhs, double* d_phi, int n_rhs, int n_c,
                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream);

@@ -111,7 +111,7 @@ const char* exx_status_string(exx_status s) {
 
 // exx_plan_create / exx_plan_create_bloch (theta == nullptr: real plan)
 static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
-                              double omega, const double* theta, int max_batch, int device) {
+                              double omega, const double* theta, int max_batch, int device, int bloch_form = 0) {
   if (!out) return EXX_ERR_INVALID_ARG;
   *out = nullptr;
   if (nx < 1 || ny < 1 || nz < 1 || !(h > 0.0) || !std::isfinite(h) || !bc || fd_order < 2 ||
@@ -153,6 +153,15 @@ static exx_status create_plan(exx_plan** out, int nx, int ny, int nz, double h, 
         p->h_Vc_re[a] = p->h_Vc_re[same];
         p->h_Vc_im[a] = p->h_Vc_im[same];
         p->bfly[a] = p->bfly[same];
+        continue;
+      }
+      if (p->theta[a] != 0.0 && bloch_form == EXX_BLOCH_FORM_EMBEDDED) {
+        // cross-check form: complex eigenvectors, products on the real embedding [[Mr, -Mi], [Mi, Mr]]
+        if (!exx::bloch_eigh(p->n[a], h, fd_order, p->theta[a], p->h_lam[a], p->h_V[a], p->h_Vi[a])) {
+          delete p;
+          return EXX_ERR_EIGENSOLVE;
+        }
+        p->bloch = true;
         continue;
       }
       if (p->theta[a] != 0.0) {
@@ -231,6 +240,12 @@ exx_status exx_plan_create_bloch(exx_plan** out, int nx, int ny, int nz, double 
                                  double omega, const double theta[3], int max_batch, int device) {
   if (!theta) return EXX_ERR_INVALID_ARG;
   return create_plan(out, nx, ny, nz, h, bc, fd_order, omega, theta, max_batch, device);
+}
+
+exx_status exx_plan_create_bloch_form(exx_plan** out, int nx, int ny, int nz, double h, const int bc[3], int fd_order,
+                                      double omega, const double theta[3], int max_batch, int device, int form) {
+  if (!theta || (form != EXX_BLOCH_FORM_REAL && form != EXX_BLOCH_FORM_EMBEDDED)) return EXX_ERR_INVALID_ARG;
+  return create_plan(out, nx, ny, nz, h, bc, fd_order, omega, theta, max_batch, device, form);
 }
 
 exx_status exx_plan_destroy(exx_plan* plan) {

@@ -103,6 +103,9 @@ def load_library():
     lib.exx_plan_create_bloch.restype = C.c_int
     lib.exx_plan_create_bloch.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, ip, C.c_int,
                                           C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int]
+    lib.exx_plan_create_bloch_form.restype = C.c_int
+    lib.exx_plan_create_bloch_form.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_double, ip, C.c_int,
+                                               C.c_double, C.POINTER(C.c_double), C.c_int, C.c_int, C.c_int]
     lib.exx_plan_workspace_bytes_bloch.restype = C.c_size_t
     lib.exx_plan_workspace_bytes_bloch.argtypes = [vp, C.c_int]
     lib.exx_poisson_solve_bloch.restype = C.c_int
@@ -164,7 +167,8 @@ def probe_fp64_peak(kind: int, device: int = 0, seconds: float = 1.0) -> float:
 class Plan:
     """exx_plan_create / exx_plan_destroy (the per-axis eigendecompositions, once)."""
 
-    def __init__(self, nx, ny, nz, h, bc=(0, 0, 0), fd_order=12, omega=0.0, max_batch=64, device=0, theta=None):
+    def __init__(self, nx, ny, nz, h, bc=(0, 0, 0), fd_order=12, omega=0.0, max_batch=64, device=0, theta=None,
+                 bloch_form=0):
         lib = load_library()
         self._lib = lib
         self._h = C.c_void_p()
@@ -179,7 +183,11 @@ class Plan:
             _check(st, "exx_plan_create")
         else:   # Bloch-periodic plan: theta[a] = (k-q)_a * n_a * h (exx_plan_create_bloch)
             th = (C.c_double * 3)(*[float(t) for t in theta])
-            st = lib.exx_plan_create_bloch(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, th, max_batch, device)
+            if bloch_form:      # exx_plan_create_bloch_form: the embedded complex products (cross-check form)
+                st = lib.exx_plan_create_bloch_form(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, th, max_batch,
+                                                    device, int(bloch_form))
+            else:
+                st = lib.exx_plan_create_bloch(C.byref(self._h), nx, ny, nz, h, bc_arr, fd_order, omega, th, max_batch, device)
             _check(st, "exx_plan_create_bloch")
         self._ws = None
 

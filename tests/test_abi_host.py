@@ -119,13 +119,15 @@ def test_reflection_adapted_eigenbasis(lib, dims, bc, h):
 
 @pytest.mark.parametrize("dims,bc,theta", [((16, 12, 9), (0, 0, 1), (0.7, -2.1, 0.5)), ((48, 48, 48), (0, 0, 0), (np.pi, 0.0, 1.0)),
                                            ((7, 60, 5), (1, 0, 0), (0.3, np.pi / 2, -np.pi))])
-def test_bloch_planner_agrees_with_bloch_oracle(lib, dims, bc, theta):
-    """exx_plan_create_bloch (real-symmetric embedding + Jacobi + complex Gram-Schmidt) against numpy's Hermitian
-    eigh on the oracle's matrix: eigenvalues, unitarity, K V = V Lambda, and the multiplier table."""
+@pytest.mark.parametrize("form", [0, 1], ids=["real_form", "embedded"])
+def test_bloch_planner_agrees_with_bloch_oracle(lib, dims, bc, theta, form):
+    """exx_plan_create_bloch (form 0: the real form K' = U^H K U = W Lambda W^T through the reflection butterfly U, Jacobi,
+    V = U W) and exx_plan_create_bloch_form(EMBEDDED) (real-symmetric embedding + Jacobi + complex Gram-Schmidt) against
+    numpy's Hermitian eigh on the oracle's matrix: eigenvalues, unitarity, K V = V Lambda, and the multiplier table."""
     from oracle import bloch_oracle as blo
     nx, ny, nz = dims
     h, omega = 0.3, 0.106
-    p = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=4, device=-1, theta=theta)
+    p = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=4, device=-1, theta=theta, bloch_form=form)
     o = blo.make_plan(nx, ny, nz, h, bc, 12, omega, theta)
     scale = abs(blo.fd_weights(12, h)[0])
     for ax, n in enumerate(dims):

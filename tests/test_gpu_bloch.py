@@ -9,7 +9,11 @@ from paper_2501_16572_b200 import exx
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-10
-VARIANTS = [pytest.param(exx.VARIANT_FUSED_DMMA, id="fused_dmma"), pytest.param(exx.VARIANT_REFERENCE, id="reference")]
+# (kernel variant, form of the phase axes): the real form (butterfly + real products, the default), the embedded complex
+# products (exx_plan_create_bloch_form, the cross-check form), and the plain kernels
+VARIANTS = [pytest.param((exx.VARIANT_FUSED_DMMA, 0), id="fused_dmma"),
+            pytest.param((exx.VARIANT_FUSED_DMMA, 1), id="fused_dmma_embedded"),
+            pytest.param((exx.VARIANT_REFERENCE, 0), id="reference")]
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -56,13 +60,14 @@ SOLVE_CASES = [
 @pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("case", SOLVE_CASES, ids=lambda c: f"{c[0][0]}x{c[0][1]}x{c[0][2]}_nrhs{c[4]}")
 def test_bloch_solve_matches_oracle(case, variant):
+    variant, form = variant
     dims, bc, theta, omega, n_rhs, n_c = case
     nx, ny, nz = dims
     h = 0.3
     rng = np.random.default_rng(31)
     C = _rand(rng, n_rhs, dims)
     ref = blo.poisson_solve(blo.make_plan(nx, ny, nz, h, bc, 12, omega, theta), C)
-    plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=8, device=0, theta=theta)
+    plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=8, device=0, theta=theta, bloch_form=form)
     plan.set_variant(variant)
     d = _planar(C)
     keep = d.clone()
@@ -86,6 +91,7 @@ def test_bloch_solve_matches_oracle(case, variant):
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_bloch_apply_two_q_points_matches_oracle(variant):
     """Targets at k, orbitals at two q-points: two plans (theta = theta_k - theta_q), second call accumulates."""
+    variant, form = variant
     dims, bc, h, omega = (16, 12, 10), (0, 0, 1), 0.35, 0.106
     nx, ny, nz = dims
     th_k = np.array([0.6, -1.0, 0.0])
@@ -101,7 +107,7 @@ def test_bloch_apply_two_q_points_matches_oracle(variant):
     d_tgt = _planar(tgt)
     vx = None
     for q in range(2):
-        plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=8, device=0, theta=tuple(th_k - th_q[q]))
+        plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=8, device=0, theta=tuple(th_k - th_q[q]), bloch_form=form)
         plan.set_variant(variant)
         vx, e_k = plan.apply_bloch(_planar(psi[q]), torch.from_numpy(occ[q]).cuda(), d_tgt, vx=vx, accumulate=q > 0,
                                    n_c=3 if q == 0 else 8)
