@@ -183,7 +183,7 @@ __device__ __forceinline__ void bfly_orbit(const Orbit& o, double (&vr)[8], doub
 }
 
 // rho_b = conj(psi_j) .* tgt_k followed by the forward butterflies; grid.y = nb, a thread per orbit
-__global__ void __launch_bounds__(256, 3) k_pair_density_c_bfly(const double* __restrict__ psi, const double* __restrict__ tgt,
+__global__ void __launch_bounds__(256, 4) k_pair_density_c_bfly(const double* __restrict__ psi, const double* __restrict__ tgt,
                                                              BatchDesc bd, long long N, BflyDims d, long long orbits,
                                                              double* __restrict__ out) {
   // blocks in (orbital, target) order with the target fastest: the nk right-hand sides that share psi_j are formed back to
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(256, 3) k_pair_density_c_bfly(const double* __
 
 // in-place butterflies of nb complex functions (the bare solver): forward before the products, inverse after them
 template <bool INVERSE>
-__global__ void __launch_bounds__(256, 3) k_bfly_c(double* __restrict__ buf, long long N, BflyDims d, long long orbits) {
+__global__ void __launch_bounds__(256, 4) k_bfly_c(double* __restrict__ buf, long long N, BflyDims d, long long orbits) {
   double* o = buf + (size_t)blockIdx.y * 2 * N;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < orbits; t += (long long)gridDim.x * blockDim.x) {
     const Orbit ob = orbit_of(d, (unsigned)t);
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(256, 3) k_bfly_c(double* __restrict__ buf, lon
 
 // vx_k (-)= sum_j occ_j psi_j .* (U phi~_jk): inverse butterflies of the solver's output, then the complex product, j
 // ascending; grid.y = nk, a thread per orbit
-__global__ void __launch_bounds__(256, 2) k_accumulate_c_bfly(const double* __restrict__ psi, const double* __restrict__ occ,
+__global__ void __launch_bounds__(256, 3) k_accumulate_c_bfly(const double* __restrict__ psi, const double* __restrict__ occ,
                                                            const double* __restrict__ phi, BatchDesc bd, bool first,
                                                            long long N, BflyDims d, long long orbits,
                                                            double* __restrict__ vx) {
