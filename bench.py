@@ -621,6 +621,18 @@ def run_b200(args):
         del psi4
         torch.cuda.empty_cache()
         extra["configs"] = configs
+        # SURVEY 8(f) NEXT-3 in the same line: the Bloch-periodic complex variant on config 2's grid (short run)
+        try:
+            bl = run_bloch(argparse.Namespace(config=2, nc=0, steps=5, warmup=3, variant=0, no_ace=True, n_orb=0, n_tgt=0),
+                           emit=False)
+            extra["bloch_cfg2"] = {"value": bl["value"], "unit": "complex pair solves/s", "ms_per_step": bl["ms_per_step"],
+                                   "n_c": bl["config"]["n_c"], "theta": bl["config"]["theta"],
+                                   "mode_products_frac_of_dmma_peak": bl["roofline"]["frac"],
+                                   "step_frac": bl["roofline"]["step_frac"],
+                                   "class_ms_per_step": bl["roofline"]["class_ms_per_step"],
+                                   "what": "exx_apply_bloch, one (k,q) pair, 64 complex orbitals on 48^3; executed real flops"}
+        except Exception as exc:   # an extra, never fatal for the headline
+            extra["bloch_cfg2"] = {"error": str(exc)[:200]}
         extra["sweep_cfg4"] = {"what": "BASELINE.json configs[3] batch-size sweep (the paper's Fig. 1 in shape): all 1,536 "
                                        "orbitals against a reduced block of 8 targets (896..903), 3 timed steps each",
                                "unit": UNIT, "rows": sweep}
@@ -681,7 +693,7 @@ def measure_e2e(plan, w, d_psi, d_occ, n_c, ms_per_step):
             "ex": ex_h}
 
 
-def run_bloch(args):
+def run_bloch(args, emit=True):
     """One (k,q) pair of the complex variant on the config's grid and orbital count: phases pi/2, pi/3, pi/5 on the
     periodic axes, complex orbitals from workloads.make_complex_orbitals.  Roofline credit = executed real flops:
     per pass 2*N*n per plane product, 2 plane products per axis (axes with a phase run in their real form)."""
@@ -769,8 +781,10 @@ def run_bloch(args):
                                "max_abs_vx": float(vx.abs().max().item()),
                                "what": "exx_ace_build_bloch(psi, W=vx) and exx_ace_apply_bloch(xi, psi): median of 5, L2 "
                                        "flushed, CUDA events; executed real flops (4x a real Gram / expand)"}
-    print(json.dumps(line), flush=True)
     plan.close()
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
 def run_solver_sweep(args):
