@@ -613,7 +613,7 @@ def run_b200(args):
         configs = {}
         configs["cfg2"], _ = measure_extra(exx, 2, dev, local, peak_dmma, flush, stream, steps=10, want_ace=not args.no_ace)
         configs["cfg3"], _ = measure_extra(exx, 3, dev, local, peak_dmma, flush, stream, steps=3, want_ace=not args.no_ace)
-        configs["cfg4"], psi4 = measure_extra(exx, 4, dev, local, peak_dmma, flush, stream, n_tgt=32, steps=3)
+        configs["cfg4"], psi4 = measure_extra(exx, 4, dev, local, peak_dmma, flush, stream, steps=2)   # all 256 targets
         sweep = []
         for nc in (16, 32, 64, 128, 256, 512):
             r, _ = measure_extra(exx, 4, dev, local, peak_dmma, flush, stream, n_tgt=8, n_c=nc, steps=3, psi=psi4)
