@@ -53,7 +53,8 @@ typedef enum {
   EXX_ERR_CUDA = 3,
   EXX_ERR_EIGENSOLVE = 4,
   EXX_ERR_WORKSPACE = 5,
-  EXX_ERR_ALIAS = 6
+  EXX_ERR_ALIAS = 6,
+  EXX_ERR_LIMIT = 7 /* a size exceeds a fixed capacity compiled into the library (exx_energy_static) */
 } exx_status;
 
 enum { EXX_BC_PERIODIC = 0, EXX_BC_DIRICHLET = 1 };
@@ -288,6 +289,39 @@ exx_status exx_ace_build_bloch(exx_plan* plan, const double* d_psi, const double
                                double* d_M, int* d_info, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 exx_status exx_ace_apply_bloch(exx_plan* plan, const double* d_xi, int n_orb, const double* d_phi, int n_trial,
                                double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * The energy step on its own, for callers that cannot allocate device memory (BASELINE.json north_star: "together with
+ * the exchange energy"; R7):
+ *   d_ex_k[k] = dv * <d_tgt[k], d_vx[k]>   for k < n_tgt      (optional, NULL)      dv = h^3, the grid weight
+ *   *d_ex     = 1/2 sum_k d_occ_tgt[k] d_ex_k[k]              (optional, NULL; overwritten; needs d_occ_tgt)
+ * d_tgt, d_vx: [n_tgt][n_points] device doubles, e.g. the targets and the d_vx an exx_apply without d_ex / d_ex_k
+ * produced; they may be real sets (n_points = N) or the two-plane complex sets of exx_apply_bloch (n_points = 2 N,
+ * which gives Re <tgt, vx>).  The values equal those exx_apply returns for the same d_vx.
+ *
+ * Who needs it.  Some host programs give all of the GPU's memory to an arena of their own when they start (a
+ * hybrid-functional code sizes its orbital arrays to fill the card), after which cudaMalloc fails; others call from a
+ * loop that keeps several streams busy, where the device-wide synchronisation inside cudaMalloc / cudaFree would stall
+ * every one of them.  Every other compute call here needs a plan (whose creation allocates) and a workspace.  This call
+ * needs no plan and no workspace and calls no cudaMalloc, cudaFree or allocating library routine, on any call: the
+ * block sums of its two-stage reduction go to a fixed array inside the library image, EXX_ENERGY_STATIC_MAX_TGT * 64
+ * doubles = 2 MiB, which every GPU that loads libexx.so holds until the process exits.
+ *
+ * Limits and rules:
+ *  - n_tgt > EXX_ENERGY_STATIC_MAX_TGT returns EXX_ERR_LIMIT and enqueues nothing (split the targets over several
+ *    calls and sum *d_ex yourself, or use exx_apply's own energy outputs).
+ *  - It runs on the CURRENT device (cudaSetDevice), which must be the one the buffers live on, on `cuda_stream`, and
+ *    never synchronises the host.  The first call on each device looks up the array's address on that device
+ *    (cudaGetSymbolAddress; thread safe) -- make that first call during set-up, outside any stream capture.
+ *  - All calls on a device share the one array.  Nothing in it has to be zero beforehand (every slot a call reads it
+ *    has written itself first), but two calls that run on the GPU at the same time -- different streams, or different
+ *    host threads on different streams -- overwrite each other's block sums: order them on one stream or with events.
+ *  - Errors: INVALID_ARG (n_tgt < 0, n_points < 1, dv <= 0, a missing input, d_ex without d_occ_tgt), LIMIT, CUDA.
+ *    n_tgt == 0 writes *d_ex = 0.
+ */
+#define EXX_ENERGY_STATIC_MAX_TGT 4096
+exx_status exx_energy_static(const double* d_tgt, const double* d_vx, const double* d_occ_tgt, int n_tgt,
+                             long long n_points, double dv, double* d_ex_k, double* d_ex, void* cuda_stream);
 
 /* Number of kernels the last exx_apply / exx_poisson_solve call on this plan enqueued. */
 long long exx_plan_last_launch_count(const exx_plan* plan);

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libexx.so")
 STAMP = os.path.join(HERE, "csrc", ".build_stamp")
 
-SOURCES = ["plan_host.cpp", "kernels_ref.cu", "kernels_dmma.cu", "kernels_tma.cu", "kernels_fused.cu", "kernels_sym.cu", "kernels_nonbatch.cu", "kernels_ace.cu", "kernels_bloch.cu", "exx_api.cu", "peak_probe.cu"]
+SOURCES = ["plan_host.cpp", "kernels_ref.cu", "kernels_dmma.cu", "kernels_tma.cu", "kernels_fused.cu", "kernels_sym.cu", "kernels_nonbatch.cu", "kernels_ace.cu", "kernels_bloch.cu", "exx_api.cu", "peak_probe.cu", "energy_static.cu"]
 HEADERS = [os.path.join(CSRC, "exx_internal.h"), os.path.join(CSRC, "tma_common.cuh"), os.path.join(ROOT, "include", "exx.h")]
 
 COMPILE_FLAGS = [

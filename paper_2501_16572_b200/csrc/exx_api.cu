@@ -73,6 +73,11 @@ inline int resolve_nc(const exx_plan* p, int n_c) {
 
 }  // namespace
 
+namespace exx {
+// for entry points that live in other files (energy_static.cu): the error exx_status_string shows for EXX_ERR_CUDA
+void note_cuda_error(cudaError_t e) { g_last_cuda = e; }
+}  // namespace exx
+
 // plan-owned extras that are not part of the struct shared with the kernels
 struct PlanExtras {
   double* d_energy_scratch = nullptr;  // kEnergyChunk * kEnergyBlocks doubles
@@ -103,6 +108,9 @@ const char* exx_status_string(exx_status s) {
     case EXX_ERR_EIGENSOLVE: return "EXX_ERR_EIGENSOLVE: Jacobi eigensolver did not converge";
     case EXX_ERR_WORKSPACE: return "EXX_ERR_WORKSPACE: workspace too small or missing";
     case EXX_ERR_ALIAS: return "EXX_ERR_ALIAS: output overlaps an input or the workspace";
+    case EXX_ERR_LIMIT:
+      return "EXX_ERR_LIMIT: size exceeds a capacity fixed at build time (exx_energy_static: at most "
+             "EXX_ENERGY_STATIC_MAX_TGT = 4096 targets per call)";
   }
   return "unknown exx_status";
 }

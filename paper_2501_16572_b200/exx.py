@@ -124,6 +124,8 @@ def load_library():
     lib.exx_plan_get_profile_passes.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     lib.exx_probe_fp64_peak.restype = C.c_int
     lib.exx_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_double)]
+    lib.exx_energy_static.restype = C.c_int
+    lib.exx_energy_static.argtypes = [dp, dp, dp, C.c_int, C.c_longlong, C.c_double, dp, dp, vp]
     lib.exx_version.restype = C.c_char_p
     lib.exx_version.argtypes = []
     _lib = lib
@@ -162,6 +164,35 @@ def probe_fp64_peak(kind: int, device: int = 0, seconds: float = 1.0) -> float:
     out = C.c_double(0.0)
     _check(load_library().exx_probe_fp64_peak(kind, device, seconds, C.byref(out)), "exx_probe_fp64_peak")
     return out.value
+
+
+ENERGY_STATIC_MAX_TGT = 4096     # EXX_ENERGY_STATIC_MAX_TGT (include/exx.h)
+
+
+def energy_static(tgt: torch.Tensor, vx: torch.Tensor, occ_tgt: torch.Tensor | None, dv: float,
+                  ex_k: torch.Tensor | None, ex: torch.Tensor | None, stream: torch.cuda.Stream | None = None) -> None:
+    """exx_energy_static: ex_k[k] = dv <tgt[k], vx[k]>, ex = 1/2 sum_k occ_tgt[k] ex_k[k], written into the tensors the
+    caller passes (either may be None).  Meant for callers that cannot allocate on the GPU -- all device memory already
+    given to their own arena, or a multi-stream loop that a cudaMalloc would stall: the library call needs no plan and
+    no workspace and allocates nothing (its block sums go to a fixed 2 MiB array inside libexx.so), which is why this
+    wrapper takes the outputs instead of creating them.  At most ENERGY_STATIC_MAX_TGT targets per call (ExxError with
+    EXX_ERR_LIMIT beyond).  Runs on the tensors' device, which is made current for the call; calls that overlap on that
+    GPU race on the shared array, so keep them on one stream."""
+    n_tgt = tgt.shape[0]
+    dev = tgt.device
+    n_points = tgt.numel() // n_tgt if n_tgt else max(1, vx.numel())
+    if vx.numel() != tgt.numel():
+        raise ValueError("tgt and vx must hold the same number of elements")
+    for t, n, what in ((occ_tgt, n_tgt, "occ_tgt"), (ex_k, n_tgt, "ex_k"), (ex, 1, "ex")):
+        if t is not None and t.numel() != n:
+            raise ValueError(f"{what}: expected {n} elements, got {t.numel()}")
+    with torch.cuda.device(dev):
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        st = load_library().exx_energy_static(_dev_ptr(tgt, dev, "tgt"), _dev_ptr(vx, dev, "vx"),
+                                              _dev_ptr(occ_tgt, dev, "occ_tgt"), n_tgt, n_points, float(dv),
+                                              _dev_ptr(ex_k, dev, "ex_k"), _dev_ptr(ex, dev, "ex"),
+                                              C.c_void_p(s.cuda_stream))
+    _check(st, "exx_energy_static")
 
 
 class Plan:
