@@ -58,8 +58,8 @@ def parse_args():
     ap.add_argument("--n-orb", type=int, default=0, help="override orbital count (debug; invalidates the headline)")
     ap.add_argument("--n-tgt", type=int, default=0)
     ap.add_argument("--fusion", type=int, default=-1,
-                    help="exx_plan_set_fusion mask (measurement hook; -1 = library default 3: fused z pass and fused "
-                         "x-backward + accumulate)")
+                    help="exx_plan_set_fusion mask (measurement hook; -1 = library default 15: fused z pass, fused "
+                         "x-backward + accumulate, half-chunk y tiles, reflection-adapted eigenbases)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the configs 2-4 / sweep_cfg4 extra objects")

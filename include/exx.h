@@ -119,8 +119,11 @@ int exx_plan_get_fusion(const exx_plan* plan);
  */
 exx_status exx_plan_set_accumulate(exx_plan* plan, int on);
 
-/* Bytes of device workspace exx_apply / exx_poisson_solve need for batches of n_c right-hand sides
- * (0 if plan is NULL or n_c is outside 1..max_batch). */
+/* Bytes of device workspace exx_apply / exx_poisson_solve need for batches of n_c right-hand sides: two buffers of n_c
+ * grid functions, 16 N n_c bytes (0 if plan is NULL or n_c is outside 1..max_batch).  n_c = 0 asks for the library's
+ * default batch -- about 4 GB of right-hand sides, at least 32, at most max_batch -- so for a plan with a large
+ * max_batch exx_plan_workspace_bytes(plan, 0) is about 8 GB (it was about 2 GB before the default grew from 1 GB to
+ * 4 GB of right-hand sides); pass an explicit n_c to bound it. */
 size_t exx_plan_workspace_bytes(const exx_plan* plan, int n_c);
 
 /* Test hook: copy out one axis' eigenpairs. h_lambda: n doubles; h_V: n*n doubles, column-major

@@ -60,7 +60,7 @@ inline bool all_axes_fast(const exx_plan* p) { return p->d_Vpad[0] && p->d_Vpad[
 inline bool is_complex_plan(const exx_plan* p) { return p->bloch || p->d_Vi[0] || p->d_Vi[1] || p->d_Vi[2] ||
                                                          !p->h_Vi[0].empty() || !p->h_Vi[1].empty() || !p->h_Vi[2].empty(); }
 
-// n_c == 0: about 1 GB of right-hand sides per batch (measured: larger batches only amortise launch ramps and tails,
+// n_c == 0: about 4 GB of right-hand sides per batch (measured: larger batches only amortise launch ramps and tails,
 // DESIGN.md section 9), at least kDefaultBatch, at most max_batch
 inline int resolve_nc(const exx_plan* p, int n_c) {
   if (n_c == 0) {
@@ -338,7 +338,9 @@ exx_status exx_plan_get_axis(const exx_plan* plan, int axis, double* h_lambda, d
 }
 
 exx_status exx_plan_get_axis_symmetric(const exx_plan* plan, int axis, double* h_lambda, double* h_V, int* n_even) {
-  if (!plan || axis < 0 || axis > 2 || !plan->h_Vi[axis].empty()) return EXX_ERR_INVALID_ARG;
+  // a Bloch axis has no reflection-adapted real basis: in the embedded form its eigenvectors are complex (h_Vi), in the
+  // real form (bfly) h_V holds W of K' = U^H K U, which the periodic reflection does not act on
+  if (!plan || axis < 0 || axis > 2 || !plan->h_Vi[axis].empty() || plan->bfly[axis]) return EXX_ERR_INVALID_ARG;
   const int n = plan->n[axis];
   std::vector<double> lam_s, Vs;
   int nh = 0;

@@ -83,7 +83,8 @@ struct exx_plan {
   // forked and joined with the two events
   int lanes;
   // bit 0: z-forward + multiplier + z-backward in one pass (k_mode_zz); bit 1: x-backward + accumulate in one pass
-  // (k_mode_xacc); bit 2: y passes on 8-column half-chunk tiles where nx == 8 (mod 16).  Default 7; exx_plan_set_fusion
+  // (k_mode_xacc); bit 2: y passes on 8-column half-chunk tiles where nx == 8 (mod 16); bit 3 (needs bit 0): the mode products
+  // on the reflection-adapted eigenbases (symmetric mode).  Default 15 = all on; exx_plan_set_fusion
   // (test / measurement hook)
   int fusion;
   cudaStream_t lane_stream;

@@ -524,6 +524,7 @@ cudaError_t fast_solve_batch(exx_plan* p, const double* src, double* work, doubl
       }
       if (!xsym && p->variant == EXX_VARIANT_FUSED_DMMA) e = tma_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
       if (e == cudaErrorNotSupported) e = fast_mode_product(p, 0, true, nullptr, cur, nb, false, fa, s);
+      if (e == cudaErrorNotSupported) ps.cancel();  // nothing ran here: the plain pair density + x product below are recorded
     }
     if (e == cudaSuccess) {
       first_done = true;

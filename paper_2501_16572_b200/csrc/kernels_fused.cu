@@ -1104,7 +1104,7 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
     z.inner = (int)inner;
     z.cpo = (int)((inner + 15) / 16);
     const long long chunks = (long long)z.cpo * nb;
-    if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+    if (chunks >= (1LL << 31) - 64) return cudaErrorUnknown;  // see below: no fallback from here
     z.total_chunks = (unsigned)chunks;
     z.outer = nb;
     z.div_cpo = make_fastdiv((unsigned)z.cpo);
@@ -1125,7 +1125,9 @@ cudaError_t fused_zz(exx_plan* p, const double* in, double* out, int nb, cudaStr
       default: e = launch_zz_sym<8, 2, 12, 1>(p, m0, m1, z, s); break;
     }
     if (e == cudaSuccess) ++p->tma_launches;
-    if (e != cudaErrorNotSupported) return e;  // else: the dense fused kernel below
+    // The table is in (even | odd) z-mode order (lam_s), the dense kernel below contracts with the ascending basis in
+    // d_img_zz: a symmetric kernel that cannot run is a hard error, not a fallback.
+    return e == cudaErrorNotSupported ? cudaErrorUnknown : e;
   }
   ZArgs a{};
   a.out = out;

@@ -1388,7 +1388,11 @@ void sym_destroy(exx_plan* p) {
 // batch runs in "symmetric" mode (sym_axis_capable(p, 1) and TMA-addressable buffers).
 cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, cudaStream_t s) {
   TmaState* st = static_cast<TmaState*>(p->tma_state);
-  if (!st || !st->ys_nh || !aligned16(buf)) return cudaErrorNotSupported;
+  // NotSupported means exactly one thing to the caller: the plan has no symmetric y axis (the table then keeps y in
+  // ascending order and the dense product serves).  Past that point the table is in (even | odd) y order, so a kernel
+  // that cannot run is a hard error, never a reason to fall back to the dense product.
+  if (!st || !st->ys_nh) return cudaErrorNotSupported;
+  if (!aligned16(buf)) return cudaErrorUnknown;
   const int n = p->n[1], nh = st->ys_nh, no = n - nh, ms = (nh + 7) / 8;
   const bool per = false, hc = st->ys_hc;  // centred reflection y -> n - 1 - y on either kind of axis (sym_init_y)
   const long long inner = p->n[0], outer = (long long)p->n[2] * nb;
@@ -1408,7 +1412,7 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
   a.inner = (int)inner;
   a.cpo = (int)((inner + cw - 1) / cw);
   const long long chunks = (long long)a.cpo * outer;
-  if (chunks >= (1LL << 31) - 64) return cudaErrorNotSupported;
+  if (chunks >= (1LL << 31) - 64) return cudaErrorUnknown;
   a.total_chunks = (unsigned)chunks;
   a.outer = (int)outer;
   a.div_cpo = make_fastdiv((unsigned)a.cpo);
@@ -1418,22 +1422,26 @@ cudaError_t sym_mode_product_y(exx_plan* p, bool forward, double* buf, int nb, c
   CUtensorMap m0;
   cudaError_t e;
   if ((e = get_map(st, buf, inner, n, outer, 16, &m0, cw)) != cudaSuccess) return e;
-  ++p->tma_launches;
+  auto launch = [&]() -> cudaError_t {
 #define EXX_SYM_CASE(MSV)                                                                       \
   case MSV:                                                                                     \
     if (forward) return hc ? launch_lf<MSV, true>(p, m0, a, s) : launch_lf<MSV, false>(p, m0, a, s); \
     return hc ? launch_lb<MSV, true>(p, m0, a, s) : launch_lb<MSV, false>(p, m0, a, s);
-  switch (ms) {
-    EXX_SYM_CASE(3)
-    EXX_SYM_CASE(4)
-    EXX_SYM_CASE(5)
-    EXX_SYM_CASE(6)
-    EXX_SYM_CASE(7)
-    default:
-      if (forward) return hc ? launch_lf<8, true>(p, m0, a, s) : launch_lf<8, false>(p, m0, a, s);
-      return hc ? launch_lb<8, true>(p, m0, a, s) : launch_lb<8, false>(p, m0, a, s);
-  }
+    switch (ms) {
+      EXX_SYM_CASE(3)
+      EXX_SYM_CASE(4)
+      EXX_SYM_CASE(5)
+      EXX_SYM_CASE(6)
+      EXX_SYM_CASE(7)
+      default:
+        if (forward) return hc ? launch_lf<8, true>(p, m0, a, s) : launch_lf<8, false>(p, m0, a, s);
+        return hc ? launch_lb<8, true>(p, m0, a, s) : launch_lb<8, false>(p, m0, a, s);
+    }
 #undef EXX_SYM_CASE
+  };
+  e = launch();
+  if (e == cudaSuccess) ++p->tma_launches;
+  return e == cudaErrorNotSupported ? cudaErrorUnknown : e;
 }
 
 // Whether the exchange-apply batch `fa` can run its x passes on the reflection-adapted basis: the plan has the images and
@@ -1494,15 +1502,18 @@ cudaError_t sym_xf(exx_plan* p, double* out, int nb, const FastArgs* fa, cudaStr
   cudaError_t e;
   if ((e = get_map(st, fa->psi, a.n, (long long)a.rows_per_rhs * fa->n_occ, 0, 8 * NT, &m0)) != cudaSuccess) return e;
   if ((e = get_map(st, fa->tgt, a.n, (long long)a.rows_per_rhs * fa->n_tgt, 0, 8 * NT, &m1)) != cudaSuccess) return e;
-  ++p->tma_launches;
   switch ((a.nh + 7) / 8) {
-    case 3: return launch_xf<3>(p, m0, m1, a, s);
-    case 4: return launch_xf<4>(p, m0, m1, a, s);
-    case 5: return launch_xf<5>(p, m0, m1, a, s);
-    case 6: return launch_xf<6>(p, m0, m1, a, s);
-    case 7: return launch_xf<7>(p, m0, m1, a, s);
-    default: return launch_xf<8>(p, m0, m1, a, s);
+    case 3: e = launch_xf<3>(p, m0, m1, a, s); break;
+    case 4: e = launch_xf<4>(p, m0, m1, a, s); break;
+    case 5: e = launch_xf<5>(p, m0, m1, a, s); break;
+    case 6: e = launch_xf<6>(p, m0, m1, a, s); break;
+    case 7: e = launch_xf<7>(p, m0, m1, a, s); break;
+    default: e = launch_xf<8>(p, m0, m1, a, s); break;
   }
+  // counted only once the kernel is enqueued: NotSupported here (shared memory) sends the caller to the dense x-forward
+  // pass, and the batch's symmetric-mode decision reads this counter
+  if (e == cudaSuccess) ++p->tma_launches;
+  return e;
 }
 
 // Bare solver (exx_poisson_solve): whether its x passes can run on the reflection-adapted basis.
@@ -1531,15 +1542,16 @@ cudaError_t sym_xf_plain(exx_plan* p, const double* in, double* out, int nb, cud
   CUtensorMap m0;
   cudaError_t e;
   if ((e = get_map(st, in, a.n, (long long)a.rows_per_rhs * nb, 0, 8 * NT, &m0)) != cudaSuccess) return e;
-  ++p->tma_launches;
   switch ((a.nh + 7) / 8) {
-    case 3: return launch_xf_plain<3>(p, m0, a, s);
-    case 4: return launch_xf_plain<4>(p, m0, a, s);
-    case 5: return launch_xf_plain<5>(p, m0, a, s);
-    case 6: return launch_xf_plain<6>(p, m0, a, s);
-    case 7: return launch_xf_plain<7>(p, m0, a, s);
-    default: return launch_xf_plain<8>(p, m0, a, s);
+    case 3: e = launch_xf_plain<3>(p, m0, a, s); break;
+    case 4: e = launch_xf_plain<4>(p, m0, a, s); break;
+    case 5: e = launch_xf_plain<5>(p, m0, a, s); break;
+    case 6: e = launch_xf_plain<6>(p, m0, a, s); break;
+    case 7: e = launch_xf_plain<7>(p, m0, a, s); break;
+    default: e = launch_xf_plain<8>(p, m0, a, s); break;
   }
+  if (e == cudaSuccess) ++p->tma_launches;  // as in sym_xf: counted once enqueued
+  return e;
 }
 
 cudaError_t sym_xb_plain(exx_plan* p, double* buf, int nb, cudaStream_t s) {

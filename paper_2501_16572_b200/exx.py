@@ -247,7 +247,8 @@ class Plan:
         _check(self._lib.exx_plan_set_lanes(self._h, lanes), "exx_plan_set_lanes")
 
     def set_fusion(self, mask: int):
-        """exx_plan_set_fusion: bit 0 = fused z products, bit 1 = fused x-backward + accumulate (default 3)."""
+        """exx_plan_set_fusion: bit 0 = fused z products, bit 1 = fused x-backward + accumulate, bit 2 = half-chunk y tiles
+        where nx is 8 (mod 16), bit 3 = reflection-adapted eigenbases (needs bit 0).  Default 15 = all on (exx.h)."""
         _check(self._lib.exx_plan_set_fusion(self._h, mask), "exx_plan_set_fusion")
 
     @property

@@ -138,6 +138,13 @@ def test_bloch_planner_agrees_with_bloch_oracle(lib, dims, bc, theta, form):
         assert np.allclose(K @ V, V * lam[None, :], rtol=0, atol=2e-12 * scale)
         if bc[ax] == 1 or theta[ax] == 0.0:
             assert np.all(V.imag == 0.0)           # real axis: the real planner was used
+            p.get_axis_symmetric(ax)               # ... and it still has its reflection-adapted basis
+        else:
+            # an axis with a phase has no reflection-adapted real basis, in either form (in the real form h_V holds W of
+            # K' = U^H K U, not eigenvectors of K): exx_plan_get_axis_symmetric says INVALID_ARG, as exx.h documents
+            with pytest.raises(exx.ExxError) as err:
+                p.get_axis_symmetric(ax)
+            assert err.value.status == 1
     assert np.allclose(p.get_multiplier(), o.mult, rtol=1e-10, atol=0)
     # the real entry points refuse a complex plan
     dummy = C.c_void_p(1 << 20)

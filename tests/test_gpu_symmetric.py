@@ -91,6 +91,46 @@ def test_symmetric_apply_matches_full_oracle(case, variant):
     torch.cuda.synchronize()
     assert plan.last_solve_count == n * n
     assert _rel(vx.cpu().numpy(), vx_f.cpu().numpy()) < 1e-12
+    if two_sided:
+        # with both sides of the accumulate fused into the x-backward pass every vx_m receives its terms in
+        # ascending partner order (target side j <= m first, orbital side k > m after), each term formed by the same
+        # instructions from the same phi bits as in the full apply: the two results are bitwise equal
+        assert torch.equal(vx, vx_f), f"max abs diff {float((vx - vx_f).abs().max()):.3e}"
+        assert ex.item() == ex_f.item()
+    plan.close()
+
+
+# The unfused route of the pair-symmetric apply on grids where the two-sided fused accumulate COULD run: the streaming
+# k_accumulate (sym) + k_accumulate_transposed pair behind mode products that still run in symmetric mode order for y and z.
+# It is taken when fusion bit 1 is off (mask 13) and when a buffer is not 16-byte aligned (TMA cannot address it).  Either
+# way exx_apply_symmetric shapes its blocks with nk_min = 1, so nk >= 2 only where the whole block is one j-chunk.
+@pytest.mark.parametrize("how", ["fusion13", "psi_offset_8_bytes"])
+@pytest.mark.parametrize("case", [((40, 36, 34), (0, 0, 1), 0.106, 0.3, 21, 16), ((36, 40, 44), (1, 0, 0), 0.0, 0.3, 11, 5)],
+                         ids=lambda c: f"{c[0][0]}x{c[0][1]}x{c[0][2]}_n{c[4]}_nc{c[5]}")
+def test_symmetric_apply_unfused_route_on_symmetric_capable_grids(case, how):
+    dims, bc, omega, h, n, n_c = case
+    nx, ny, nz = dims
+    rng = np.random.default_rng(29)
+    psi = rng.standard_normal((n, nz, ny, nx))
+    occ = np.linspace(2.0, 1e-6, n)
+    o = orc.make_plan(nx, ny, nz, h, bc, 12, omega)
+    vx_o, e_o, ex_o = orc.exx_apply(o, psi, occ, psi, occ)
+    plan = exx.Plan(nx, ny, nz, h, bc, 12, omega, max_batch=64, device=0)
+    d_occ = torch.from_numpy(occ).cuda()
+    if how == "fusion13":
+        plan.set_fusion(13)
+        d_psi = torch.from_numpy(psi).cuda()
+    else:
+        flat = torch.empty(psi.size + 1, dtype=torch.float64, device="cuda")
+        d_psi = flat[1:].view(n, nz, ny, nx)
+        d_psi.copy_(torch.from_numpy(psi))
+        assert d_psi.data_ptr() % 16 == 8
+    vx, e_k, ex = plan.apply_symmetric(d_psi, d_occ, n_c=n_c)
+    torch.cuda.synchronize()
+    assert plan.last_solve_count == _expected_solves(n, n_c, 1)      # nk_min = 1: the two-sided pass was not chosen
+    assert _rel(vx.cpu().numpy(), vx_o) < TOL
+    assert np.abs(e_k.cpu().numpy() - e_o).max() < TOL * np.abs(e_o).max()
+    assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
     plan.close()
 
 
