@@ -128,3 +128,39 @@ def test_ace_on_config2_full_size():
     assert _rel(xi.cpu().numpy(), xi_o) < TOL
     assert _rel(own.cpu().numpy(), W_o) < TOL
     plan.close()
+
+
+def test_ace_at_the_measured_size_config3_256_orbitals():
+    """The ACE case bench.py times: BASELINE.json configs[2] (60x60x120 slab), n = 256 orbitals = four 64-wide Cholesky
+    blocks, n_trial = 256.  The oracle cannot produce W = Vx Psi at this size in test time (65,536 CPU solves), and no
+    oracle input may come from the CUDA path, so W is synthetic and made here on the CPU: W = -Psi S + 0.3 (1 - P) R with
+    S symmetric positive definite (condition number about 50), P the projector on the orbitals and R seeded noise.  The
+    orbitals are orthonormal under h^3, so M = h^3 Psi^T W = -S is negative definite as the method needs, and the part
+    outside the orbitals' span makes xi more than a recombination of Psi.  exx_ace_build and exx_ace_apply then have
+    exactly the measured shapes; the exchange apply that feeds them at this size is pinned by test_gpu_fullsize.py."""
+    w = wl.WORKLOADS[3]
+    n = w.n_orb
+    psi = wl.make_inputs(w, "cpu")[0].numpy()
+    dV = w.h ** 3
+    rng = np.random.default_rng(61)
+    Q, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    S = (Q * np.geomspace(0.02, 1.0, n)[None, :]) @ Q.T
+    S = 0.5 * (S + S.T)
+    P2 = psi.reshape(n, -1)
+    R = rng.standard_normal(P2.shape)
+    R -= (dV * (R @ P2.T)) @ P2                               # (1 - P) R, rows orthogonal to every orbital
+    W = (-(S @ P2) + 0.3 * R).reshape(psi.shape)
+    xi_o, M_o = ace.ace_build(psi, W, dV)
+    assert np.abs(M_o + S).max() < 1e-9                       # the construction did what it says
+    out_o = ace.ace_apply(xi_o, psi, dV)
+
+    plan = exx.Plan.for_workload(w, device=0)
+    d_psi, d_W = torch.from_numpy(psi).cuda(), torch.from_numpy(W).cuda()
+    xi, M, info = plan.ace_build(d_psi, d_W)
+    out = plan.ace_apply(xi, d_psi)
+    torch.cuda.synchronize()
+    assert int(info.item()) == 0
+    assert _rel(M.cpu().numpy(), M_o) < TOL
+    assert _rel(xi.cpu().numpy(), xi_o) < TOL
+    assert _rel(out.cpu().numpy(), out_o) < TOL
+    plan.close()

@@ -117,6 +117,42 @@ def test_bloch_apply_two_q_points_matches_oracle(variant):
     assert np.abs(e_k.cpu().numpy() - e_o).max() < TOL * np.abs(e_o).max()
 
 
+@pytest.mark.parametrize("form", [0, 1], ids=["real_form", "embedded"])
+@pytest.mark.parametrize("cfg,n_orb,n_c,cols", [(2, 64, 512, [0, 31, 63]), (3, 16, 256, [0, 15])],
+                         ids=["cfg2_48c_64orb", "cfg3_60x60x120_16orb"])
+def test_bloch_apply_at_the_benchmarked_sizes(cfg, n_orb, n_c, cols, form):
+    """exx_apply_bloch on the grids its throughput is quoted on, set up exactly as `bench.py --bloch --config 2` does
+    (48^3, 64 complex orbitals from workloads.make_complex_orbitals, n_c 512, phases pi/2, pi/3, pi/5 on the periodic
+    axes), and on the 60x60x120 slab with 16 orbitals: the GPU applies the operator to ALL targets in its own batch
+    shapes (the 16-byte butterfly kernels, orbits of up to 8 points, L2-ordered blocks); the oracle computes sampled
+    target columns with the full sum over the orbitals."""
+    from paper_2501_16572_b200 import workloads as wl
+    w = wl.WORKLOADS[cfg]
+    if n_orb != w.n_orb:
+        w = wl.scaled(w, n_orb, n_orb, 0)
+    theta = tuple(t if b == wl.PERIODIC else 0.0 for t, b in zip((np.pi / 2, np.pi / 3, np.pi / 5), w.bc))
+    d_psi = wl.make_complex_orbitals(w, "cpu").cuda()
+    occ = wl.occupations(w)
+    plan = exx.Plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, max_batch=max(128, n_c), device=0, theta=theta,
+                    bloch_form=form)
+    tma0 = plan.tma_launch_count
+    vx, e_k = plan.apply_bloch(d_psi, torch.from_numpy(occ).cuda(), d_psi, n_c=n_c)
+    torch.cuda.synchronize()
+    assert plan.tma_launch_count > tma0                     # the tensor-core kernels served it
+    psi = _cplx(d_psi)
+    o = blo.make_plan(w.nx, w.ny, w.nz, w.h, w.bc, w.order, w.omega, theta)
+    vx_o, e_o = blo.exx_apply_bloch(o, psi, occ, psi[cols])
+    assert _rel(_cplx(vx[cols]), vx_o) < TOL
+    e_all = e_k.cpu().numpy()
+    assert np.abs(e_all[cols] - e_o).max() < TOL * np.abs(e_o).max()
+    # whole block, any size: Vx is Hermitian negative semidefinite -- M_ab = <psi_a|Vx psi_b> = conj(M_ba), e_k < 0
+    z = _cplx(vx).reshape(n_orb, -1)
+    M = psi.reshape(n_orb, -1).conj() @ z.T
+    assert np.abs(M - M.conj().T).max() < 1e-9 * np.abs(M).max()
+    assert np.all(e_all < 0)
+    plan.close()
+
+
 def test_bloch_theta_zero_equals_the_real_apply():
     dims, bc, h, omega = (16, 16, 16), (0, 0, 0), 0.5, 0.0
     rng = np.random.default_rng(41)

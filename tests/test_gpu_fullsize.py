@@ -1,7 +1,9 @@
-"""Full-size parity (BASELINE.json configs 3-5 at their real orbital counts, default n_c, the launch
-configuration bench.py times): the oracle computes sampled target columns with the FULL sum over all
-occupied orbitals (SURVEY.md 8(c) "column sub-sampling"); the GPU's e_k makes the energy check exact per
-column.  The oracle streams the orbitals from the GPU in chunks, so no host copy of the 44 GB set is needed.
+"""Full-size parity (BASELINE.json configs 3-5 at their real orbital counts AND their real target blocks, default n_c:
+the batch shapes bench.py times -- 26 x 3 batches of 10 orbitals x up to 102 targets at cfg3, 119 x 7 of 13 x 39 at cfg4,
+320 x 6 of 10 x 25 at cfg5 on a 148-SM B200; the launch count is asserted so the shape cannot drift).  The GPU applies
+the whole block; the oracle computes sampled target columns INSIDE that block with the FULL sum over all occupied
+orbitals (SURVEY.md 8(c) "column sub-sampling"), and the GPU's e_k makes the energy check exact per column.  The
+oracle streams the orbitals from the GPU in chunks, so no host copy of the 44 GB set is needed.
 Set EXX_SKIP_SLOW=1 to skip (the oracle needs 1-3 minutes of CPU per config)."""
 import os
 
@@ -30,33 +32,63 @@ def _oracle_columns(w, d_psi, occ, cols, chunk=64):
     return np.stack(vx), e
 
 
-@pytest.mark.parametrize("cfg,cols", [(3, [0, 36, 73, 109, 146, 182, 219, 255]), (4, [896, 1151]), (5, [2176])])
+def _batch_shape(w, n_c, sms):
+    """exx_apply's batch shaping rule (exx_api.cu), restated: a k_mode_xacc work item is (row tile, target), 16 rows up to
+    64 x points and 8 above; a batch takes enough targets for about 24 items per warp (12 warps per SM), the rest of n_c
+    goes to orbitals (at least 8).  Returns (orbitals per batch, targets per batch)."""
+    rows = 16 if w.nx <= 64 else 8
+    tiles = (w.ny * w.nz + rows - 1) // rows
+    nk_want = min(-(-24 * 12 * sms // tiles), w.n_tgt, n_c)
+    nj = min(max(n_c // nk_want, min(8, w.n_orb)), n_c, w.n_orb)
+    return nj, n_c // nj
+
+
+@pytest.mark.parametrize("cfg,cols", [(3, [0, 36, 73, 109, 146, 182, 219, 255]), (4, [896, 1151]), (5, [2176, 2303])])
 def test_full_size_sampled_columns(cfg, cols):
     if os.environ.get("EXX_SKIP_SLOW") == "1":
         pytest.skip("EXX_SKIP_SLOW=1")
     w = wl.WORKLOADS[cfg]
-    need = w.n_orb * w.N * 8 + (len(cols) * 2 + 2 * w.default_nc) * w.N * 8
+    need = w.n_orb * w.N * 8 + (w.n_tgt + 2 * w.default_nc) * w.N * 8
     free, _ = torch.cuda.mem_get_info()
     if free < need + (4 << 30):
         pytest.skip(f"needs {need / 2**30:.0f} GiB of device memory")
-    psi, occ, _, _ = wl.make_inputs(w, "cuda")
-    idx = torch.tensor(cols, device="cuda")
-    tgt = psi[idx].contiguous()
-    occ_t = occ[idx].contiguous()
+    psi, occ, tgt, occ_t = wl.make_inputs(w, "cuda")        # tgt = psi[tgt_start : tgt_start + n_tgt], the config's block
+    assert tgt.shape[0] == w.n_tgt and all(w.tgt_start <= c < w.tgt_start + w.n_tgt for c in cols)
     plan = exx.Plan.for_workload(w, device=0)
-    vx, e_k, ex = plan.apply(psi, occ, tgt, occ_t)          # default n_c, all n_orb occupied orbitals
+    vx, e_k, ex = plan.apply(psi, occ, tgt, occ_t, n_c=w.default_nc)   # what bench.py runs: whole block, all orbitals
     torch.cuda.synchronize()
-    assert plan.last_launch_count > 0
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    nj, nk = _batch_shape(w, w.default_nc, sms)
+    n_batches = -(-w.n_orb // nj) * -(-w.n_tgt // nk)
+    assert nk > 8 and plan.last_launch_count == 5 * n_batches + 3, (plan.last_launch_count, nj, nk)   # 5 passes per batch
+    if sms == 148:
+        assert plan.last_launch_count == {3: 393, 4: 4168, 5: 9603}[cfg]     # bench.py's launches per step (profiles/)
+    loc = [c - w.tgt_start for c in cols]
     vx_o, e_o = _oracle_columns(w, psi, occ, cols)
-    err = np.abs(vx.cpu().numpy() - vx_o).max() / np.abs(vx_o).max()
+    vx_s = vx[loc].cpu().numpy()
+    err = np.abs(vx_s - vx_o).max() / np.abs(vx_o).max()
     assert err < TOL, err
-    assert np.abs(e_k.cpu().numpy() - e_o).max() / np.abs(e_o).max() < TOL
-    ex_o = 0.5 * float(np.sum(occ_t.cpu().numpy() * e_o))
-    assert abs(ex.item() - ex_o) < TOL * abs(ex_o)
-    # properties that hold at any size: e_k < 0 (Vx is negative semidefinite), pair symmetry of the
-    # Hermitian form <psi_a|Vx psi_b> on the sampled block
-    assert np.all(e_k.cpu().numpy() < 0)
-    if len(cols) > 1:
-        M = (tgt.view(len(cols), -1) @ vx.view(len(cols), -1).T).cpu().numpy()
-        assert np.abs(M - M.T).max() < 1e-9 * np.abs(M).max()
+    e_all = e_k.cpu().numpy()
+    assert np.abs(e_all[loc] - e_o).max() / np.abs(e_o).max() < TOL
+    # E_x of the whole block: the library's sum over its own e_k (the sampled ones are pinned above), recomputed here
+    ex_blk = 0.5 * float(np.sum(occ_t.cpu().numpy() * e_all))
+    assert abs(ex.item() - ex_blk) < 1e-12 * abs(ex_blk)
+    # properties that hold at any size, over the whole block: e_k < 0 (Vx is negative semidefinite) and the symmetry
+    # of the Hermitian form <psi_a|Vx psi_b>, whose diagonal is e_k / h^3
+    assert np.all(e_all < 0)
+    M = (tgt.reshape(w.n_tgt, -1) @ vx.reshape(w.n_tgt, -1).T).cpu().numpy()
+    assert np.abs(M - M.T).max() < 1e-9 * np.abs(M).max()
+    assert np.abs(np.diag(M) * w.h ** 3 - e_all).max() < 1e-12 * np.abs(e_all).max()
+    if w.tgt_start == 0 and w.n_tgt == w.n_orb:
+        # targets == orbitals (cfg3): the pair-symmetric apply at the size bench.py measures it, against the same oracle
+        # columns (the oracle's FULL sum over j; about half of the pairs are solved here)
+        del M
+        vx_s2, e_s2, ex_s2 = plan.apply_symmetric(psi, occ, n_c=w.default_nc)
+        torch.cuda.synchronize()
+        assert w.n_orb * (w.n_orb + 1) // 2 <= plan.last_solve_count < 0.6 * w.n_orb ** 2
+        err = np.abs(vx_s2[loc].cpu().numpy() - vx_o).max() / np.abs(vx_o).max()
+        assert err < TOL, err
+        assert np.abs(e_s2.cpu().numpy()[loc] - e_o).max() / np.abs(e_o).max() < TOL
+        assert float((vx_s2 - vx).abs().max()) < 1e-12 * float(vx.abs().max())
+        assert abs(ex_s2.item() - ex.item()) < 1e-12 * abs(ex.item())
     plan.close()
