@@ -54,6 +54,11 @@ def parse_args():
     ap.add_argument("--nc", type=int, default=0, help="right-hand sides per batch (0 = workload default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process-group backend for --gpus N > 1.  nccl (default): one rank per GPU.  gloo: a DEBUG mode that "
+                         "lets several ranks share the GPUs present (rank r uses cuda:(r mod device_count)), so the whole "
+                         "multi-rank branch can be executed on a one-GPU box; its throughput is not a scaling number and "
+                         "the line says so")
     ap.add_argument("--variant", type=int, default=0, help="0 = DMMA path (default), 1 = plain-kernel cross-check variant")
     ap.add_argument("--n-orb", type=int, default=0, help="override orbital count (debug; invalidates the headline)")
     ap.add_argument("--n-tgt", type=int, default=0)
@@ -91,7 +96,9 @@ def config_dict(w: wl.Workload, n_c: int, extra=None) -> dict:
     d = {"workload": f"BASELINE.json configs[{w.cfg - 1}]: {w.name}", "grid": [w.nx, w.ny, w.nz], "h_bohr": w.h,
          "bc_xyz": bcs, "fd_order": w.order, "omega": w.omega, "n_occ": w.n_orb, "n_tgt": w.n_tgt,
          "tgt_start": w.tgt_start, "pair_solves_per_step": w.pair_solves, "n_c": n_c,
-         "flops_per_solve": w.flops_per_solve, "l2": "flushed between timed steps (256 MiB write)"}
+         "flops_per_solve": w.flops_per_solve,
+         # one text for both arms, so that their `config` objects compare equal
+         "l2": "B200 arm: flushed between timed steps (256 MiB write outside the event pair); reference arm: n/a (CPU)"}
     if extra:
         d.update(extra)
     return d
@@ -161,7 +168,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": steps, "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(w, args.nc or w.default_nc, {"l2": "n/a (CPU)"}),
+            "config": config_dict(w, args.nc or w.default_nc),
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -246,21 +253,37 @@ def hbm_peak():
         return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-# Algorithmic HBM bytes per grid point and pair solve of the five-pass structure: pass 1 writes the batch
-# (8; psi_j and tgt_k tiles are shared by the nk / nj pairs of a batch: 8/nk + 8/nj), passes 2-4 read and write it (48),
-# pass 5 reads it (8) plus the psi tiles (8/nk) and vx_k (16/nj): 64 + 16/nk + 24/nj.  The bound below uses 64.
-ALG_BYTES_PER_POINT = 64.0
+# Algorithmic HBM bytes per grid point and pair solve: SURVEY.md 8(d) counts 48 (its three-fused-pass structure: two
+# round trips of the batch between the passes plus one more pass's worth for psi/tgt/vx tiles).  The five-pass structure
+# this library runs moves 64 + 16/nk + 24/nj (pass 1 writes the batch, passes 2-4 read and write it, pass 5
+# reads it).  The HBM leg of the step roofline uses the survey's 48; the fraction against the structure's own 64 is
+# reported beside it (`frac_vs_structure_bytes`), so that "how close to the roofline" and "how close to what this design
+# can reach" are both in the line.
+ALG_BYTES_PER_POINT = 48.0
+STRUCTURE_BYTES_PER_POINT = 64.0
 
 
-def step_roofline(flops_exec_per_solve: float, N: int, peak_tflops: float, us_per_solve: float) -> dict:
-    """Whole-step roofline: the slower of (executed FP64 operations / DMMA peak) and (algorithmic bytes / copy bandwidth)."""
+def step_roofline(flops_exec_per_solve: float, N: int, peak_tflops: float, us_per_solve: float,
+                  flops_dense_per_solve: float | None = None) -> dict:
+    """Whole-step roofline: the slower of (executed FP64 operations / DMMA peak) and (SURVEY.md 8(d)'s algorithmic bytes /
+    copy bandwidth).  `frac` = `frac_vs_survey_bytes` uses the survey's 48 B per point; `frac_vs_structure_bytes` the 64 B
+    of the five-pass structure; `frac_dense_count` credits the tensor leg with the dense algorithmic operations
+    4 N (nx+ny+nz) of SURVEY.md 8(d) (above 1 where the reflection-adapted bases halve the executed ones)."""
     hbm, src = hbm_peak()
     t_tensor = flops_exec_per_solve / (peak_tflops * 1e12) * 1e6
     t_hbm = ALG_BYTES_PER_POINT * N / (hbm * 1e9) * 1e6
+    t_hbm_structure = STRUCTURE_BYTES_PER_POINT * N / (hbm * 1e9) * 1e6
     bound = "tensor" if t_tensor >= t_hbm else "hbm"
-    return {"bound": bound, "us_per_solve_tensor": t_tensor, "us_per_solve_hbm": t_hbm, "us_per_solve_measured": us_per_solve,
-            "frac": max(t_tensor, t_hbm) / us_per_solve, "hbm_peak_gbs": hbm, "hbm_peak_source": src,
-            "algorithmic_bytes_per_solve": ALG_BYTES_PER_POINT * N}
+    out = {"bound": bound, "us_per_solve_tensor": t_tensor, "us_per_solve_hbm": t_hbm, "us_per_solve_measured": us_per_solve,
+           "frac": max(t_tensor, t_hbm) / us_per_solve, "frac_vs_survey_bytes": max(t_tensor, t_hbm) / us_per_solve,
+           "frac_vs_structure_bytes": max(t_tensor, t_hbm_structure) / us_per_solve,
+           "us_per_solve_hbm_structure": t_hbm_structure, "hbm_peak_gbs": hbm, "hbm_peak_source": src,
+           "algorithmic_bytes_per_solve": ALG_BYTES_PER_POINT * N, "algorithmic_bytes_per_point": ALG_BYTES_PER_POINT,
+           "structure_bytes_per_point": STRUCTURE_BYTES_PER_POINT}
+    if flops_dense_per_solve:
+        t_dense = flops_dense_per_solve / (peak_tflops * 1e12) * 1e6
+        out["frac_dense_count"] = max(t_dense, t_hbm) / us_per_solve
+    return out
 
 
 def timed_apply(step, steps: int, warmup: int, flush, stream, barrier=None):
@@ -314,7 +337,8 @@ def instrumented(plan, step, flush, prof_steps: int, flops_step: float, peak: fl
         kernels[name] = {"kernel": KERNEL_OF_PASS[name][0 if sym else 1], "launches_per_step": cnt // prof_steps,
                          "avg_launch_ms": ms / max(cnt, 1), "ms_per_step": ms / prof_steps,
                          "share_of_step": ms / all_ms if all_ms > 0 else None, "executed_flops_per_solve": fl,
-                         "achieved_tflops": tf, "frac_of_dmma_peak": tf / peak}
+                         "dense_flops_per_solve": dense, "achieved_tflops": tf, "frac_of_dmma_peak": tf / peak,
+                         "frac_dense_count": tf / peak * dense / fl if fl > 0 else None}
     return {"achieved": achieved, "frac": achieved / peak, "avg_launch_ms": mp_ms / max(mp_cnt, 1),
             "launches": mp_cnt // prof_steps, "share_of_step": mp_ms / all_ms if all_ms > 0 else None,
             "class_ms_per_step": {k: v[0] / prof_steps for k, v in prof.items()}, "kernels": kernels}
@@ -347,7 +371,7 @@ def measure_extra(exx, cfg: int, dev, local: int, peak: float, flush, stream, n_
            "n_c": n_c, "pair_solves_per_step": w.pair_solves, "steps": steps, "ms_per_step": ms,
            "value": w.pair_solves / (ms * 1e-3), "unit": UNIT, "applies_per_s": w.n_tgt / (ms * 1e-3),
            "step_frac": flops / (ms * 1e-3) / 1e12 / peak,
-           "step_roofline": step_roofline(plan.executed_flops_per_solve, w.N, peak, ms * 1e3 / w.pair_solves),
+           "step_roofline": step_roofline(plan.executed_flops_per_solve, w.N, peak, ms * 1e3 / w.pair_solves, w.flops_per_solve),
            "executed_over_algorithmic_flops": plan.executed_flops_per_solve / w.flops_per_solve, "E_x": float(ex.item()),
            "launches_per_step": plan.last_launch_count}
     if want_ace and w.n_tgt == w.n_orb and w.tgt_start == 0:
@@ -431,10 +455,15 @@ def run_b200(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if args.backend == "gloo":      # debug: ranks may share a GPU (NCCL refuses two ranks on one device, gloo does not)
+        local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if args.backend == "gloo":
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
 
     import __graft_entry__ as ge
     if rank == 0:
@@ -526,17 +555,23 @@ def run_b200(args):
     traffic = None
     if dom is not None:
         traffic = traffic_tab.get((w.cfg, n_c), {}).get(dom["kernel"].split("<")[0])
-    n_batch = min(n_c, w.n_orb * n_tgt_local)
+    # right-hand sides of one launch of the dominant kernel: the step's pair solves over its launches (the batches are
+    # nj x nk <= n_c, the last target block smaller), not n_c itself
+    n_batch = (w.n_orb * n_tgt_local / dom["launches_per_step"]) if dom is not None and dom["launches_per_step"] else \
+        min(n_c, w.n_orb * n_tgt_local)
     us_per_solve = ms_per_step * 1e3 / (w.n_orb * n_tgt_local)
     roofline = {"bound": "tensor",
                 "kernel": (f"{dom['kernel']} ({dom_pass} pass of a batch; FP64 mma.sync -> DMMA.8x8x4, operands by TMA)"
                            if dom is not None else "mode products"),
                 "achieved": dom["achieved_tflops"] if dom is not None else inst["achieved"], "peak": peak_dmma,
                 "unit": "TFLOP/s", "frac": dom["frac_of_dmma_peak"] if dom is not None else inst["frac"],
+                "frac_executed_count": dom["frac_of_dmma_peak"] if dom is not None else inst["frac"],
+                "frac_dense_count": dom["frac_dense_count"] if dom is not None else None,
                 "traffic": traffic,
                 "traffic_note": (f"dram read + write bytes per launch of this kernel from the committed ncu --set full capture "
                                  f"profiles/{traffic_file}" if traffic else "no committed ncu capture for this (config, n_c)")
-                                + f"; algorithmic bytes of an in-place pass over one batch = {2 * 8 * w.N * n_batch:.4g}",
+                                + f"; algorithmic bytes of an in-place pass over one launch's {n_batch:.1f} right-hand sides (average over "
+                                  f"the step's batches) = {2 * 8 * w.N * n_batch:.4g}",
                 "achieved_note": "FP64 operations this kernel EXECUTES per launch (exx_plan_get_profile_passes; the dense "
                                  "algorithmic count of its products would be higher where it runs on the reflection-adapted "
                                  "basis, DESIGN.md 6.9) / its average launch duration (CUDA events, live)",
@@ -550,13 +585,16 @@ def run_b200(args):
                 "all_mode_products": {"achieved": inst["achieved"], "frac": inst["frac"], "launches": inst["launches"],
                                       "avg_launch_ms": inst["avg_launch_ms"], "share_of_step": inst["share_of_step"]},
                 "step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
-                "step": step_roofline(flops_exec, w.N, peak_dmma, us_per_solve),
+                "step": step_roofline(flops_exec, w.N, peak_dmma, us_per_solve, w.flops_per_solve),
+                "step_frac_dense_count": w.n_orb * n_tgt_local * w.flops_per_solve / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
                 "flops_per_solve_executed": flops_exec, "flops_per_solve_algorithmic": w.flops_per_solve,
                 "executed_over_algorithmic_flops": flops_exec / w.flops_per_solve,
                 "algorithmic_tflops_whole_step": w.n_orb * n_tgt_local * w.flops_per_solve / (ms_per_step * 1e-3) / 1e12,
-                "flops_note": "achieved / frac / step_frac count the FP64 operations the kernels execute (padding excluded); "
-                              "the reflection-adapted bases halve the operations of the products, so the dense "
-                              "algorithmic count would give fractions above 1",
+                "flops_note": "achieved / frac (= frac_executed_count) / step_frac count the FP64 operations the kernels "
+                              "execute (padding excluded): how busy the tensor pipe is.  frac_dense_count / "
+                              "step_frac_dense_count credit the same time with SURVEY.md 8(d)'s dense algorithmic count "
+                              "(2 N n per product): the reflection-adapted bases halve the executed operations, so these "
+                              "exceed 1",
                 "class_ms_per_step": inst["class_ms_per_step"],
                 "measured": f"{prof_steps} separate instrumented step(s) (CUDA-event pair around every launch, caller's stream)"}
     if roofline["step"]["bound"] == "hbm" and dom is not None:
@@ -644,9 +682,12 @@ def run_b200(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(w, n_c, {"parallelism": f"targets sharded over {world} rank(s) ({args.scaling} scaling), "
-                                                           "orbitals replicated; one all-reduce of the per-target energies",
-                                           "pair_solves_all_ranks": solves_all_ranks}),
+            "config": config_dict(w, n_c),
+            "parallelism": f"targets sharded over {world} rank(s) ({args.scaling} scaling), orbitals replicated; one "
+                           "all-reduce of the per-target energies",
+            "pair_solves_all_ranks": solves_all_ranks,
+            "backend": (args.backend if world > 1 else None) if args.backend == "nccl" else
+                       f"gloo (DEBUG: {world} rank(s) on {torch.cuda.device_count()} GPU(s); not a scaling measurement)",
             "applies_per_s": n_tgt_union / (ms_per_step * 1e-3), "E_x": ex_val,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches_per_step * args.steps * world),
             "roofline": roofline, "cpu_baseline": cpu_baseline,

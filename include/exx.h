@@ -28,9 +28,12 @@
  *  - All work is enqueued on `cuda_stream` (a cudaStream_t passed as void*, NULL = default stream).
  *    exx_apply / exx_poisson_solve never synchronise the host; results (including *d_ex) are valid once
  *    the caller has synchronised that stream.  The calls are CUDA-graph capturable.
- *  - Every entry point returns an exx_status; nothing throws, exits or aborts.  Arguments are validated
+ *  - Every entry point returns an exx_status; no host code throws, exits or aborts.  Arguments are validated
  *    before the first launch, so a call that returns EXX_ERR_INVALID_ARG / _WORKSPACE / _ALIAS has
- *    enqueued nothing.
+ *    enqueued nothing.  One device-side exception: a TMA-pipeline kernel whose mbarrier wait has not completed
+ *    after 2^30 polls (minutes; only a hardware fault or a corrupted tensor map can cause it) executes a trap
+ *    rather than hang the stream, which the next synchronising CUDA call reports (EXX_ERR_CUDA from this library;
+ *    the CUDA context is lost, as after any device-side fault).
  *  - occ is used exactly as passed: no mixing fraction, spin factor or Brillouin weight (R8), no
  *    thresholding of small occupations (R9).
  *  - There is no CPU fallback: without a CUDA device every compute call returns EXX_ERR_CUDA.

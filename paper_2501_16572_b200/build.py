@@ -25,7 +25,7 @@ COMPILE_FLAGS = [
     "-Xcompiler", "-fPIC,-O3,-Wall,-Wno-unused-function",
     "-Xptxas", "-v",
 ]
-LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "--shared"]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-ldl"]   # -ldl: header-only NVTX v3 dlopens its tool
 
 
 def _nvcc() -> str:

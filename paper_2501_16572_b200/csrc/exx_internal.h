@@ -1,5 +1,6 @@
 // Internal declarations shared by the host planner, the kernels and the C-ABI layer of libexx.so.
 #pragma once
+#include <nvtx3/nvToolsExt.h>
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -156,11 +157,24 @@ struct DeviceScope {
 };
 
 // RAII event pair around one launch when profiling is on (no-op otherwise).
+// Every scope is also an NVTX range on the host thread (a range per stage), named after the pass of a
+// batch or the kernel class, so a tool that understands NVTX (ncu --nvtx --nvtx-include "exx:z/", a timeline viewer) can
+// select or label the launches of one pass.  Header-only NVTX v3: without a tool attached a push/pop is a null-pointer test.
+inline const char* prof_scope_name(int cls, int pass) {
+  static const char* const kPassName[PASS_COUNT] = {"exx:x_forward", "exx:y_forward", "exx:z", "exx:z_backward",
+                                                    "exx:y_backward", "exx:x_backward", "exx:x_backward_orbital_side",
+                                                    "exx:mode_product"};
+  static const char* const kClassName[KC_COUNT] = {"exx:mode_product", "exx:pair_density", "exx:accumulate", "exx:energy"};
+  if (cls == KC_MODE_PRODUCT && pass >= 0 && pass < PASS_COUNT) return kPassName[pass];
+  return cls >= 0 && cls < KC_COUNT ? kClassName[cls] : "exx";
+}
+
 struct ProfScope {
   exx_plan* p;
   cudaStream_t s;
   cudaEvent_t e1;
   ProfScope(exx_plan* plan, int cls, cudaStream_t stream, int pass = -1) : p(plan), s(stream), e1(nullptr) {
+    nvtxRangePushA(prof_scope_name(cls, pass));
     if (!p->prof_on) return;
     cudaEvent_t e0;
     if (cudaEventCreate(&e0) != cudaSuccess) return;
@@ -170,6 +184,7 @@ struct ProfScope {
   }
   ~ProfScope() {
     if (e1) cudaEventRecord(e1, s);
+    nvtxRangePop();
   }
   void cancel() {  // nothing was launched inside this scope: drop the record
     if (!e1) return;

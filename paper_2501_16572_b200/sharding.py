@@ -25,16 +25,16 @@ def weak_scaling_targets(tgt_start: int, n_tgt: int, n_orb: int, rank: int) -> t
 
 
 def reduce_energy(e_k_local: torch.Tensor, occ_tgt_local: torch.Tensor, k0: int, n_tgt: int, group=None):
-    """All-reduce the per-target energies into the full [n_tgt] vector and E_x = 1/2 sum_k occ_k e_k.
+    """All-reduce the per-target energies into the full [n_tgt] vector and E_x = 1/2 sum_k occ_k e_k: ONE collective
+    over a buffer of n_tgt + 1 doubles (the energies in their slots, this rank's partial E_x in the last one).
     Works with any backend (nccl on GPUs, gloo in the CPU tests); a no-op without torch.distributed."""
     import torch.distributed as dist
-    e_k = torch.zeros(n_tgt, dtype=torch.float64, device=e_k_local.device)
-    e_k[k0:k0 + e_k_local.numel()] = e_k_local
-    ex = 0.5 * torch.sum(occ_tgt_local * e_k_local).reshape(1)
+    buf = torch.zeros(n_tgt + 1, dtype=torch.float64, device=e_k_local.device)
+    buf[k0:k0 + e_k_local.numel()] = e_k_local
+    buf[n_tgt] = 0.5 * torch.sum(occ_tgt_local * e_k_local)
     if dist.is_available() and dist.is_initialized():
-        dist.all_reduce(e_k, op=dist.ReduceOp.SUM, group=group)
-        dist.all_reduce(ex, op=dist.ReduceOp.SUM, group=group)
-    return e_k, ex[0]
+        dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+    return buf[:n_tgt], buf[n_tgt]
 
 
 def shard_orbitals(n_orb: int, rank: int, world: int) -> tuple[int, int, int]:
