@@ -96,3 +96,22 @@ def test_energy_static_rejects_more_targets_than_its_array_holds():
     exx.energy_static(tgt[:n - 1], tgt[:n - 1], occ[:n - 1], 1.0, e_k[:n - 1], ex)
     torch.cuda.synchronize()
     assert bool((e_k[:n - 1] == 4.0).all()) and float(ex) == 0.5 * 4.0 * (n - 1)
+
+
+def test_energy_static_on_the_two_plane_complex_sets_of_the_bloch_variant():
+    """n_points = 2 N: a complex function is a real plane followed by an imaginary plane, and the plain dot product over
+    both planes is Re <tgt, vx> -- the e_k exx_apply_bloch returns (its existing path, same tolerance)."""
+    dev = torch.device("cuda", 0)
+    nx, ny, nz, h = 16, 12, 10, 0.35
+    plan = exx.Plan(nx, ny, nz, h, (0, 0, 1), 12, 0.106, max_batch=8, device=0, theta=(0.6, -1.0, 0.0))
+    g = torch.Generator().manual_seed(11)
+    psi = torch.randn((5, 2, nz, ny, nx), dtype=torch.float64, generator=g).to(dev)
+    tgt = torch.randn((3, 2, nz, ny, nx), dtype=torch.float64, generator=g).to(dev)
+    occ = torch.linspace(2.0, 0.1, 5, dtype=torch.float64).to(dev)
+    vx, e_k = plan.apply_bloch(psi, occ, tgt, n_c=4)
+    torch.cuda.synchronize()
+    s_e = torch.full((3,), float("nan"), dtype=torch.float64, device=dev)
+    exx.energy_static(tgt, vx, None, h * h * h, s_e, None)      # no occupations: e_k only
+    torch.cuda.synchronize()
+    assert _close(s_e, e_k)
+    plan.close()
