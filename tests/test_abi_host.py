@@ -68,6 +68,26 @@ def test_host_only_plan_refuses_compute_loudly(lib):
     p.close()
 
 
+def test_energy_static_validates_before_touching_a_device(lib):
+    """exx_energy_static (the entry point for callers that cannot allocate device memory): argument errors and the
+    fixed capacity of its in-library scratch array are reported before any CUDA call, so they can be checked without a
+    GPU; with valid arguments and no device the call fails loudly (there is no CPU fallback)."""
+    d = C.c_void_p(1 << 20)
+    f = lib.exx_energy_static
+    assert f(d, d, d, exx.ENERGY_STATIC_MAX_TGT + 1, 10, 1.0, d, d, None) == 7           # EXX_ERR_LIMIT
+    assert b"EXX_ERR_LIMIT" in lib.exx_status_string(7) and b"4096" in lib.exx_status_string(7)
+    assert f(d, d, d, -1, 10, 1.0, d, d, None) == 1                                       # n_tgt < 0
+    assert f(d, d, d, 2, 0, 1.0, d, d, None) == 1                                         # n_points < 1
+    assert f(d, d, d, 2, 10, 0.0, d, d, None) == 1                                        # dv <= 0
+    assert f(None, d, d, 2, 10, 1.0, d, d, None) == 1                                     # missing input
+    assert f(d, d, None, 2, 10, 1.0, d, d, None) == 1                                     # E_x without occupations
+    assert f(d, d, d, 2, 10, 1.0, None, None, None) == 0                                  # nothing asked for: a no-op
+    import torch
+    if not torch.cuda.is_available():
+        st = f(d, d, d, 2, 10, 1.0, d, d, None)
+        assert st == 3 and b"EXX_ERR_CUDA" in lib.exx_status_string(st)
+
+
 @pytest.mark.parametrize("dims,bc,omega,h", [((16, 16, 16), (0, 0, 0), 0.0, 0.5), ((12, 10, 30), (0, 0, 1), 0.106, 0.25),
                                              ((48, 48, 48), (0, 0, 0), 0.106, 0.25), ((7, 9, 5), (1, 0, 1), 0.106, 0.3),
                                              ((120, 60, 1), (1, 0, 0), 0.106, 0.2)])
